@@ -1,0 +1,152 @@
+/*
+ * ulens.h -- C ABI of the B200-native image-centred ray-shooting (ICRS) hot path.
+ *
+ * What is computed (citations are to /root/reference/PAPER.md, "P:<line>"):
+ *
+ *   finite-source, limb-darkened magnification of an N-point-mass lens (N = 1, 2, 3)
+ *
+ *       A(w_c, rho, u1) = (1/F0) Int Int Theta(rho - |w(z) - w_c|) I(|w(z) - w_c| / rho) d^2 z   Eqs. 5-6
+ *       w(z) = z - sum_i eps_i / conj(z - a_i),  sum_i eps_i = 1                                 Eq. 1,
+ *       I(x) = 1 - u1 (1 - sqrt(1 - x^2)),       F0 = pi rho^2 (1 - u1/3)                         Eq. A6,
+ *
+ *   by the paper's method: Ehrlich-Aberth roots of the lens polynomial (Eq. 4, Eq. 7),
+ *   image-limb points (Eq. 8) -> polar (r, theta) sectors -> fixed polar grid of
+ *   rays per sector with cubic edge location along theta and a limb-singularity-aware ring quadrature
+ *   (Sec. 3.3, App. A), summed over rings and sectors and normalised (Eq. A5).
+ *
+ * Conventions
+ *   - every function returns int: 0 = ULENS_OK, negative = error (below); ulens_strerror() names it.
+ *   - "device" pointers are CUDA device memory OWNED BY THE CALLER (e.g. torch tensors); the library
+ *     never frees or keeps them beyond the work it enqueues. "host" pointers are ordinary memory, read
+ *     (or written, for *_host entry points) before the call returns.
+ *   - all device work is enqueued on the caller's stream (a cudaStream_t passed as void*, NULL = the
+ *     legacy default stream) and the call does NOT synchronise, except the *_host entry points, the
+ *     stats/peak calls and ulens_destroy, which say so.
+ *   - one context = one device = one stream at a time (the context owns the workspace the kernels share).
+ *   - lengths are in Einstein radii of the TOTAL lens mass; complex numbers are passed as
+ *     separate re / im arrays (SoA); doubles are IEEE binary64.
+ *   - per-point trouble (root iteration not converged, patch cap hit, resolution cap hit, image
+ *     touching a patch border, ...) is reported in the optional status bitmask, not as an error code.
+ *   - there is NO CPU fallback: every step runs in the CUDA kernels of this library.
+ */
+#ifndef ULENS_H
+#define ULENS_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define ULENS_OK            0
+#define ULENS_EINVAL       -1   /* NULL where not allowed, non-finite or out-of-domain scalar, negative size */
+#define ULENS_ECUDA        -2   /* a CUDA runtime call failed (ulens_last_cuda_error has the text) */
+#define ULENS_ENOMEM       -3   /* workspace allocation failed */
+#define ULENS_EUNSUPPORTED -4   /* valid request that this build does not implement */
+
+/* per-point status bits (status_out) */
+#define ULENS_ST_EA_NOCONV   0x0001u  /* an Ehrlich-Aberth solve hit its iteration cap (Eq. 7) */
+#define ULENS_ST_IMG_PARITY  0x0002u  /* centre image count not congruent N+1 (mod 2) */
+#define ULENS_ST_PATCH_CAP   0x0004u  /* more sectors than the cap: merged into one */
+#define ULENS_ST_RES_CAP     0x0008u  /* a sector wanted more rings / rays than the cap allows */
+#define ULENS_ST_CLIPPED     0x0010u  /* an inside ray sat on a sector border (margin too small) */
+#define ULENS_ST_UNIT_OVF    0x0020u  /* work-queue overflow: point not integrated, A = NaN */
+#define ULENS_ST_ERR_HIGH    0x0040u  /* half-resolution self-check differs by more than rel_tol */
+#define ULENS_ST_NO_IMAGE    0x0080u  /* no image-limb point found (A = NaN) */
+#define ULENS_ST_NIMG_SHIFT  8        /* bits 8..11: number of images of the source centre */
+
+typedef struct ulens_ctx ulens_ctx;
+
+/* Tunables; a zeroed struct (or NULL) selects the defaults in brackets. */
+typedef struct {
+    int    n_limb;        /* source-limb samples per point, multiple of 32 (Eq. 8: ~500) [512]   */
+    int    n_r;           /* rings per image half-extent in r (P:139 N_r)                        [384]   */
+    int    n_theta;       /* rays per image half-extent in theta (P:139 N_theta)                 [48]    */
+    double rel_tol;       /* self-check threshold for ULENS_ST_ERR_HIGH                          [1e-4]  */
+    int    chunk_pts;     /* points processed per internal pass (workspace size)                 [65536] */
+    int    flags;         /* reserved, 0 */
+} ulens_options;
+
+/* Lens: n_lens in {1,2,3}; eps sums to 1; positions in Einstein radii of the total mass. */
+typedef struct {
+    int    n_lens;
+    double eps[3];
+    double ax[3];
+    double ay[3];
+} ulens_lens;
+
+typedef struct {
+    uint64_t n_points;     /* source points integrated since create / reset */
+    uint64_t n_rays;       /* lens-map evaluations in the ray-shooting kernel */
+    uint64_t n_patches;    /* sectors integrated */
+    uint64_t n_units;      /* 32-ring work units integrated */
+    uint64_t n_limb_solves;/* polynomial solves at limb points */
+    uint64_t n_flagged;    /* points with any status bit 0x00ff set */
+} ulens_stats;
+
+int  ulens_create (ulens_ctx** out, int cuda_device, const ulens_options* opt);
+void ulens_destroy(ulens_ctx* ctx);                       /* synchronises the device, frees the workspace */
+
+/* Geometry (Fig. 3 caption P:203; readings G4/G5 in DESIGN.md).
+ * binary: origin = barycentre of M1, M2; M1 (eps 1/(1+q)) at x = -s q/(1+q), M2 (eps q/(1+q)) at x = +s/(1+q).
+ * triple: q3 = M3/M1, M3 at polar (r3, psi) from the MIDPOINT of M1-M2; eps = (1, q, q3)/(1+q+q3).
+ * EINVAL unless s > 0, q > 0, q3 >= 0, r3 > 0, all finite. Host-only helpers. */
+int  ulens_lens_binary(ulens_lens* out, double s, double q);
+int  ulens_lens_triple(ulens_lens* out, double s, double q, double q3, double r3, double psi);
+
+/* (i) Source positions in -> magnification out.
+ * n_cfg lens/source configurations, n_pts source centres each, row-major [cfg][pt].
+ *   lenses_host, rho_host, u1_host : host arrays of n_cfg entries, copied during the call
+ *                                    (rho > 0, 0 <= u1 <= 1, else EINVAL).
+ *   w_re, w_im   : device, n_cfg*n_pts doubles, source centres w_c.
+ *   A_out        : device, n_cfg*n_pts doubles, magnification (Eq. 6 / A5).
+ *   err_out      : device or NULL, n_cfg*n_pts doubles: |A - A(half radial resolution)| / A.
+ *   status_out   : device or NULL, n_cfg*n_pts uint32 bitmasks (ULENS_ST_*).
+ * n_cfg == 0 or n_pts == 0 is a successful no-op. */
+int  ulens_mag(ulens_ctx* ctx, int n_cfg, int n_pts,
+               const ulens_lens* lenses_host, const double* rho_host, const double* u1_host,
+               const double* w_re, const double* w_im,
+               double* A_out, double* err_out, uint32_t* status_out, void* stream);
+
+/* Same with HOST arrays for w_re, w_im, A_out, err_out, status_out: copies in, computes, copies out and
+ * synchronises the stream before returning (the end-to-end entry point). */
+int  ulens_mag_host(ulens_ctx* ctx, int n_cfg, int n_pts,
+               const ulens_lens* lenses_host, const double* rho_host, const double* u1_host,
+               const double* w_re_host, const double* w_im_host,
+               double* A_out_host, double* err_out_host, uint32_t* status_out_host, void* stream);
+
+/* (ii) Trajectory parameters in -> light curve out (binary lens, reading G3):
+ *   theta_host [n_cfg][7] = (t0, u0, tE, s, q, rho, alpha), host; u1 shared; t device [n_epochs].
+ *   tau = (t - t0)/tE,  w_c = (tau cos a - u0 sin a) + i (tau sin a + u0 cos a).
+ *   A_out device [n_cfg][n_epochs]; dA_out device [n_cfg][n_epochs][7] or NULL (forward-mode
+ *   derivatives dA/d(t0,u0,tE,s,q,rho,alpha), Sec. 3.5). */
+int  ulens_lightcurve_binary(ulens_ctx* ctx, int n_cfg, int n_epochs,
+               const double* theta_host, double u1, const double* t,
+               double* A_out, double* dA_out, double* err_out, uint32_t* status_out, void* stream);
+
+/* (iii) Root export (Eq. 4, Eq. 7): all N^2+1 roots of the lens polynomial for
+ * each source position and which of them are images (validated on Eq. 1; images are polished
+ * on Eq. 1). roots_re/im device [n_pts][n_deg], is_image device [n_pts][n_deg] bytes, n_deg = N^2+1. */
+int  ulens_roots(ulens_ctx* ctx, const ulens_lens* lens_host, int n_pts,
+               const double* w_re, const double* w_im,
+               double* roots_re, double* roots_im, uint8_t* is_image, void* stream);
+
+/* Counters (synchronises the device). ulens_reset_stats zeroes them. */
+int  ulens_get_stats(ulens_ctx* ctx, ulens_stats* out);
+int  ulens_reset_stats(ulens_ctx* ctx);
+
+/* Names of the kernels a call launches, for launch accounting: number of kernel launches the last
+ * ulens_mag / ulens_lightcurve_binary / ulens_roots call on this context enqueued. */
+int  ulens_last_launch_count(ulens_ctx* ctx);
+
+/* FP64 FMA roofline denominator: runs a dependent-chain-free DFMA kernel on every SM for about
+ * `ms` milliseconds and returns the achieved rate in DFMA/s (one DFMA = 2 flop). Synchronises. */
+int  ulens_fp64_peak(ulens_ctx* ctx, double ms, double* dfma_per_s);
+
+const char* ulens_strerror(int code);
+const char* ulens_last_cuda_error(ulens_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ULENS_H */

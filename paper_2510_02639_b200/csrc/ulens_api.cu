@@ -1,0 +1,640 @@
+// ulens_api.cu -- kernels and C ABI (include/ulens.h) of the B200-native ICRS hot path.
+//
+// Pipeline per chunk of source points (all on the caller's stream, no host round trip in between):
+//   k_traj      (lightcurve entry only)  trajectory -> source centres
+//   k_roots     thread per point: lens polynomial, Ehrlich-Aberth, validate + polish         Eq. 4, 7
+//   k_regions   warp per point: limb images -> polar sectors -> 32-ring work units           Sec. 3.2
+//   k_shoot     warp per work unit, lane per ring: rays along theta, edge events, ring sums  Sec. 3.3, App. A
+//   k_finalize  thread per point: ordered sum of its units, normalise                        Eq. A5
+//
+// There is no CPU implementation behind this ABI: without a CUDA device every entry point fails.
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <string.h>
+#include <new>
+#include <vector>
+
+#include "../../include/ulens.h"
+#include "ulens_core.cuh"
+#include "ulens_regions.cuh"
+#include "ulens_host.hpp"
+
+using namespace ulens;
+
+// ------------------------------------------------------------------------------------------------ context
+
+struct DevCounters {
+    unsigned long long n_rays, n_patches, n_units, n_limb_solves, n_flagged, n_points;
+};
+
+struct ChunkCounters {          // reset per chunk
+    unsigned int n_units;       // units allocated by k_regions
+    unsigned int next_unit;     // dynamic scheduler of k_shoot
+};
+
+struct ulens_ctx {
+    int device;
+    ulens_options opt;
+    RegionParams rp;
+    int chunk;
+    size_t cap_units;
+    // workspace (device)
+    Patch* patches;             // [chunk][UL_MAXP]
+    int* n_patch;               // [chunk]
+    unsigned* status_ws;        // [chunk]
+    unsigned* unit_desc;        // [cap_units]  (patch slot << 8) | ring block
+    double* unit_sum;           // [cap_units]  all rings
+    double* unit_odd;           // [cap_units]  odd rings only (half-resolution self-check)
+    ChunkCounters* cc;
+    DevCounters* counters;
+    PointCfg* cfg_dev; LensPoly* poly_dev; size_t cfg_cap;
+    double* traj_w; size_t traj_cap;    // lightcurve entry: source centres [2][n]
+    double* io_buf; size_t io_cap;      // *_host entry: staging
+    int last_launches;
+    char cuda_err[256];
+};
+
+static int fail_cuda(ulens_ctx* c, cudaError_t e, const char* where)
+{
+    if (c) snprintf(c->cuda_err, sizeof c->cuda_err, "%s: %s", where, cudaGetErrorString(e));
+    return ULENS_ECUDA;
+}
+#define CK(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return fail_cuda(ctx, e_, #call); } while (0)
+
+// ------------------------------------------------------------------------------------------------ host geometry
+
+static bool finite_pos(double x) { return isfinite(x) && x > 0.0; }
+
+extern "C" int ulens_lens_binary(ulens_lens* out, double s, double q)
+{
+    if (!out || !finite_pos(s) || !finite_pos(q)) return ULENS_EINVAL;
+    memset(out, 0, sizeof *out);
+    out->n_lens = 2;
+    out->eps[0] = 1.0 / (1.0 + q);
+    out->eps[1] = q / (1.0 + q);
+    out->ax[0] = -s * q / (1.0 + q);          // G4: primary at negative x, barycentre of M1, M2 at the origin
+    out->ax[1] = s / (1.0 + q);
+    return ULENS_OK;
+}
+
+extern "C" int ulens_lens_triple(ulens_lens* out, double s, double q, double q3, double r3, double psi)
+{
+    if (!out || !finite_pos(s) || !finite_pos(q) || !(q3 >= 0.0) || !isfinite(q3) || !finite_pos(r3) || !isfinite(psi))
+        return ULENS_EINVAL;
+    memset(out, 0, sizeof *out);
+    double tot = 1.0 + q + q3;
+    out->n_lens = 3;
+    out->eps[0] = 1.0 / tot; out->eps[1] = q / tot; out->eps[2] = q3 / tot;
+    out->ax[0] = -s * q / (1.0 + q);
+    out->ax[1] = s / (1.0 + q);
+    double mid = 0.5 * (out->ax[0] + out->ax[1]);      // G5: M3 at polar (r3, psi) from the midpoint of M1-M2
+    out->ax[2] = mid + r3 * cos(psi);
+    out->ay[2] = r3 * sin(psi);
+    return ULENS_OK;
+}
+
+
+// ------------------------------------------------------------------------------------------------ kernels
+
+__device__ __forceinline__ double warp_sum(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// trajectory (G3): tau = (t - t0)/tE,  w = (tau cos a - u0 sin a) + i (tau sin a + u0 cos a)
+__global__ void k_traj(int n_cfg, int n_ep, const double* __restrict__ theta, const double* __restrict__ t,
+                       double* __restrict__ w_re, double* __restrict__ w_im)
+{
+    long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= (long long)n_cfg * n_ep) return;
+    int c = (int)(i / n_ep), e = (int)(i % n_ep);
+    const double* th = theta + 7 * c;
+    double tau = (t[e] - th[0]) / th[2];
+    double ca = cos(th[6]), sa = sin(th[6]);
+    w_re[i] = tau * ca - th[1] * sa;
+    w_im[i] = tau * sa + th[1] * ca;
+}
+
+// One thread per source point: all roots, image flags, images polished on Eq. 1.
+// out_* may be NULL (then only the status word is produced).
+template <int N>
+__global__ void k_roots(int n, int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cfg,
+                        const LensPoly* __restrict__ poly, const double* __restrict__ w_re,
+                        const double* __restrict__ w_im, double* __restrict__ out_re, double* __restrict__ out_im,
+                        uint8_t* __restrict__ out_img, unsigned* __restrict__ status)
+{
+    constexpr int DEG = N * N + 1;
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    long long gp = (long long)pt_base + i;
+    int c = (int)(gp / n_pts_per_cfg);
+    Lens L = cfg[c].lens;
+    double wx = w_re[gp], wy = w_im[gp];
+    double br[DEG + 1], bi[DEG + 1], zr[DEG], zi[DEG];
+    poly_coeffs<N>(L, poly[c], wx, wy, br, bi);
+    ea_init<DEG>(br, bi, zr, zi);
+    int it = ea_iterate<DEG>(br, bi, zr, zi, 100);
+    unsigned st = (it > 100) ? UL_ST_EA_NOCONV : 0u;
+    // validate + polish (G7): damped Newton on Eq. 1 from every root; accept converged, un-moved, distinct ones
+    double ix[DEG], iy[DEG];
+    int n_img = 0;
+    unsigned mask = 0;
+#pragma unroll
+    for (int k = 0; k < DEG; ++k) {
+        double zx = zr[k], zy = zi[k], detJ, resid, gx, gy;
+        double dm2 = 1e300;
+#pragma unroll
+        for (int a = 0; a < N; ++a) { double dx = zx - L.ax[a], dy = zy - L.ay[a]; dm2 = ul_min(dm2, dx * dx + dy * dy); }
+        bool ok = polish_image<N>(L, wx, wy, zx, zy, 8, 1e-13, detJ, resid, gx, gy);
+        double mv2 = (zx - zr[k]) * (zx - zr[k]) + (zy - zi[k]) * (zy - zi[k]);
+        ok = ok && (mv2 <= 0.01 * dm2);
+        if (ok) {
+            double sc = ul_max(1.0, zx * zx + zy * zy);
+            for (int q = 0; q < n_img; ++q) {
+                double ddx = zx - ix[q], ddy = zy - iy[q];
+                if (ddx * ddx + ddy * ddy < 1e-18 * sc) ok = false;
+            }
+        }
+        if (ok) { ix[n_img] = zx; iy[n_img] = zy; ++n_img; mask |= 1u << k; zr[k] = zx; zi[k] = zy; }
+    }
+    if (((n_img - (N + 1)) & 1) != 0 || n_img < N + 1) st |= UL_ST_IMG_PARITY;
+    st |= (unsigned)(n_img & 0xf) << 8;
+    if (status) status[i] = st;
+    if (out_re) {
+#pragma unroll
+        for (int k = 0; k < DEG; ++k) {
+            out_re[(long long)i * DEG + k] = zr[k];
+            out_im[(long long)i * DEG + k] = zi[k];
+            out_img[(long long)i * DEG + k] = (mask >> k) & 1u;
+        }
+    }
+}
+
+// One warp per source point.
+template <int N>
+__global__ void __launch_bounds__(128)
+k_regions(int n, int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cfg, const LensPoly* __restrict__ poly,
+          const double* __restrict__ w_re, const double* __restrict__ w_im, RegionParams rp,
+          Patch* __restrict__ patches, int* __restrict__ n_patch, unsigned* __restrict__ status,
+          unsigned* __restrict__ unit_desc, unsigned cap_units, ChunkCounters* cc, DevCounters* ctr)
+{
+    constexpr int DEG = N * N + 1;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    RegionWork<DEG>* Wall = reinterpret_cast<RegionWork<DEG>*>(smem_raw);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    int i = blockIdx.x * (blockDim.x >> 5) + warp;
+    if (i >= n) return;                                  // whole warp leaves together
+    RegionWork<DEG>& W = Wall[warp];
+    long long gp = (long long)pt_base + i;
+    int c = (int)(gp / n_pts_per_cfg);
+    Lens L = cfg[c].lens;
+    double rho = cfg[c].rho;
+    double wcx = w_re[gp], wcy = w_im[gp];
+    unsigned st = 0; int n_solves = 0;
+    regions_phaseA<N>(lane, L, poly[c], wcx, wcy, rho, rp, W, st, n_solves);
+    st = __reduce_or_sync(0xffffffffu, st);
+    __syncwarp();
+    regions_phaseB<DEG>(lane, W);
+    __syncwarp();
+    int np = 0; unsigned base = 0; int total_units = 0;
+    if (lane == 0) {
+        np = regions_phaseC<N>(W, rp, i, L, wcx, wcy, rho, st);
+        for (int p = 0; p < np; ++p) total_units += W.patch[p].n_units;
+        base = atomicAdd(&cc->n_units, (unsigned)total_units);
+        if ((unsigned long long)base + total_units > cap_units) { st |= UL_ST_UNIT_OVF; np = 0; total_units = 0; }
+        int u = base;
+        for (int p = 0; p < np; ++p) { W.patch[p].unit0 = u; u += W.patch[p].n_units; patches[(long long)i * UL_MAXP + p] = W.patch[p]; }
+        n_patch[i] = np;
+        status[i] |= st;                                 // k_roots wrote the word first
+        atomicAdd(&ctr->n_limb_solves, (unsigned long long)(32 * (rp.n_limb / 32 + 1)));
+        atomicAdd(&ctr->n_patches, (unsigned long long)np);
+    }
+    np = __shfl_sync(0xffffffffu, np, 0);
+    __syncwarp();
+    for (int p = 0; p < np; ++p) {
+        int nu = W.patch[p].n_units, u0 = W.patch[p].unit0;
+        for (int b = lane; b < nu; b += 32) unit_desc[u0 + b] = ((unsigned)(i * UL_MAXP + p) << 8) | (unsigned)b;
+    }
+}
+
+// One warp per 32-ring work unit, one lane per ring (Sec. 3.3; App. A). Units are pulled from a device counter.
+template <int N, bool LD>
+__global__ void __launch_bounds__(128)
+k_shoot(int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cfg, const double* __restrict__ w_re,
+        const double* __restrict__ w_im, const Patch* __restrict__ patches, const unsigned* __restrict__ unit_desc,
+        double* __restrict__ unit_sum, double* __restrict__ unit_odd, unsigned* __restrict__ status,
+        ChunkCounters* cc, DevCounters* ctr)
+{
+    const int lane = threadIdx.x & 31;
+    const unsigned n_units = cc->n_units;
+    unsigned long long rays = 0;
+    for (;;) {
+        unsigned u = 0;
+        if (lane == 0) u = atomicAdd(&cc->next_unit, 1u);
+        u = __shfl_sync(0xffffffffu, u, 0);
+        if (u >= n_units) break;
+        unsigned d = unit_desc[u];
+        const Patch P = patches[d >> 8];
+        int blk = (int)(d & 0xffu);
+        long long gp = (long long)pt_base + P.point;
+        int c = (int)(gp / n_pts_per_cfg);
+        Lens L = cfg[c].lens;
+        double rho = cfg[c].rho, u1 = cfg[c].u1;
+        double wcx = w_re[gp], wcy = w_im[gp];
+        int line = blk * 32 + lane;
+        double U, S, f; bool edge, clipped;
+        // line flux: (1-u1) Int chi dA + (u1/rho) Int chi sqrt(-F) dA      (Eq. A6 split, G12)
+        if (P.flags & UL_PATCH_SCAN_R) {
+            double th = P.th0 + (line + 0.5) * P.dth;
+            shoot_col<N, LD>(L, wcx, wcy, rho * rho, th, P.r0, P.dr, P.n_r, U, S, edge);
+            f = ((1.0 - u1) * U + (LD ? (u1 / rho) * S : 0.0)) * P.dth;
+            clipped = edge;
+        } else {
+            double r = P.r0 + (line + 0.5) * P.dr;
+            bool periodic = (P.flags & UL_PATCH_PERIODIC) != 0;
+            shoot_ring<N, LD>(L, wcx, wcy, rho * rho, r, P.th0, P.dth, P.n_th, periodic, U, S, edge);
+            f = r * ((1.0 - u1) * U + (LD ? (u1 / rho) * S : 0.0)) * P.dth * P.dr;
+            clipped = edge || ((line < 1 || line >= P.n_r - 1) && U > 0.0 && P.r0 > 0.0);
+        }
+        double tot = warp_sum(f);
+        double odd = warp_sum((lane & 1) ? f : 0.0);
+        unsigned any_clip = __ballot_sync(0xffffffffu, clipped);
+        if (lane == 0) {
+            unit_sum[u] = tot;
+            unit_odd[u] = 2.0 * odd;
+            if (any_clip) atomicOr(&status[P.point], UL_ST_CLIPPED);
+            rays += 32ull * (unsigned long long)(((P.flags & UL_PATCH_SCAN_R) ? P.n_r : P.n_th) + 4);
+        }
+    }
+    if (lane == 0 && rays) atomicAdd(&ctr->n_rays, rays);
+}
+
+// One thread per point: ordered (deterministic) sum over its sectors' units, normalisation (Eq. A5; F0 of P:99).
+__global__ void k_finalize(int n, int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cfg,
+                           const Patch* __restrict__ patches, const int* __restrict__ n_patch,
+                           const double* __restrict__ unit_sum, const double* __restrict__ unit_odd,
+                           const unsigned* __restrict__ status_ws, double rel_tol,
+                           double* __restrict__ A_out, double* __restrict__ err_out, unsigned* __restrict__ status_out,
+                           DevCounters* ctr)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    long long gp = (long long)pt_base + i;
+    int c = (int)(gp / n_pts_per_cfg);
+    double rho = cfg[c].rho, u1 = cfg[c].u1;
+    double F0 = UL_PI * rho * rho * (1.0 - u1 / 3.0);
+    int np = n_patch[i];
+    double s = 0.0, so = 0.0;
+    unsigned long long nu_tot = 0;
+    for (int p = 0; p < np; ++p) {
+        const Patch& P = patches[(long long)i * UL_MAXP + p];
+        int nu = P.n_units;
+        nu_tot += nu;
+        for (int b = 0; b < nu; ++b) { s += unit_sum[P.unit0 + b]; so += unit_odd[P.unit0 + b]; }
+    }
+    unsigned st = status_ws[i];
+    double A = s / F0, Ao = so / F0;
+    if (np == 0) { A = nan(""); Ao = A; }
+    // half-resolution self check: the radial rule errs like dr^1.5 (square-root ring ends), so the error
+    // of the full sum is about |A - A_half| / (2^1.5 - 1)
+    double err = fabs(A - Ao) / (1.8284271247461903 * fabs(A));
+    if (!(err <= rel_tol)) st |= UL_ST_ERR_HIGH;
+    A_out[gp] = A;
+    if (err_out) err_out[gp] = err;
+    if (status_out) status_out[gp] = st;
+    atomicAdd(&ctr->n_units, nu_tot);
+    if (i == 0) atomicAdd(&ctr->n_points, (unsigned long long)n);
+    if (st & 0xffu) atomicAdd(&ctr->n_flagged, 1ull);
+}
+
+// FP64 FMA peak: 8 independent chains per thread
+__global__ void k_dfma_peak(int iters, double* out)
+{
+    double a0 = threadIdx.x * 1e-9, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6, a7 = a0 + 7;
+    const double m = 1.0000001, b = 1e-9;
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            a0 = fma(a0, m, b); a1 = fma(a1, m, b); a2 = fma(a2, m, b); a3 = fma(a3, m, b);
+            a4 = fma(a4, m, b); a5 = fma(a5, m, b); a6 = fma(a6, m, b); a7 = fma(a7, m, b);
+        }
+    }
+    double s = a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7;
+    if (s == 12345.678) out[0] = s;
+}
+
+// ------------------------------------------------------------------------------------------------ C ABI
+
+extern "C" const char* ulens_strerror(int code)
+{
+    switch (code) {
+        case ULENS_OK: return "ok";
+        case ULENS_EINVAL: return "invalid argument";
+        case ULENS_ECUDA: return "CUDA error";
+        case ULENS_ENOMEM: return "out of memory";
+        case ULENS_EUNSUPPORTED: return "unsupported";
+        default: return "unknown error";
+    }
+}
+
+extern "C" const char* ulens_last_cuda_error(ulens_ctx* ctx) { return ctx ? ctx->cuda_err : ""; }
+
+extern "C" int ulens_create(ulens_ctx** out, int cuda_device, const ulens_options* opt)
+{
+    if (!out) return ULENS_EINVAL;
+    *out = nullptr;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || cuda_device < 0 || cuda_device >= ndev) return ULENS_ECUDA;
+    ulens_ctx* ctx = new (std::nothrow) ulens_ctx();
+    if (!ctx) return ULENS_ENOMEM;
+    memset(ctx, 0, sizeof *ctx);
+    ctx->device = cuda_device;
+    ulens_options o; memset(&o, 0, sizeof o);
+    if (opt) o = *opt;
+    if (o.n_limb <= 0) o.n_limb = 512;
+    o.n_limb = (o.n_limb + 31) & ~31;
+    if (o.n_limb > 8192) o.n_limb = 8192;
+    if (o.n_r <= 0) o.n_r = 384;
+    if (o.n_theta <= 0) o.n_theta = 48;
+    if (!(o.rel_tol > 0.0)) o.rel_tol = 1e-4;
+    if (o.chunk_pts <= 0) o.chunk_pts = 65536;
+    if (o.chunk_pts > (1 << 24) / UL_MAXP) o.chunk_pts = (1 << 24) / UL_MAXP;
+    ctx->opt = o;
+    ctx->rp.n_limb = o.n_limb; ctx->rp.n_r = o.n_r; ctx->rp.n_theta = o.n_theta;
+    ctx->rp.max_nr = 8192; ctx->rp.max_nth = 32768; ctx->rp.max_units_pt = 1024;
+    ctx->chunk = o.chunk_pts;
+    ctx->cap_units = (size_t)ctx->chunk * 192;
+    if (ctx->cap_units > 0x7fffff00u) ctx->cap_units = 0x7fffff00u;
+    cudaError_t e = cudaSetDevice(cuda_device);
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->patches, sizeof(Patch) * UL_MAXP * (size_t)ctx->chunk);
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->n_patch, sizeof(int) * (size_t)ctx->chunk);
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->status_ws, sizeof(unsigned) * (size_t)ctx->chunk);
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->unit_desc, sizeof(unsigned) * ctx->cap_units);
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->unit_sum, sizeof(double) * ctx->cap_units);
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->unit_odd, sizeof(double) * ctx->cap_units);
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->cc, sizeof(ChunkCounters));
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->counters, sizeof(DevCounters));
+    if (e == cudaSuccess) e = cudaMemset(ctx->counters, 0, sizeof(DevCounters));
+    if (e != cudaSuccess) { ulens_destroy(ctx); return e == cudaErrorMemoryAllocation ? ULENS_ENOMEM : ULENS_ECUDA; }
+    *out = ctx;
+    return ULENS_OK;
+}
+
+extern "C" void ulens_destroy(ulens_ctx* ctx)
+{
+    if (!ctx) return;
+    cudaSetDevice(ctx->device);
+    cudaDeviceSynchronize();
+    cudaFree(ctx->patches); cudaFree(ctx->n_patch); cudaFree(ctx->status_ws); cudaFree(ctx->unit_desc);
+    cudaFree(ctx->unit_sum); cudaFree(ctx->unit_odd); cudaFree(ctx->cc); cudaFree(ctx->counters);
+    cudaFree(ctx->cfg_dev); cudaFree(ctx->poly_dev); cudaFree(ctx->traj_w); cudaFree(ctx->io_buf);
+    delete ctx;
+}
+
+static int upload_cfgs(ulens_ctx* ctx, int n_cfg, const ulens_lens* lenses, const double* rho, const double* u1,
+                       cudaStream_t st, int* n_lens_out, bool* any_ld)
+{
+    int N = lenses[0].n_lens;
+    if (N < 1 || N > 3) return ULENS_EINVAL;
+    std::vector<PointCfg> cfg(n_cfg);
+    std::vector<LensPoly> poly(n_cfg);
+    *any_ld = false;
+    for (int c = 0; c < n_cfg; ++c) {
+        const ulens_lens& L = lenses[c];
+        if (L.n_lens != N) return ULENS_EUNSUPPORTED;       // one lens multiplicity per call
+        double tot = 0.0;
+        for (int a = 0; a < N; ++a) {
+            if (!isfinite(L.eps[a]) || !(L.eps[a] >= 0.0) || !isfinite(L.ax[a]) || !isfinite(L.ay[a])) return ULENS_EINVAL;
+            tot += L.eps[a];
+        }
+        if (fabs(tot - 1.0) > 1e-9) return ULENS_EINVAL;
+        if (!finite_pos(rho[c]) || !(u1[c] >= 0.0 && u1[c] <= 1.0)) return ULENS_EINVAL;
+        memset(&cfg[c], 0, sizeof(PointCfg));
+        cfg[c].lens.n = N;
+        for (int a = 0; a < N; ++a) { cfg[c].lens.eps[a] = L.eps[a]; cfg[c].lens.ax[a] = L.ax[a]; cfg[c].lens.ay[a] = L.ay[a]; }
+        cfg[c].rho = rho[c]; cfg[c].u1 = u1[c];
+        if (u1[c] > 0.0) *any_ld = true;
+        lens_poly_basis(L.n_lens, L.eps, L.ax, L.ay, &poly[c]);
+    }
+    if ((size_t)n_cfg > ctx->cfg_cap) {
+        cudaFree(ctx->cfg_dev); cudaFree(ctx->poly_dev); ctx->cfg_dev = nullptr; ctx->poly_dev = nullptr; ctx->cfg_cap = 0;
+        size_t cap = (size_t)n_cfg + 64;
+        if (cudaMalloc(&ctx->cfg_dev, sizeof(PointCfg) * cap) != cudaSuccess) return ULENS_ENOMEM;
+        if (cudaMalloc(&ctx->poly_dev, sizeof(LensPoly) * cap) != cudaSuccess) return ULENS_ENOMEM;
+        ctx->cfg_cap = cap;
+    }
+    // pageable source: the runtime stages the bytes before returning, so the vectors may die here
+    CK(cudaMemcpyAsync(ctx->cfg_dev, cfg.data(), sizeof(PointCfg) * n_cfg, cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(ctx->poly_dev, poly.data(), sizeof(LensPoly) * n_cfg, cudaMemcpyHostToDevice, st));
+    CK(cudaStreamSynchronize(st));
+    *n_lens_out = N;
+    return ULENS_OK;
+}
+
+template <int N>
+static int run_chunks(ulens_ctx* ctx, long long n_total, int n_pts, bool ld, const double* w_re, const double* w_im,
+                      double* A_out, double* err_out, unsigned* status_out, cudaStream_t st)
+{
+    constexpr int DEG = N * N + 1;
+    const size_t smem = 4 * sizeof(RegionWork<DEG>);
+    CK(cudaFuncSetAttribute(k_regions<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int sm_count = 148;
+    cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, ctx->device);
+    for (long long base = 0; base < n_total; base += ctx->chunk) {
+        int n = (int)((n_total - base < ctx->chunk) ? (n_total - base) : ctx->chunk);
+        CK(cudaMemsetAsync(ctx->cc, 0, sizeof(ChunkCounters), st));
+        k_roots<N><<<(n + 127) / 128, 128, 0, st>>>(n, (int)base, n_pts, ctx->cfg_dev, ctx->poly_dev, w_re, w_im,
+                                                    nullptr, nullptr, nullptr, ctx->status_ws);
+        k_regions<N><<<(n + 3) / 4, 128, smem, st>>>(n, (int)base, n_pts, ctx->cfg_dev, ctx->poly_dev, w_re, w_im, ctx->rp,
+                                                     ctx->patches, ctx->n_patch, ctx->status_ws, ctx->unit_desc,
+                                                     (unsigned)ctx->cap_units, ctx->cc, ctx->counters);
+        int grid = sm_count * 4;
+        if (ld)
+            k_shoot<N, true><<<grid, 128, 0, st>>>((int)base, n_pts, ctx->cfg_dev, w_re, w_im, ctx->patches, ctx->unit_desc,
+                                                   ctx->unit_sum, ctx->unit_odd, ctx->status_ws, ctx->cc, ctx->counters);
+        else
+            k_shoot<N, false><<<grid, 128, 0, st>>>((int)base, n_pts, ctx->cfg_dev, w_re, w_im, ctx->patches, ctx->unit_desc,
+                                                    ctx->unit_sum, ctx->unit_odd, ctx->status_ws, ctx->cc, ctx->counters);
+        k_finalize<<<(n + 127) / 128, 128, 0, st>>>(n, (int)base, n_pts, ctx->cfg_dev, ctx->patches, ctx->n_patch,
+                                                    ctx->unit_sum, ctx->unit_odd, ctx->status_ws, ctx->opt.rel_tol,
+                                                    A_out, err_out, status_out, ctx->counters);
+        ctx->last_launches += 4;
+        CK(cudaGetLastError());
+    }
+    return ULENS_OK;
+}
+
+static int mag_device(ulens_ctx* ctx, int n_cfg, int n_pts, const ulens_lens* lenses, const double* rho, const double* u1,
+                      const double* w_re, const double* w_im, double* A_out, double* err_out, unsigned* status_out,
+                      cudaStream_t st)
+{
+    int N = 0; bool ld = false;
+    int rc = upload_cfgs(ctx, n_cfg, lenses, rho, u1, st, &N, &ld);
+    if (rc != ULENS_OK) return rc;
+    long long n_total = (long long)n_cfg * n_pts;
+    if (n_total > 0x7fffffffLL) return ULENS_EUNSUPPORTED;
+    ctx->last_launches = 0;
+    switch (N) {
+        case 1: rc = run_chunks<1>(ctx, n_total, n_pts, ld, w_re, w_im, A_out, err_out, status_out, st); break;
+        case 2: rc = run_chunks<2>(ctx, n_total, n_pts, ld, w_re, w_im, A_out, err_out, status_out, st); break;
+        default: rc = run_chunks<3>(ctx, n_total, n_pts, ld, w_re, w_im, A_out, err_out, status_out, st); break;
+    }
+    return rc;
+}
+
+extern "C" int ulens_mag(ulens_ctx* ctx, int n_cfg, int n_pts, const ulens_lens* lenses_host, const double* rho_host,
+                         const double* u1_host, const double* w_re, const double* w_im, double* A_out, double* err_out,
+                         uint32_t* status_out, void* stream)
+{
+    if (!ctx || n_cfg < 0 || n_pts < 0) return ULENS_EINVAL;
+    if (n_cfg == 0 || n_pts == 0) return ULENS_OK;
+    if (!lenses_host || !rho_host || !u1_host || !w_re || !w_im || !A_out) return ULENS_EINVAL;
+    CK(cudaSetDevice(ctx->device));
+    return mag_device(ctx, n_cfg, n_pts, lenses_host, rho_host, u1_host, w_re, w_im, A_out, err_out, status_out,
+                      (cudaStream_t)stream);
+}
+
+extern "C" int ulens_mag_host(ulens_ctx* ctx, int n_cfg, int n_pts, const ulens_lens* lenses_host, const double* rho_host,
+                              const double* u1_host, const double* w_re_host, const double* w_im_host, double* A_out_host,
+                              double* err_out_host, uint32_t* status_out_host, void* stream)
+{
+    if (!ctx || n_cfg < 0 || n_pts < 0) return ULENS_EINVAL;
+    if (n_cfg == 0 || n_pts == 0) return ULENS_OK;
+    if (!lenses_host || !rho_host || !u1_host || !w_re_host || !w_im_host || !A_out_host) return ULENS_EINVAL;
+    CK(cudaSetDevice(ctx->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    size_t n = (size_t)n_cfg * n_pts;
+    size_t need = n * 5;                                 // w_re, w_im, A, err, status (as 8-byte slots)
+    if (need > ctx->io_cap) {
+        cudaFree(ctx->io_buf); ctx->io_buf = nullptr; ctx->io_cap = 0;
+        if (cudaMalloc(&ctx->io_buf, sizeof(double) * need) != cudaSuccess) return ULENS_ENOMEM;
+        ctx->io_cap = need;
+    }
+    double* d_wre = ctx->io_buf; double* d_wim = d_wre + n; double* d_A = d_wim + n; double* d_err = d_A + n;
+    unsigned* d_st = reinterpret_cast<unsigned*>(d_err + n);
+    CK(cudaMemcpyAsync(d_wre, w_re_host, sizeof(double) * n, cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(d_wim, w_im_host, sizeof(double) * n, cudaMemcpyHostToDevice, st));
+    int rc = mag_device(ctx, n_cfg, n_pts, lenses_host, rho_host, u1_host, d_wre, d_wim, d_A, d_err, d_st, st);
+    if (rc != ULENS_OK) return rc;
+    CK(cudaMemcpyAsync(A_out_host, d_A, sizeof(double) * n, cudaMemcpyDeviceToHost, st));
+    if (err_out_host) CK(cudaMemcpyAsync(err_out_host, d_err, sizeof(double) * n, cudaMemcpyDeviceToHost, st));
+    if (status_out_host) CK(cudaMemcpyAsync(status_out_host, d_st, sizeof(unsigned) * n, cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    return ULENS_OK;
+}
+
+extern "C" int ulens_lightcurve_binary(ulens_ctx* ctx, int n_cfg, int n_epochs, const double* theta_host, double u1,
+                                       const double* t, double* A_out, double* dA_out, double* err_out,
+                                       uint32_t* status_out, void* stream)
+{
+    if (!ctx || n_cfg < 0 || n_epochs < 0) return ULENS_EINVAL;
+    if (n_cfg == 0 || n_epochs == 0) return ULENS_OK;
+    if (!theta_host || !t || !A_out || !(u1 >= 0.0 && u1 <= 1.0)) return ULENS_EINVAL;
+    if (dA_out) return ULENS_EUNSUPPORTED;               // forward-mode variant: not in this build yet
+    CK(cudaSetDevice(ctx->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    std::vector<ulens_lens> lenses(n_cfg);
+    std::vector<double> rho(n_cfg), u1v(n_cfg, u1);
+    for (int c = 0; c < n_cfg; ++c) {
+        const double* th = theta_host + 7 * c;
+        for (int k = 0; k < 7; ++k) if (!isfinite(th[k])) return ULENS_EINVAL;
+        if (!(th[2] > 0.0)) return ULENS_EINVAL;
+        int rc = ulens_lens_binary(&lenses[c], th[3], th[4]);
+        if (rc != ULENS_OK) return rc;
+        rho[c] = th[5];
+    }
+    size_t n = (size_t)n_cfg * n_epochs;
+    size_t need = 2 * n + 7 * (size_t)n_cfg;
+    if (need > ctx->traj_cap) {
+        cudaFree(ctx->traj_w); ctx->traj_w = nullptr; ctx->traj_cap = 0;
+        if (cudaMalloc(&ctx->traj_w, sizeof(double) * need) != cudaSuccess) return ULENS_ENOMEM;
+        ctx->traj_cap = need;
+    }
+    double* w_re = ctx->traj_w; double* w_im = w_re + n; double* th_dev = w_im + n;
+    CK(cudaMemcpyAsync(th_dev, theta_host, sizeof(double) * 7 * n_cfg, cudaMemcpyHostToDevice, st));
+    k_traj<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(n_cfg, n_epochs, th_dev, t, w_re, w_im);
+    CK(cudaGetLastError());
+    int rc = mag_device(ctx, n_cfg, n_epochs, lenses.data(), rho.data(), u1v.data(), w_re, w_im, A_out, err_out, status_out, st);
+    ctx->last_launches += 1;
+    return rc;
+}
+
+extern "C" int ulens_roots(ulens_ctx* ctx, const ulens_lens* lens_host, int n_pts, const double* w_re, const double* w_im,
+                           double* roots_re, double* roots_im, uint8_t* is_image, void* stream)
+{
+    if (!ctx || n_pts < 0) return ULENS_EINVAL;
+    if (n_pts == 0) return ULENS_OK;
+    if (!lens_host || !w_re || !w_im || !roots_re || !roots_im || !is_image) return ULENS_EINVAL;
+    CK(cudaSetDevice(ctx->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    int N = 0; bool ld = false;
+    double rho = 1.0, u1 = 0.0;
+    int rc = upload_cfgs(ctx, 1, lens_host, &rho, &u1, st, &N, &ld);
+    if (rc != ULENS_OK) return rc;
+    int grid = (n_pts + 127) / 128;
+    switch (N) {
+        case 1: k_roots<1><<<grid, 128, 0, st>>>(n_pts, 0, n_pts, ctx->cfg_dev, ctx->poly_dev, w_re, w_im, roots_re, roots_im, is_image, nullptr); break;
+        case 2: k_roots<2><<<grid, 128, 0, st>>>(n_pts, 0, n_pts, ctx->cfg_dev, ctx->poly_dev, w_re, w_im, roots_re, roots_im, is_image, nullptr); break;
+        default: k_roots<3><<<grid, 128, 0, st>>>(n_pts, 0, n_pts, ctx->cfg_dev, ctx->poly_dev, w_re, w_im, roots_re, roots_im, is_image, nullptr); break;
+    }
+    ctx->last_launches = 1;
+    CK(cudaGetLastError());
+    return ULENS_OK;
+}
+
+extern "C" int ulens_get_stats(ulens_ctx* ctx, ulens_stats* out)
+{
+    if (!ctx || !out) return ULENS_EINVAL;
+    CK(cudaSetDevice(ctx->device));
+    CK(cudaDeviceSynchronize());
+    DevCounters h;
+    CK(cudaMemcpy(&h, ctx->counters, sizeof h, cudaMemcpyDeviceToHost));
+    out->n_points = h.n_points; out->n_rays = h.n_rays; out->n_patches = h.n_patches; out->n_units = h.n_units;
+    out->n_limb_solves = h.n_limb_solves; out->n_flagged = h.n_flagged;
+    return ULENS_OK;
+}
+
+extern "C" int ulens_reset_stats(ulens_ctx* ctx)
+{
+    if (!ctx) return ULENS_EINVAL;
+    CK(cudaSetDevice(ctx->device));
+    CK(cudaDeviceSynchronize());
+    CK(cudaMemset(ctx->counters, 0, sizeof(DevCounters)));
+    return ULENS_OK;
+}
+
+extern "C" int ulens_last_launch_count(ulens_ctx* ctx) { return ctx ? ctx->last_launches : ULENS_EINVAL; }
+
+extern "C" int ulens_fp64_peak(ulens_ctx* ctx, double ms, double* dfma_per_s)
+{
+    if (!ctx || !dfma_per_s || !(ms > 0.0)) return ULENS_EINVAL;
+    CK(cudaSetDevice(ctx->device));
+    int sm_count = 148;
+    cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, ctx->device);
+    double* d = nullptr;
+    CK(cudaMalloc(&d, sizeof(double)));
+    cudaEvent_t e0, e1;
+    CK(cudaEventCreate(&e0)); CK(cudaEventCreate(&e1));
+    const int blocks = sm_count * 8, threads = 256;
+    int iters = 2000;
+    double best = 0.0;
+    float el = 0.f;
+    // calibrate then run ~ms
+    for (int pass = 0; pass < 3; ++pass) {
+        CK(cudaEventRecord(e0));
+        k_dfma_peak<<<blocks, threads>>>(iters, d);
+        CK(cudaEventRecord(e1));
+        CK(cudaEventSynchronize(e1));
+        CK(cudaEventElapsedTime(&el, e0, e1));
+        double rate = (double)blocks * threads * 64.0 * iters / (el * 1e-3);
+        if (pass > 0 && rate > best) best = rate;
+        if (pass == 0) { double scale = ms / (el > 1e-3 ? el : 1e-3); iters = (int)(iters * scale); if (iters < 100) iters = 100; if (iters > 50000000) iters = 50000000; }
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d);
+    *dfma_per_s = best;
+    return ULENS_OK;
+}

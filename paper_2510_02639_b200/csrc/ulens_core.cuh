@@ -1,0 +1,499 @@
+// ulens_core.cuh -- per-thread arithmetic of the ICRS hot path (device code; also compiles as plain
+// C++ so that host logic tests can include it -- the product has no CPU path, see ulens_api.cu).
+//
+// Citations "P:<line>" are to /root/reference/PAPER.md. Readings "G<n>" are listed in DESIGN.md.
+//
+//   lens map, Jacobian                      Eq. 1-3
+//   lens polynomial (own derivation, G1)    Eq. 4
+//   Ehrlich-Aberth iteration (G6)           Eq. 7
+//   root validation + polish on Eq. 1 (G7)
+//   ring quadrature along theta (G9-G13)    App. A
+//
+// This file shares nothing with oracle/ (different polynomial construction, different integration
+// rule, different code).
+#pragma once
+#include <math.h>
+#include <stdint.h>
+
+#if defined(__CUDACC__)
+#define UL_HD __host__ __device__ __forceinline__
+#define UL_HDN __host__ __device__
+#else
+#define UL_HD inline
+#define UL_HDN inline
+#endif
+
+namespace ulens {
+
+// ------------------------------------------------------------------------------------------------
+// data shared by the kernels
+// ------------------------------------------------------------------------------------------------
+
+struct Lens {            // same layout as ulens_lens (include/ulens.h)
+    int n;
+    double eps[3], ax[3], ay[3];
+};
+
+// Polynomial basis of one lens: T_k(z) = Q(z)^k G(z)^(N-k), k = 0..N, where
+//   Q(z) = prod_i (z - a_i),  G(z) = sum_i eps_i prod_{m != i} (z - a_m)      (conj of Eq. 1: conj z = conj w + G/Q).
+// With c_i = conj(w) - conj(a_i):  conj(z) - conj(a_i) = (c_i Q + G)/Q, so Eq. 1 times prod_i (c_i Q + G) is
+//   P(z) = (z - w) sum_{k=0..N} e_k(c) T_k(z)  -  sum_{k=0..N-1} f_k(c) T_{k+1}(z),      degree N^2 + 1,
+// e_k = k-th elementary symmetric polynomial of c_1..c_N, f_k = sum_i eps_i e_k(c without c_i).
+// T_k has degree N(N-1) + k <= N^2 (<= 9): 10 coefficients each, filled on the host once per lens.
+struct LensPoly {
+    double tr[4][10], ti[4][10];
+};
+
+struct PointCfg {        // per (lens, source) configuration
+    Lens lens;
+    double rho, u1;
+};
+
+// sector ("patch") descriptor, written by k_regions and read by k_shoot
+struct Patch {
+    double r0, dr;       // ring i at r0 + (i + 1/2) dr, i = 0..n_r-1   (G11: midpoint nodes, empty end rings)
+    double th0, dth;     // ray j at th0 + (j + 1/2) dth, j = 0..n_th-1
+    int n_r, n_th;
+    int point;           // global point index
+    int unit0;           // first 32-ring work unit of this patch in the unit arrays
+    int flags;           // bit 0: periodic in theta (full ring); bit 1: scan lines are radial (lanes = theta)
+    int n_units;         // 32-line work units
+};
+
+#define UL_PATCH_PERIODIC 1
+#define UL_PATCH_SCAN_R 2
+
+// status bits (mirror include/ulens.h)
+#define UL_ST_EA_NOCONV  0x0001u
+#define UL_ST_IMG_PARITY 0x0002u
+#define UL_ST_PATCH_CAP  0x0004u
+#define UL_ST_RES_CAP    0x0008u
+#define UL_ST_CLIPPED    0x0010u
+#define UL_ST_UNIT_OVF   0x0020u
+#define UL_ST_ERR_HIGH   0x0040u
+#define UL_ST_NO_IMAGE   0x0080u
+
+#define UL_PI 3.14159265358979323846
+#define UL_BIG 1e100
+
+UL_HD double ul_min(double a, double b) { return a < b ? a : b; }
+UL_HD double ul_max(double a, double b) { return a > b ? a : b; }
+
+// ------------------------------------------------------------------------------------------------
+// Eq. 1-3: lens map residual and its conj-derivative g = sum eps_i / conj(z - a_i)^2
+// ------------------------------------------------------------------------------------------------
+
+// f = z - sum eps_i/conj(z - a_i) - w ;  g = d w / d conj(z) = sum eps_i / conj(z - a_i)^2 ;  dmin2 = min |z - a_i|^2
+template <int N>
+UL_HD void lens_resid(const Lens& L, double zx, double zy, double wx, double wy,
+                      double& fx, double& fy, double& gx, double& gy, double& dmin2)
+{
+    double sx = 0.0, sy = 0.0;
+    gx = 0.0; gy = 0.0; dmin2 = 1e300;
+#pragma unroll
+    for (int i = 0; i < N; ++i) {
+        double dx = zx - L.ax[i], dy = zy - L.ay[i];
+        double r2 = dx * dx + dy * dy;
+        double inv = 1.0 / r2;
+        dmin2 = ul_min(dmin2, r2);
+        // eps/conj(d) = eps d/|d|^2
+        sx += L.eps[i] * dx * inv;
+        sy += L.eps[i] * dy * inv;
+        // eps/conj(d)^2 = eps d^2/|d|^4
+        double inv2 = inv * inv;
+        gx += L.eps[i] * (dx * dx - dy * dy) * inv2;
+        gy += L.eps[i] * (2.0 * dx * dy) * inv2;
+    }
+    fx = zx - sx - wx;
+    fy = zy - sy - wy;
+}
+
+// Damped Newton on Eq. 1 itself (G7 "polish"): delta w = dz + g conj(dz)  =>  dz = (b - g conj(b))/(1 - |g|^2), b = -f.
+// The step is limited to half the distance to the nearest lens. Returns true when the final residual
+// is below tol * max(1, |z|); z is updated in place; detJ = 1 - |g|^2 (Eq. 3).
+template <int N>
+UL_HD bool polish_image(const Lens& L, double wx, double wy, double& zx, double& zy, int max_it,
+                        double tol, double& detJ, double& resid, double& gx, double& gy)
+{
+    double fx, fy, dmin2;
+    bool ok = false;
+    resid = 1e300; detJ = 0.0;
+    for (int it = 0; it <= max_it; ++it) {
+        lens_resid<N>(L, zx, zy, wx, wy, fx, fy, gx, gy, dmin2);
+        detJ = 1.0 - (gx * gx + gy * gy);
+        resid = sqrt(fx * fx + fy * fy);
+        double scale = ul_max(1.0, sqrt(zx * zx + zy * zy));
+        if (!(resid == resid)) return false;
+        if (resid <= tol * scale) { ok = true; if (resid <= 4e-16 * scale) break; }
+        if (it == max_it) break;
+        if (fabs(detJ) < 1e-14) break;
+        double bx = -fx, by = -fy;
+        // g conj(b)
+        double qx = gx * bx + gy * by, qy = gy * bx - gx * by;
+        double sx = (bx - qx) / detJ, sy = (by - qy) / detJ;
+        double s2 = sx * sx + sy * sy;
+        double lim2 = 0.25 * dmin2;
+        if (s2 > lim2) { double k = sqrt(lim2 / s2); sx *= k; sy *= k; }
+        zx += sx; zy += sy;
+    }
+    return ok;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Eq. 4: coefficients b_0..b_DEG of the lens polynomial for source position w
+// ------------------------------------------------------------------------------------------------
+
+template <int N>
+UL_HD void poly_coeffs(const Lens& L, const LensPoly& T, double wx, double wy, double* br, double* bi)
+{
+    constexpr int DEG = N * N + 1;
+    // c_i = conj(w) - conj(a_i)
+    double cx[N], cy[N];
+#pragma unroll
+    for (int i = 0; i < N; ++i) { cx[i] = wx - L.ax[i]; cy[i] = -(wy - L.ay[i]); }
+    // a source centre exactly on a projected lens position makes the leading coefficient vanish
+    // (prod c_i): nudge that c_i (images move by ~1e-13, far below every tolerance here)
+#pragma unroll
+    for (int i = 0; i < N; ++i)
+        if (cx[i] * cx[i] + cy[i] * cy[i] < 1e-26) cx[i] += 1e-13;
+    // elementary symmetric polynomials e_0..e_N of c, and f_k = sum_i eps_i e_k(c \ c_i)
+    double ex[N + 1], ey[N + 1], fx[N], fy[N];
+    ex[0] = 1.0; ey[0] = 0.0;
+#pragma unroll
+    for (int k = 1; k <= N; ++k) { ex[k] = 0.0; ey[k] = 0.0; }
+#pragma unroll
+    for (int i = 0; i < N; ++i) {
+#pragma unroll
+        for (int k = N; k >= 1; --k) {
+            if (k <= i + 1) {
+                ex[k] += ex[k - 1] * cx[i] - ey[k - 1] * cy[i];
+                ey[k] += ex[k - 1] * cy[i] + ey[k - 1] * cx[i];
+            }
+        }
+    }
+    if constexpr (N == 1) {
+        fx[0] = L.eps[0]; fy[0] = 0.0;
+    } else if constexpr (N == 2) {
+        fx[0] = L.eps[0] + L.eps[1]; fy[0] = 0.0;
+        fx[1] = L.eps[0] * cx[1] + L.eps[1] * cx[0];
+        fy[1] = L.eps[0] * cy[1] + L.eps[1] * cy[0];
+    } else {
+        fx[0] = L.eps[0] + L.eps[1] + L.eps[2]; fy[0] = 0.0;
+        fx[1] = L.eps[0] * (cx[1] + cx[2]) + L.eps[1] * (cx[0] + cx[2]) + L.eps[2] * (cx[0] + cx[1]);
+        fy[1] = L.eps[0] * (cy[1] + cy[2]) + L.eps[1] * (cy[0] + cy[2]) + L.eps[2] * (cy[0] + cy[1]);
+        double p12x = cx[1] * cx[2] - cy[1] * cy[2], p12y = cx[1] * cy[2] + cy[1] * cx[2];
+        double p02x = cx[0] * cx[2] - cy[0] * cy[2], p02y = cx[0] * cy[2] + cy[0] * cx[2];
+        double p01x = cx[0] * cx[1] - cy[0] * cy[1], p01y = cx[0] * cy[1] + cy[0] * cx[1];
+        fx[2] = L.eps[0] * p12x + L.eps[1] * p02x + L.eps[2] * p01x;
+        fy[2] = L.eps[0] * p12y + L.eps[1] * p02y + L.eps[2] * p01y;
+    }
+    // S(z) = sum_k e_k T_k(z)   (degree N^2),  R(z) = sum_k f_k T_{k+1}(z)   (degree N^2)
+    // P = (z - w) S - R :  b_l = S_{l-1} - w S_l - R_l
+    double sr[DEG], si[DEG];          // S_0..S_{N^2}  (DEG = N^2+1 entries)
+#pragma unroll
+    for (int l = 0; l < DEG; ++l) {
+        double ar = 0.0, ai = 0.0, rr = 0.0, ri = 0.0;
+#pragma unroll
+        for (int k = 0; k <= N; ++k) {
+            double tr = T.tr[k][l], ti = T.ti[k][l];
+            ar += ex[k] * tr - ey[k] * ti;
+            ai += ex[k] * ti + ey[k] * tr;
+            if (k >= 1) {
+                rr += fx[k - 1] * tr - fy[k - 1] * ti;
+                ri += fx[k - 1] * ti + fy[k - 1] * tr;
+            }
+        }
+        sr[l] = ar; si[l] = ai;
+        br[l] = -(wx * ar - wy * ai) - rr;
+        bi[l] = -(wx * ai + wy * ar) - ri;
+    }
+    br[DEG] = 0.0; bi[DEG] = 0.0;
+#pragma unroll
+    for (int l = 1; l <= DEG; ++l) { br[l] += sr[l - 1]; bi[l] += si[l - 1]; }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Eq. 7: Ehrlich-Aberth simultaneous iteration (Newton form, G6), Gauss-Seidel order
+// ------------------------------------------------------------------------------------------------
+
+template <int DEG>
+UL_HD void horner2(const double* br, const double* bi, double x, double y,
+                   double& pr, double& pi, double& dr, double& di)
+{
+    pr = br[DEG]; pi = bi[DEG]; dr = 0.0; di = 0.0;
+#pragma unroll
+    for (int l = DEG - 1; l >= 0; --l) {
+        double t = dr * x - di * y + pr;
+        di = dr * y + di * x + pi;
+        dr = t;
+        t = pr * x - pi * y + br[l];
+        pi = pr * y + pi * x + bi[l];
+        pr = t;
+    }
+}
+
+// Initial guesses on the Cauchy-bound circle (G6: radius 1 + max_{l<n} |b_l/b_n|, phase offset 0.4 rad).
+template <int DEG>
+UL_HD void ea_init(const double* br, const double* bi, double* zr, double* zi)
+{
+    double ln2 = br[DEG] * br[DEG] + bi[DEG] * bi[DEG];
+    double m2 = 0.0;
+#pragma unroll
+    for (int l = 0; l < DEG; ++l) m2 = ul_max(m2, br[l] * br[l] + bi[l] * bi[l]);
+    double R = 1.0 + sqrt(m2 / ln2);
+    // the lens-polynomial roots all lie within a few Einstein radii; a huge Cauchy bound (tiny leading
+    // coefficient) only slows the first iterations down, so start no further out than 8
+    R = ul_min(R, 8.0);
+    // centroid of the roots = -b_{n-1}/(n b_n)
+    double qx = (br[DEG - 1] * br[DEG] + bi[DEG - 1] * bi[DEG]) / ln2;
+    double qy = (bi[DEG - 1] * br[DEG] - br[DEG - 1] * bi[DEG]) / ln2;
+    double cx = -qx / DEG, cy = -qy / DEG;
+    if (!(cx * cx + cy * cy < 16.0)) { cx = 0.0; cy = 0.0; }
+#pragma unroll
+    for (int k = 0; k < DEG; ++k) {
+        double ph = 0.4 + 2.0 * UL_PI * k / DEG;
+        zr[k] = cx + R * cos(ph);
+        zi[k] = cy + R * sin(ph);
+    }
+}
+
+// Iterate until every relative step is < 1e-14, or the steps stagnate at the evaluation-noise floor
+// (largest step < 1e-8 and no longer halving), or max_it. Returns the iterations used (max_it+1 if
+// the cap was hit without meeting either criterion).
+template <int DEG>
+UL_HD int ea_iterate(const double* br, const double* bi, double* zr, double* zi, int max_it)
+{
+    double e_prev = 1e300;
+    for (int it = 1; it <= max_it; ++it) {
+        double e = 0.0;
+#pragma unroll
+        for (int k = 0; k < DEG; ++k) {
+            double pr, pi, dr, di;
+            horner2<DEG>(br, bi, zr[k], zi[k], pr, pi, dr, di);
+            double p2 = pr * pr + pi * pi;
+            if (p2 == 0.0) continue;
+            // Newton ratio n = P/P'
+            double d2 = dr * dr + di * di;
+            double nx, ny;
+            if (d2 > 0.0) { nx = (pr * dr + pi * di) / d2; ny = (pi * dr - pr * di) / d2; }
+            else { nx = 1e-3; ny = 1e-3; }
+            // repulsion S = sum_{j != k} 1/(z_k - z_j)
+            double sx = 0.0, sy = 0.0;
+#pragma unroll
+            for (int j = 0; j < DEG; ++j) {
+                if (j == k) continue;
+                double ux = zr[k] - zr[j], uy = zi[k] - zi[j];
+                double u2 = ux * ux + uy * uy;
+                if (u2 > 0.0) { double iu = 1.0 / u2; sx += ux * iu; sy -= uy * iu; }
+            }
+            // step = n / (1 - n S)
+            double ax = 1.0 - (nx * sx - ny * sy), ay = -(nx * sy + ny * sx);
+            double a2 = ax * ax + ay * ay;
+            double stx, sty;
+            if (a2 > 1e-300) { stx = (nx * ax + ny * ay) / a2; sty = (ny * ax - nx * ay) / a2; }
+            else { stx = nx; sty = ny; }
+            zr[k] -= stx; zi[k] -= sty;
+            double z2 = zr[k] * zr[k] + zi[k] * zi[k];
+            double rel = (stx * stx + sty * sty) / (z2 + 1e-12);
+            e = ul_max(e, rel);
+        }
+        if (!(e == e)) return max_it + 1;
+        if (e < 1e-28) return it;                            // (1e-14)^2
+        if (e < 1e-16 && e > 0.25 * e_prev) return it;       // stagnation at the noise floor (1e-8 ^2, halving ^2)
+        e_prev = e;
+    }
+    return max_it + 1;
+}
+
+// ------------------------------------------------------------------------------------------------
+// App. A: ring quadrature along theta
+// ------------------------------------------------------------------------------------------------
+
+// zeta(-1/2, u) and zeta(-3/2, u) for u in (0, 1]: Hurwitz zeta = u^(-s) + zeta(s, 1+u); the smooth
+// part is a degree-9 Chebyshev fit on [0,1] (max error 7e-10 / 2e-10).
+UL_HD double zeta_m12(double u)
+{
+    const double c[10] = {-0.207886224314425946, -0.730177387536053191, -0.326542433690562406,
+                          0.0837832566266219698, -0.0435998186937335486, 0.0271396135617846347,
+                          -0.0165300041688832568, 0.00823252937110980637, -0.00274063185833692022,
+                          0.000434876090612478912};
+    double p = c[9];
+#pragma unroll
+    for (int i = 8; i >= 0; --i) p = p * u + c[i];
+    return sqrt(u) + p;
+}
+UL_HD double zeta_m32(double u)
+{
+    const double c[10] = {-0.0254852020522020475, -0.311829304876540199, -0.547634035662697937,
+                          -0.163258961591498412, 0.0313415948971861593, -0.0127998326381573904,
+                          0.00616325441161647825, -0.00268571587959467142, 0.000828839924548779593,
+                          -0.0001258385180165005};
+    double p = c[9];
+#pragma unroll
+    for (int i = 8; i >= 0; --i) p = p * u + c[i];
+    return u * sqrt(u) + p;
+}
+
+// F(z) = |w(z) - w_c|^2 - rho^2  (inside the source image <=> F < 0), one reciprocal per ray.
+// A ray on a lens gives inf/NaN -> clamped to +UL_BIG (outside), never NaN.
+template <int N>
+UL_HD double ray_F(const Lens& L, double x, double y, double wcx, double wcy, double rho2)
+{
+    double ux = x - wcx, uy = y - wcy;
+    double F;
+    if constexpr (N == 1) {
+        double dx = x - L.ax[0], dy = y - L.ay[0];
+        double inv = L.eps[0] / (dx * dx + dy * dy);
+        double ex = ux - dx * inv, ey = uy - dy * inv;
+        F = ex * ex + ey * ey - rho2;
+    } else if constexpr (N == 2) {
+        double d1x = x - L.ax[0], d1y = y - L.ay[0];
+        double d2x = x - L.ax[1], d2y = y - L.ay[1];
+        double D1 = d1x * d1x + d1y * d1y, D2 = d2x * d2x + d2y * d2y;
+        double inv = 1.0 / (D1 * D2);
+        double e1 = L.eps[0] * D2 * inv, e2 = L.eps[1] * D1 * inv;
+        double ex = ux - e1 * d1x - e2 * d2x, ey = uy - e1 * d1y - e2 * d2y;
+        F = ex * ex + ey * ey - rho2;
+    } else {
+        double d1x = x - L.ax[0], d1y = y - L.ay[0];
+        double d2x = x - L.ax[1], d2y = y - L.ay[1];
+        double d3x = x - L.ax[2], d3y = y - L.ay[2];
+        double D1 = d1x * d1x + d1y * d1y, D2 = d2x * d2x + d2y * d2y, D3 = d3x * d3x + d3y * d3y;
+        double D12 = D1 * D2;
+        double inv = 1.0 / (D12 * D3);
+        double e1 = L.eps[0] * D2 * D3 * inv, e2 = L.eps[1] * D1 * D3 * inv, e3 = L.eps[2] * D12 * inv;
+        double ex = ux - e1 * d1x - e2 * d2x - e3 * d3x, ey = uy - e1 * d1y - e2 * d2y - e3 * d3y;
+        F = ex * ex + ey * ey - rho2;
+    }
+    return fmin(F, UL_BIG);    // fmin returns the non-NaN operand
+}
+
+// One boundary crossing between nodes 1 and 2 of the window (f0, f1, f2, f3) at x = -1, 0, 1, 2
+// (cubic Lagrange interpolant, App. A.1, G13; linear fallback if the cubic has no root in the cell).
+// Returns u = distance (in cells) from the crossing to the first inside node, entering = node 1 outside,
+// and dS = the end correction of the midpoint sum of sqrt(-F) over the inside run (in cells):
+//   sum - integral = sqrt(sigma) [ zeta(-1/2,u) + t2 zeta(-3/2,u) ],   -F ~ sigma xi (1 + 2 t2 xi) from the edge
+// (Navot's correction for an x^(1/2) end singularity; its first cell is the paper's f(delta) b(delta),
+// Eqs. A7-A8, G12). The uniform part follows from u: zeta(0,u) = 1/2 - u (== Eq. A3 point-centred, G9/G10).
+// t2_extra adds the logarithmic slope of a smooth weight (the r of r dr on radial scan lines).
+UL_HD void edge_event(double f0, double f1, double f2, double f3, bool want_S, double t2_extra,
+                      double& u, bool& entering, double& dS)
+{
+    double c0 = f1;
+    double c1 = (-2.0 * f0 - 3.0 * f1 + 6.0 * f2 - f3) * (1.0 / 6.0);
+    double c2 = (f0 - 2.0 * f1 + f2) * 0.5;
+    double c3 = (-f0 + 3.0 * f1 - 3.0 * f2 + f3) * (1.0 / 6.0);
+    double x = f1 / (f1 - f2);                       // linear guess, in (0,1) because the signs differ
+    bool cubic_ok = true;
+#pragma unroll 1
+    for (int it = 0; it < 4; ++it) {
+        double p = c0 + x * (c1 + x * (c2 + x * c3));
+        double dp = c1 + x * (2.0 * c2 + 3.0 * x * c3);
+        double xn = x - p / dp;
+        if (!(xn >= 0.0 && xn <= 1.0)) { cubic_ok = false; break; }
+        x = xn;
+    }
+    double dp, d2p;
+    if (cubic_ok) {
+        dp = c1 + x * (2.0 * c2 + 3.0 * x * c3);
+        d2p = 2.0 * c2 + 6.0 * x * c3;
+    } else {                                        // G13 fallback: linear interpolation
+        x = f1 / (f1 - f2);
+        dp = f2 - f1; d2p = 0.0;
+    }
+    entering = !(f1 < 0.0);                         // node 1 outside, node 2 inside
+    u = entering ? 1.0 - x : x;
+    dS = 0.0;
+    if (want_S) {
+        double sigma = entering ? -dp : dp;         // slope of -F away from the edge, per cell
+        double tau = -0.5 * d2p;
+        if (sigma > 0.0) {
+            double ss = sqrt(sigma);
+            double corr = ss * zeta_m12(u);
+            double t2 = tau / (2.0 * sigma) + (entering ? t2_extra : -t2_extra);
+            if (fabs(t2) < 0.5) corr += ss * t2 * zeta_m32(u);
+            dS = -corr;
+        }
+    }
+}
+
+// Integrate one ring r over theta:  U = Int chi dtheta / dth,  S = Int chi sqrt(-F) dtheta / dth  (both in cells).
+// Rays at th0 + (j + 1/2) dth, j = -2 .. n_th+1 (two halo rays per side feed the cubic stencil; for a
+// periodic sector they are the wrapped rays). edge = true if one of the first / last two rays of a
+// bounded sector is inside (the margin was too small).
+template <int N, bool LD>
+UL_HD void shoot_ring(const Lens& L, double wcx, double wcy, double rho2, double r, double th0, double dth,
+                      int n_th, bool periodic, double& U_out, double& S_out, bool& edge)
+{
+    double cd = cos(dth), sd = sin(dth);
+    double t = th0 - 1.5 * dth;
+    double c = cos(t), s = sin(t);
+    double f0 = UL_BIG, f1 = UL_BIG, f2 = UL_BIG, f3;
+    double U = 0.0, S = 0.0;
+    edge = false;
+    const int j_first = periodic ? 2 : 1;
+    for (int j = -2; j <= n_th + 1; ++j) {
+        f3 = ray_F<N>(L, r * c, r * s, wcx, wcy, rho2);
+        if (j >= 0 && j < n_th && f3 < 0.0) {
+            U += 1.0;
+            if (LD) S += sqrt(-f3);
+            if (!periodic && (j < 2 || j >= n_th - 2)) edge = true;
+        }
+        // pair (j-2, j-1) = (f1, f2), stencil complete once f0 = F_{j-3} exists (j >= 1). In a periodic
+        // sector pair (-1, 0) is pair (n_th-1, n_th) again: take it once.
+        if (j >= j_first && ((f1 < 0.0) != (f2 < 0.0))) {
+            double u, dS; bool en;
+            edge_event(f0, f1, f2, f3, LD, 0.0, u, en, dS);
+            U += u - 0.5; S += dS;
+        }
+        f0 = f1; f1 = f2; f2 = f3;
+        double cn = c * cd - s * sd;
+        s = s * cd + c * sd;
+        c = cn;
+    }
+    U_out = U; S_out = S;
+}
+
+UL_HD bool en_dummy(double f1) { return !(f1 < 0.0); }
+
+// Integrate one radial line theta over r (filled ring / disk sectors):
+//   U = Int chi r dr,  S = Int chi sqrt(-F) r dr   (length^2 units). Nodes at r0 + (i + 1/2) dr, i = -2 .. n_r+1.
+// A node with r < 0 is the point on the opposite side of the origin: F is smooth along the whole line, so
+// the stencil stays valid; the inside run of a disk simply starts at node 0 (midpoint rule exact for r dr).
+template <int N, bool LD>
+UL_HD void shoot_col(const Lens& L, double wcx, double wcy, double rho2, double th, double r0, double dr,
+                     int n_r, double& U_out, double& S_out, bool& edge)
+{
+    double c = cos(th), s = sin(th);
+    double f0 = UL_BIG, f1 = UL_BIG, f2 = UL_BIG, f3;
+    double U = 0.0, S = 0.0, U2 = 0.0;
+    edge = false;
+    for (int i = -2; i <= n_r + 1; ++i) {
+        double r = r0 + (i + 0.5) * dr;
+        f3 = ray_F<N>(L, r * c, r * s, wcx, wcy, rho2);
+        if (i >= 0 && i < n_r && f3 < 0.0) {
+            U += r;
+            if (LD) S += r * sqrt(-f3);
+            if ((i < 2 && r0 > 0.0) || i >= n_r - 2) edge = true;
+        }
+        // pair (i-2, i-1) = (f1, f2)
+        if (i >= 1 && ((f1 < 0.0) != (f2 < 0.0))) {
+            double r1 = r0 + (i - 1.5) * dr;             // node i-2
+            double rh = r1 + 0.5 * dr;                   // cell face between the pair
+            if (rh > 0.0) {
+                double u, dS; bool en;
+                double rin = en_dummy(f1) ? r1 + dr : r1; // first inside node
+                double t2x = dr / ul_max(rin, 0.5 * dr);
+                edge_event(f0, f1, f2, f3, LD, t2x, u, en, dS);
+                double rc = en ? (r1 + dr) - u * dr : r1 + u * dr;
+                rc = ul_max(rc, 0.0);
+                U2 += en ? 0.5 * (rh * rh - rc * rc) : 0.5 * (rc * rc - rh * rh);
+                S += dS * rc;
+            }
+        }
+        f0 = f1; f1 = f2; f2 = f3;
+    }
+    U_out = U * dr + U2; S_out = S * dr;
+}
+
+}  // namespace ulens
