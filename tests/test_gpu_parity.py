@@ -1,0 +1,212 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle and the closed forms. Needs a B200.
+
+Tolerance (BASELINE.json north_star): |A_gpu / A_oracle - 1| <= 1e-4 on points the oracle resolves
+(err_est <= 2e-5); image roots to 1e-10.
+"""
+import math
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+TOL_A = 1e-4
+TOL_ROOT = 1e-10
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    return torch
+
+
+@pytest.fixture(scope="module")
+def ctx(torch_cuda):
+    from paper_2510_02639_b200 import binding, build
+    build.build()
+    c = binding.Context(0)
+    yield c
+    c.close()
+
+
+def _to_dev(torch, w):
+    w = np.asarray(w, dtype=complex)
+    return (torch.tensor(np.ascontiguousarray(w.real), device="cuda:0"),
+            torch.tensor(np.ascontiguousarray(w.imag), device="cuda:0"))
+
+
+def _gpu_mag(ctx, torch, lenses, rho, u1, w):
+    """w: [n_cfg, n_pts] complex."""
+    w = np.atleast_2d(np.asarray(w, dtype=complex))
+    wre, wim = _to_dev(torch, w)
+    A, err, st = ctx.ulens_mag(lenses, rho, u1, wre.contiguous(), wim.contiguous())
+    torch.cuda.synchronize()
+    return A.cpu().numpy(), err.cpu().numpy(), st.cpu().numpy().astype(np.uint32)
+
+
+def _workload_lens(binding, O, wl, c):
+    p = wl.lens_params[c]
+    if wl.kind == "binary":
+        return binding.ulens_lens_binary(*p), O.lens_binary(*p)
+    return binding.ulens_lens_triple(*p), O.lens_triple(*p)
+
+
+# ------------------------------------------------------------------ closed forms (single lens)
+
+@pytest.mark.parametrize("rho", [0.1, 0.01, 1e-3])
+def test_single_lens_centre_closed_form(ctx, torch_cuda, rho):
+    """A = sqrt(1 + 4/rho^2) at u = 0 (north_star): a full Einstein ring."""
+    from paper_2510_02639_b200 import binding
+    A, _, st = _gpu_mag(ctx, torch_cuda, [binding.lens_single()], [rho], [0.0], [[0j]])
+    assert abs(A[0, 0] / math.sqrt(1 + 4 / rho ** 2) - 1) < 1e-6
+    assert (st[0, 0] & 0xff) == 0
+
+
+@pytest.mark.parametrize("u,rho,u1", [(0.3, 0.05, 0.0), (0.02, 0.05, 0.0), (1.2, 0.3, 0.0), (0.011, 0.01, 0.0),
+                                      (0.3, 0.05, 0.5), (0.03, 0.05, 1.0), (0.2, 0.1, 0.3), (0.0005, 0.05, 0.5)])
+def test_single_lens_witt_mao_and_limb_darkened(ctx, torch_cuda, u, rho, u1):
+    from paper_2510_02639_b200 import binding
+    from test_oracle_pins import A_ld_single, A_witt_mao
+    ref = float(A_ld_single(u, rho, u1)) if u1 > 0 else float(A_witt_mao(u, rho))
+    w = u * complex(math.cos(0.83), math.sin(0.83))
+    A, _, _ = _gpu_mag(ctx, torch_cuda, [binding.lens_single()], [rho], [u1], [[w]])
+    assert abs(A[0, 0] / ref - 1) < 5e-5
+
+
+def test_wide_binary_reduces_to_single_lens(ctx, torch_cuda):
+    from paper_2510_02639_b200 import binding
+    from test_oracle_pins import A_witt_mao
+    L = binding.ulens_lens_binary(50.0, 1e-6)
+    u, rho = 0.3, 0.05
+    w = complex(L.ax[0], 0) + u * complex(math.cos(1.0), math.sin(1.0))
+    A, _, _ = _gpu_mag(ctx, torch_cuda, [L], [rho], [0.0], [[w]])
+    assert abs(A[0, 0] / float(A_witt_mao(u, rho)) - 1) < 5e-5
+
+
+# ------------------------------------------------------------------ config C0: all 500 points
+
+def test_config0_all_points(ctx, torch_cuda, oracle):
+    from paper_2510_02639_b200 import binding, inputs
+    wl = inputs.get(0)
+    lens, olens = _workload_lens(binding, oracle, wl, 0)
+    A, err, st = _gpu_mag(ctx, torch_cuda, [lens], wl.rho, wl.u1, wl.w)
+    ref = oracle.mag_fs_batch([olens], 0, wl.w[0].real, wl.w[0].imag, wl.rho[0], wl.u1[0], 100, 8)
+    adm = ref["err_est"] <= 2e-5
+    assert adm.sum() >= 495
+    rel = np.abs(A[0] / ref["A"] - 1)
+    assert rel[adm].max() <= TOL_A, (rel.argmax(), rel.max())
+    nimg = (st[0] >> 8) & 0xf
+    assert set(np.unique(nimg)) <= {3, 5} and (nimg == 5).sum() >= 1      # the trajectory crosses the caustic
+    assert A[0].max() > 20
+
+
+# ------------------------------------------------------------------ configs C1..C3: seeded stratified subsample
+
+@pytest.mark.parametrize("cfg,n_cfg_used,n_per_cfg", [(1, 8, 24), (2, 6, 16), (3, 4, 16)])
+def test_config_subsample(ctx, torch_cuda, oracle, cfg, n_cfg_used, n_per_cfg):
+    from paper_2510_02639_b200 import binding, inputs
+    wl = inputs.get(cfg)
+    idx = inputs.subsample(wl, n_per_cfg, seed=cfg)
+    cs = list(range(0, wl.n_cfg, wl.n_cfg // n_cfg_used))[:n_cfg_used]
+    lenses, olenses = zip(*[_workload_lens(binding, oracle, wl, c) for c in cs])
+    w = np.stack([wl.w[c][idx[c]] for c in cs])
+    A, err, st = _gpu_mag(ctx, torch_cuda, lenses, wl.rho[cs], wl.u1[cs], w)
+    n_bad = n_adm = 0
+    worst = 0.0
+    for k, c in enumerate(cs):
+        ref = oracle.mag_fs_batch([olenses[k]], 0, w[k].real, w[k].imag, wl.rho[c], wl.u1[c], 100, 8)
+        adm = ref["err_est"] <= 2e-5
+        rel = np.abs(A[k] / ref["A"] - 1)
+        n_adm += int(adm.sum())
+        n_bad += int((rel[adm] > TOL_A).sum())
+        if adm.any():
+            worst = max(worst, float(np.nanmax(rel[adm])))
+    assert n_adm >= 0.9 * w.size
+    assert n_bad == 0, (n_bad, n_adm, worst)
+
+
+# ------------------------------------------------------------------ roots
+
+@pytest.mark.parametrize("kind", ["single", "binary", "triple"])
+def test_root_sets_match_oracle(ctx, torch_cuda, oracle, kind):
+    from paper_2510_02639_b200 import binding
+    rng = np.random.default_rng(11)
+    if kind == "single":
+        lens, olens = binding.lens_single(), oracle.lens_single()
+    elif kind == "binary":
+        lens, olens = binding.ulens_lens_binary(0.9, 0.03), oracle.lens_binary(0.9, 0.03)
+    else:
+        lens, olens = binding.ulens_lens_triple(1.1, 0.5, 0.03, 1.24, 1.3), oracle.lens_triple(1.1, 0.5, 0.03, 1.24, 1.3)
+    n = 200
+    w = rng.uniform(-1.2, 1.2, n) + 1j * rng.uniform(-1.2, 1.2, n)
+    wre, wim = _to_dev(torch_cuda, w)
+    z, img = ctx.ulens_roots(lens, wre, wim)
+    torch_cuda.cuda.synchronize()
+    z, img = z.cpu().numpy(), img.cpu().numpy()
+    n_cmp = 0
+    for k in range(n):
+        r = oracle.roots(olens, complex(w[k]))
+        zo = r["z"][r["is_image"]]
+        if np.min(np.abs(r["detJ"][r["is_image"]])) < 1e-6:      # on a caustic: image pair ill-defined
+            continue
+        zg = z[k][img[k]]
+        assert len(zg) == len(zo), (k, len(zg), len(zo))
+        for a in zo:                                            # compare as sets (root order is arbitrary)
+            d = np.abs(zg - a)
+            assert d.min() <= TOL_ROOT * max(1.0, abs(a)), (k, a, d.min())
+        n_cmp += 1
+    assert n_cmp > 0.9 * n
+
+
+# ------------------------------------------------------------------ edge cases of the boundary
+
+def test_empty_and_invalid_inputs(ctx, torch_cuda):
+    from paper_2510_02639_b200 import binding
+    torch = torch_cuda
+    L = binding.ulens_lens_binary(1.0, 0.1)
+    e = torch.empty((0,), dtype=torch.float64, device="cuda:0")
+    A, _, _ = ctx.ulens_mag([L], [1e-2], [0.0], e, e)                      # zero points: no-op success
+    assert A.numel() == 0
+    one = torch.zeros((1, 1), dtype=torch.float64, device="cuda:0") + 0.3
+    for rho, u1 in [(-1.0, 0.0), (0.0, 0.0), (float("nan"), 0.0), (1e-2, 1.5), (1e-2, -0.1)]:
+        with pytest.raises(binding.UlensError):
+            ctx.ulens_mag([L], [rho], [u1], one, one)
+
+
+def test_source_on_lens_position_and_ragged_batch(ctx, torch_cuda, oracle):
+    """Degenerate inputs: w_c exactly on a projected lens position; a batch that is not a
+    multiple of any tile size (37 points)."""
+    from paper_2510_02639_b200 import binding
+    L, OL = binding.ulens_lens_binary(0.8, 0.3), oracle.lens_binary(0.8, 0.3)
+    rng = np.random.default_rng(3)
+    w = rng.uniform(-0.6, 0.6, 37) + 1j * rng.uniform(-0.6, 0.6, 37)
+    w[0] = complex(L.ax[0], 0.0)
+    w[1] = complex(L.ax[1], 0.0)
+    w[2] = 0j
+    A, _, st = _gpu_mag(ctx, torch_cuda, [L], [0.02], [0.4], [w])
+    ref = oracle.mag_fs_batch([OL], 0, w.real, w.imag, 0.02, 0.4, 100, 8)
+    adm = ref["err_est"] <= 2e-5
+    assert np.all(np.isfinite(A))
+    assert np.abs(A[0] / ref["A"] - 1)[adm].max() <= TOL_A
+
+
+def test_host_entry_matches_device_entry(ctx, torch_cuda):
+    from paper_2510_02639_b200 import binding, inputs
+    wl = inputs.get(0)
+    L = binding.ulens_lens_binary(1.0, 0.01)
+    w = wl.w[:, ::10]
+    A_dev, _, _ = _gpu_mag(ctx, torch_cuda, [L], wl.rho, wl.u1, w)
+    A_host, _, _ = ctx.ulens_mag_host([L], wl.rho, wl.u1, w.real, w.imag)
+    assert np.array_equal(A_dev, A_host)                                   # deterministic reduction order
+
+
+def test_lightcurve_entry_matches_positions_entry(ctx, torch_cuda, oracle):
+    from paper_2510_02639_b200 import binding, inputs
+    wl = inputs.get(0)
+    t = torch_cuda.tensor(wl.t[::5].copy(), device="cuda:0")
+    A, dA, err, st = ctx.ulens_lightcurve_binary(wl.theta, 0.0, t)
+    torch_cuda.cuda.synchronize()
+    wx, wy = oracle.trajectory(0.0, 0.05, 1.0, 0.7, wl.t[::5])             # trajectory pinned in test_oracle_pins
+    A2, _, _ = _gpu_mag(ctx, torch_cuda, [binding.ulens_lens_binary(1.0, 0.01)], [1e-2], [0.0], [wx + 1j * wy])
+    assert np.allclose(A.cpu().numpy(), A2, rtol=1e-9)
