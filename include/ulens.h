@@ -139,6 +139,20 @@ int  ulens_reset_stats(ulens_ctx* ctx);
  * ulens_mag / ulens_lightcurve_binary / ulens_roots call on this context enqueued. */
 int  ulens_last_launch_count(ulens_ctx* ctx);
 
+/* Per-kernel device time (measurement): while timing is on, every kernel launch of the
+ * pipeline is bracketed by a CUDA event pair recorded on the CALLER'S stream (no synchronisation, no
+ * serialisation beyond stream order). ulens_get_kernel_ms synchronises those events and returns the
+ * total device milliseconds and the launch count of kernel `which` accumulated since the last
+ * ulens_set_timing(ctx, 1) call (which also clears the totals). */
+#define ULENS_K_TRAJ     0   /* trajectory -> source centres            (step a1) */
+#define ULENS_K_ROOTS    1   /* centre roots: polynomial, EA, polish    (step a2) */
+#define ULENS_K_REGIONS  2   /* limb images + sector builder            (steps a3, a4) */
+#define ULENS_K_SHOOT    3   /* ray shooting + ring quadrature          (steps a5, a6) */
+#define ULENS_K_FINALIZE 4   /* per-point sum, normalisation            (step a7) */
+#define ULENS_K_COUNT    5
+int  ulens_set_timing(ulens_ctx* ctx, int on);
+int  ulens_get_kernel_ms(ulens_ctx* ctx, int which, double* ms_total, int* launches);
+
 /* FP64 FMA roofline denominator: runs a dependent-chain-free DFMA kernel on every SM for about
  * `ms` milliseconds and returns the achieved rate in DFMA/s (one DFMA = 2 flop). Synchronises. */
 int  ulens_fp64_peak(ulens_ctx* ctx, double ms, double* dfma_per_s);

@@ -17,10 +17,11 @@ ULENS_OK, ULENS_EINVAL, ULENS_ECUDA, ULENS_ENOMEM, ULENS_EUNSUPPORTED = 0, -1, -
 ST_EA_NOCONV, ST_IMG_PARITY, ST_PATCH_CAP, ST_RES_CAP = 0x1, 0x2, 0x4, 0x8
 ST_CLIPPED, ST_UNIT_OVF, ST_ERR_HIGH, ST_NO_IMAGE = 0x10, 0x20, 0x40, 0x80
 ST_NIMG_SHIFT = 8
+KERNEL_NAMES = ["k_traj", "k_roots", "k_regions", "k_shoot", "k_finalize"]     # ULENS_K_* order
 
 EXPORTS = ["ulens_create", "ulens_destroy", "ulens_lens_binary", "ulens_lens_triple", "ulens_mag",
            "ulens_mag_host", "ulens_lightcurve_binary", "ulens_roots", "ulens_get_stats",
-           "ulens_reset_stats", "ulens_last_launch_count", "ulens_fp64_peak", "ulens_strerror",
+           "ulens_reset_stats", "ulens_last_launch_count", "ulens_set_timing", "ulens_get_kernel_ms", "ulens_fp64_peak", "ulens_strerror",
            "ulens_last_cuda_error"]
 
 
@@ -66,6 +67,8 @@ def lib() -> C.CDLL:
         L.ulens_get_stats.argtypes = [vp, C.POINTER(ulens_stats)]
         L.ulens_reset_stats.argtypes = [vp]
         L.ulens_last_launch_count.argtypes = [vp]
+        L.ulens_set_timing.argtypes = [vp, ip]
+        L.ulens_get_kernel_ms.argtypes = [vp, ip, dp, C.POINTER(C.c_int)]
         L.ulens_fp64_peak.argtypes = [vp, C.c_double, dp]
         L.ulens_strerror.argtypes = [ip]
         L.ulens_strerror.restype = C.c_char_p
@@ -228,6 +231,18 @@ class Context:
 
     def ulens_last_launch_count(self) -> int:
         return int(lib().ulens_last_launch_count(self._h))
+
+    def ulens_set_timing(self, on: bool):
+        _check(lib().ulens_set_timing(self._h, int(bool(on))), self._h)
+
+    def ulens_get_kernel_ms(self) -> dict:
+        """{kernel name: (total device ms, launches)} since ulens_set_timing(True). Synchronises."""
+        out = {}
+        for which, name in enumerate(KERNEL_NAMES):
+            ms, n = C.c_double(), C.c_int()
+            _check(lib().ulens_get_kernel_ms(self._h, which, C.byref(ms), C.byref(n)), self._h)
+            out[name] = (ms.value, n.value)
+        return out
 
     def ulens_fp64_peak(self, ms: float = 200.0) -> float:
         out = C.c_double()

@@ -53,7 +53,25 @@ struct ulens_ctx {
     double* traj_w; size_t traj_cap;    // lightcurve entry: source centres [2][n]
     double* io_buf; size_t io_cap;      // *_host entry: staging
     int last_launches;
+    // optional per-kernel device timing (ulens_set_timing): event pairs recorded on the caller's stream
+    int timing_on;
+    struct TimedLaunch { cudaEvent_t a, b; int which; };
+    std::vector<TimedLaunch>* timed;
+    double k_ms[ULENS_K_COUNT]; int k_launches[ULENS_K_COUNT];
     char cuda_err[256];
+};
+
+// RAII-free helper: record an event pair around one launch when timing is on
+struct KTimer {
+    ulens_ctx* c; cudaStream_t st; cudaEvent_t a, b; int which; bool on;
+    KTimer(ulens_ctx* ctx, int w, cudaStream_t s) : c(ctx), st(s), a(nullptr), b(nullptr), which(w), on(ctx->timing_on != 0)
+    {
+        if (on) { cudaEventCreate(&a); cudaEventCreate(&b); cudaEventRecord(a, st); }
+    }
+    ~KTimer()
+    {
+        if (on) { cudaEventRecord(b, st); c->timed->push_back({a, b, which}); }
+    }
 };
 
 static int fail_cuda(ulens_ctx* c, cudaError_t e, const char* where)
@@ -353,6 +371,8 @@ extern "C" int ulens_create(ulens_ctx** out, int cuda_device, const ulens_option
     if (!ctx) return ULENS_ENOMEM;
     memset(ctx, 0, sizeof *ctx);
     ctx->device = cuda_device;
+    ctx->timed = new (std::nothrow) std::vector<ulens_ctx::TimedLaunch>();
+    if (!ctx->timed) { delete ctx; return ULENS_ENOMEM; }
     ulens_options o; memset(&o, 0, sizeof o);
     if (opt) o = *opt;
     if (o.n_limb <= 0) o.n_limb = 512;
@@ -392,6 +412,10 @@ extern "C" void ulens_destroy(ulens_ctx* ctx)
     cudaFree(ctx->patches); cudaFree(ctx->n_patch); cudaFree(ctx->status_ws); cudaFree(ctx->unit_desc);
     cudaFree(ctx->unit_sum); cudaFree(ctx->unit_odd); cudaFree(ctx->cc); cudaFree(ctx->counters);
     cudaFree(ctx->cfg_dev); cudaFree(ctx->poly_dev); cudaFree(ctx->traj_w); cudaFree(ctx->io_buf);
+    if (ctx->timed) {
+        for (auto& t : *ctx->timed) { cudaEventDestroy(t.a); cudaEventDestroy(t.b); }
+        delete ctx->timed;
+    }
     delete ctx;
 }
 
@@ -447,21 +471,33 @@ static int run_chunks(ulens_ctx* ctx, long long n_total, int n_pts, bool ld, con
     for (long long base = 0; base < n_total; base += ctx->chunk) {
         int n = (int)((n_total - base < ctx->chunk) ? (n_total - base) : ctx->chunk);
         CK(cudaMemsetAsync(ctx->cc, 0, sizeof(ChunkCounters), st));
-        k_roots<N><<<(n + 127) / 128, 128, 0, st>>>(n, (int)base, n_pts, ctx->cfg_dev, ctx->poly_dev, w_re, w_im,
-                                                    nullptr, nullptr, nullptr, ctx->status_ws);
-        k_regions<N><<<(n + 3) / 4, 128, smem, st>>>(n, (int)base, n_pts, ctx->cfg_dev, ctx->poly_dev, w_re, w_im, ctx->rp,
-                                                     ctx->patches, ctx->n_patch, ctx->status_ws, ctx->unit_desc,
-                                                     (unsigned)ctx->cap_units, ctx->cc, ctx->counters);
+        {
+            KTimer kt(ctx, ULENS_K_ROOTS, st);
+            k_roots<N><<<(n + 127) / 128, 128, 0, st>>>(n, (int)base, n_pts, ctx->cfg_dev, ctx->poly_dev, w_re, w_im,
+                                                        nullptr, nullptr, nullptr, ctx->status_ws);
+        }
+        {
+            KTimer kt(ctx, ULENS_K_REGIONS, st);
+            k_regions<N><<<(n + 3) / 4, 128, smem, st>>>(n, (int)base, n_pts, ctx->cfg_dev, ctx->poly_dev, w_re, w_im, ctx->rp,
+                                                         ctx->patches, ctx->n_patch, ctx->status_ws, ctx->unit_desc,
+                                                         (unsigned)ctx->cap_units, ctx->cc, ctx->counters);
+        }
         int grid = sm_count * 4;
-        if (ld)
-            k_shoot<N, true><<<grid, 128, 0, st>>>((int)base, n_pts, ctx->cfg_dev, w_re, w_im, ctx->patches, ctx->unit_desc,
-                                                   ctx->unit_sum, ctx->unit_odd, ctx->status_ws, ctx->cc, ctx->counters);
-        else
-            k_shoot<N, false><<<grid, 128, 0, st>>>((int)base, n_pts, ctx->cfg_dev, w_re, w_im, ctx->patches, ctx->unit_desc,
-                                                    ctx->unit_sum, ctx->unit_odd, ctx->status_ws, ctx->cc, ctx->counters);
-        k_finalize<<<(n + 127) / 128, 128, 0, st>>>(n, (int)base, n_pts, ctx->cfg_dev, ctx->patches, ctx->n_patch,
-                                                    ctx->unit_sum, ctx->unit_odd, ctx->status_ws, ctx->opt.rel_tol,
-                                                    A_out, err_out, status_out, ctx->counters);
+        {
+            KTimer kt(ctx, ULENS_K_SHOOT, st);
+            if (ld)
+                k_shoot<N, true><<<grid, 128, 0, st>>>((int)base, n_pts, ctx->cfg_dev, w_re, w_im, ctx->patches, ctx->unit_desc,
+                                                       ctx->unit_sum, ctx->unit_odd, ctx->status_ws, ctx->cc, ctx->counters);
+            else
+                k_shoot<N, false><<<grid, 128, 0, st>>>((int)base, n_pts, ctx->cfg_dev, w_re, w_im, ctx->patches, ctx->unit_desc,
+                                                        ctx->unit_sum, ctx->unit_odd, ctx->status_ws, ctx->cc, ctx->counters);
+        }
+        {
+            KTimer kt(ctx, ULENS_K_FINALIZE, st);
+            k_finalize<<<(n + 127) / 128, 128, 0, st>>>(n, (int)base, n_pts, ctx->cfg_dev, ctx->patches, ctx->n_patch,
+                                                        ctx->unit_sum, ctx->unit_odd, ctx->status_ws, ctx->opt.rel_tol,
+                                                        A_out, err_out, status_out, ctx->counters);
+        }
         ctx->last_launches += 4;
         CK(cudaGetLastError());
     }
@@ -556,7 +592,10 @@ extern "C" int ulens_lightcurve_binary(ulens_ctx* ctx, int n_cfg, int n_epochs, 
     }
     double* w_re = ctx->traj_w; double* w_im = w_re + n; double* th_dev = w_im + n;
     CK(cudaMemcpyAsync(th_dev, theta_host, sizeof(double) * 7 * n_cfg, cudaMemcpyHostToDevice, st));
-    k_traj<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(n_cfg, n_epochs, th_dev, t, w_re, w_im);
+    {
+        KTimer kt(ctx, ULENS_K_TRAJ, st);
+        k_traj<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(n_cfg, n_epochs, th_dev, t, w_re, w_im);
+    }
     CK(cudaGetLastError());
     int rc = mag_device(ctx, n_cfg, n_epochs, lenses.data(), rho.data(), u1v.data(), w_re, w_im, A_out, err_out, status_out, st);
     ctx->last_launches += 1;
@@ -604,6 +643,42 @@ extern "C" int ulens_reset_stats(ulens_ctx* ctx)
     CK(cudaSetDevice(ctx->device));
     CK(cudaDeviceSynchronize());
     CK(cudaMemset(ctx->counters, 0, sizeof(DevCounters)));
+    return ULENS_OK;
+}
+
+// fold finished event pairs into the per-kernel totals (synchronises on each pair)
+static int drain_timed(ulens_ctx* ctx)
+{
+    for (auto& t : *ctx->timed) {
+        float ms = 0.f;
+        CK(cudaEventSynchronize(t.b));
+        CK(cudaEventElapsedTime(&ms, t.a, t.b));
+        ctx->k_ms[t.which] += ms; ctx->k_launches[t.which] += 1;
+        cudaEventDestroy(t.a); cudaEventDestroy(t.b);
+    }
+    ctx->timed->clear();
+    return ULENS_OK;
+}
+
+extern "C" int ulens_set_timing(ulens_ctx* ctx, int on)
+{
+    if (!ctx) return ULENS_EINVAL;
+    CK(cudaSetDevice(ctx->device));
+    int rc = drain_timed(ctx);
+    if (rc != ULENS_OK) return rc;
+    ctx->timing_on = on ? 1 : 0;
+    if (on) for (int k = 0; k < ULENS_K_COUNT; ++k) { ctx->k_ms[k] = 0.0; ctx->k_launches[k] = 0; }
+    return ULENS_OK;
+}
+
+extern "C" int ulens_get_kernel_ms(ulens_ctx* ctx, int which, double* ms_total, int* launches)
+{
+    if (!ctx || which < 0 || which >= ULENS_K_COUNT || !ms_total) return ULENS_EINVAL;
+    CK(cudaSetDevice(ctx->device));
+    int rc = drain_timed(ctx);
+    if (rc != ULENS_OK) return rc;
+    *ms_total = ctx->k_ms[which];
+    if (launches) *launches = ctx->k_launches[which];
     return ULENS_OK;
 }
 
