@@ -176,15 +176,21 @@ class Context:
                                _dev(status_out, torch.int32, n), self._stream(stream)), self._h)
         return A_out, err_out, status_out
 
-    def ulens_mag_host(self, lenses, rho, u1, w_re, w_im, stream=None):
-        """Host numpy arrays in / out; copies and synchronisation happen inside the C call."""
+    def ulens_mag_host(self, lenses, rho, u1, w_re, w_im, A=None, err=None, st=None, stream=None):
+        """Host numpy arrays in / out (optionally caller-provided, e.g. views of pinned tensors); the
+        copies and the synchronisation happen inside the C call."""
         n_cfg, arr, rho, u1 = self._cfg_arrays(lenses, rho, u1)
         w_re = np.ascontiguousarray(w_re, dtype=np.float64)
         w_im = np.ascontiguousarray(w_im, dtype=np.float64)
         n_pts = w_re.size // max(n_cfg, 1)
-        A = np.empty((n_cfg, n_pts))
-        err = np.empty((n_cfg, n_pts))
-        st = np.empty((n_cfg, n_pts), dtype=np.uint32)
+        A = np.empty((n_cfg, n_pts)) if A is None else A
+        err = np.empty((n_cfg, n_pts)) if err is None else err
+        st = np.empty((n_cfg, n_pts), dtype=np.uint32) if st is None else st
+        for a, dt in ((A, np.float64), (err, np.float64)):
+            if a.dtype != dt or not a.flags.c_contiguous or a.size != n_cfg * n_pts:
+                raise UlensError("output arrays must be C-contiguous float64 of n_cfg*n_pts elements")
+        if st.dtype.itemsize != 4 or not st.flags.c_contiguous or st.size != n_cfg * n_pts:
+            raise UlensError("status array must be C-contiguous 32-bit of n_cfg*n_pts elements")
         _check(lib().ulens_mag_host(self._h, n_cfg, n_pts, arr, _dptr(rho), _dptr(u1),
                                     w_re.ctypes.data_as(C.c_void_p), w_im.ctypes.data_as(C.c_void_p),
                                     A.ctypes.data_as(C.c_void_p), err.ctypes.data_as(C.c_void_p),
