@@ -239,13 +239,25 @@ static void orc_descend(orc_fs *S, int64_t ix, int64_t iy, int64_t size)
 /* A at lattice pitch rho/n_rho. Returns 0, or -1 on a bad argument.
  * Outside |Re z|,|Im z| <= R = 2 + |w_c| + rho + max|a_i| no point can map into the source:
  * there |z - a_i| > 2 + |w_c| + rho  so  |w - z| <= sum eps_i/|z-a_i| < 1/2  while  |z - w_c| > 2 + rho. */
+int orc_mag_fs_pitch(const orc_lens *L, double wcx, double wcy, double rho, double u1, double h, int ss,
+                     double *A_out, long long *n_eval_out);
+
 int orc_mag_fs(const orc_lens *L, double wcx, double wcy, double rho, double u1, int n_rho, int ss,
                double *A_out, long long *n_eval_out)
 {
-    if (!L || L->n < 1 || L->n > 3 || !(rho > 0) || !(u1 >= 0 && u1 <= 1) || n_rho < 1 || ss < 1) return -1;
+    if (!(rho > 0) || n_rho < 1) return -1;
+    return orc_mag_fs_pitch(L, wcx, wcy, rho, u1, rho / n_rho, ss, A_out, n_eval_out);
+}
+
+/* The same with the lattice pitch h given explicitly, so that a finite-difference derivative with respect
+ * to rho (or anything else) can hold the lattice fixed (DESIGN.md 7.2 "derivative reference"). */
+int orc_mag_fs_pitch(const orc_lens *L, double wcx, double wcy, double rho, double u1, double h, int ss,
+                     double *A_out, long long *n_eval_out)
+{
+    if (!L || L->n < 1 || L->n > 3 || !(rho > 0) || !(u1 >= 0 && u1 <= 1) || !(h > 0) || ss < 1) return -1;
     orc_fs S;
     S.L = L; S.wcx = wcx; S.wcy = wcy; S.rho = rho; S.rho2 = rho * rho; S.u1 = u1;
-    S.h = rho / n_rho; S.ss = ss; S.x2_smooth = 0.81; S.flux = 0.0; S.n_eval = 0;
+    S.h = h; S.ss = ss; S.x2_smooth = 0.81; S.flux = 0.0; S.n_eval = 0;
     double amax = 0.0;
     for (int i = 0; i < L->n; ++i) { double a = hypot(L->ax[i], L->ay[i]); if (a > amax) amax = a; }
     double R = 2.0 + hypot(wcx, wcy) + rho + amax;
@@ -280,6 +292,25 @@ int orc_mag_fs_batch(const orc_lens *lenses, const int *lens_idx, int n_pts, con
         int r2 = orc_mag_fs(L, wcx[k], wcy[k], rho[k], u1[k], 2 * n_rho, ss, &A_fine[k], &e2);
         if (n_eval) n_eval[k] = e1 + e2;
         if (r1 || r2) bad |= 1;
+    }
+    return bad ? -1 : 0;
+}
+
+/* Batch at one explicit pitch per point and one lens per point (finite-difference stencils: every
+ * perturbed evaluation has its own lens, source and radius but the unperturbed point's lattice). */
+int orc_mag_fs_pitch_batch(const orc_lens *lenses, int n_pts, const double *wcx, const double *wcy,
+                           const double *rho, const double *u1, const double *h, int ss, int n_threads,
+                           double *A, long long *n_eval)
+{
+    int bad = 0;
+#ifdef _OPENMP
+    if (n_threads > 0) omp_set_num_threads(n_threads);
+#endif
+#pragma omp parallel for schedule(dynamic, 1) reduction(| : bad)
+    for (int k = 0; k < n_pts; ++k) {
+        long long e = 0;
+        if (orc_mag_fs_pitch(&lenses[k], wcx[k], wcy[k], rho[k], u1[k], h[k], ss, &A[k], &e)) bad |= 1;
+        if (n_eval) n_eval[k] = e;
     }
     return bad ? -1 : 0;
 }

@@ -179,6 +179,47 @@ __global__ void k_roots(int n, int pt_base, int n_pts_per_cfg, const PointCfg* _
         }
         if (ok) { ix[n_img] = zx; iy[n_img] = zy; ++n_img; mask |= 1u << k; zr[k] = zx; zi[k] = zy; }
     }
+    // An image count of the wrong parity almost always means the ultra-faint image next to a light
+    // lens was lost: it sits at z ~ a_i + eps_i / conj(a_i - w - sum_{j!=i} eps_j/conj(a_i - a_j)), inside
+    // the cluster of spurious roots around a_i that EA cannot resolve in double (degree 10). Seed it there.
+    if constexpr (N > 1) {
+        if (((n_img - (N + 1)) & 1) != 0 || n_img < N + 1) {
+#pragma unroll
+            for (int a = 0; a < N; ++a) {
+                double tx = L.ax[a] - wx, ty = L.ay[a] - wy;
+#pragma unroll
+                for (int b = 0; b < N; ++b) {
+                    if (b == a) continue;
+                    double dx = L.ax[a] - L.ax[b], dy = L.ay[a] - L.ay[b];
+                    double i2 = L.eps[b] / (dx * dx + dy * dy);
+                    tx -= dx * i2; ty -= dy * i2;               // eps_b / conj(d) = eps_b d / |d|^2
+                }
+                double t2 = tx * tx + ty * ty;
+                if (!(t2 > 0.0)) continue;
+                double zx = L.ax[a] + L.eps[a] * tx / t2, zy = L.ay[a] + L.eps[a] * ty / t2;   // eps/conj(t) = eps t/|t|^2
+                double detJ, resid, gx, gy;
+                bool ok = polish_image<N>(L, wx, wy, zx, zy, 12, 1e-13, detJ, resid, gx, gy);
+                if (ok) {
+                    double sc = ul_max(1.0, zx * zx + zy * zy);
+                    for (int q = 0; q < n_img; ++q) {
+                        double ddx = zx - ix[q], ddy = zy - iy[q];
+                        if (ddx * ddx + ddy * ddy < 1e-18 * sc) ok = false;
+                    }
+                }
+                if (!ok) continue;
+                // put it in the non-image slot nearest to it
+                int slot = -1; double bd = 1e300;
+#pragma unroll
+                for (int k = 0; k < DEG; ++k) {
+                    if (mask & (1u << k)) continue;
+                    double ddx = zr[k] - zx, ddy = zi[k] - zy, d = ddx * ddx + ddy * ddy;
+                    if (d < bd) { bd = d; slot = k; }
+                }
+                if (slot < 0) continue;
+                ix[n_img] = zx; iy[n_img] = zy; ++n_img; mask |= 1u << slot; zr[slot] = zx; zi[slot] = zy;
+            }
+        }
+    }
     if (((n_img - (N + 1)) & 1) != 0 || n_img < N + 1) st |= UL_ST_IMG_PARITY;
     st |= (unsigned)(n_img & 0xf) << 8;
     if (status) status[i] = st;

@@ -257,25 +257,33 @@ UL_HD void ea_init(const double* br, const double* bi, double* zr, double* zi)
     }
 }
 
-// Iterate until every relative step is < 1e-14, or the steps stagnate at the evaluation-noise floor
-// (largest step < 1e-8 and no longer halving), or max_it. Returns the iterations used (max_it+1 if
-// the cap was hit without meeting either criterion).
+// Iterate until every root is settled, or max_it. A root is settled (frozen, but still repelling the others)
+// once its relative step is < sqrt(tol2), or its step is below 1e-3 and no longer shrinking by 1.41x per
+// iteration: the evaluation-noise floor, which for the spurious-root clusters next to a light lens is as
+// high as 1e-5 relative (degree 10). Near-double roots converge linearly at rate 1/2 and are NOT stopped by
+// the second rule. The images are polished on Eq. 1 afterwards, so EA only has to reach Newton's basin.
+// Returns the iterations used (max_it+1 if the cap was hit with a root still moving).
 template <int DEG>
-UL_HD int ea_iterate(const double* br, const double* bi, double* zr, double* zi, int max_it)
+UL_HD int ea_iterate(const double* br, const double* bi, double* zr, double* zi, int max_it, double tol2 = 1e-28)
 {
-    double e_prev = 1e300;
+    double prev[DEG];
+#pragma unroll
+    for (int k = 0; k < DEG; ++k) prev[k] = 1e300;
+    unsigned done = 0;
+    const unsigned all = (1u << DEG) - 1u;
     for (int it = 1; it <= max_it; ++it) {
-        double e = 0.0;
+        bool bad = false;
 #pragma unroll
         for (int k = 0; k < DEG; ++k) {
+            if (done & (1u << k)) continue;
             double pr, pi, dr, di;
             horner2<DEG>(br, bi, zr[k], zi[k], pr, pi, dr, di);
             double p2 = pr * pr + pi * pi;
-            if (p2 == 0.0) continue;
+            if (p2 == 0.0) { done |= 1u << k; continue; }
             // Newton ratio n = P/P'
             double d2 = dr * dr + di * di;
             double nx, ny;
-            if (d2 > 0.0) { nx = (pr * dr + pi * di) / d2; ny = (pi * dr - pr * di) / d2; }
+            if (d2 > 0.0) { double id = 1.0 / d2; nx = (pr * dr + pi * di) * id; ny = (pi * dr - pr * di) * id; }
             else { nx = 1e-3; ny = 1e-3; }
             // repulsion S = sum_{j != k} 1/(z_k - z_j)
             double sx = 0.0, sy = 0.0;
@@ -290,19 +298,48 @@ UL_HD int ea_iterate(const double* br, const double* bi, double* zr, double* zi,
             double ax = 1.0 - (nx * sx - ny * sy), ay = -(nx * sy + ny * sx);
             double a2 = ax * ax + ay * ay;
             double stx, sty;
-            if (a2 > 1e-300) { stx = (nx * ax + ny * ay) / a2; sty = (ny * ax - nx * ay) / a2; }
+            if (a2 > 1e-300) { double ia = 1.0 / a2; stx = (nx * ax + ny * ay) * ia; sty = (ny * ax - nx * ay) * ia; }
             else { stx = nx; sty = ny; }
             zr[k] -= stx; zi[k] -= sty;
             double z2 = zr[k] * zr[k] + zi[k] * zi[k];
             double rel = (stx * stx + sty * sty) / (z2 + 1e-12);
-            e = ul_max(e, rel);
+            if (!(rel == rel)) bad = true;
+            if (rel < tol2 || (rel < 1e-6 && rel > 0.5 * prev[k])) done |= 1u << k;
+            prev[k] = rel;
         }
-        if (!(e == e)) return max_it + 1;
-        if (e < 1e-28) return it;                            // (1e-14)^2
-        if (e < 1e-16 && e > 0.25 * e_prev) return it;       // stagnation at the noise floor (1e-8 ^2, halving ^2)
-        e_prev = e;
+        if (bad) return max_it + 1;
+        if (done == all) return it;
     }
     return max_it + 1;
+}
+
+// Keep root identities along a path in w: permute the new roots so that slot j holds the one nearest to
+// slot j's previous position (greedy in slot order). Roots move continuously with w, so after this a slot
+// can only confuse roots that are closer to each other than one step of the path.
+template <int DEG>
+UL_HD void match_roots(const double* ozr, const double* ozi, double* zr, double* zi)
+{
+    double nr[DEG], ni[DEG];
+    unsigned used = 0;
+    bool ident = true;
+#pragma unroll
+    for (int j = 0; j < DEG; ++j) {
+        int best = -1; double bd = 1e300;
+#pragma unroll
+        for (int k = 0; k < DEG; ++k) {
+            if (used & (1u << k)) continue;
+            double dx = zr[k] - ozr[j], dy = zi[k] - ozi[j];
+            double d = dx * dx + dy * dy;
+            if (d < bd || best < 0) { bd = d; best = k; }
+        }
+        used |= 1u << best;
+        nr[j] = zr[best]; ni[j] = zi[best];
+        ident = ident && (best == j);
+    }
+    if (!ident) {
+#pragma unroll
+        for (int j = 0; j < DEG; ++j) { zr[j] = nr[j]; zi[j] = ni[j]; }
+    }
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -103,7 +103,7 @@ UL_HDN void regions_phaseA(int lane, const Lens& L, const LensPoly& T, double wc
     const int chunk = P.n_limb / 32;
     SubBox* B = &W.box[lane * DEG];
     double t_cur[DEG];
-    double zr[DEG], zi[DEG], pvx[DEG], pvy[DEG];
+    double zr[DEG], zi[DEG], ozr[DEG], ozi[DEG], pvx[DEG], pvy[DEG];
     double br[DEG + 1], bi[DEG + 1];
     unsigned valid_prev = 0;
 #pragma unroll
@@ -115,14 +115,20 @@ UL_HDN void regions_phaseA(int lane, const Lens& L, const LensPoly& T, double wc
         double ph = dphi * k;
         double wx = wcx + rho * cos(ph), wy = wcy + rho * sin(ph);      // Eq. 8 (G2)
         poly_coeffs<N>(L, T, wx, wy, br, bi);
+        // limb solves only have to land in the basin of the Eq.-1 polish: relative step 1e-7
         int it;
-        if (s == 0) { ea_init<DEG>(br, bi, zr, zi); it = ea_iterate<DEG>(br, bi, zr, zi, 64); }
+        bool cold = (s == 0);
+        if (s == 0) { ea_init<DEG>(br, bi, zr, zi); it = ea_iterate<DEG>(br, bi, zr, zi, 64, 1e-14); }
         else {
-            it = ea_iterate<DEG>(br, bi, zr, zi, 32);
-            if (it > 32) { ea_init<DEG>(br, bi, zr, zi); it = ea_iterate<DEG>(br, bi, zr, zi, 64); if (it <= 64) it = 1; }
+#pragma unroll
+            for (int j = 0; j < DEG; ++j) { ozr[j] = zr[j]; ozi[j] = zi[j]; }
+            it = ea_iterate<DEG>(br, bi, zr, zi, 24, 1e-14);
+            if (it > 24) { cold = true; ea_init<DEG>(br, bi, zr, zi); it = ea_iterate<DEG>(br, bi, zr, zi, 64, 1e-14); if (it <= 64) it = 1; }
+            match_roots<DEG>(ozr, ozi, zr, zi);          // slot j keeps following the same root
         }
         ++n_solves;
-        if ((s == 0 && it > 64) || (s > 0 && it > 32)) status |= UL_ST_EA_NOCONV;
+        if ((s == 0 && it > 64) || (s > 0 && it > 24)) status |= UL_ST_EA_NOCONV;
+        (void)cold;
 
         unsigned valid = 0;
         double px[DEG], py[DEG], hrr[DEG], htt[DEG], crr[DEG], ctt[DEG];
@@ -148,21 +154,33 @@ UL_HDN void regions_phaseA(int lane, const Lens& L, const LensPoly& T, double wc
         for (int j = 0; j < DEG; ++j)
             if (valid & (1u << j))
                 box_add(B[j], t_cur[j], sqrt(px[j] * px[j] + py[j] * py[j]), atan2(py[j], px[j]), hrr[j], htt[j], crr[j], ctt[j], true);
-        // links: slots that switched off (their last point) and on (their first point) between s-1 and s
+        // links: a slot that switched off (its last point) or on (its first point) between s-1 and s is one
+        // half of an image pair destroyed / created on a critical curve somewhere between the two partners'
+        // end points: each partner's box takes the other's end point, so that the pair's boxes overlap.
+        // Partner = the nearest other switching slot, if closer than 0.5 (unrelated flips are not linked).
         if (s > 0) {
             unsigned off = valid_prev & ~valid, on = valid & ~valid_prev;
             unsigned grp = off | on;
             if (grp && (grp & (grp - 1))) {             // at least two members
+                double ex[DEG], ey[DEG];
+#pragma unroll
+                for (int a = 0; a < DEG; ++a) { ex[a] = (off & (1u << a)) ? pvx[a] : px[a]; ey[a] = (off & (1u << a)) ? pvy[a] : py[a]; }
 #pragma unroll
                 for (int a = 0; a < DEG; ++a) {
                     if (!(grp & (1u << a))) continue;
-                    double ax_ = (off & (1u << a)) ? pvx[a] : px[a];
-                    double ay_ = (off & (1u << a)) ? pvy[a] : py[a];
-                    double ra = sqrt(ax_ * ax_ + ay_ * ay_), ta = atan2(ay_, ax_);
+                    int nb = -1; double bd = 0.25;
 #pragma unroll
                     for (int b = 0; b < DEG; ++b) {
                         if (b == a || !(grp & (1u << b))) continue;
-                        box_add(B[b], t_cur[b], ra, ta, 1e300, 1e300, 1e300, 1e300, false);
+                        double dx = ex[a] - ex[b], dy = ey[a] - ey[b];
+                        double d = dx * dx + dy * dy;
+                        if (d < bd) { bd = d; nb = b; }
+                    }
+                    if (nb >= 0) {
+                        double ra = sqrt(ex[a] * ex[a] + ey[a] * ey[a]), ta = atan2(ey[a], ex[a]);
+                        double rb = sqrt(ex[nb] * ex[nb] + ey[nb] * ey[nb]), tb = atan2(ey[nb], ex[nb]);
+                        box_add(B[nb], t_cur[nb], ra, ta, 1e300, 1e300, 1e300, 1e300, false);
+                        box_add(B[a], t_cur[a], rb, tb, 1e300, 1e300, 1e300, 1e300, false);
                     }
                 }
             }

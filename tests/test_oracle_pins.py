@@ -289,3 +289,31 @@ def test_single_lens_roots_closed_form(oracle):
     zs = np.sort(r["z"][r["is_image"]].real)
     assert np.allclose(zs, [(u - math.sqrt(u * u + 4)) / 2, (u + math.sqrt(u * u + 4)) / 2], atol=1e-15)
     assert abs(oracle.mag_point_source(L, complex(u, 0)) - float(A_ps_single(mp.mpf(u)))) < 1e-13
+
+
+# ---------------------------------------------------------------- derivative reference (finite differences)
+
+@pytest.mark.parametrize("u,rho,u1", [(0.3, 0.05, 0.0), (0.03, 0.05, 0.0), (0.0, 0.05, 0.0), (0.3, 0.05, 0.5)])
+def test_fd_derivative_reference_single_lens(oracle, u, rho, u1):
+    """oracle.mag_fd against closed forms: dA/drho = -4/(rho^3 sqrt(1+4/rho^2)) at u = 0 and
+    mpmath derivatives of the Witt-Mao / limb-darkened closed forms elsewhere."""
+    S = oracle.lens_single()
+
+    def case(p):
+        return S, complex(p[0] * math.cos(0.83), p[0] * math.sin(0.83)), p[1]
+
+    ss = 16 if u1 == 0 else 8
+    steps = [[0.2 * rho, 0.1 * rho], [0.1 * rho, 0.05 * rho]]
+    A0, dA = oracle.mag_fd(case, [u, rho], steps, u1, 100, ss)
+    D, corr = oracle.fd_extrapolate(dA)
+    if u == 0.0:
+        exact_rho = -4.0 / (rho ** 3 * math.sqrt(1 + 4 / rho ** 2))
+        assert abs(D[1] / exact_rho - 1) < 2e-4
+        assert abs(D[0]) < 2e-4 * abs(exact_rho)            # symmetric in u
+        return
+    f = (lambda uu, rr: A_ld_single(uu, rr, u1)) if u1 > 0 else A_witt_mao
+    du = float(mp.diff(lambda x: f(x, mp.mpf(rho)), u))
+    dr = float(mp.diff(lambda x: f(mp.mpf(u), x), rho))
+    scale = A0 / rho                                       # natural size of a derivative in source-plane units
+    assert abs(D[0] - du) < 1e-3 * max(abs(du), 0.02 * scale)
+    assert abs(D[1] - dr) < 1e-3 * max(abs(dr), 0.02 * scale)
