@@ -152,76 +152,9 @@ __global__ void k_roots(int n, int pt_base, int n_pts_per_cfg, const PointCfg* _
     int c = (int)(gp / n_pts_per_cfg);
     Lens L = cfg[c].lens;
     double wx = w_re[gp], wy = w_im[gp];
-    double br[DEG + 1], bi[DEG + 1], zr[DEG], zi[DEG];
-    poly_coeffs<N>(L, poly[c], wx, wy, br, bi);
-    ea_init<DEG>(br, bi, zr, zi);
-    int it = ea_iterate<DEG>(br, bi, zr, zi, 100);
-    unsigned st = (it > 100) ? UL_ST_EA_NOCONV : 0u;
-    // validate + polish (G7): damped Newton on Eq. 1 from every root; accept converged, un-moved, distinct ones
-    double ix[DEG], iy[DEG];
-    int n_img = 0;
+    double zr[DEG], zi[DEG];
     unsigned mask = 0;
-#pragma unroll
-    for (int k = 0; k < DEG; ++k) {
-        double zx = zr[k], zy = zi[k], detJ, resid, gx, gy;
-        double dm2 = 1e300;
-#pragma unroll
-        for (int a = 0; a < N; ++a) { double dx = zx - L.ax[a], dy = zy - L.ay[a]; dm2 = ul_min(dm2, dx * dx + dy * dy); }
-        bool ok = polish_image<N>(L, wx, wy, zx, zy, 8, 1e-13, detJ, resid, gx, gy);
-        double mv2 = (zx - zr[k]) * (zx - zr[k]) + (zy - zi[k]) * (zy - zi[k]);
-        ok = ok && (mv2 <= 0.01 * dm2);
-        if (ok) {
-            double sc = ul_max(1.0, zx * zx + zy * zy);
-            for (int q = 0; q < n_img; ++q) {
-                double ddx = zx - ix[q], ddy = zy - iy[q];
-                if (ddx * ddx + ddy * ddy < 1e-18 * sc) ok = false;
-            }
-        }
-        if (ok) { ix[n_img] = zx; iy[n_img] = zy; ++n_img; mask |= 1u << k; zr[k] = zx; zi[k] = zy; }
-    }
-    // An image count of the wrong parity almost always means the ultra-faint image next to a light
-    // lens was lost: it sits at z ~ a_i + eps_i / conj(a_i - w - sum_{j!=i} eps_j/conj(a_i - a_j)), inside
-    // the cluster of spurious roots around a_i that EA cannot resolve in double (degree 10). Seed it there.
-    if constexpr (N > 1) {
-        if (((n_img - (N + 1)) & 1) != 0 || n_img < N + 1) {
-#pragma unroll
-            for (int a = 0; a < N; ++a) {
-                double tx = L.ax[a] - wx, ty = L.ay[a] - wy;
-#pragma unroll
-                for (int b = 0; b < N; ++b) {
-                    if (b == a) continue;
-                    double dx = L.ax[a] - L.ax[b], dy = L.ay[a] - L.ay[b];
-                    double i2 = L.eps[b] / (dx * dx + dy * dy);
-                    tx -= dx * i2; ty -= dy * i2;               // eps_b / conj(d) = eps_b d / |d|^2
-                }
-                double t2 = tx * tx + ty * ty;
-                if (!(t2 > 0.0)) continue;
-                double zx = L.ax[a] + L.eps[a] * tx / t2, zy = L.ay[a] + L.eps[a] * ty / t2;   // eps/conj(t) = eps t/|t|^2
-                double detJ, resid, gx, gy;
-                bool ok = polish_image<N>(L, wx, wy, zx, zy, 12, 1e-13, detJ, resid, gx, gy);
-                if (ok) {
-                    double sc = ul_max(1.0, zx * zx + zy * zy);
-                    for (int q = 0; q < n_img; ++q) {
-                        double ddx = zx - ix[q], ddy = zy - iy[q];
-                        if (ddx * ddx + ddy * ddy < 1e-18 * sc) ok = false;
-                    }
-                }
-                if (!ok) continue;
-                // put it in the non-image slot nearest to it
-                int slot = -1; double bd = 1e300;
-#pragma unroll
-                for (int k = 0; k < DEG; ++k) {
-                    if (mask & (1u << k)) continue;
-                    double ddx = zr[k] - zx, ddy = zi[k] - zy, d = ddx * ddx + ddy * ddy;
-                    if (d < bd) { bd = d; slot = k; }
-                }
-                if (slot < 0) continue;
-                ix[n_img] = zx; iy[n_img] = zy; ++n_img; mask |= 1u << slot; zr[slot] = zx; zi[slot] = zy;
-            }
-        }
-    }
-    if (((n_img - (N + 1)) & 1) != 0 || n_img < N + 1) st |= UL_ST_IMG_PARITY;
-    st |= (unsigned)(n_img & 0xf) << 8;
+    unsigned st = centre_images<N>(L, poly[c], wx, wy, zr, zi, mask);
     if (status) status[i] = st;
     if (out_re) {
 #pragma unroll
@@ -256,6 +189,7 @@ k_regions(int n, int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cf
     unsigned st = 0; int n_solves = 0;
     regions_phaseA<N>(lane, L, poly[c], wcx, wcy, rho, rp, W, st, n_solves);
     st = __reduce_or_sync(0xffffffffu, st);
+    const int tot_solves = __reduce_add_sync(0xffffffffu, n_solves);
     __syncwarp();
     regions_phaseB<DEG>(lane, W);
     __syncwarp();
@@ -269,7 +203,7 @@ k_regions(int n, int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cf
         for (int p = 0; p < np; ++p) { W.patch[p].unit0 = u; u += W.patch[p].n_units; patches[(long long)i * UL_MAXP + p] = W.patch[p]; }
         n_patch[i] = np;
         status[i] |= st;                                 // k_roots wrote the word first
-        atomicAdd(&ctr->n_limb_solves, (unsigned long long)(32 * (rp.n_limb / 32 + 1)));
+        atomicAdd(&ctr->n_limb_solves, (unsigned long long)tot_solves);
         atomicAdd(&ctr->n_patches, (unsigned long long)np);
     }
     np = __shfl_sync(0xffffffffu, np, 0);

@@ -110,7 +110,7 @@ UL_HD void lens_resid(const Lens& L, double zx, double zy, double wx, double wy,
 
 // Damped Newton on Eq. 1 itself (G7 "polish"): delta w = dz + g conj(dz)  =>  dz = (b - g conj(b))/(1 - |g|^2), b = -f.
 // The step is limited to half the distance to the nearest lens. Returns true when the final residual
-// is below tol * max(1, |z|); z is updated in place; detJ = 1 - |g|^2 (Eq. 3).
+// (or the last Newton step) is below tol * max(1, |z|); z is updated in place; detJ = 1 - |g|^2 (Eq. 3).
 template <int N>
 UL_HD bool polish_image(const Lens& L, double wx, double wy, double& zx, double& zy, int max_it,
                         double tol, double& detJ, double& resid, double& gx, double& gy)
@@ -135,6 +135,9 @@ UL_HD bool polish_image(const Lens& L, double wx, double wy, double& zx, double&
         double lim2 = 0.25 * dmin2;
         if (s2 > lim2) { double k = sqrt(lim2 / s2); sx *= k; sy *= k; }
         zx += sx; zy += sy;
+        // converged in POSITION: next to a light lens |g| ~ 1e5 and the rounding floor of the residual
+        // (~1e-16 |a| |g|) is far above tol although the image is located to ~1e-16
+        if (s2 <= tol * tol * scale * scale && resid <= 1e-6 * scale) { ok = true; break; }
     }
     return ok;
 }
@@ -340,6 +343,88 @@ UL_HD void match_roots(const double* ozr, const double* ozi, double* zr, double*
 #pragma unroll
         for (int j = 0; j < DEG; ++j) { zr[j] = nr[j]; zi[j] = ni[j]; }
     }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Step a2 for one source position: all N^2+1 roots (Eq. 4, Eq. 7), validated and polished on Eq. 1 (G7).
+// zr/zi: the roots (images polished); mask: which slots are images. Returns the status word
+// (UL_ST_EA_NOCONV, UL_ST_IMG_PARITY, image count << 8).
+// ------------------------------------------------------------------------------------------------
+template <int N>
+UL_HDN unsigned centre_images(const Lens& L, const LensPoly& T, double wx, double wy, double* zr, double* zi, unsigned& mask)
+{
+    constexpr int DEG = N * N + 1;
+    double br[DEG + 1], bi[DEG + 1];
+    poly_coeffs<N>(L, T, wx, wy, br, bi);
+    ea_init<DEG>(br, bi, zr, zi);
+    int it = ea_iterate<DEG>(br, bi, zr, zi, 100);
+    unsigned st = (it > 100) ? UL_ST_EA_NOCONV : 0u;
+    // validate + polish (G7): damped Newton on Eq. 1 from every root; accept converged, un-moved, distinct ones
+    double ix[DEG], iy[DEG];
+    int n_img = 0;
+    mask = 0;
+#pragma unroll
+    for (int k = 0; k < DEG; ++k) {
+        double zx = zr[k], zy = zi[k], detJ, resid, gx, gy;
+        double dm2 = 1e300;
+#pragma unroll
+        for (int a = 0; a < N; ++a) { double dx = zx - L.ax[a], dy = zy - L.ay[a]; dm2 = ul_min(dm2, dx * dx + dy * dy); }
+        bool ok = polish_image<N>(L, wx, wy, zx, zy, 8, 1e-13, detJ, resid, gx, gy);
+        double mv2 = (zx - zr[k]) * (zx - zr[k]) + (zy - zi[k]) * (zy - zi[k]);
+        ok = ok && (mv2 <= 0.01 * dm2);
+        if (ok) {
+            double sc = ul_max(1.0, zx * zx + zy * zy);
+            for (int q = 0; q < n_img; ++q) {
+                double ddx = zx - ix[q], ddy = zy - iy[q];
+                if (ddx * ddx + ddy * ddy < 1e-18 * sc) ok = false;
+            }
+        }
+        if (ok) { ix[n_img] = zx; iy[n_img] = zy; ++n_img; mask |= 1u << k; zr[k] = zx; zi[k] = zy; }
+    }
+    // An image count of the wrong parity almost always means the ultra-faint image next to a light
+    // lens was lost: it sits at z ~ a_i + eps_i / conj(a_i - w - sum_{j!=i} eps_j/conj(a_i - a_j)), inside
+    // the cluster of spurious roots around a_i that EA cannot resolve in double (degree 10). Seed it there.
+    if constexpr (N > 1) {
+        if (((n_img - (N + 1)) & 1) != 0 || n_img < N + 1) {
+#pragma unroll
+            for (int a = 0; a < N; ++a) {
+                double tx = L.ax[a] - wx, ty = L.ay[a] - wy;
+#pragma unroll
+                for (int b = 0; b < N; ++b) {
+                    if (b == a) continue;
+                    double dx = L.ax[a] - L.ax[b], dy = L.ay[a] - L.ay[b];
+                    double i2 = L.eps[b] / (dx * dx + dy * dy);
+                    tx -= dx * i2; ty -= dy * i2;               // eps_b / conj(d) = eps_b d / |d|^2
+                }
+                double t2 = tx * tx + ty * ty;
+                if (!(t2 > 0.0)) continue;
+                double zx = L.ax[a] + L.eps[a] * tx / t2, zy = L.ay[a] + L.eps[a] * ty / t2;   // eps/conj(t) = eps t/|t|^2
+                double detJ, resid, gx, gy;
+                bool ok = polish_image<N>(L, wx, wy, zx, zy, 12, 1e-13, detJ, resid, gx, gy);
+                if (ok) {
+                    double sc = ul_max(1.0, zx * zx + zy * zy);
+                    for (int q = 0; q < n_img; ++q) {
+                        double ddx = zx - ix[q], ddy = zy - iy[q];
+                        if (ddx * ddx + ddy * ddy < 1e-18 * sc) ok = false;
+                    }
+                }
+                if (!ok) continue;
+                // put it in the non-image slot nearest to it
+                int slot = -1; double bd = 1e300;
+#pragma unroll
+                for (int k = 0; k < DEG; ++k) {
+                    if (mask & (1u << k)) continue;
+                    double ddx = zr[k] - zx, ddy = zi[k] - zy, d = ddx * ddx + ddy * ddy;
+                    if (d < bd) { bd = d; slot = k; }
+                }
+                if (slot < 0) continue;
+                ix[n_img] = zx; iy[n_img] = zy; ++n_img; mask |= 1u << slot; zr[slot] = zx; zi[slot] = zy;
+            }
+        }
+    }
+    if (((n_img - (N + 1)) & 1) != 0 || n_img < N + 1) st |= UL_ST_IMG_PARITY;
+    st |= (unsigned)(n_img & 0xf) << 8;
+    return st;
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -109,28 +109,38 @@ UL_HDN void regions_phaseA(int lane, const Lens& L, const LensPoly& T, double wc
 #pragma unroll
     for (int j = 0; j < DEG; ++j) { B[j].r_lo = 1.0; B[j].r_hi = -1.0; B[j].t_lo = B[j].t_hi = 0.0; B[j].hr = B[j].ht = B[j].cr = B[j].ct = 1e300; t_cur[j] = 0.0; pvx[j] = pvy[j] = 0.0; }
 
+    // The lane walks its arc of the limb, phi in [phi0, phi0 + chunk dphi], with an ADAPTIVE step: the base
+    // step is dphi = 2 pi / n_limb (Eq. 8); a step is halved and retried (down to dphi / 4096) when an image
+    // moved by more than ~4 % of its distance from the origin -- where the limb passes close to a lens or to a
+    // cusp the image boundary races along a long arc within a fraction of dphi and uniform limb sampling
+    // would leave most of that arc unsampled -- and (down to dphi / 8) when the set of images
+    // changed, which localises the creation / destruction of an image pair on a caustic.
     const double dphi = 2.0 * UL_PI / P.n_limb;
-    for (int s = 0; s <= chunk; ++s) {
-        int k = lane * chunk + s;                       // limb index; k = n_limb wraps to 0 (same point)
-        double ph = dphi * k;
-        double wx = wcx + rho * cos(ph), wy = wcy + rho * sin(ph);      // Eq. 8 (G2)
+    const double ph0 = dphi * (lane * chunk), ph_end = dphi * (lane * chunk + chunk);
+    double ph = ph0, step = dphi;
+    bool first = true;
+    int guard = 0;
+    while (first || ph < ph_end - 1e-9 * dphi) {
+        const int s = first ? 0 : 1;
+        double st_try = step;
+        if (ph + st_try > ph_end - 1e-9 * dphi) st_try = ph_end - ph;      // land exactly on the arc's end
+        const double ph_new = first ? ph0 : ph + st_try;
+        double wx = wcx + rho * cos(ph_new), wy = wcy + rho * sin(ph_new);      // Eq. 8 (G2)
         poly_coeffs<N>(L, T, wx, wy, br, bi);
         // limb solves only have to land in the basin of the Eq.-1 polish: relative step 1e-7
         int it;
-        bool cold = (s == 0);
-        if (s == 0) { ea_init<DEG>(br, bi, zr, zi); it = ea_iterate<DEG>(br, bi, zr, zi, 64, 1e-14); }
+        if (first) { ea_init<DEG>(br, bi, zr, zi); it = ea_iterate<DEG>(br, bi, zr, zi, 64, 1e-14); }
         else {
 #pragma unroll
             for (int j = 0; j < DEG; ++j) { ozr[j] = zr[j]; ozi[j] = zi[j]; }
             it = ea_iterate<DEG>(br, bi, zr, zi, 24, 1e-14);
-            if (it > 24) { cold = true; ea_init<DEG>(br, bi, zr, zi); it = ea_iterate<DEG>(br, bi, zr, zi, 64, 1e-14); if (it <= 64) it = 1; }
+            if (it > 24) { ea_init<DEG>(br, bi, zr, zi); it = ea_iterate<DEG>(br, bi, zr, zi, 64, 1e-14); if (it <= 64) it = 1; }
             match_roots<DEG>(ozr, ozi, zr, zi);          // slot j keeps following the same root
         }
         ++n_solves;
-        if ((s == 0 && it > 64) || (s > 0 && it > 24)) status |= UL_ST_EA_NOCONV;
-        (void)cold;
+        const bool noconv = (first && it > 64) || (!first && it > 24);
 
-        unsigned valid = 0;
+        unsigned valid = 0, faint = 0;
         double px[DEG], py[DEG], hrr[DEG], htt[DEG], crr[DEG], ctt[DEG];
 #pragma unroll
         for (int j = 0; j < DEG; ++j) {
@@ -147,12 +157,37 @@ UL_HDN void regions_phaseA(int lane, const Lens& L, const LensPoly& T, double wc
                 valid |= 1u << j;
                 zr[j] = zx; zi[j] = zy;                 // polished image = better warm start
                 local_extents(zx, zy, gx, gy, rho, hrr[j], htt[j], crr[j], ctt[j]);
+                // an image of magnification 1/|det J| < 1e-7 (the one sitting on top of a light lens) is
+                // tracked but gets no sector: at most N of them, i.e. < 3e-7 of A >= 1
+                if (fabs(detJ) > 1e7) faint |= 1u << j;
             } else { hrr[j] = htt[j] = crr[j] = ctt[j] = 1e300; }
         }
+        if (!first && ++guard < 4096) {
+            // largest image displacement over this step, relative to the image's distance from the origin
+            bool too_far = false;
+#pragma unroll
+            for (int j = 0; j < DEG; ++j) {
+                if (!(valid & valid_prev & (1u << j))) continue;
+                double dx = px[j] - pvx[j], dy = py[j] - pvy[j];
+                double z2 = px[j] * px[j] + py[j] * py[j];
+                if (dx * dx + dy * dy > 0.0016 * ul_max(z2, 0.04)) too_far = true;
+            }
+            const bool flipped = (valid != valid_prev);
+            if ((too_far && st_try > dphi * (1.0 / 4096.0)) || (flipped && st_try > dphi * 0.126)) {
+#pragma unroll
+                for (int j = 0; j < DEG; ++j) { zr[j] = ozr[j]; zi[j] = ozi[j]; }
+                step = 0.5 * st_try;
+                continue;                                 // retry from the previous point with half the step
+            }
+        }
+        if (noconv) status |= UL_ST_EA_NOCONV;
+#ifdef UL_DEBUG_PHASEA
+        if (lane == UL_DEBUG_PHASEA) { printf("lane %d ph %.6f step %.3g it %d valid %x:", lane, ph_new / dphi, st_try / dphi, it, valid); for (int j = 0; j < DEG; ++j) printf(" (%.6f,%.6f)", px[j], py[j]); printf("\n"); }
+#endif
         // own points
 #pragma unroll
         for (int j = 0; j < DEG; ++j)
-            if (valid & (1u << j))
+            if (valid & ~faint & (1u << j))
                 box_add(B[j], t_cur[j], sqrt(px[j] * px[j] + py[j] * py[j]), atan2(py[j], px[j]), hrr[j], htt[j], crr[j], ctt[j], true);
         // links: a slot that switched off (its last point) or on (its first point) between s-1 and s is one
         // half of an image pair destroyed / created on a critical curve somewhere between the two partners'
@@ -188,6 +223,8 @@ UL_HDN void regions_phaseA(int lane, const Lens& L, const LensPoly& T, double wc
 #pragma unroll
         for (int j = 0; j < DEG; ++j) { pvx[j] = px[j]; pvy[j] = py[j]; }
         valid_prev = valid;
+        if (!first) { ph = ph_new; step = ul_min(2.0 * st_try, dphi); }
+        first = false;
     }
     // normalise theta intervals: t_lo in [-pi, pi)
 #pragma unroll
@@ -237,7 +274,74 @@ UL_HDN void regions_phaseB(int lane, RegionWork<DEG>& W)
 }
 
 // ---------------------------------------------------------------------------------------------- phase C
+// One sector -> its ray grid (Sec. 3.3 "fixed-resolution polar grid"; spacing from the local image scale).
+// Scan lines (one per lane, 32 per work unit) are rings scanned along theta for a bounded sector and radial
+// lines scanned along r for a filled ring / disk, whose boundary runs along theta.
+//   [rl, rh] x [tl, th]   tight bounds of the member boxes (already expanded by the box margin)
+//   hr, ht / cr, ct       smallest projected half-extent / half-chord of the image along r / theta
+//   gap_*                 free space to the neighbouring group on each side: margins never use more than
+//                         45 % of it, so sectors stay disjoint
+UL_HD void emit_patch(Patch& out, const RegionParams& P, int point, double rl, double rh, double tl, double th,
+                      double hr_, double ht_, double cr_, double ct_, bool periodic, bool scan_r,
+                      double gap_r_lo, double gap_r_hi, double gap_t_lo, double gap_t_hi, int& units_left,
+                      unsigned& status)
+{
+    double r_ext = rh - rl;
+    double t_ext = periodic ? 2.0 * UL_PI : (th - tl);
+    // lines: spaced by the projected half-extent / n_r; nodes on a line: by the half-chord / n_theta
+    double hr = ul_min(scan_r ? cr_ : hr_, 0.5 * r_ext);
+    double ht = ul_min(scan_r ? ht_ : ct_, 0.5 * t_ext * rh);
+    int per_r = scan_r ? P.n_theta : P.n_r, per_t = scan_r ? P.n_r : P.n_theta;
+    double want_r = ceil(r_ext / hr * per_r);
+    double want_t = ceil(t_ext * rh / ht * per_t);
+    int n_r = want_r > (double)P.max_nr ? P.max_nr : (int)want_r;
+    int n_th = want_t > (double)P.max_nth ? P.max_nth : (int)want_t;
+    if (want_r > (double)P.max_nr || want_t > (double)P.max_nth) status |= UL_ST_RES_CAP;
+    if (n_th < 16) n_th = 16;
+    if (n_r < 16) n_r = 16;
+    double dth = t_ext / n_th;
+    if (!periodic) {
+        // 3 extra cells of margin per side (cubic stencil + empty border rays)
+        double e_lo = ul_min(3.0 * dth, 0.45 * gap_t_lo), e_hi = ul_min(3.0 * dth, 0.45 * gap_t_hi);
+        tl -= e_lo;
+        double span = t_ext + e_lo + e_hi;
+        n_th = (int)ceil(span / dth);
+        if (n_th > P.max_nth) { n_th = P.max_nth; status |= UL_ST_RES_CAP; }
+        dth = span / n_th;
+    }
+    double dr = r_ext / n_r;
+    double span_r;
+    {
+        double e_lo = ul_min(3.0 * dr, 0.45 * gap_r_lo), e_hi = ul_min(3.0 * dr, 0.45 * gap_r_hi);
+        if (rl <= 0.0) e_lo = 0.0;
+        rl -= e_lo;
+        span_r = r_ext + e_lo + e_hi;
+        n_r = (int)ceil(span_r / dr);
+        if (n_r > P.max_nr) { n_r = P.max_nr; status |= UL_ST_RES_CAP; }
+    }
+    // the line count is a multiple of 32 (one lane per line)
+    int n_units;
+    if (scan_r) { n_th = (n_th + 31) & ~31; n_units = n_th / 32; }
+    else { n_r = (n_r + 31) & ~31; n_units = n_r / 32; }
+    if (n_units > units_left) {                          // per-point unit budget
+        status |= UL_ST_RES_CAP;
+        n_units = units_left > 1 ? units_left : 1;
+        if (scan_r) n_th = 32 * n_units; else n_r = 32 * n_units;
+    }
+    units_left -= n_units;
+    if (units_left < 0) units_left = 0;
+    if (periodic) dth = 2.0 * UL_PI / n_th;
+    dr = span_r / n_r;
+    out.r0 = rl; out.dr = dr; out.th0 = tl; out.dth = dth; out.n_r = n_r; out.n_th = n_th;
+    out.point = point; out.unit0 = 0;
+    out.flags = (periodic ? UL_PATCH_PERIODIC : 0) | (scan_r ? UL_PATCH_SCAN_R : 0);
+    out.n_units = n_units;
+}
+
 // Returns the number of sectors (0 if no image-limb point was found).
+// The paper's "1-D binning in r and theta, all combinations, empty ones dropped" as interval sweeps:
+// boxes -> disjoint r-groups; inside each r-group its member boxes -> periodic theta-groups; every
+// (r-group, theta-group) is one sector with the tight bounds of its members.
 // The boxes only follow image BOUNDARIES. A circle r = const that lies in a gap between two r-groups (or
 // inside the innermost one) meets no boundary, so it is entirely inside or entirely outside the image:
 // one ray on it decides. Where it is inside (ring-like image around the origin, or a disk that contains
@@ -270,7 +374,6 @@ UL_HDN int regions_phaseC(RegionWork<N * N + 1>& W, const RegionParams& P, int p
     bool ring_group[UL_MAXG];
     {
         int m = 0;                                       // groups after merging
-        bool fill_prev = false;
         for (int g = 0; g < ngr; ++g) {
             double lo_edge = (g == 0) ? 0.0 : gr_hi[g - 1];
             bool fill = false;
@@ -285,116 +388,81 @@ UL_HDN int regions_phaseC(RegionWork<N * N + 1>& W, const RegionParams& P, int p
             } else {
                 gr_lo[m] = gr_lo[g]; gr_hi[m] = gr_hi[g]; ring_group[m] = false; ++m;
             }
-            fill_prev = fill;
         }
-        (void)fill_prev;
         ngr = m;
     }
-    // ---- theta groups (periodic)
-    double gt_lo[UL_MAXG], gt_hi[UL_MAXG];
-    int ngt = 0;
-    {
-        double cur_hi = -1e300;
-        for (int q = 0; q < nb; ++q) {
-            double rl, rh, tl, th;
-            box_expanded(W.box[W.order_t[q]], rl, rh, tl, th);
-            if (ngt == 0 || (tl > cur_hi && ngt < UL_MAXG)) { gt_lo[ngt] = tl; gt_hi[ngt] = th; cur_hi = th; ++ngt; }
-            else { cur_hi = ul_max(cur_hi, th); gt_hi[ngt - 1] = cur_hi; }
-        }
-        // wrap: the group reaching furthest past +pi swallows the leading groups it covers
-        for (;;) {
-            if (ngt <= 1) break;
-            int im = 0;
-            for (int g = 1; g < ngt; ++g) if (gt_hi[g] > gt_hi[im]) im = g;
-            if (im == 0 || gt_hi[im] - 2.0 * UL_PI < gt_lo[0]) break;
-            // merge group 0 into group im (shifted by 2 pi), drop group 0
-            gt_hi[im] = ul_max(gt_hi[im], gt_hi[0] + 2.0 * UL_PI);
-            for (int g = 1; g < ngt; ++g) { gt_lo[g - 1] = gt_lo[g]; gt_hi[g - 1] = gt_hi[g]; }
-            --ngt;
-        }
-        for (int g = 0; g < ngt; ++g) if (gt_hi[g] - gt_lo[g] >= 2.0 * UL_PI) { gt_lo[0] = -UL_PI; gt_hi[0] = UL_PI; ngt = 1; break; }
-    }
-    const bool full_ring_only = (ngt == 1 && gt_hi[0] - gt_lo[0] >= 2.0 * UL_PI - 1e-12);
 
-    // ---- occupied cells -> sectors (tight bbox of the members, expanded)
-    signed char cell[UL_MAXG][UL_MAXG];
-    for (int a = 0; a < UL_MAXG; ++a) for (int b = 0; b < UL_MAXG; ++b) cell[a][b] = -1;
-    double p_rl[UL_MAXP], p_rh[UL_MAXP], p_tl[UL_MAXP], p_th[UL_MAXP], p_hr[UL_MAXP], p_ht[UL_MAXP], p_cr[UL_MAXP], p_ct[UL_MAXP];
-    int p_gr[UL_MAXP], p_gt[UL_MAXP];
     int np = 0;
+    int units_left = P.max_units_pt;
     bool capped = false;
-    for (int i = 0; i < n; ++i) {
-        const SubBox& b = W.box[i];
-        if (b.r_lo > b.r_hi) continue;
-        double rl, rh, tl, th;
-        box_expanded(b, rl, rh, tl, th);
-        int a = 0;
-        for (int g = 0; g < ngr; ++g) if (rl >= gr_lo[g] && rl <= gr_hi[g]) { a = g; break; }
-        int c = 0;
-        if (ring_group[a]) { rl = gr_lo[a]; rh = gr_hi[a]; }
-        if (full_ring_only || ring_group[a]) { tl = -UL_PI; th = UL_PI; }
-        else {
-            bool found = false;
-            for (int g = 0; g < ngt && !found; ++g) {
-                if (tl >= gt_lo[g] && tl <= gt_hi[g]) { c = g; found = true; }
-                else if (tl + 2.0 * UL_PI >= gt_lo[g] && tl + 2.0 * UL_PI <= gt_hi[g]) { c = g; tl += 2.0 * UL_PI; th += 2.0 * UL_PI; found = true; }
+    for (int a = 0; a < ngr && !capped; ++a) {
+        const double gap_r_lo = (a == 0) ? gr_lo[0] : gr_lo[a] - gr_hi[a - 1];
+        const double gap_r_hi = (a == ngr - 1) ? 1e300 : gr_lo[a + 1] - gr_hi[a];
+        if (ring_group[a]) {
+            // filled ring / disk: one full-ring sector scanned along radial lines
+            double hr = 1e300, ht = 1e300, cr = 1e300, ct = 1e300;
+            for (int i = 0; i < n; ++i) {
+                const SubBox& b = W.box[i];
+                if (b.r_lo > b.r_hi) continue;
+                double rl, rh, tl, th;
+                box_expanded(b, rl, rh, tl, th);
+                if (!(rl >= gr_lo[a] && rl <= gr_hi[a])) continue;
+                hr = ul_min(hr, b.hr); ht = ul_min(ht, b.ht); cr = ul_min(cr, b.cr); ct = ul_min(ct, b.ct);
             }
+            if (np == UL_MAXP) { capped = true; break; }
+            emit_patch(W.patch[np++], P, point, gr_lo[a], gr_hi[a], -UL_PI, UL_PI, hr, ht, cr, ct, true, true,
+                       gap_r_lo, gap_r_hi, 0.0, 0.0, units_left, status);
+            continue;
         }
-        int p = cell[a][c];
-        if (p < 0) {
-            if (np == UL_MAXP) { capped = true; p = UL_MAXP - 1; }
-            else {
-                p = np++; cell[a][c] = (signed char)p;
-                p_rl[p] = rl; p_rh[p] = rh; p_tl[p] = tl; p_th[p] = th; p_hr[p] = b.hr; p_ht[p] = b.ht; p_cr[p] = b.cr; p_ct[p] = b.ct; p_gr[p] = a; p_gt[p] = c;
-                continue;
+        // ---- theta groups of this r-group's members (periodic)
+        double gt_lo[UL_MAXG], gt_hi[UL_MAXG];
+        int ngt = 0;
+        {
+            double cur_hi = -1e300;
+            for (int q = 0; q < nb; ++q) {
+                double rl, rh, tl, th;
+                box_expanded(W.box[W.order_t[q]], rl, rh, tl, th);
+                if (!(rl >= gr_lo[a] && rl <= gr_hi[a])) continue;
+                if (ngt == 0 || (tl > cur_hi && ngt < UL_MAXG)) { gt_lo[ngt] = tl; gt_hi[ngt] = th; cur_hi = th; ++ngt; }
+                else { cur_hi = ul_max(cur_hi, th); gt_hi[ngt - 1] = cur_hi; }
             }
+            // wrap: the group reaching furthest past +pi swallows the leading groups it covers
+            for (;;) {
+                if (ngt <= 1) break;
+                int im = 0;
+                for (int g = 1; g < ngt; ++g) if (gt_hi[g] > gt_hi[im]) im = g;
+                if (im == 0 || gt_hi[im] - 2.0 * UL_PI < gt_lo[0]) break;
+                gt_hi[im] = ul_max(gt_hi[im], gt_hi[0] + 2.0 * UL_PI);
+                for (int g = 1; g < ngt; ++g) { gt_lo[g - 1] = gt_lo[g]; gt_hi[g - 1] = gt_hi[g]; }
+                --ngt;
+            }
+            for (int g = 0; g < ngt; ++g) if (gt_hi[g] - gt_lo[g] >= 2.0 * UL_PI) { gt_lo[0] = -UL_PI; gt_hi[0] = UL_PI; ngt = 1; break; }
         }
-        p_rl[p] = ul_min(p_rl[p], rl); p_rh[p] = ul_max(p_rh[p], rh);
-        p_tl[p] = ul_min(p_tl[p], tl); p_th[p] = ul_max(p_th[p], th);
-        p_hr[p] = ul_min(p_hr[p], b.hr); p_ht[p] = ul_min(p_ht[p], b.ht);
-        p_cr[p] = ul_min(p_cr[p], b.cr); p_ct[p] = ul_min(p_ct[p], b.ct);
-    }
-    if (capped) {
-        // more sectors than the cap: one sector around everything (never drop an image)
-        status |= UL_ST_PATCH_CAP;
-        double rl = 1e300, rh = 0.0, hr = 1e300, ht = 1e300, cr = 1e300, ct = 1e300;
+        const bool full_ring = (ngt == 1 && gt_hi[0] - gt_lo[0] >= 2.0 * UL_PI - 1e-12);
+        // ---- tight bounds of each theta-group's members
+        double c_rl[UL_MAXG], c_rh[UL_MAXG], c_tl[UL_MAXG], c_th[UL_MAXG], c_hr[UL_MAXG], c_ht[UL_MAXG], c_cr[UL_MAXG], c_ct[UL_MAXG];
+        for (int g = 0; g < ngt; ++g) { c_rl[g] = 1e300; c_rh[g] = -1e300; c_tl[g] = 1e300; c_th[g] = -1e300; c_hr[g] = c_ht[g] = c_cr[g] = c_ct[g] = 1e300; }
         for (int i = 0; i < n; ++i) {
             const SubBox& b = W.box[i];
             if (b.r_lo > b.r_hi) continue;
-            double a1, a2, a3, a4; box_expanded(b, a1, a2, a3, a4);
-            rl = ul_min(rl, a1); rh = ul_max(rh, a2); hr = ul_min(hr, b.hr); ht = ul_min(ht, b.ht); cr = ul_min(cr, b.cr); ct = ul_min(ct, b.ct);
+            double rl, rh, tl, th;
+            box_expanded(b, rl, rh, tl, th);
+            if (!(rl >= gr_lo[a] && rl <= gr_hi[a])) continue;
+            int c = 0;
+            if (full_ring) { tl = -UL_PI; th = UL_PI; }
+            else {
+                for (int g = 0; g < ngt; ++g) {
+                    if (tl >= gt_lo[g] && tl <= gt_hi[g]) { c = g; break; }
+                    if (tl + 2.0 * UL_PI >= gt_lo[g] && tl + 2.0 * UL_PI <= gt_hi[g]) { c = g; tl += 2.0 * UL_PI; th += 2.0 * UL_PI; break; }
+                }
+            }
+            c_rl[c] = ul_min(c_rl[c], rl); c_rh[c] = ul_max(c_rh[c], rh);
+            c_tl[c] = ul_min(c_tl[c], tl); c_th[c] = ul_max(c_th[c], th);
+            c_hr[c] = ul_min(c_hr[c], b.hr); c_ht[c] = ul_min(c_ht[c], b.ht);
+            c_cr[c] = ul_min(c_cr[c], b.cr); c_ct[c] = ul_min(c_ct[c], b.ct);
         }
-        np = 1; p_rl[0] = rl; p_rh[0] = rh; p_tl[0] = -UL_PI; p_th[0] = UL_PI; p_hr[0] = hr; p_ht[0] = ht; p_cr[0] = cr; p_ct[0] = ct; p_gr[0] = 0; p_gt[0] = 0;
-        ngr = 1; gr_lo[0] = rl; gr_hi[0] = rh; ngt = 1; gt_lo[0] = -UL_PI; gt_hi[0] = UL_PI;
-    }
-
-    // ---- grid per sector. Scan lines (one per lane, 32 per work unit) are rings scanned along theta for a
-    // bounded sector (Sec. 3.3) and radial lines scanned along r for a filled ring / disk, whose boundary
-    // runs along theta: there the line integral is a smooth periodic function of theta.
-    int units_left = P.max_units_pt;
-    for (int p = 0; p < np; ++p) {
-        Patch& out = W.patch[p];
-        bool periodic = (p_th[p] - p_tl[p] >= 2.0 * UL_PI - 1e-12);
-        bool scan_r = periodic && ring_group[p_gr[p]];
-        double r_ext = p_rh[p] - p_rl[p];
-        double t_ext = periodic ? 2.0 * UL_PI : (p_th[p] - p_tl[p]);
-        // lines: spaced by the projected half-extent / n_r; nodes on a line: by the half-chord / n_theta
-        double hr = ul_min(scan_r ? p_cr[p] : p_hr[p], 0.5 * r_ext);
-        double ht = ul_min(scan_r ? p_ht[p] : p_ct[p], 0.5 * t_ext * p_rh[p]);
-        int per_r = scan_r ? P.n_theta : P.n_r, per_t = scan_r ? P.n_r : P.n_theta;
-        double want_r = ceil(r_ext / hr * per_r);
-        double want_t = ceil(t_ext * p_rh[p] / ht * per_t);
-        int n_r = want_r > (double)P.max_nr ? P.max_nr : (int)want_r;
-        int n_th = want_t > (double)P.max_nth ? P.max_nth : (int)want_t;
-        if (want_r > (double)P.max_nr || want_t > (double)P.max_nth) status |= UL_ST_RES_CAP;
-        if (n_th < 16) n_th = 16;
-        if (n_r < 16) n_r = 16;
-        double dth = t_ext / n_th;
-        double tl = p_tl[p];
-        if (!periodic) {
-            // 3 extra cells of margin per side (cubic stencil + empty border rays), but never more than
-            // 45 % of the gap to the neighbouring theta-group so that sectors stay disjoint
-            int c = p_gt[p];
+        for (int c = 0; c < ngt; ++c) {
+            if (c_rl[c] > c_rh[c]) continue;
             double gap_lo, gap_hi;
             if (ngt == 1) { gap_lo = gap_hi = 2.0 * UL_PI - (gt_hi[0] - gt_lo[0]); }
             else {
@@ -405,45 +473,24 @@ UL_HDN int regions_phaseC(RegionWork<N * N + 1>& W, const RegionParams& P, int p
                 gap_lo -= 2.0 * UL_PI * floor(gap_lo / (2.0 * UL_PI));
                 gap_hi -= 2.0 * UL_PI * floor(gap_hi / (2.0 * UL_PI));
             }
-            double e_lo = ul_min(3.0 * dth, 0.45 * gap_lo), e_hi = ul_min(3.0 * dth, 0.45 * gap_hi);
-            tl -= e_lo;
-            double span = t_ext + e_lo + e_hi;
-            n_th = (int)ceil(span / dth);
-            if (n_th > P.max_nth) { n_th = P.max_nth; status |= UL_ST_RES_CAP; }
-            dth = span / n_th;
+            if (np == UL_MAXP) { capped = true; break; }
+            emit_patch(W.patch[np++], P, point, c_rl[c], c_rh[c], c_tl[c], c_th[c], c_hr[c], c_ht[c], c_cr[c], c_ct[c],
+                       full_ring, false, gap_r_lo, gap_r_hi, gap_lo, gap_hi, units_left, status);
         }
-        // r: 3 extra cells of margin per side within 45 % of the gap to the neighbouring r-group
-        double dr = r_ext / n_r;
-        double rl = p_rl[p];
-        double span_r = r_ext;
-        {
-            int a = p_gr[p];
-            double gap_lo = (a == 0) ? gr_lo[0] : gr_lo[a] - gr_hi[a - 1];
-            double gap_hi = (a == ngr - 1) ? 1e300 : gr_lo[a + 1] - gr_hi[a];
-            double e_lo = ul_min(3.0 * dr, 0.45 * gap_lo), e_hi = ul_min(3.0 * dr, 0.45 * gap_hi);
-            if (p_rl[p] <= 0.0) e_lo = 0.0;
-            rl -= e_lo;
-            span_r = r_ext + e_lo + e_hi;
-            n_r = (int)ceil(span_r / dr);
-            if (n_r > P.max_nr) { n_r = P.max_nr; status |= UL_ST_RES_CAP; }
+    }
+    if (capped) {
+        // more sectors than the cap: one full-ring sector around everything (never drop an image)
+        status |= UL_ST_PATCH_CAP;
+        double rl = 1e300, rh = 0.0, hr = 1e300, ht = 1e300, cr = 1e300, ct = 1e300;
+        for (int i = 0; i < n; ++i) {
+            const SubBox& b = W.box[i];
+            if (b.r_lo > b.r_hi) continue;
+            double a1, a2, a3, a4; box_expanded(b, a1, a2, a3, a4);
+            rl = ul_min(rl, a1); rh = ul_max(rh, a2); hr = ul_min(hr, b.hr); ht = ul_min(ht, b.ht); cr = ul_min(cr, b.cr); ct = ul_min(ct, b.ct);
         }
-        // the line count is a multiple of 32 (one lane per line)
-        int n_units;
-        if (scan_r) { n_th = (n_th + 31) & ~31; n_units = n_th / 32; }
-        else { n_r = (n_r + 31) & ~31; n_units = n_r / 32; }
-        if (n_units > units_left) {                      // per-point unit budget
-            status |= UL_ST_RES_CAP;
-            n_units = units_left > 1 ? units_left : 1;
-            if (scan_r) n_th = 32 * n_units; else n_r = 32 * n_units;
-        }
-        units_left -= n_units;
-        if (units_left < 0) units_left = 0;
-        if (periodic) dth = 2.0 * UL_PI / n_th;
-        dr = span_r / n_r;
-        out.r0 = rl; out.dr = dr; out.th0 = tl; out.dth = dth; out.n_r = n_r; out.n_th = n_th;
-        out.point = point; out.unit0 = 0;
-        out.flags = (periodic ? UL_PATCH_PERIODIC : 0) | (scan_r ? UL_PATCH_SCAN_R : 0);
-        out.n_units = n_units;
+        np = 0; units_left = P.max_units_pt;
+        emit_patch(W.patch[np++], P, point, rl, rh, -UL_PI, UL_PI, hr, ht, cr, ct, true, false, rl, 1e300, 0.0, 0.0,
+                   units_left, status);
     }
     W.n_patch = np;
     return np;
