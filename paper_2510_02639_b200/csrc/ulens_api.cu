@@ -44,7 +44,9 @@ struct ulens_ctx {
     Patch* patches;             // [chunk][UL_MAXP]
     int* n_patch;               // [chunk]
     unsigned* status_ws;        // [chunk]
-    unsigned* unit_desc;        // [cap_units]  (patch slot << 8) | ring block
+    double* c_zr; double* c_zi; // [chunk][10] roots of the source centre (k_roots -> k_regions)
+    unsigned* c_mask;           // [chunk]     which of them are images
+    unsigned* unit_desc;        // [cap_units]  (patch slot << 11) | line block (< 2048)
     double* unit_sum;           // [cap_units]  all rings
     double* unit_odd;           // [cap_units]  odd rings only (half-resolution self-check)
     ChunkCounters* cc;
@@ -143,7 +145,8 @@ template <int N>
 __global__ void k_roots(int n, int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cfg,
                         const LensPoly* __restrict__ poly, const double* __restrict__ w_re,
                         const double* __restrict__ w_im, double* __restrict__ out_re, double* __restrict__ out_im,
-                        uint8_t* __restrict__ out_img, unsigned* __restrict__ status)
+                        uint8_t* __restrict__ out_img, unsigned* __restrict__ status,
+                        double* __restrict__ c_zr, double* __restrict__ c_zi, unsigned* __restrict__ c_mask)
 {
     constexpr int DEG = N * N + 1;
     int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -156,6 +159,11 @@ __global__ void k_roots(int n, int pt_base, int n_pts_per_cfg, const PointCfg* _
     unsigned mask = 0;
     unsigned st = centre_images<N>(L, poly[c], wx, wy, zr, zi, mask);
     if (status) status[i] = st;
+    if (c_zr) {
+#pragma unroll
+        for (int k = 0; k < DEG; ++k) { c_zr[(long long)i * 10 + k] = zr[k]; c_zi[(long long)i * 10 + k] = zi[k]; }
+        c_mask[i] = mask;
+    }
     if (out_re) {
 #pragma unroll
         for (int k = 0; k < DEG; ++k) {
@@ -172,7 +180,8 @@ __global__ void __launch_bounds__(128)
 k_regions(int n, int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cfg, const LensPoly* __restrict__ poly,
           const double* __restrict__ w_re, const double* __restrict__ w_im, RegionParams rp,
           Patch* __restrict__ patches, int* __restrict__ n_patch, unsigned* __restrict__ status,
-          unsigned* __restrict__ unit_desc, unsigned cap_units, ChunkCounters* cc, DevCounters* ctr)
+          unsigned* __restrict__ unit_desc, unsigned cap_units, ChunkCounters* cc, DevCounters* ctr,
+          const double* __restrict__ c_zr, const double* __restrict__ c_zi, const unsigned* __restrict__ c_mask)
 {
     constexpr int DEG = N * N + 1;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -187,7 +196,7 @@ k_regions(int n, int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cf
     double rho = cfg[c].rho;
     double wcx = w_re[gp], wcy = w_im[gp];
     unsigned st = 0; int n_solves = 0;
-    regions_phaseA<N>(lane, L, poly[c], wcx, wcy, rho, rp, W, st, n_solves);
+    regions_phaseA<N>(lane, L, poly[c], wcx, wcy, rho, rp, W, st, n_solves, c_zr + (long long)i * 10, c_zi + (long long)i * 10, c_mask[i]);
     st = __reduce_or_sync(0xffffffffu, st);
     const int tot_solves = __reduce_add_sync(0xffffffffu, n_solves);
     __syncwarp();
@@ -210,7 +219,7 @@ k_regions(int n, int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cf
     __syncwarp();
     for (int p = 0; p < np; ++p) {
         int nu = W.patch[p].n_units, u0 = W.patch[p].unit0;
-        for (int b = lane; b < nu; b += 32) unit_desc[u0 + b] = ((unsigned)(i * UL_MAXP + p) << 8) | (unsigned)b;
+        for (int b = lane; b < nu; b += 32) unit_desc[u0 + b] = ((unsigned)(i * UL_MAXP + p) << 11) | (unsigned)b;
     }
 }
 
@@ -220,10 +229,10 @@ __global__ void __launch_bounds__(128)
 k_shoot(int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cfg, const double* __restrict__ w_re,
         const double* __restrict__ w_im, const Patch* __restrict__ patches, const unsigned* __restrict__ unit_desc,
         double* __restrict__ unit_sum, double* __restrict__ unit_odd, unsigned* __restrict__ status,
-        ChunkCounters* cc, DevCounters* ctr)
+        ChunkCounters* cc, DevCounters* ctr, unsigned cap_units)
 {
     const int lane = threadIdx.x & 31;
-    const unsigned n_units = cc->n_units;
+    const unsigned n_units = min(cc->n_units, cap_units);       // an overflowing point allocated nothing (UL_ST_UNIT_OVF)
     unsigned long long rays = 0;
     for (;;) {
         unsigned u = 0;
@@ -231,8 +240,8 @@ k_shoot(int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cfg, const 
         u = __shfl_sync(0xffffffffu, u, 0);
         if (u >= n_units) break;
         unsigned d = unit_desc[u];
-        const Patch P = patches[d >> 8];
-        int blk = (int)(d & 0xffu);
+        const Patch P = patches[d >> 11];
+        int blk = (int)(d & 0x7ffu);
         long long gp = (long long)pt_base + P.point;
         int c = (int)(gp / n_pts_per_cfg);
         Lens L = cfg[c].lens;
@@ -245,7 +254,7 @@ k_shoot(int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cfg, const 
             double th = P.th0 + (line + 0.5) * P.dth;
             shoot_col<N, LD>(L, wcx, wcy, rho * rho, th, P.r0, P.dr, P.n_r, U, S, edge);
             f = ((1.0 - u1) * U + (LD ? (u1 / rho) * S : 0.0)) * P.dth;
-            clipped = edge;
+            clipped = edge || (!(P.flags & UL_PATCH_PERIODIC) && (line < 1 || line >= P.n_th - 1) && U > 0.0);
         } else {
             double r = P.r0 + (line + 0.5) * P.dr;
             bool periodic = (P.flags & UL_PATCH_PERIODIC) != 0;
@@ -357,7 +366,7 @@ extern "C" int ulens_create(ulens_ctx** out, int cuda_device, const ulens_option
     if (o.n_theta <= 0) o.n_theta = 48;
     if (!(o.rel_tol > 0.0)) o.rel_tol = 1e-4;
     if (o.chunk_pts <= 0) o.chunk_pts = 65536;
-    if (o.chunk_pts > (1 << 24) / UL_MAXP) o.chunk_pts = (1 << 24) / UL_MAXP;
+    if (o.chunk_pts > (1 << 21) / UL_MAXP) o.chunk_pts = (1 << 21) / UL_MAXP;
     ctx->opt = o;
     ctx->rp.n_limb = o.n_limb; ctx->rp.n_r = o.n_r; ctx->rp.n_theta = o.n_theta;
     ctx->rp.max_nr = 8192; ctx->rp.max_nth = 32768; ctx->rp.max_units_pt = 1024;
@@ -368,6 +377,9 @@ extern "C" int ulens_create(ulens_ctx** out, int cuda_device, const ulens_option
     if (e == cudaSuccess) e = cudaMalloc(&ctx->patches, sizeof(Patch) * UL_MAXP * (size_t)ctx->chunk);
     if (e == cudaSuccess) e = cudaMalloc(&ctx->n_patch, sizeof(int) * (size_t)ctx->chunk);
     if (e == cudaSuccess) e = cudaMalloc(&ctx->status_ws, sizeof(unsigned) * (size_t)ctx->chunk);
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->c_zr, sizeof(double) * 10 * (size_t)ctx->chunk);
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->c_zi, sizeof(double) * 10 * (size_t)ctx->chunk);
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->c_mask, sizeof(unsigned) * (size_t)ctx->chunk);
     if (e == cudaSuccess) e = cudaMalloc(&ctx->unit_desc, sizeof(unsigned) * ctx->cap_units);
     if (e == cudaSuccess) e = cudaMalloc(&ctx->unit_sum, sizeof(double) * ctx->cap_units);
     if (e == cudaSuccess) e = cudaMalloc(&ctx->unit_odd, sizeof(double) * ctx->cap_units);
@@ -384,6 +396,7 @@ extern "C" void ulens_destroy(ulens_ctx* ctx)
     if (!ctx) return;
     cudaSetDevice(ctx->device);
     cudaDeviceSynchronize();
+    cudaFree(ctx->c_zr); cudaFree(ctx->c_zi); cudaFree(ctx->c_mask);
     cudaFree(ctx->patches); cudaFree(ctx->n_patch); cudaFree(ctx->status_ws); cudaFree(ctx->unit_desc);
     cudaFree(ctx->unit_sum); cudaFree(ctx->unit_odd); cudaFree(ctx->cc); cudaFree(ctx->counters);
     cudaFree(ctx->cfg_dev); cudaFree(ctx->poly_dev); cudaFree(ctx->traj_w); cudaFree(ctx->io_buf);
@@ -449,23 +462,23 @@ static int run_chunks(ulens_ctx* ctx, long long n_total, int n_pts, bool ld, con
         {
             KTimer kt(ctx, ULENS_K_ROOTS, st);
             k_roots<N><<<(n + 127) / 128, 128, 0, st>>>(n, (int)base, n_pts, ctx->cfg_dev, ctx->poly_dev, w_re, w_im,
-                                                        nullptr, nullptr, nullptr, ctx->status_ws);
+                                                        nullptr, nullptr, nullptr, ctx->status_ws, ctx->c_zr, ctx->c_zi, ctx->c_mask);
         }
         {
             KTimer kt(ctx, ULENS_K_REGIONS, st);
             k_regions<N><<<(n + 3) / 4, 128, smem, st>>>(n, (int)base, n_pts, ctx->cfg_dev, ctx->poly_dev, w_re, w_im, ctx->rp,
                                                          ctx->patches, ctx->n_patch, ctx->status_ws, ctx->unit_desc,
-                                                         (unsigned)ctx->cap_units, ctx->cc, ctx->counters);
+                                                         (unsigned)ctx->cap_units, ctx->cc, ctx->counters, ctx->c_zr, ctx->c_zi, ctx->c_mask);
         }
         int grid = sm_count * 4;
         {
             KTimer kt(ctx, ULENS_K_SHOOT, st);
             if (ld)
                 k_shoot<N, true><<<grid, 128, 0, st>>>((int)base, n_pts, ctx->cfg_dev, w_re, w_im, ctx->patches, ctx->unit_desc,
-                                                       ctx->unit_sum, ctx->unit_odd, ctx->status_ws, ctx->cc, ctx->counters);
+                                                       ctx->unit_sum, ctx->unit_odd, ctx->status_ws, ctx->cc, ctx->counters, (unsigned)ctx->cap_units);
             else
                 k_shoot<N, false><<<grid, 128, 0, st>>>((int)base, n_pts, ctx->cfg_dev, w_re, w_im, ctx->patches, ctx->unit_desc,
-                                                        ctx->unit_sum, ctx->unit_odd, ctx->status_ws, ctx->cc, ctx->counters);
+                                                        ctx->unit_sum, ctx->unit_odd, ctx->status_ws, ctx->cc, ctx->counters, (unsigned)ctx->cap_units);
         }
         {
             KTimer kt(ctx, ULENS_K_FINALIZE, st);
@@ -591,9 +604,9 @@ extern "C" int ulens_roots(ulens_ctx* ctx, const ulens_lens* lens_host, int n_pt
     if (rc != ULENS_OK) return rc;
     int grid = (n_pts + 127) / 128;
     switch (N) {
-        case 1: k_roots<1><<<grid, 128, 0, st>>>(n_pts, 0, n_pts, ctx->cfg_dev, ctx->poly_dev, w_re, w_im, roots_re, roots_im, is_image, nullptr); break;
-        case 2: k_roots<2><<<grid, 128, 0, st>>>(n_pts, 0, n_pts, ctx->cfg_dev, ctx->poly_dev, w_re, w_im, roots_re, roots_im, is_image, nullptr); break;
-        default: k_roots<3><<<grid, 128, 0, st>>>(n_pts, 0, n_pts, ctx->cfg_dev, ctx->poly_dev, w_re, w_im, roots_re, roots_im, is_image, nullptr); break;
+        case 1: k_roots<1><<<grid, 128, 0, st>>>(n_pts, 0, n_pts, ctx->cfg_dev, ctx->poly_dev, w_re, w_im, roots_re, roots_im, is_image, nullptr, nullptr, nullptr, nullptr); break;
+        case 2: k_roots<2><<<grid, 128, 0, st>>>(n_pts, 0, n_pts, ctx->cfg_dev, ctx->poly_dev, w_re, w_im, roots_re, roots_im, is_image, nullptr, nullptr, nullptr, nullptr); break;
+        default: k_roots<3><<<grid, 128, 0, st>>>(n_pts, 0, n_pts, ctx->cfg_dev, ctx->poly_dev, w_re, w_im, roots_re, roots_im, is_image, nullptr, nullptr, nullptr, nullptr); break;
     }
     ctx->last_launches = 1;
     CK(cudaGetLastError());

@@ -369,9 +369,10 @@ UL_HDN unsigned centre_images(const Lens& L, const LensPoly& T, double wx, doubl
         double dm2 = 1e300;
 #pragma unroll
         for (int a = 0; a < N; ++a) { double dx = zx - L.ax[a], dy = zy - L.ay[a]; dm2 = ul_min(dm2, dx * dx + dy * dy); }
-        bool ok = polish_image<N>(L, wx, wy, zx, zy, 8, 1e-13, detJ, resid, gx, gy);
-        double mv2 = (zx - zr[k]) * (zx - zr[k]) + (zy - zi[k]) * (zy - zi[k]);
-        ok = ok && (mv2 <= 0.01 * dm2);
+        // a polish that converges IS an image wherever it started (Eq. 1 is the definition); starts
+        // from spurious roots may land on an image already found: the duplicate test below drops those
+        bool ok = polish_image<N>(L, wx, wy, zx, zy, 16, 1e-13, detJ, resid, gx, gy);
+        (void)dm2;
         if (ok) {
             double sc = ul_max(1.0, zx * zx + zy * zy);
             for (int q = 0; q < n_img; ++q) {

@@ -97,15 +97,20 @@ UL_HD void local_extents(double zx, double zy, double gx, double gy, double rho,
 // ---------------------------------------------------------------------------------------------- phase A
 template <int N>
 UL_HDN void regions_phaseA(int lane, const Lens& L, const LensPoly& T, double wcx, double wcy, double rho,
-                           const RegionParams& P, RegionWork<N * N + 1>& W, unsigned& status, int& n_solves)
+                           const RegionParams& P, RegionWork<N * N + 1>& W, unsigned& status, int& n_solves,
+                           const double* czr, const double* czi, unsigned cmask)
 {
     constexpr int DEG = N * N + 1;
     const int chunk = P.n_limb / 32;
     SubBox* B = &W.box[lane * DEG];
-    double t_cur[DEG];
+    double t_cur[DEG];              // per BOX: unwrapped theta of its last point
+    double lastx[DEG], lasty[DEG];  // per BOX: its last point
+    int bmap[DEG];                  // slot -> the box that slot's current arc writes to
+#pragma unroll
+    for (int j = 0; j < DEG; ++j) { bmap[j] = -1; lastx[j] = lasty[j] = 0.0; }
     double zr[DEG], zi[DEG], ozr[DEG], ozi[DEG], pvx[DEG], pvy[DEG];
     double br[DEG + 1], bi[DEG + 1];
-    unsigned valid_prev = 0;
+    unsigned valid_prev = 0, faint_prev = 0;
 #pragma unroll
     for (int j = 0; j < DEG; ++j) { B[j].r_lo = 1.0; B[j].r_hi = -1.0; B[j].t_lo = B[j].t_hi = 0.0; B[j].hr = B[j].ht = B[j].cr = B[j].ct = 1e300; t_cur[j] = 0.0; pvx[j] = pvy[j] = 0.0; }
 
@@ -149,9 +154,28 @@ UL_HDN void regions_phaseA(int lane, const Lens& L, const LensPoly& T, double wc
             double dm2 = 1e300;
 #pragma unroll
             for (int i = 0; i < N; ++i) { double dx = zx - L.ax[i], dy = zy - L.ay[i]; dm2 = ul_min(dm2, dx * dx + dy * dy); }
-            bool ok = polish_image<N>(L, wx, wy, zx, zy, 4, 1e-9, detJ, resid, gx, gy);
+            bool ok = polish_image<N>(L, wx, wy, zx, zy, 6, 1e-9, detJ, resid, gx, gy);
+            // along the limb a slot must follow ONE image continuously: a polish that carries the EA root
+            // further than 10 % of its distance to the nearest lens has jumped to some other image
             double mv2 = (zx - zr[j]) * (zx - zr[j]) + (zy - zi[j]) * (zy - zi[j]);
             ok = ok && (mv2 <= 0.01 * dm2);
+            // continuation: a slot that held an image at the previous limb point and lost it (EA cannot
+            // resolve the root clusters next to a light lens in double) is re-polished from that image
+            if (!ok && (valid_prev & (1u << j))) {
+                zx = pvx[j]; zy = pvy[j];
+                ok = polish_image<N>(L, wx, wy, zx, zy, 10, 1e-9, detJ, resid, gx, gy);
+                double jx = zx - pvx[j], jy = zy - pvy[j];
+                ok = ok && (jx * jx + jy * jy <= 0.0016 * ul_max(zx * zx + zy * zy, 0.04));
+            }
+            // two slots on one image: the later one is not an image of its own
+            if (ok) {
+#pragma unroll
+                for (int q = 0; q < DEG; ++q) {
+                    if (q >= j || !(valid & (1u << q))) continue;
+                    double ddx = zx - px[q], ddy = zy - py[q];
+                    if (ddx * ddx + ddy * ddy < 1e-10 * ul_max(1.0, zx * zx + zy * zy)) ok = false;
+                }
+            }
             px[j] = zx; py[j] = zy;
             if (ok) {
                 valid |= 1u << j;
@@ -162,12 +186,38 @@ UL_HDN void regions_phaseA(int lane, const Lens& L, const LensPoly& T, double wc
                 if (fabs(detJ) > 1e7) faint |= 1u << j;
             } else { hrr[j] = htt[j] = crr[j] = ctt[j] = 1e300; }
         }
+        if (first) {
+            // seed the arc's first point from the images of the source CENTRE (step a2, found with an
+            // unrestricted polish, duplicates removed, faint images seeded): damped Newton on Eq. 1 for this
+            // limb point from each of them. Whatever it converges to is an image of the limb point; if no
+            // slot holds it yet it takes a free one.
+#pragma unroll
+            for (int m = 0; m < DEG; ++m) {
+                if (!(cmask & (1u << m))) continue;
+                double zx = czr[m], zy = czi[m], detJ, resid, gx, gy;
+                if (!polish_image<N>(L, wx, wy, zx, zy, 12, 1e-9, detJ, resid, gx, gy)) continue;
+                bool dup = false;
+                int free_slot = -1;
+#pragma unroll
+                for (int q = 0; q < DEG; ++q) {
+                    if (valid & (1u << q)) {
+                        double ddx = zx - px[q], ddy = zy - py[q];
+                        if (ddx * ddx + ddy * ddy < 1e-10 * ul_max(1.0, zx * zx + zy * zy)) dup = true;
+                    } else if (free_slot < 0) free_slot = q;
+                }
+                if (dup || free_slot < 0) continue;
+                const int q = free_slot;
+                valid |= 1u << q; px[q] = zx; py[q] = zy; zr[q] = zx; zi[q] = zy;
+                local_extents(zx, zy, gx, gy, rho, hrr[q], htt[q], crr[q], ctt[q]);
+                if (fabs(detJ) > 1e7) faint |= 1u << q;
+            }
+        }
         if (!first && ++guard < 4096) {
             // largest image displacement over this step, relative to the image's distance from the origin
             bool too_far = false;
 #pragma unroll
             for (int j = 0; j < DEG; ++j) {
-                if (!(valid & valid_prev & (1u << j))) continue;
+                if (!(valid & valid_prev & ~faint & (1u << j))) continue;
                 double dx = px[j] - pvx[j], dy = py[j] - pvy[j];
                 double z2 = px[j] * px[j] + py[j] * py[j];
                 if (dx * dx + dy * dy > 0.0016 * ul_max(z2, 0.04)) too_far = true;
@@ -186,9 +236,33 @@ UL_HDN void regions_phaseA(int lane, const Lens& L, const LensPoly& T, double wc
 #endif
         // own points
 #pragma unroll
-        for (int j = 0; j < DEG; ++j)
-            if (valid & ~faint & (1u << j))
-                box_add(B[j], t_cur[j], sqrt(px[j] * px[j] + py[j] * py[j]), atan2(py[j], px[j]), hrr[j], htt[j], crr[j], ctt[j], true);
+        for (int j = 0; j < DEG; ++j) {
+            if (!(valid & ~faint & (1u << j))) continue;
+            // A box holds ONE arc. If this slot's image is nowhere near the last point of its box (the slot
+            // swapped identity with another root, or lost its image and found a different one), its new
+            // arc goes to an unused box of this lane if there is one.
+            int bi = bmap[j];
+            const double far2 = 0.0036 * ul_max(px[j] * px[j] + py[j] * py[j], 0.04);
+            if (bi >= 0) {
+                double dx = px[j] - lastx[bi], dy = py[j] - lasty[bi];
+                if (dx * dx + dy * dy > far2) bi = -1;
+            }
+            if (bi < 0) {
+                // an empty box no slot writes to; failing that, the box whose last point is nearest
+                double bd = 1e300; int nearest = 0;
+                for (int b = 0; b < DEG && bi < 0; ++b) {
+                    bool in_use = false;
+                    for (int q = 0; q < DEG; ++q) in_use = in_use || (q != j && bmap[q] == b);
+                    if (B[b].r_lo > B[b].r_hi) { if (!in_use) bi = b; continue; }
+                    double dx = px[j] - lastx[b], dy = py[j] - lasty[b], d = dx * dx + dy * dy;
+                    if (d < bd) { bd = d; nearest = b; }
+                }
+                if (bi < 0) bi = nearest;
+                bmap[j] = bi;
+            }
+            box_add(B[bi], t_cur[bi], sqrt(px[j] * px[j] + py[j] * py[j]), atan2(py[j], px[j]), hrr[j], htt[j], crr[j], ctt[j], true);
+            lastx[bi] = px[j]; lasty[bi] = py[j];
+        }
         // links: a slot that switched off (its last point) or on (its first point) between s-1 and s is one
         // half of an image pair destroyed / created on a critical curve somewhere between the two partners'
         // end points: each partner's box takes the other's end point, so that the pair's boxes overlap.
@@ -202,11 +276,11 @@ UL_HDN void regions_phaseA(int lane, const Lens& L, const LensPoly& T, double wc
                 for (int a = 0; a < DEG; ++a) { ex[a] = (off & (1u << a)) ? pvx[a] : px[a]; ey[a] = (off & (1u << a)) ? pvy[a] : py[a]; }
 #pragma unroll
                 for (int a = 0; a < DEG; ++a) {
-                    if (!(grp & (1u << a))) continue;
+                    if (!(grp & ~(faint | faint_prev) & (1u << a))) continue;
                     int nb = -1; double bd = 0.25;
 #pragma unroll
                     for (int b = 0; b < DEG; ++b) {
-                        if (b == a || !(grp & (1u << b))) continue;
+                        if (b == a || !(grp & ~(faint | faint_prev) & (1u << b))) continue;
                         double dx = ex[a] - ex[b], dy = ey[a] - ey[b];
                         double d = dx * dx + dy * dy;
                         if (d < bd) { bd = d; nb = b; }
@@ -214,15 +288,15 @@ UL_HDN void regions_phaseA(int lane, const Lens& L, const LensPoly& T, double wc
                     if (nb >= 0) {
                         double ra = sqrt(ex[a] * ex[a] + ey[a] * ey[a]), ta = atan2(ey[a], ex[a]);
                         double rb = sqrt(ex[nb] * ex[nb] + ey[nb] * ey[nb]), tb = atan2(ey[nb], ex[nb]);
-                        box_add(B[nb], t_cur[nb], ra, ta, 1e300, 1e300, 1e300, 1e300, false);
-                        box_add(B[a], t_cur[a], rb, tb, 1e300, 1e300, 1e300, 1e300, false);
+                        if (bmap[nb] >= 0) box_add(B[bmap[nb]], t_cur[bmap[nb]], ra, ta, 1e300, 1e300, 1e300, 1e300, false);
+                        if (bmap[a] >= 0) box_add(B[bmap[a]], t_cur[bmap[a]], rb, tb, 1e300, 1e300, 1e300, 1e300, false);
                     }
                 }
             }
         }
 #pragma unroll
         for (int j = 0; j < DEG; ++j) { pvx[j] = px[j]; pvy[j] = py[j]; }
-        valid_prev = valid;
+        valid_prev = valid; faint_prev = faint;
         if (!first) { ph = ph_new; step = ul_min(2.0 * st_try, dphi); }
         first = false;
     }
@@ -474,8 +548,11 @@ UL_HDN int regions_phaseC(RegionWork<N * N + 1>& W, const RegionParams& P, int p
                 gap_hi -= 2.0 * UL_PI * floor(gap_hi / (2.0 * UL_PI));
             }
             if (np == UL_MAXP) { capped = true; break; }
+            // a sector that closes on itself in theta is cut by radial lines: the line integral is then a
+            // smooth periodic function of theta (spectral convergence of the midpoint rule across lines)
+            const bool scan_r = full_ring;
             emit_patch(W.patch[np++], P, point, c_rl[c], c_rh[c], c_tl[c], c_th[c], c_hr[c], c_ht[c], c_cr[c], c_ct[c],
-                       full_ring, false, gap_r_lo, gap_r_hi, gap_lo, gap_hi, units_left, status);
+                       full_ring, scan_r, gap_r_lo, gap_r_hi, gap_lo, gap_hi, units_left, status);
         }
     }
     if (capped) {
