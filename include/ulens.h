@@ -60,8 +60,8 @@ typedef struct ulens_ctx ulens_ctx;
 /* Tunables; a zeroed struct (or NULL) selects the defaults in brackets. */
 typedef struct {
     int    n_limb;        /* source-limb samples per point, multiple of 32 (Eq. 8: ~500) [512]   */
-    int    n_r;           /* rings per image half-extent in r (P:139 N_r)                        [384]   */
-    int    n_theta;       /* rays per image half-extent in theta (P:139 N_theta)                 [48]    */
+    int    n_r;           /* scan lines per image half-extent across the lines (P:139 N_r)       [96]    */
+    int    n_theta;       /* rays per image half-chord along a scan line (P:139 N_theta)         [48]    */
     double rel_tol;       /* self-check threshold for ULENS_ST_ERR_HIGH                          [1e-4]  */
     int    chunk_pts;     /* points processed per internal pass (workspace size)                 [65536] */
     int    flags;         /* reserved, 0 */
@@ -107,6 +107,15 @@ int  ulens_mag(ulens_ctx* ctx, int n_cfg, int n_pts,
                const ulens_lens* lenses_host, const double* rho_host, const double* u1_host,
                const double* w_re, const double* w_im,
                double* A_out, double* err_out, uint32_t* status_out, void* stream);
+
+/* (i') The same with forward-mode derivatives (Sec. 3.5) with respect to
+ * the intrinsic inputs: dA5_out device [n_cfg*n_pts][5] = dA/d(w_cx, w_cy, s, q, rho). The s and q columns
+ * are defined for binary lenses in the geometry of ulens_lens_binary (EUNSUPPORTED otherwise) and are zero
+ * for n_lens = 1; n_lens = 3 is EUNSUPPORTED in this build. */
+int  ulens_mag_grad(ulens_ctx* ctx, int n_cfg, int n_pts,
+               const ulens_lens* lenses_host, const double* rho_host, const double* u1_host,
+               const double* w_re, const double* w_im,
+               double* A_out, double* dA5_out, double* err_out, uint32_t* status_out, void* stream);
 
 /* Same with HOST arrays for w_re, w_im, A_out, err_out, status_out: copies in, computes, copies out and
  * synchronises the stream before returning (the end-to-end entry point). */

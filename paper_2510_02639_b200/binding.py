@@ -19,7 +19,7 @@ ST_CLIPPED, ST_UNIT_OVF, ST_ERR_HIGH, ST_NO_IMAGE = 0x10, 0x20, 0x40, 0x80
 ST_NIMG_SHIFT = 8
 KERNEL_NAMES = ["k_traj", "k_roots", "k_regions", "k_shoot", "k_finalize"]     # ULENS_K_* order
 
-EXPORTS = ["ulens_create", "ulens_destroy", "ulens_lens_binary", "ulens_lens_triple", "ulens_mag",
+EXPORTS = ["ulens_create", "ulens_destroy", "ulens_lens_binary", "ulens_lens_triple", "ulens_mag", "ulens_mag_grad",
            "ulens_mag_host", "ulens_lightcurve_binary", "ulens_roots", "ulens_get_stats",
            "ulens_reset_stats", "ulens_last_launch_count", "ulens_set_timing", "ulens_get_kernel_ms", "ulens_fp64_peak", "ulens_strerror",
            "ulens_last_cuda_error"]
@@ -61,6 +61,7 @@ def lib() -> C.CDLL:
         L.ulens_lens_binary.argtypes = [C.POINTER(ulens_lens), C.c_double, C.c_double]
         L.ulens_lens_triple.argtypes = [C.POINTER(ulens_lens)] + [C.c_double] * 5
         L.ulens_mag.argtypes = [vp, ip, ip, C.POINTER(ulens_lens), dp, dp, vp, vp, vp, vp, vp, vp]
+        L.ulens_mag_grad.argtypes = [vp, ip, ip, C.POINTER(ulens_lens), dp, dp, vp, vp, vp, vp, vp, vp, vp]
         L.ulens_mag_host.argtypes = [vp, ip, ip, C.POINTER(ulens_lens), dp, dp, vp, vp, vp, vp, vp, vp]
         L.ulens_lightcurve_binary.argtypes = [vp, ip, ip, dp, C.c_double, vp, vp, vp, vp, vp, vp]
         L.ulens_roots.argtypes = [vp, C.POINTER(ulens_lens), ip, vp, vp, vp, vp, vp, vp]
@@ -175,6 +176,23 @@ class Context:
                                _dev(A_out, torch.float64, n), _dev(err_out, torch.float64, n),
                                _dev(status_out, torch.int32, n), self._stream(stream)), self._h)
         return A_out, err_out, status_out
+
+    def ulens_mag_grad(self, lenses, rho, u1, w_re, w_im, stream=None):
+        """As ulens_mag, plus dA/d(w_cx, w_cy, s, q, rho): returns (A, dA5 [n_cfg, n_pts, 5], err, status)."""
+        torch = self._torch
+        n_cfg, arr, rho, u1 = self._cfg_arrays(lenses, rho, u1)
+        n_pts = w_re.numel() // max(n_cfg, 1)
+        n = n_cfg * n_pts
+        dev = w_re.device
+        A = torch.empty((n_cfg, n_pts), dtype=torch.float64, device=dev)
+        dA = torch.empty((n_cfg, n_pts, 5), dtype=torch.float64, device=dev)
+        err = torch.empty((n_cfg, n_pts), dtype=torch.float64, device=dev)
+        st = torch.empty((n_cfg, n_pts), dtype=torch.int32, device=dev)
+        _check(lib().ulens_mag_grad(self._h, n_cfg, n_pts, arr, _dptr(rho), _dptr(u1),
+                                    _dev(w_re, torch.float64, n), _dev(w_im, torch.float64, n),
+                                    _dev(A, torch.float64, n), _dev(dA, torch.float64, 5 * n),
+                                    _dev(err, torch.float64, n), _dev(st, torch.int32, n), self._stream(stream)), self._h)
+        return A, dA, err, st
 
     def ulens_mag_host(self, lenses, rho, u1, w_re, w_im, A=None, err=None, st=None, stream=None):
         """Host numpy arrays in / out (optionally caller-provided, e.g. views of pinned tensors); the

@@ -19,6 +19,7 @@
 #include "../../include/ulens.h"
 #include "ulens_core.cuh"
 #include "ulens_regions.cuh"
+#include "ulens_dual.cuh"
 #include "ulens_host.hpp"
 
 using namespace ulens;
@@ -46,6 +47,11 @@ struct ulens_ctx {
     unsigned* status_ws;        // [chunk]
     double* c_zr; double* c_zi; // [chunk][10] roots of the source centre (k_roots -> k_regions)
     unsigned* c_mask;           // [chunk]     which of them are images
+    // forward-mode variant (allocated on first use)
+    PatchTan* ptans;            // [chunk][UL_MAXP] tangents of the sectors' radial bounds
+    double* unit_tan;           // [cap_units][UL_NT] tangent sums of the units
+    double* grad5;              // [chunk][UL_NT] intrinsic gradient dA/d(w_cx, w_cy, s, q, rho)
+    TangentTable* tan_dev; size_t tan_cap;
     unsigned* unit_desc;        // [cap_units]  (patch slot << 11) | line block (< 2048)
     double* unit_sum;           // [cap_units]  all rings
     double* unit_odd;           // [cap_units]  odd rings only (half-resolution self-check)
@@ -181,15 +187,20 @@ k_regions(int n, int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cf
           const double* __restrict__ w_re, const double* __restrict__ w_im, RegionParams rp,
           Patch* __restrict__ patches, int* __restrict__ n_patch, unsigned* __restrict__ status,
           unsigned* __restrict__ unit_desc, unsigned cap_units, ChunkCounters* cc, DevCounters* ctr,
-          const double* __restrict__ c_zr, const double* __restrict__ c_zi, const unsigned* __restrict__ c_mask)
+          const double* __restrict__ c_zr, const double* __restrict__ c_zi, const unsigned* __restrict__ c_mask,
+          const TangentTable* __restrict__ tans, PatchTan* __restrict__ ptans)
 {
     constexpr int DEG = N * N + 1;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     RegionWork<DEG>* Wall = reinterpret_cast<RegionWork<DEG>*>(smem_raw);
+    // dual run: the boxes' extreme points live behind the per-warp work areas
+    BoxExt* ext_all = reinterpret_cast<BoxExt*>(smem_raw + (blockDim.x >> 5) * sizeof(RegionWork<DEG>));
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     int i = blockIdx.x * (blockDim.x >> 5) + warp;
     if (i >= n) return;                                  // whole warp leaves together
     RegionWork<DEG>& W = Wall[warp];
+    if (lane == 0) W.ext = tans ? ext_all + warp * 32 * DEG : nullptr;
+    __syncwarp();
     long long gp = (long long)pt_base + i;
     int c = (int)(gp / n_pts_per_cfg);
     Lens L = cfg[c].lens;
@@ -204,12 +215,12 @@ k_regions(int n, int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cf
     __syncwarp();
     int np = 0; unsigned base = 0; int total_units = 0;
     if (lane == 0) {
-        np = regions_phaseC<N>(W, rp, i, L, wcx, wcy, rho, st);
+        np = regions_phaseC<N>(W, rp, i, L, wcx, wcy, rho, st, tans ? &tans[c] : nullptr);
         for (int p = 0; p < np; ++p) total_units += W.patch[p].n_units;
         base = atomicAdd(&cc->n_units, (unsigned)total_units);
         if ((unsigned long long)base + total_units > cap_units) { st |= UL_ST_UNIT_OVF; np = 0; total_units = 0; }
         int u = base;
-        for (int p = 0; p < np; ++p) { W.patch[p].unit0 = u; u += W.patch[p].n_units; patches[(long long)i * UL_MAXP + p] = W.patch[p]; }
+        for (int p = 0; p < np; ++p) { W.patch[p].unit0 = u; u += W.patch[p].n_units; patches[(long long)i * UL_MAXP + p] = W.patch[p]; if (tans) ptans[(long long)i * UL_MAXP + p] = W.ptan[p]; }
         n_patch[i] = np;
         status[i] |= st;                                 // k_roots wrote the word first
         atomicAdd(&ctr->n_limb_solves, (unsigned long long)tot_solves);
@@ -251,15 +262,15 @@ k_shoot(int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cfg, const 
         double U, S, f; bool edge, clipped;
         // line flux: (1-u1) Int chi dA + (u1/rho) Int chi sqrt(-F) dA      (Eq. A6 split, G12)
         if (P.flags & UL_PATCH_SCAN_R) {
-            double th = P.th0 + (line + 0.5) * P.dth;
+            double th, wt; line_node(P.flags, P.n_th, line, P.th0, P.dth, th, wt);
             shoot_col<N, LD>(L, wcx, wcy, rho * rho, th, P.r0, P.dr, P.n_r, U, S, edge);
-            f = ((1.0 - u1) * U + (LD ? (u1 / rho) * S : 0.0)) * P.dth;
+            f = ((1.0 - u1) * U + (LD ? (u1 / rho) * S : 0.0)) * wt;
             clipped = edge || (!(P.flags & UL_PATCH_PERIODIC) && (line < 1 || line >= P.n_th - 1) && U > 0.0);
         } else {
-            double r = P.r0 + (line + 0.5) * P.dr;
+            double r, wr; line_node(P.flags, P.n_r, line, P.r0, P.dr, r, wr);
             bool periodic = (P.flags & UL_PATCH_PERIODIC) != 0;
             shoot_ring<N, LD>(L, wcx, wcy, rho * rho, r, P.th0, P.dth, P.n_th, periodic, U, S, edge);
-            f = r * ((1.0 - u1) * U + (LD ? (u1 / rho) * S : 0.0)) * P.dth * P.dr;
+            f = r * ((1.0 - u1) * U + (LD ? (u1 / rho) * S : 0.0)) * P.dth * wr;
             clipped = edge || ((line < 1 || line >= P.n_r - 1) && U > 0.0 && P.r0 > 0.0);
         }
         double tot = warp_sum(f);
@@ -313,6 +324,133 @@ __global__ void k_finalize(int n, int pt_base, int n_pts_per_cfg, const PointCfg
     if (st & 0xffu) atomicAdd(&ctr->n_flagged, 1ull);
 }
 
+// ------------------------------------------------------------------------------------------------ forward-mode variant (a8)
+
+// k_shoot with tangents: same unit queue, same lines; every quantity of the line rule is a dual number with
+// UL_NT tangents (ulens_dual.cuh). The sector's radial grid moves with the image: r0' = r_lo', dr' = (r_hi' - r_lo') / n_r.
+template <int N, bool LD>
+__global__ void __launch_bounds__(128)
+k_shoot_dual(int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cfg, const TangentTable* __restrict__ tans,
+             const double* __restrict__ w_re, const double* __restrict__ w_im, const Patch* __restrict__ patches,
+             const PatchTan* __restrict__ ptans, const unsigned* __restrict__ unit_desc, double* __restrict__ unit_sum,
+             double* __restrict__ unit_odd, double* __restrict__ unit_tan, unsigned* __restrict__ status,
+             ChunkCounters* cc, DevCounters* ctr, unsigned cap_units)
+{
+    const int lane = threadIdx.x & 31;
+    const unsigned n_units = min(cc->n_units, cap_units);
+    unsigned long long rays = 0;
+    for (;;) {
+        unsigned u = 0;
+        if (lane == 0) u = atomicAdd(&cc->next_unit, 1u);
+        u = __shfl_sync(0xffffffffu, u, 0);
+        if (u >= n_units) break;
+        unsigned d = unit_desc[u];
+        const Patch P = patches[d >> 11];
+        const PatchTan PT = ptans[d >> 11];
+        int blk = (int)(d & 0x7ffu);
+        long long gp = (long long)pt_base + P.point;
+        int c = (int)(gp / n_pts_per_cfg);
+        Lens L = cfg[c].lens;
+        const TangentTable& T = tans[c];
+        double rho = cfg[c].rho, u1 = cfg[c].u1;
+        double wcx = w_re[gp], wcy = w_im[gp];
+        int line = blk * 32 + lane;
+        // co-moving radial grid
+        D5 r0, dr;
+        r0.v = P.r0; dr.v = P.dr;
+#pragma unroll
+        for (int k = 0; k < UL_NT; ++k) { r0.d[k] = PT.rlo_dot[k]; dr.d[k] = (PT.rhi_dot[k] - PT.rlo_dot[k]) / P.n_r; }
+        D5 U, S, f; bool edge, clipped;
+        D5 rho_d = d5_const(rho);
+#pragma unroll
+        for (int k = 0; k < UL_NT; ++k) rho_d.d[k] = T.drho[k];
+        if (P.flags & UL_PATCH_SCAN_R) {
+            double th = P.th0 + (line + 0.5) * P.dth;
+            shoot_col_d<N, LD>(L, T, wcx, wcy, rho, th, r0, dr, P.n_r, U, S, edge);
+            f = U * (1.0 - u1);
+            if (LD) f += (S / rho_d) * u1;
+            f = f * P.dth;
+            clipped = edge || (!(P.flags & UL_PATCH_PERIODIC) && (line < 1 || line >= P.n_th - 1) && U.v > 0.0);
+        } else {
+            D5 r = r0 + dr * (line + 0.5);
+            bool periodic = (P.flags & UL_PATCH_PERIODIC) != 0;
+            shoot_ring_d<N, LD>(L, T, wcx, wcy, rho, r, P.th0, P.dth, P.n_th, periodic, U, S, edge);
+            f = U * (1.0 - u1);
+            if (LD) f += (S / rho_d) * u1;
+            f = r * f * dr * P.dth;
+            clipped = edge || ((line < 1 || line >= P.n_r - 1) && U.v > 0.0 && P.r0 > 0.0);
+        }
+        double tot = warp_sum(f.v);
+        double odd = warp_sum((lane & 1) ? f.v : 0.0);
+        double tk[UL_NT];
+#pragma unroll
+        for (int k = 0; k < UL_NT; ++k) tk[k] = warp_sum(f.d[k]);
+        unsigned any_clip = __ballot_sync(0xffffffffu, clipped);
+        if (lane == 0) {
+            unit_sum[u] = tot;
+            unit_odd[u] = 2.0 * odd;
+#pragma unroll
+            for (int k = 0; k < UL_NT; ++k) unit_tan[(size_t)u * UL_NT + k] = tk[k];
+            if (any_clip) atomicOr(&status[P.point], UL_ST_CLIPPED);
+            rays += 32ull * (unsigned long long)(((P.flags & UL_PATCH_SCAN_R) ? P.n_r : P.n_th) + 4);
+        }
+    }
+    if (lane == 0 && rays) atomicAdd(&ctr->n_rays, rays);
+}
+
+// per point: ordered sum of the units' tangents, normalisation A = flux / F0(rho) differentiated:
+//   dA/dp_k = (dflux_k - A dF0_k) / F0,  F0 = pi rho^2 (1 - u1/3)
+__global__ void k_finalize_dual(int n, int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cfg,
+                                const TangentTable* __restrict__ tans, const Patch* __restrict__ patches,
+                                const int* __restrict__ n_patch, const double* __restrict__ unit_sum,
+                                const double* __restrict__ unit_tan, double* __restrict__ grad5)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    long long gp = (long long)pt_base + i;
+    int c = (int)(gp / n_pts_per_cfg);
+    double rho = cfg[c].rho, u1 = cfg[c].u1;
+    double F0 = UL_PI * rho * rho * (1.0 - u1 / 3.0);
+    int np = n_patch[i];
+    double s = 0.0, tk[UL_NT];
+    for (int k = 0; k < UL_NT; ++k) tk[k] = 0.0;
+    for (int p = 0; p < np; ++p) {
+        const Patch& P = patches[(long long)i * UL_MAXP + p];
+        for (int b = 0; b < P.n_units; ++b) {
+            s += unit_sum[P.unit0 + b];
+            for (int k = 0; k < UL_NT; ++k) tk[k] += unit_tan[(size_t)(P.unit0 + b) * UL_NT + k];
+        }
+    }
+    double A = s / F0;
+    for (int k = 0; k < UL_NT; ++k) {
+        double dF0 = 2.0 * UL_PI * rho * (1.0 - u1 / 3.0) * tans[c].drho[k];
+        grad5[gp * UL_NT + k] = np ? (tk[k] - A * dF0) / F0 : nan("");
+    }
+}
+
+// chain rule through the trajectory (reading G3): (w_cx, w_cy, s, q, rho) -> (t0, u0, tE, s, q, rho, alpha)
+__global__ void k_chain7(int n_cfg, int n_ep, const double* __restrict__ theta, const double* __restrict__ t,
+                         const double* __restrict__ w_re, const double* __restrict__ w_im,
+                         const double* __restrict__ grad5, double* __restrict__ dA)
+{
+    long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= (long long)n_cfg * n_ep) return;
+    int c = (int)(i / n_ep), e = (int)(i % n_ep);
+    const double* th = theta + 7 * c;
+    double tE = th[2], tau = (t[e] - th[0]) / tE;
+    double ca = cos(th[6]), sa = sin(th[6]);
+    const double* g = grad5 + i * UL_NT;
+    double along = g[0] * ca + g[1] * sa;
+    double* o = dA + i * 7;
+    o[0] = -along / tE;
+    o[1] = -g[0] * sa + g[1] * ca;
+    o[2] = -tau * along / tE;
+    o[3] = g[2];
+    o[4] = g[3];
+    o[5] = g[4];
+    o[6] = -g[0] * w_im[i] + g[1] * w_re[i];
+}
+
 // FP64 FMA peak: 8 independent chains per thread
 __global__ void k_dfma_peak(int iters, double* out)
 {
@@ -362,7 +500,7 @@ extern "C" int ulens_create(ulens_ctx** out, int cuda_device, const ulens_option
     if (o.n_limb <= 0) o.n_limb = 512;
     o.n_limb = (o.n_limb + 31) & ~31;
     if (o.n_limb > 8192) o.n_limb = 8192;
-    if (o.n_r <= 0) o.n_r = 384;
+    if (o.n_r <= 0) o.n_r = 96;
     if (o.n_theta <= 0) o.n_theta = 48;
     if (!(o.rel_tol > 0.0)) o.rel_tol = 1e-4;
     if (o.chunk_pts <= 0) o.chunk_pts = 65536;
@@ -397,6 +535,7 @@ extern "C" void ulens_destroy(ulens_ctx* ctx)
     cudaSetDevice(ctx->device);
     cudaDeviceSynchronize();
     cudaFree(ctx->c_zr); cudaFree(ctx->c_zi); cudaFree(ctx->c_mask);
+    cudaFree(ctx->ptans); cudaFree(ctx->unit_tan); cudaFree(ctx->grad5); cudaFree(ctx->tan_dev);
     cudaFree(ctx->patches); cudaFree(ctx->n_patch); cudaFree(ctx->status_ws); cudaFree(ctx->unit_desc);
     cudaFree(ctx->unit_sum); cudaFree(ctx->unit_odd); cudaFree(ctx->cc); cudaFree(ctx->counters);
     cudaFree(ctx->cfg_dev); cudaFree(ctx->poly_dev); cudaFree(ctx->traj_w); cudaFree(ctx->io_buf);
@@ -449,10 +588,17 @@ static int upload_cfgs(ulens_ctx* ctx, int n_cfg, const ulens_lens* lenses, cons
 
 template <int N>
 static int run_chunks(ulens_ctx* ctx, long long n_total, int n_pts, bool ld, const double* w_re, const double* w_im,
-                      double* A_out, double* err_out, unsigned* status_out, cudaStream_t st)
+                      double* A_out, double* err_out, unsigned* status_out, cudaStream_t st, double* grad5_out = nullptr)
 {
     constexpr int DEG = N * N + 1;
-    const size_t smem = 4 * sizeof(RegionWork<DEG>);
+    const bool dual = grad5_out != nullptr;
+    const TangentTable* tans = dual ? ctx->tan_dev : nullptr;
+    if (dual && N == 3) return ULENS_EUNSUPPORTED;
+    if (dual && !ctx->ptans) {
+        if (cudaMalloc(&ctx->ptans, sizeof(PatchTan) * UL_MAXP * (size_t)ctx->chunk) != cudaSuccess) return ULENS_ENOMEM;
+        if (cudaMalloc(&ctx->unit_tan, sizeof(double) * UL_NT * ctx->cap_units) != cudaSuccess) return ULENS_ENOMEM;
+    }
+    const size_t smem = 4 * sizeof(RegionWork<DEG>) + (dual ? 4 * 32 * DEG * sizeof(BoxExt) : 0);
     CK(cudaFuncSetAttribute(k_regions<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int sm_count = 148;
     cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, ctx->device);
@@ -468,12 +614,23 @@ static int run_chunks(ulens_ctx* ctx, long long n_total, int n_pts, bool ld, con
             KTimer kt(ctx, ULENS_K_REGIONS, st);
             k_regions<N><<<(n + 3) / 4, 128, smem, st>>>(n, (int)base, n_pts, ctx->cfg_dev, ctx->poly_dev, w_re, w_im, ctx->rp,
                                                          ctx->patches, ctx->n_patch, ctx->status_ws, ctx->unit_desc,
-                                                         (unsigned)ctx->cap_units, ctx->cc, ctx->counters, ctx->c_zr, ctx->c_zi, ctx->c_mask);
+                                                         (unsigned)ctx->cap_units, ctx->cc, ctx->counters, ctx->c_zr, ctx->c_zi, ctx->c_mask, tans, ctx->ptans);
         }
         int grid = sm_count * 4;
         {
             KTimer kt(ctx, ULENS_K_SHOOT, st);
-            if (ld)
+            if constexpr (N < 3) {
+                if (dual && ld)
+                    k_shoot_dual<N, true><<<grid, 128, 0, st>>>((int)base, n_pts, ctx->cfg_dev, tans, w_re, w_im, ctx->patches, ctx->ptans,
+                                                                ctx->unit_desc, ctx->unit_sum, ctx->unit_odd, ctx->unit_tan, ctx->status_ws,
+                                                                ctx->cc, ctx->counters, (unsigned)ctx->cap_units);
+                else if (dual)
+                    k_shoot_dual<N, false><<<grid, 128, 0, st>>>((int)base, n_pts, ctx->cfg_dev, tans, w_re, w_im, ctx->patches, ctx->ptans,
+                                                                 ctx->unit_desc, ctx->unit_sum, ctx->unit_odd, ctx->unit_tan, ctx->status_ws,
+                                                                 ctx->cc, ctx->counters, (unsigned)ctx->cap_units);
+            }
+            if (dual) {}
+            else if (ld)
                 k_shoot<N, true><<<grid, 128, 0, st>>>((int)base, n_pts, ctx->cfg_dev, w_re, w_im, ctx->patches, ctx->unit_desc,
                                                        ctx->unit_sum, ctx->unit_odd, ctx->status_ws, ctx->cc, ctx->counters, (unsigned)ctx->cap_units);
             else
@@ -485,6 +642,11 @@ static int run_chunks(ulens_ctx* ctx, long long n_total, int n_pts, bool ld, con
             k_finalize<<<(n + 127) / 128, 128, 0, st>>>(n, (int)base, n_pts, ctx->cfg_dev, ctx->patches, ctx->n_patch,
                                                         ctx->unit_sum, ctx->unit_odd, ctx->status_ws, ctx->opt.rel_tol,
                                                         A_out, err_out, status_out, ctx->counters);
+            if (dual) {
+                k_finalize_dual<<<(n + 127) / 128, 128, 0, st>>>(n, (int)base, n_pts, ctx->cfg_dev, tans, ctx->patches, ctx->n_patch,
+                                                                 ctx->unit_sum, ctx->unit_tan, grad5_out);
+                ctx->last_launches += 1;
+            }
         }
         ctx->last_launches += 4;
         CK(cudaGetLastError());
@@ -492,20 +654,55 @@ static int run_chunks(ulens_ctx* ctx, long long n_total, int n_pts, bool ld, con
     return ULENS_OK;
 }
 
+// tangent tables of the UL_NT intrinsic directions (w_cx, w_cy, s, q, rho). The lens-parameter directions
+// exist for a binary in the geometry of ulens_lens_binary (G4): s = a_2 - a_1, q = eps_2 / eps_1.
+static int upload_tangents(ulens_ctx* ctx, int n_cfg, const ulens_lens* lenses, cudaStream_t st)
+{
+    std::vector<TangentTable> tt(n_cfg);
+    for (int c = 0; c < n_cfg; ++c) {
+        TangentTable& T = tt[c];
+        memset(&T, 0, sizeof T);
+        T.dwx[0] = 1.0; T.dwy[1] = 1.0; T.drho[4] = 1.0;
+        const ulens_lens& L = lenses[c];
+        if (L.n_lens == 2) {
+            double s = L.ax[1] - L.ax[0], q = L.eps[1] / L.eps[0];
+            if (L.ay[0] != 0.0 || L.ay[1] != 0.0 || fabs(L.eps[0] * L.ax[0] + L.eps[1] * L.ax[1]) > 1e-12 * (1.0 + fabs(s)))
+                return ULENS_EUNSUPPORTED;               // not the ulens_lens_binary geometry
+            double o = 1.0 / (1.0 + q);
+            T.dax[2][0] = -q * o; T.dax[2][1] = o;                       // d/ds
+            T.deps[3][0] = -o * o; T.deps[3][1] = o * o;                 // d/dq
+            T.dax[3][0] = -s * o * o; T.dax[3][1] = -s * o * o;
+        }
+    }
+    if ((size_t)n_cfg > ctx->tan_cap) {
+        cudaFree(ctx->tan_dev); ctx->tan_dev = nullptr; ctx->tan_cap = 0;
+        if (cudaMalloc(&ctx->tan_dev, sizeof(TangentTable) * ((size_t)n_cfg + 64)) != cudaSuccess) return ULENS_ENOMEM;
+        ctx->tan_cap = (size_t)n_cfg + 64;
+    }
+    CK(cudaMemcpyAsync(ctx->tan_dev, tt.data(), sizeof(TangentTable) * n_cfg, cudaMemcpyHostToDevice, st));
+    CK(cudaStreamSynchronize(st));
+    return ULENS_OK;
+}
+
 static int mag_device(ulens_ctx* ctx, int n_cfg, int n_pts, const ulens_lens* lenses, const double* rho, const double* u1,
                       const double* w_re, const double* w_im, double* A_out, double* err_out, unsigned* status_out,
-                      cudaStream_t st)
+                      cudaStream_t st, double* grad5_out = nullptr)
 {
     int N = 0; bool ld = false;
     int rc = upload_cfgs(ctx, n_cfg, lenses, rho, u1, st, &N, &ld);
     if (rc != ULENS_OK) return rc;
+    if (grad5_out) {
+        if (N == 3) return ULENS_EUNSUPPORTED;
+        rc = upload_tangents(ctx, n_cfg, lenses, st);
+        if (rc != ULENS_OK) return rc;
+    }
     long long n_total = (long long)n_cfg * n_pts;
     if (n_total > 0x7fffffffLL) return ULENS_EUNSUPPORTED;
     ctx->last_launches = 0;
     switch (N) {
-        case 1: rc = run_chunks<1>(ctx, n_total, n_pts, ld, w_re, w_im, A_out, err_out, status_out, st); break;
-        case 2: rc = run_chunks<2>(ctx, n_total, n_pts, ld, w_re, w_im, A_out, err_out, status_out, st); break;
-        default: rc = run_chunks<3>(ctx, n_total, n_pts, ld, w_re, w_im, A_out, err_out, status_out, st); break;
+        case 1: rc = run_chunks<1>(ctx, n_total, n_pts, ld, w_re, w_im, A_out, err_out, status_out, st, grad5_out); break;
+        case 2: rc = run_chunks<2>(ctx, n_total, n_pts, ld, w_re, w_im, A_out, err_out, status_out, st, grad5_out); break;
+        default: rc = run_chunks<3>(ctx, n_total, n_pts, ld, w_re, w_im, A_out, err_out, status_out, st, grad5_out); break;
     }
     return rc;
 }
@@ -520,6 +717,18 @@ extern "C" int ulens_mag(ulens_ctx* ctx, int n_cfg, int n_pts, const ulens_lens*
     CK(cudaSetDevice(ctx->device));
     return mag_device(ctx, n_cfg, n_pts, lenses_host, rho_host, u1_host, w_re, w_im, A_out, err_out, status_out,
                       (cudaStream_t)stream);
+}
+
+extern "C" int ulens_mag_grad(ulens_ctx* ctx, int n_cfg, int n_pts, const ulens_lens* lenses_host, const double* rho_host,
+                              const double* u1_host, const double* w_re, const double* w_im, double* A_out, double* dA5_out,
+                              double* err_out, uint32_t* status_out, void* stream)
+{
+    if (!ctx || n_cfg < 0 || n_pts < 0) return ULENS_EINVAL;
+    if (n_cfg == 0 || n_pts == 0) return ULENS_OK;
+    if (!lenses_host || !rho_host || !u1_host || !w_re || !w_im || !A_out || !dA5_out) return ULENS_EINVAL;
+    CK(cudaSetDevice(ctx->device));
+    return mag_device(ctx, n_cfg, n_pts, lenses_host, rho_host, u1_host, w_re, w_im, A_out, err_out, status_out,
+                      (cudaStream_t)stream, dA5_out);
 }
 
 extern "C" int ulens_mag_host(ulens_ctx* ctx, int n_cfg, int n_pts, const ulens_lens* lenses_host, const double* rho_host,
@@ -558,7 +767,6 @@ extern "C" int ulens_lightcurve_binary(ulens_ctx* ctx, int n_cfg, int n_epochs, 
     if (!ctx || n_cfg < 0 || n_epochs < 0) return ULENS_EINVAL;
     if (n_cfg == 0 || n_epochs == 0) return ULENS_OK;
     if (!theta_host || !t || !A_out || !(u1 >= 0.0 && u1 <= 1.0)) return ULENS_EINVAL;
-    if (dA_out) return ULENS_EUNSUPPORTED;               // forward-mode variant: not in this build yet
     CK(cudaSetDevice(ctx->device));
     cudaStream_t st = (cudaStream_t)stream;
     std::vector<ulens_lens> lenses(n_cfg);
@@ -572,21 +780,28 @@ extern "C" int ulens_lightcurve_binary(ulens_ctx* ctx, int n_cfg, int n_epochs, 
         rho[c] = th[5];
     }
     size_t n = (size_t)n_cfg * n_epochs;
-    size_t need = 2 * n + 7 * (size_t)n_cfg;
+    size_t need = 2 * n + 7 * (size_t)n_cfg + (dA_out ? UL_NT * n : 0);
     if (need > ctx->traj_cap) {
         cudaFree(ctx->traj_w); ctx->traj_w = nullptr; ctx->traj_cap = 0;
         if (cudaMalloc(&ctx->traj_w, sizeof(double) * need) != cudaSuccess) return ULENS_ENOMEM;
         ctx->traj_cap = need;
     }
     double* w_re = ctx->traj_w; double* w_im = w_re + n; double* th_dev = w_im + n;
+    double* g5 = dA_out ? th_dev + 7 * (size_t)n_cfg : nullptr;
     CK(cudaMemcpyAsync(th_dev, theta_host, sizeof(double) * 7 * n_cfg, cudaMemcpyHostToDevice, st));
     {
         KTimer kt(ctx, ULENS_K_TRAJ, st);
         k_traj<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(n_cfg, n_epochs, th_dev, t, w_re, w_im);
     }
     CK(cudaGetLastError());
-    int rc = mag_device(ctx, n_cfg, n_epochs, lenses.data(), rho.data(), u1v.data(), w_re, w_im, A_out, err_out, status_out, st);
+    int rc = mag_device(ctx, n_cfg, n_epochs, lenses.data(), rho.data(), u1v.data(), w_re, w_im, A_out, err_out, status_out, st, g5);
     ctx->last_launches += 1;
+    if (rc != ULENS_OK) return rc;
+    if (dA_out) {
+        k_chain7<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(n_cfg, n_epochs, th_dev, t, w_re, w_im, g5, dA_out);
+        ctx->last_launches += 1;
+        CK(cudaGetLastError());
+    }
     return rc;
 }
 

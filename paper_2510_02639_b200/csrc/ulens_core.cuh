@@ -56,12 +56,13 @@ struct Patch {
     int n_r, n_th;
     int point;           // global point index
     int unit0;           // first 32-ring work unit of this patch in the unit arrays
-    int flags;           // bit 0: periodic in theta (full ring); bit 1: scan lines are radial (lanes = theta)
+    int flags;           // UL_PATCH_*: periodic in theta (full ring); scan lines are radial (lanes = theta); sin-spaced rings
     int n_units;         // 32-line work units
 };
 
 #define UL_PATCH_PERIODIC 1
 #define UL_PATCH_SCAN_R 2
+#define UL_PATCH_SINR 4      // ring i of n_r at r_c + h sin(phi_i), phi_i = -pi/2 + (i + 1/2) pi / n_r, weight h cos(phi_i) pi / n_r
 
 // status bits (mirror include/ulens.h)
 #define UL_ST_EA_NOCONV  0x0001u
@@ -575,6 +576,21 @@ UL_HD void shoot_ring(const Lens& L, double wcx, double wcy, double rho2, double
         c = cn;
     }
     U_out = U; S_out = S;
+}
+
+// Scan line `line` of a sector: its coordinate across the lines (radius of a ring, or theta of a radial line)
+// and its quadrature weight. r0, dr describe the span [r0, r0 + n_r dr]; with UL_PATCH_SINR the rings sit at Chebyshev-like radii
+// r_c + h sin(phi) (midpoint rule in phi): where the span ends at the radial extremes of a convex image the
+// integrand chord(r) ~ sqrt((r - r_lo)(r_hi - r)) becomes smooth in phi and the rule converges spectrally
+// instead of like dr^1.5 (measured on the single-lens closed form in DESIGN.md).
+UL_HD void line_node(int flags, int n_r, int line, double r0, double dr, double& r, double& w)
+{
+    if (flags & UL_PATCH_SINR) {
+        double h = 0.5 * n_r * dr, ph = (line + 0.5) * (UL_PI / n_r);      // phi + pi/2
+        double s, c; s = sin(ph); c = cos(ph);
+        r = r0 + h * (1.0 - c);                                              // r_c - h cos(ph) = r_c + h sin(phi)
+        w = h * s * (UL_PI / n_r);
+    } else { r = r0 + (line + 0.5) * dr; w = dr; }
 }
 
 UL_HD bool en_dummy(double f1) { return !(f1 < 0.0); }

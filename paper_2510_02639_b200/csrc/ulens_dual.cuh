@@ -1,0 +1,280 @@
+// ulens_dual.cuh -- forward-mode (dual-number) variant of the ray-shooting integrator (step a8).
+//
+// PAPER.md Sec. 3.5: derivatives of the magnification by forward-mode differentiation THROUGH
+// the region construction and the quadrature. What is differentiated here is the discrete rule of
+// ulens_core.cuh with the inside flags piecewise constant:
+//   * the radial grid of a sector moves with the image: r0 and dr carry tangents obtained from the extreme
+//     image-limb points by implicit differentiation of Eq. 1 (P:163-175 uses the polynomial; the lens
+//     equation itself is better conditioned) -- without this the square-root behaviour of the chord
+//     length at the radial ends of an image ruins the derivative;
+//   * every ray carries dF/dp_k for the NT = 5 intrinsic directions p = (w_cx, w_cy, s, q, rho): grid motion
+//     + explicit dependence of Eq. 1 on the lens parameters + the source centre / radius;
+//   * the edge position from the cubic, the uniform weight u - 1/2 and the square-root end correction
+//     (Hurwitz zetas) are evaluated in dual arithmetic, so the edge-motion (Reynolds boundary) term is exact
+//     for the rule and the paper's sigmoid surrogate for the Heaviside function (Eq. 9) is not needed.
+#pragma once
+#include "ulens_core.cuh"
+
+namespace ulens {
+
+#define UL_NT 5          // tangent directions: w_cx, w_cy, s, q, rho
+
+// how the inputs of Eq. 1 / Eq. 5 move in each direction (filled on the host per configuration)
+struct TangentTable {
+    double dwx[UL_NT], dwy[UL_NT], drho[UL_NT];
+    double deps[UL_NT][3], dax[UL_NT][3], day[UL_NT][3];
+};
+
+struct D5 {
+    double v;
+    double d[UL_NT];
+};
+
+UL_HD D5 d5_const(double a) { D5 r; r.v = a; for (int k = 0; k < UL_NT; ++k) r.d[k] = 0.0; return r; }
+UL_HD D5 operator+(const D5& a, const D5& b) { D5 r; r.v = a.v + b.v; for (int k = 0; k < UL_NT; ++k) r.d[k] = a.d[k] + b.d[k]; return r; }
+UL_HD D5 operator-(const D5& a, const D5& b) { D5 r; r.v = a.v - b.v; for (int k = 0; k < UL_NT; ++k) r.d[k] = a.d[k] - b.d[k]; return r; }
+UL_HD D5 operator-(const D5& a) { D5 r; r.v = -a.v; for (int k = 0; k < UL_NT; ++k) r.d[k] = -a.d[k]; return r; }
+UL_HD D5 operator+(const D5& a, double b) { D5 r = a; r.v += b; return r; }
+UL_HD D5 operator-(const D5& a, double b) { D5 r = a; r.v -= b; return r; }
+UL_HD D5 operator+(double b, const D5& a) { D5 r = a; r.v += b; return r; }
+UL_HD D5 operator-(double b, const D5& a) { D5 r; r.v = b - a.v; for (int k = 0; k < UL_NT; ++k) r.d[k] = -a.d[k]; return r; }
+UL_HD D5 operator*(const D5& a, const D5& b) { D5 r; r.v = a.v * b.v; for (int k = 0; k < UL_NT; ++k) r.d[k] = a.d[k] * b.v + a.v * b.d[k]; return r; }
+UL_HD D5 operator*(const D5& a, double b) { D5 r; r.v = a.v * b; for (int k = 0; k < UL_NT; ++k) r.d[k] = a.d[k] * b; return r; }
+UL_HD D5 operator*(double b, const D5& a) { return a * b; }
+UL_HD D5 operator/(const D5& a, const D5& b)
+{
+    D5 r; double ib = 1.0 / b.v; r.v = a.v * ib;
+    for (int k = 0; k < UL_NT; ++k) r.d[k] = (a.d[k] - r.v * b.d[k]) * ib;
+    return r;
+}
+UL_HD D5 d5_sqrt(const D5& a)
+{
+    D5 r; r.v = sqrt(a.v); double h = 0.5 / r.v;
+    for (int k = 0; k < UL_NT; ++k) r.d[k] = a.d[k] * h;
+    return r;
+}
+UL_HD D5& operator+=(D5& a, const D5& b) { a.v += b.v; for (int k = 0; k < UL_NT; ++k) a.d[k] += b.d[k]; return a; }
+
+// zeta(-1/2, u), zeta(-3/2, u) of ulens_core.cuh in dual arithmetic (same coefficients, same fit)
+UL_HD D5 zeta_m12_d(const D5& u)
+{
+    const double c[10] = {-0.207886224314425946, -0.730177387536053191, -0.326542433690562406,
+                          0.0837832566266219698, -0.0435998186937335486, 0.0271396135617846347,
+                          -0.0165300041688832568, 0.00823252937110980637, -0.00274063185833692022,
+                          0.000434876090612478912};
+    double p = c[9], dp = 0.0;
+    for (int i = 8; i >= 0; --i) { dp = dp * u.v + p; p = p * u.v + c[i]; }
+    D5 r; double su = sqrt(u.v);
+    r.v = su + p;
+    double g = (u.v > 0.0 ? 0.5 / su : 0.0) + dp;
+    for (int k = 0; k < UL_NT; ++k) r.d[k] = g * u.d[k];
+    return r;
+}
+UL_HD D5 zeta_m32_d(const D5& u)
+{
+    const double c[10] = {-0.0254852020522020475, -0.311829304876540199, -0.547634035662697937,
+                          -0.163258961591498412, 0.0313415948971861593, -0.0127998326381573904,
+                          0.00616325441161647825, -0.00268571587959467142, 0.000828839924548779593,
+                          -0.0001258385180165005};
+    double p = c[9], dp = 0.0;
+    for (int i = 8; i >= 0; --i) { dp = dp * u.v + p; p = p * u.v + c[i]; }
+    D5 r; double su = sqrt(u.v);
+    r.v = u.v * su + p;
+    double g = 1.5 * su + dp;
+    for (int k = 0; k < UL_NT; ++k) r.d[k] = g * u.d[k];
+    return r;
+}
+
+// F(z) = |w(z) - w_c|^2 - rho^2 with its tangents. The ray sits at z = r (c, s), r = r.v with tangent r.d[k]
+// (co-moving grid); along a radial scan line c, s are constants, along a ring they rotate -- either way
+// dz_k = r.d[k] (c, s). Explicit dependences: -d w_c, -d eps_i / conj(z - a_i), -eps_i conj(d a_i) / conj(z - a_i)^2
+// and, through the moving ray, dw = dz + g conj(dz) (Eq. 1 differentiated; g = sum eps_i / conj(z - a_i)^2).
+template <int N>
+UL_HD D5 ray_F_dual(const Lens& L, const TangentTable& T, const D5& r, double c, double s, double wcx, double wcy,
+                    double rho)
+{
+    const double x = r.v * c, y = r.v * s;
+    double px[N], py[N], qx[N], qy[N];
+    double ex = x - wcx, ey = y - wcy;
+#pragma unroll
+    for (int i = 0; i < N; ++i) {
+        double dx = x - L.ax[i], dy = y - L.ay[i];
+        double inv = 1.0 / (dx * dx + dy * dy);
+        px[i] = dx * inv; py[i] = dy * inv;                       // 1/conj(d) = d/|d|^2
+        qx[i] = px[i] * px[i] - py[i] * py[i]; qy[i] = 2.0 * px[i] * py[i];   // 1/conj(d)^2
+        ex -= L.eps[i] * px[i]; ey -= L.eps[i] * py[i];
+    }
+    D5 F;
+    F.v = ex * ex + ey * ey - rho * rho;
+#pragma unroll
+    for (int k = 0; k < UL_NT; ++k) {
+        double zdx = r.d[k] * c, zdy = r.d[k] * s;
+        double edx = zdx - T.dwx[k], edy = zdy - T.dwy[k];
+#pragma unroll
+        for (int i = 0; i < N; ++i) {
+            edx -= T.deps[k][i] * px[i]; edy -= T.deps[k][i] * py[i];
+            double ddx = zdx - T.dax[k][i], ddy = zdy - T.day[k][i];       // d(z - a_i)
+            // - eps_i d(1/conj d) = + eps_i conj(dd) / conj(d)^2
+            edx += L.eps[i] * (ddx * qx[i] + ddy * qy[i]);
+            edy += L.eps[i] * (ddx * qy[i] - ddy * qx[i]);
+        }
+        F.d[k] = 2.0 * (ex * edx + ey * edy) - 2.0 * rho * T.drho[k];
+    }
+    if (!(F.v < UL_BIG)) { F = d5_const(UL_BIG); }               // ray on a lens: outside, never NaN
+    return F;
+}
+
+// edge_event of ulens_core.cuh in dual arithmetic: u and dS carry the tangents of the edge position
+// (implicit differentiation of the cubic's root comes for free from Newton's iteration on dual numbers).
+UL_HD void edge_event_d(const D5& f0, const D5& f1, const D5& f2, const D5& f3, bool want_S, double t2_extra,
+                        D5& u, bool& entering, D5& dS)
+{
+    D5 c0 = f1;
+    D5 c1 = (f0 * -2.0 - f1 * 3.0 + f2 * 6.0 - f3) * (1.0 / 6.0);
+    D5 c2 = (f0 - f1 * 2.0 + f2) * 0.5;
+    D5 c3 = (f1 * 3.0 - f0 - f2 * 3.0 + f3) * (1.0 / 6.0);
+    D5 x = f1 / (f1 - f2);
+    D5 xl = x;
+    bool cubic_ok = true;
+#pragma unroll 1
+    for (int it = 0; it < 5; ++it) {
+        D5 p = c0 + x * (c1 + x * (c2 + x * c3));
+        D5 dp = c1 + x * (c2 * 2.0 + x * c3 * 3.0);
+        D5 xn = x - p / dp;
+        if (!(xn.v >= 0.0 && xn.v <= 1.0)) { cubic_ok = false; break; }
+        x = xn;
+    }
+    D5 dp, d2p;
+    if (cubic_ok) {
+        dp = c1 + x * (c2 * 2.0 + x * c3 * 3.0);
+        d2p = c2 * 2.0 + x * c3 * 6.0;
+    } else {
+        x = xl;
+        dp = f2 - f1; d2p = d5_const(0.0);
+    }
+    entering = !(f1.v < 0.0);
+    u = entering ? (1.0 - x) : x;
+    dS = d5_const(0.0);
+    if (want_S) {
+        D5 sigma = entering ? -dp : dp;
+        D5 tau = d2p * -0.5;
+        if (sigma.v > 0.0) {
+            D5 ss = d5_sqrt(sigma);
+            D5 corr = ss * zeta_m12_d(u);
+            D5 t2 = tau / (sigma * 2.0) + (entering ? t2_extra : -t2_extra);
+            if (fabs(t2.v) < 0.5) corr += ss * t2 * zeta_m32_d(u);
+            dS = -corr;
+        }
+    }
+}
+
+// shoot_ring of ulens_core.cuh with tangents. r = ring radius (dual); theta grid frozen.
+template <int N, bool LD>
+UL_HD void shoot_ring_d(const Lens& L, const TangentTable& T, double wcx, double wcy, double rho, const D5& r,
+                        double th0, double dth, int n_th, bool periodic, D5& U_out, D5& S_out, bool& edge)
+{
+    double cd = cos(dth), sd = sin(dth);
+    double t = th0 - 1.5 * dth;
+    double c = cos(t), s = sin(t);
+    D5 big = d5_const(UL_BIG);
+    D5 f0 = big, f1 = big, f2 = big, f3;
+    D5 U = d5_const(0.0), S = d5_const(0.0);
+    edge = false;
+    const int j_first = periodic ? 2 : 1;
+    for (int j = -2; j <= n_th + 1; ++j) {
+        f3 = ray_F_dual<N>(L, T, r, c, s, wcx, wcy, rho);
+        if (j >= 0 && j < n_th && f3.v < 0.0) {
+            U.v += 1.0;
+            if (LD) S += d5_sqrt(-f3);
+            if (!periodic && (j < 2 || j >= n_th - 2)) edge = true;
+        }
+        if (j >= j_first && ((f1.v < 0.0) != (f2.v < 0.0))) {
+            D5 u, dS; bool en;
+            edge_event_d(f0, f1, f2, f3, LD, 0.0, u, en, dS);
+            U += u - 0.5; S += dS;
+        }
+        f0 = f1; f1 = f2; f2 = f3;
+        double cn = c * cd - s * sd;
+        s = s * cd + c * sd;
+        c = cn;
+    }
+    U_out = U; S_out = S;
+}
+
+// shoot_col of ulens_core.cuh with tangents: radial line at fixed theta, nodes r0 + (i + 1/2) dr with dual r0, dr.
+template <int N, bool LD>
+UL_HD void shoot_col_d(const Lens& L, const TangentTable& T, double wcx, double wcy, double rho, double th,
+                       const D5& r0, const D5& dr, int n_r, D5& U_out, D5& S_out, bool& edge)
+{
+    double c = cos(th), s = sin(th);
+    D5 big = d5_const(UL_BIG);
+    D5 f0 = big, f1 = big, f2 = big, f3;
+    D5 U = d5_const(0.0), S = d5_const(0.0), U2 = d5_const(0.0);
+    edge = false;
+    for (int i = -2; i <= n_r + 1; ++i) {
+        D5 r = r0 + dr * (i + 0.5);
+        f3 = ray_F_dual<N>(L, T, r, c, s, wcx, wcy, rho);
+        if (i >= 0 && i < n_r && f3.v < 0.0) {
+            U += r;
+            if (LD) S += r * d5_sqrt(-f3);
+            if ((i < 2 && r0.v > 0.0) || i >= n_r - 2) edge = true;
+        }
+        if (i >= 1 && ((f1.v < 0.0) != (f2.v < 0.0))) {
+            D5 r1 = r0 + dr * (i - 1.5);
+            D5 rh = r1 + dr * 0.5;
+            if (rh.v > 0.0) {
+                D5 u, dS; bool en;
+                bool ent = !(f1.v < 0.0);
+                D5 rin = ent ? r1 + dr : r1;
+                double t2x = dr.v / ul_max(rin.v, 0.5 * dr.v);
+                edge_event_d(f0, f1, f2, f3, LD, t2x, u, en, dS);
+                D5 rc = en ? (r1 + dr) - u * dr : r1 + u * dr;
+                if (rc.v < 0.0) rc = d5_const(0.0);
+                U2 += en ? (rh * rh - rc * rc) * 0.5 : (rc * rc - rh * rh) * 0.5;
+                S += dS * rc;
+            }
+        }
+        f0 = f1; f1 = f2; f2 = f3;
+    }
+    U_out = U * dr + U2; S_out = S * dr;
+}
+
+// d z / d p_k of an image point z of the limb point w_c + rho e^{i phi}: Eq. 1 differentiated at fixed phi,
+// dz + g conj(dz) = b_k,  b_k = dw_c + drho e^{i phi} + sum_i [ deps_i / conj(d_i) + eps_i conj(da_i) / conj(d_i)^2 ]
+// => dz = (b - g conj(b)) / (1 - |g|^2)   (P:163-175 by the implicit-function theorem, here on Eq. 1 itself).
+// Returns d|z|/dp_k in out[k]; the tangents are capped (they only have to follow the edge).
+template <int N>
+UL_HD void limb_point_rdot(const Lens& L, const TangentTable& T, double zx, double zy, double phi, double* out)
+{
+    double gx = 0.0, gy = 0.0, px[N], py[N], qx[N], qy[N];
+#pragma unroll
+    for (int i = 0; i < N; ++i) {
+        double dx = zx - L.ax[i], dy = zy - L.ay[i];
+        double inv = 1.0 / (dx * dx + dy * dy);
+        px[i] = dx * inv; py[i] = dy * inv;
+        qx[i] = px[i] * px[i] - py[i] * py[i]; qy[i] = 2.0 * px[i] * py[i];
+        gx += L.eps[i] * qx[i]; gy += L.eps[i] * qy[i];
+    }
+    double det = 1.0 - (gx * gx + gy * gy);
+    double rr = sqrt(zx * zx + zy * zy);
+    double cp = cos(phi), sp = sin(phi);
+#pragma unroll
+    for (int k = 0; k < UL_NT; ++k) {
+        double bx = T.dwx[k] + T.drho[k] * cp, by = T.dwy[k] + T.drho[k] * sp;
+#pragma unroll
+        for (int i = 0; i < N; ++i) {
+            bx += T.deps[k][i] * px[i]; by += T.deps[k][i] * py[i];
+            // eps_i conj(da_i) / conj(d_i)^2 = eps_i (dax - i day)(qx + i qy)
+            bx += L.eps[i] * (T.dax[k][i] * qx[i] + T.day[k][i] * qy[i]);
+            by += L.eps[i] * (T.dax[k][i] * qy[i] - T.day[k][i] * qx[i]);
+        }
+        // g conj(b)
+        double hx = gx * bx + gy * by, hy = gy * bx - gx * by;
+        double dzx = (bx - hx) / det, dzy = (by - hy) / det;
+        double v = rr > 0.0 ? (zx * dzx + zy * dzy) / rr : 0.0;
+        if (!(fabs(v) < 1e3)) v = 0.0;                            // on a critical curve: give up following
+        out[k] = v;
+    }
+}
+
+}  // namespace ulens

@@ -16,8 +16,13 @@
 //                       min/max of its members plus a margin, with n_r x n_theta from the local image scale.
 #pragma once
 #include "ulens_core.cuh"
+#include "ulens_dual.cuh"
 
 namespace ulens {
+
+#ifdef UL_EXPERIMENT
+static double g_mscale = 1.0;
+#endif
 
 struct SubBox {
     double r_lo, r_hi;      // r_lo > r_hi: empty
@@ -36,8 +41,21 @@ struct RegionParams {
     int max_units_pt;       // cap on 32-ring units per point
 };
 
+// dual variant only: the box's own image-limb points of smallest / largest |z| and their limb angles
+struct BoxExt {
+    double lo_r, lo_x, lo_y, lo_ph;
+    double hi_r, hi_x, hi_y, hi_ph;
+};
+
+// dual variant only: how a sector's radial bounds move (d r_lo / d p_k, d r_hi / d p_k)
+struct PatchTan {
+    double rlo_dot[UL_NT], rhi_dot[UL_NT];
+};
+
 template <int DEG>
 struct RegionWork {
+    BoxExt* ext;            // [32 * DEG] or nullptr (primal run)
+    PatchTan ptan[UL_MAXP];
     SubBox box[32 * DEG];
     short order_r[32 * DEG], order_t[32 * DEG];
     int n_sorted;
@@ -67,6 +85,24 @@ UL_HD void box_add(SubBox& b, double& t_cur, double r, double th, double hr, dou
     b.t_lo = ul_min(b.t_lo, t); b.t_hi = ul_max(b.t_hi, t);
     b.hr = ul_min(b.hr, hr); b.ht = ul_min(b.ht, ht); b.cr = ul_min(b.cr, cr); b.ct = ul_min(b.ct, ct);
     if (advance) t_cur = t;
+}
+
+// extreme of the parabola through three consecutive boundary samples (x = limb angle, y = r or theta), if the
+// middle sample is a local extreme: the image boundary bulges beyond its samples by ~ (step)^2 / 8 x curvature,
+// which matters now that the sector margins are tight
+UL_HD bool parabola_vertex(double x0, double y0, double x1, double y1, double x2, double y2, double& yv)
+{
+    if (!((y1 >= y0 && y1 >= y2) || (y1 <= y0 && y1 <= y2))) return false;
+    double h0 = x1 - x0, h1 = x2 - x1;
+    if (!(h0 > 0.0 && h1 > 0.0)) return false;
+    double s0 = (y1 - y0) / h0, s1 = (y2 - y1) / h1;
+    double a = (s1 - s0) / (h0 + h1);
+    if (a == 0.0) return false;
+    double slope1 = s0 + a * h0;                         // derivative at x1
+    double dx = -slope1 / (2.0 * a);
+    if (!(dx >= -h0 && dx <= h1)) return false;
+    yv = y1 - slope1 * slope1 / (4.0 * a);
+    return true;
 }
 
 // local image scale at an image point z with g = sum eps_i/conj(z-a_i)^2: the image of a small disk of
@@ -106,11 +142,16 @@ UL_HDN void regions_phaseA(int lane, const Lens& L, const LensPoly& T, double wc
     double t_cur[DEG];              // per BOX: unwrapped theta of its last point
     double lastx[DEG], lasty[DEG];  // per BOX: its last point
     int bmap[DEG];                  // slot -> the box that slot's current arc writes to
+    double h_ph[DEG][2], h_r[DEG][2], h_t[DEG][2];   // per BOX: its last two own points (limb angle, r, theta)
+    int h_n[DEG];
 #pragma unroll
-    for (int j = 0; j < DEG; ++j) { bmap[j] = -1; lastx[j] = lasty[j] = 0.0; }
+    for (int j = 0; j < DEG; ++j) { bmap[j] = -1; lastx[j] = lasty[j] = 0.0; h_n[j] = 0; }
     double zr[DEG], zi[DEG], ozr[DEG], ozi[DEG], pvx[DEG], pvy[DEG];
     double br[DEG + 1], bi[DEG + 1];
     unsigned valid_prev = 0, faint_prev = 0;
+#pragma unroll
+    BoxExt* E = W.ext ? &W.ext[lane * DEG] : nullptr;
+    if (E) for (int j = 0; j < DEG; ++j) { E[j].lo_r = 1e300; E[j].hi_r = -1.0; E[j].lo_x = E[j].lo_y = E[j].lo_ph = E[j].hi_x = E[j].hi_y = E[j].hi_ph = 0.0; }
 #pragma unroll
     for (int j = 0; j < DEG; ++j) { B[j].r_lo = 1.0; B[j].r_hi = -1.0; B[j].t_lo = B[j].t_hi = 0.0; B[j].hr = B[j].ht = B[j].cr = B[j].ct = 1e300; t_cur[j] = 0.0; pvx[j] = pvy[j] = 0.0; }
 
@@ -259,9 +300,31 @@ UL_HDN void regions_phaseA(int lane, const Lens& L, const LensPoly& T, double wc
                 }
                 if (bi < 0) bi = nearest;
                 bmap[j] = bi;
+                h_n[bi] = 0;                             // a new arc starts: forget the old arc's samples
             }
             box_add(B[bi], t_cur[bi], sqrt(px[j] * px[j] + py[j] * py[j]), atan2(py[j], px[j]), hrr[j], htt[j], crr[j], ctt[j], true);
             lastx[bi] = px[j]; lasty[bi] = py[j];
+            {
+                // bulge of the boundary between samples: vertex of the parabola through the last three
+                const double rr = sqrt(px[j] * px[j] + py[j] * py[j]), tt = t_cur[bi];
+                if (h_n[bi] >= 2) {
+                    double yv;
+                    if (parabola_vertex(h_ph[bi][0], h_r[bi][0], h_ph[bi][1], h_r[bi][1], ph_new, rr, yv)) {
+                        B[bi].r_lo = ul_min(B[bi].r_lo, ul_max(yv, 0.0)); B[bi].r_hi = ul_max(B[bi].r_hi, yv);
+                    }
+                    if (parabola_vertex(h_ph[bi][0], h_t[bi][0], h_ph[bi][1], h_t[bi][1], ph_new, tt, yv)) {
+                        B[bi].t_lo = ul_min(B[bi].t_lo, yv); B[bi].t_hi = ul_max(B[bi].t_hi, yv);
+                    }
+                }
+                h_ph[bi][0] = h_ph[bi][1]; h_r[bi][0] = h_r[bi][1]; h_t[bi][0] = h_t[bi][1];
+                h_ph[bi][1] = ph_new; h_r[bi][1] = rr; h_t[bi][1] = tt;
+                if (h_n[bi] < 2) ++h_n[bi];
+            }
+            if (E) {
+                double rr = sqrt(px[j] * px[j] + py[j] * py[j]);
+                if (rr < E[bi].lo_r) { E[bi].lo_r = rr; E[bi].lo_x = px[j]; E[bi].lo_y = py[j]; E[bi].lo_ph = ph_new; }
+                if (rr > E[bi].hi_r) { E[bi].hi_r = rr; E[bi].hi_x = px[j]; E[bi].hi_y = py[j]; E[bi].hi_ph = ph_new; }
+            }
         }
         // links: a slot that switched off (its last point) or on (its first point) between s-1 and s is one
         // half of an image pair destroyed / created on a critical curve somewhere between the two partners'
@@ -315,9 +378,15 @@ UL_HDN void regions_phaseA(int lane, const Lens& L, const LensPoly& T, double wc
 UL_HD void box_expanded(const SubBox& b, double& rl, double& rh, double& tl, double& th)
 {
     double m = ul_min(b.cr, b.ct);
-    double mr = 0.25 * m + 0.02 * (b.r_hi - b.r_lo);
+    // radial margin: TIGHT (0.5 % of the local width + 0.04 % of the box). The rings of a sector are placed
+    // at Chebyshev-like radii r_c + h sin(phi) (emit_patch), which removes the square-root behaviour of the
+    // chord length at the radial ends of an image only if the sector ends where the image ends.
+    double mr = 0.02 * (0.25 * m + 0.02 * (b.r_hi - b.r_lo));
+#ifdef UL_EXPERIMENT
+    mr *= g_mscale;
+#endif
     double rmid = ul_max(0.5 * (b.r_lo + b.r_hi), 1e-300);
-    double mt = 0.25 * m / rmid + 0.02 * (b.t_hi - b.t_lo);
+    double mt = 0.02 * (0.25 * m / rmid + 0.02 * (b.t_hi - b.t_lo));   // tight, as in r
     mt = ul_min(mt, 0.5);
     rl = ul_max(b.r_lo - mr, 0.0); rh = b.r_hi + mr;
     tl = b.t_lo - mt; th = b.t_hi + mt;
@@ -347,6 +416,16 @@ UL_HDN void regions_phaseB(int lane, RegionWork<DEG>& W)
     }
 }
 
+// dual variant: tangents of a sector's radial bounds from its extreme image-limb points
+template <int N>
+UL_HD void patch_tangents(const Lens& L, const TangentTable& T, const BoxExt& x, bool from_origin, PatchTan& out)
+{
+    for (int k = 0; k < UL_NT; ++k) { out.rlo_dot[k] = 0.0; out.rhi_dot[k] = 0.0; }
+    if (x.hi_r < 0.0) return;                           // no own point (links only): frozen
+    if (!from_origin) limb_point_rdot<N>(L, T, x.lo_x, x.lo_y, x.lo_ph, out.rlo_dot);
+    limb_point_rdot<N>(L, T, x.hi_x, x.hi_y, x.hi_ph, out.rhi_dot);
+}
+
 // ---------------------------------------------------------------------------------------------- phase C
 // One sector -> its ray grid (Sec. 3.3 "fixed-resolution polar grid"; spacing from the local image scale).
 // Scan lines (one per lane, 32 per work unit) are rings scanned along theta for a bounded sector and radial
@@ -374,11 +453,16 @@ UL_HD void emit_patch(Patch& out, const RegionParams& P, int point, double rl, d
     if (n_th < 16) n_th = 16;
     if (n_r < 16) n_r = 16;
     double dth = t_ext / n_th;
+    double span_t = t_ext;
     if (!periodic) {
         // 3 extra cells of margin per side (cubic stencil + empty border rays)
-        double e_lo = ul_min(3.0 * dth, 0.45 * gap_t_lo), e_hi = ul_min(3.0 * dth, 0.45 * gap_t_hi);
+        // ALONG the scan lines a generous margin costs only a few nodes: 3 cells for the cubic stencil + 5 % of
+        // the span; ACROSS the lines the sector must end where the image ends (sin-spaced lines): no margin
+        double e_lo = ul_min(3.0 * dth + 0.05 * t_ext, 0.45 * gap_t_lo), e_hi = ul_min(3.0 * dth + 0.05 * t_ext, 0.45 * gap_t_hi);
+        if (scan_r) e_lo = e_hi = 0.0;
         tl -= e_lo;
-        double span = t_ext + e_lo + e_hi;
+        span_t = t_ext + e_lo + e_hi;
+        const double span = span_t;
         n_th = (int)ceil(span / dth);
         if (n_th > P.max_nth) { n_th = P.max_nth; status |= UL_ST_RES_CAP; }
         dth = span / n_th;
@@ -386,7 +470,9 @@ UL_HD void emit_patch(Patch& out, const RegionParams& P, int point, double rl, d
     double dr = r_ext / n_r;
     double span_r;
     {
-        double e_lo = ul_min(3.0 * dr, 0.45 * gap_r_lo), e_hi = ul_min(3.0 * dr, 0.45 * gap_r_hi);
+        // radial scan lines need 3 empty nodes per side for the cubic stencil; rings need none
+        double e_lo = ul_min(3.0 * dr + 0.05 * r_ext, 0.45 * gap_r_lo), e_hi = ul_min(3.0 * dr + 0.05 * r_ext, 0.45 * gap_r_hi);
+        if (!scan_r) e_lo = e_hi = 0.0;
         if (rl <= 0.0) e_lo = 0.0;
         rl -= e_lo;
         span_r = r_ext + e_lo + e_hi;
@@ -404,11 +490,11 @@ UL_HD void emit_patch(Patch& out, const RegionParams& P, int point, double rl, d
     }
     units_left -= n_units;
     if (units_left < 0) units_left = 0;
-    if (periodic) dth = 2.0 * UL_PI / n_th;
+    dth = (periodic ? 2.0 * UL_PI : span_t) / n_th;    // the line count was rounded to a multiple of 32
     dr = span_r / n_r;
     out.r0 = rl; out.dr = dr; out.th0 = tl; out.dth = dth; out.n_r = n_r; out.n_th = n_th;
     out.point = point; out.unit0 = 0;
-    out.flags = (periodic ? UL_PATCH_PERIODIC : 0) | (scan_r ? UL_PATCH_SCAN_R : 0);
+    out.flags = (periodic ? UL_PATCH_PERIODIC : 0) | (scan_r ? UL_PATCH_SCAN_R : 0) | ((scan_r && periodic) ? 0 : UL_PATCH_SINR);
     out.n_units = n_units;
 }
 
@@ -422,7 +508,7 @@ UL_HD void emit_patch(Patch& out, const RegionParams& P, int point, double rl, d
 // the origin) the gap is filled: the groups on both sides merge into one full-ring sector.
 template <int N>
 UL_HDN int regions_phaseC(RegionWork<N * N + 1>& W, const RegionParams& P, int point, const Lens& L, double wcx,
-                          double wcy, double rho, unsigned& status)
+                          double wcy, double rho, unsigned& status, const TangentTable* TT = nullptr)
 {
     constexpr int DEG = N * N + 1;
     const int n = 32 * DEG;
@@ -443,6 +529,16 @@ UL_HDN int regions_phaseC(RegionWork<N * N + 1>& W, const RegionParams& P, int p
             if (ngr == 0 || (rl > cur_hi && ngr < UL_MAXG)) { gr_lo[ngr] = rl; gr_hi[ngr] = rh; cur_hi = rh; ++ngr; }
             else { cur_hi = ul_max(cur_hi, rh); gr_hi[ngr - 1] = cur_hi; }
         }
+    }
+    // a gap much narrower than the groups on both sides is the neck between two arcs of one image (an image
+    // pair about to merge on a critical curve): one group, so that the sector ends where the image ends
+    for (int g = 0; g + 1 < ngr;) {
+        double gap = gr_lo[g + 1] - gr_hi[g];
+        if (gap < 0.05 * ul_min(gr_hi[g] - gr_lo[g], gr_hi[g + 1] - gr_lo[g + 1])) {
+            gr_hi[g] = gr_hi[g + 1];
+            for (int k = g + 1; k + 1 < ngr; ++k) { gr_lo[k] = gr_lo[k + 1]; gr_hi[k] = gr_hi[k + 1]; }
+            --ngr;
+        } else ++g;
     }
     // ---- fill gaps whose circles are inside the image
     bool ring_group[UL_MAXG];
@@ -475,6 +571,7 @@ UL_HDN int regions_phaseC(RegionWork<N * N + 1>& W, const RegionParams& P, int p
         if (ring_group[a]) {
             // filled ring / disk: one full-ring sector scanned along radial lines
             double hr = 1e300, ht = 1e300, cr = 1e300, ct = 1e300;
+            BoxExt xlo; xlo.lo_r = 1e300; xlo.hi_r = -1.0; xlo.lo_x = xlo.lo_y = xlo.lo_ph = xlo.hi_x = xlo.hi_y = xlo.hi_ph = 0.0;
             for (int i = 0; i < n; ++i) {
                 const SubBox& b = W.box[i];
                 if (b.r_lo > b.r_hi) continue;
@@ -482,8 +579,14 @@ UL_HDN int regions_phaseC(RegionWork<N * N + 1>& W, const RegionParams& P, int p
                 box_expanded(b, rl, rh, tl, th);
                 if (!(rl >= gr_lo[a] && rl <= gr_hi[a])) continue;
                 hr = ul_min(hr, b.hr); ht = ul_min(ht, b.ht); cr = ul_min(cr, b.cr); ct = ul_min(ct, b.ct);
+                if (W.ext) {
+                    const BoxExt& e = W.ext[i];
+                    if (e.lo_r < xlo.lo_r) { xlo.lo_r = e.lo_r; xlo.lo_x = e.lo_x; xlo.lo_y = e.lo_y; xlo.lo_ph = e.lo_ph; }
+                    if (e.hi_r > xlo.hi_r) { xlo.hi_r = e.hi_r; xlo.hi_x = e.hi_x; xlo.hi_y = e.hi_y; xlo.hi_ph = e.hi_ph; }
+                }
             }
             if (np == UL_MAXP) { capped = true; break; }
+            if (W.ext && TT) patch_tangents<N>(L, *TT, xlo, gr_lo[a] <= 0.0, W.ptan[np]);
             emit_patch(W.patch[np++], P, point, gr_lo[a], gr_hi[a], -UL_PI, UL_PI, hr, ht, cr, ct, true, true,
                        gap_r_lo, gap_r_hi, 0.0, 0.0, units_left, status);
             continue;
@@ -500,6 +603,14 @@ UL_HDN int regions_phaseC(RegionWork<N * N + 1>& W, const RegionParams& P, int p
                 if (ngt == 0 || (tl > cur_hi && ngt < UL_MAXG)) { gt_lo[ngt] = tl; gt_hi[ngt] = th; cur_hi = th; ++ngt; }
                 else { cur_hi = ul_max(cur_hi, th); gt_hi[ngt - 1] = cur_hi; }
             }
+            for (int g = 0; g + 1 < ngt;) {               // necks, as for r
+                double gap = gt_lo[g + 1] - gt_hi[g];
+                if (gap < 0.05 * ul_min(gt_hi[g] - gt_lo[g], gt_hi[g + 1] - gt_lo[g + 1])) {
+                    gt_hi[g] = gt_hi[g + 1];
+                    for (int k = g + 1; k + 1 < ngt; ++k) { gt_lo[k] = gt_lo[k + 1]; gt_hi[k] = gt_hi[k + 1]; }
+                    --ngt;
+                } else ++g;
+            }
             // wrap: the group reaching furthest past +pi swallows the leading groups it covers
             for (;;) {
                 if (ngt <= 1) break;
@@ -515,6 +626,8 @@ UL_HDN int regions_phaseC(RegionWork<N * N + 1>& W, const RegionParams& P, int p
         const bool full_ring = (ngt == 1 && gt_hi[0] - gt_lo[0] >= 2.0 * UL_PI - 1e-12);
         // ---- tight bounds of each theta-group's members
         double c_rl[UL_MAXG], c_rh[UL_MAXG], c_tl[UL_MAXG], c_th[UL_MAXG], c_hr[UL_MAXG], c_ht[UL_MAXG], c_cr[UL_MAXG], c_ct[UL_MAXG];
+        BoxExt c_ext[UL_MAXG];
+        for (int g = 0; g < ngt; ++g) { c_ext[g].lo_r = 1e300; c_ext[g].hi_r = -1.0; c_ext[g].lo_x = c_ext[g].lo_y = c_ext[g].lo_ph = c_ext[g].hi_x = c_ext[g].hi_y = c_ext[g].hi_ph = 0.0; }
         for (int g = 0; g < ngt; ++g) { c_rl[g] = 1e300; c_rh[g] = -1e300; c_tl[g] = 1e300; c_th[g] = -1e300; c_hr[g] = c_ht[g] = c_cr[g] = c_ct[g] = 1e300; }
         for (int i = 0; i < n; ++i) {
             const SubBox& b = W.box[i];
@@ -534,6 +647,12 @@ UL_HDN int regions_phaseC(RegionWork<N * N + 1>& W, const RegionParams& P, int p
             c_tl[c] = ul_min(c_tl[c], tl); c_th[c] = ul_max(c_th[c], th);
             c_hr[c] = ul_min(c_hr[c], b.hr); c_ht[c] = ul_min(c_ht[c], b.ht);
             c_cr[c] = ul_min(c_cr[c], b.cr); c_ct[c] = ul_min(c_ct[c], b.ct);
+            if (W.ext) {
+                const BoxExt& e = W.ext[i];
+                BoxExt& x = c_ext[c];
+                if (e.lo_r < x.lo_r) { x.lo_r = e.lo_r; x.lo_x = e.lo_x; x.lo_y = e.lo_y; x.lo_ph = e.lo_ph; }
+                if (e.hi_r > x.hi_r) { x.hi_r = e.hi_r; x.hi_x = e.hi_x; x.hi_y = e.hi_y; x.hi_ph = e.hi_ph; }
+            }
         }
         for (int c = 0; c < ngt; ++c) {
             if (c_rl[c] > c_rh[c]) continue;
@@ -548,9 +667,13 @@ UL_HDN int regions_phaseC(RegionWork<N * N + 1>& W, const RegionParams& P, int p
                 gap_hi -= 2.0 * UL_PI * floor(gap_hi / (2.0 * UL_PI));
             }
             if (np == UL_MAXP) { capped = true; break; }
-            // a sector that closes on itself in theta is cut by radial lines: the line integral is then a
-            // smooth periodic function of theta (spectral convergence of the midpoint rule across lines)
-            const bool scan_r = full_ring;
+            // Scan lines run ACROSS the long axis of the sector. Images near the Einstein ring are arcs that
+            // hug a circle r = const: along rings their chord length jumps from zero to the full arc within
+            // a tiny step in r, while radial lines cut the arc once each and the line integral varies smoothly
+            // with theta up to the two tips, which the sin-spaced lines (UL_PATCH_SINR) take care of. A sector
+            // that closes on itself in theta has no tips at all (spectral convergence).
+            const bool scan_r = full_ring || ((c_th[c] - c_tl[c]) * c_rh[c] > (c_rh[c] - c_rl[c]));
+            if (W.ext && TT) patch_tangents<N>(L, *TT, c_ext[c], false, W.ptan[np]);
             emit_patch(W.patch[np++], P, point, c_rl[c], c_rh[c], c_tl[c], c_th[c], c_hr[c], c_ht[c], c_cr[c], c_ct[c],
                        full_ring, scan_r, gap_r_lo, gap_r_hi, gap_lo, gap_hi, units_left, status);
         }
@@ -566,6 +689,7 @@ UL_HDN int regions_phaseC(RegionWork<N * N + 1>& W, const RegionParams& P, int p
             rl = ul_min(rl, a1); rh = ul_max(rh, a2); hr = ul_min(hr, b.hr); ht = ul_min(ht, b.ht); cr = ul_min(cr, b.cr); ct = ul_min(ct, b.ct);
         }
         np = 0; units_left = P.max_units_pt;
+        for (int k = 0; k < UL_NT; ++k) { W.ptan[0].rlo_dot[k] = 0.0; W.ptan[0].rhi_dot[k] = 0.0; }
         emit_patch(W.patch[np++], P, point, rl, rh, -UL_PI, UL_PI, hr, ht, cr, ct, true, false, rl, 1e300, 0.0, 0.0,
                    units_left, status);
     }
