@@ -355,29 +355,35 @@ k_shoot_dual(int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cfg, c
         double rho = cfg[c].rho, u1 = cfg[c].u1;
         double wcx = w_re[gp], wcy = w_im[gp];
         int line = blk * 32 + lane;
-        // co-moving radial grid
-        D5 r0, dr;
-        r0.v = P.r0; dr.v = P.dr;
+        // co-moving grid ACROSS the scan lines: the span's two ends follow the image's extreme
+        // limb points; ALONG the lines the nodes are frozen (the margins there are generous)
+        const bool scan_r = (P.flags & UL_PATCH_SCAN_R) != 0, periodic = (P.flags & UL_PATCH_PERIODIC) != 0;
+        D5 x0 = d5_const(scan_r ? P.th0 : P.r0), dx = d5_const(scan_r ? P.dth : P.dr);
+        const int n_lines = scan_r ? P.n_th : P.n_r;
+        if (!(scan_r && periodic)) {
 #pragma unroll
-        for (int k = 0; k < UL_NT; ++k) { r0.d[k] = PT.rlo_dot[k]; dr.d[k] = (PT.rhi_dot[k] - PT.rlo_dot[k]) / P.n_r; }
+            for (int k = 0; k < UL_NT; ++k) {
+                double lo = scan_r ? PT.tlo_dot[k] : PT.rlo_dot[k], hi = scan_r ? PT.thi_dot[k] : PT.rhi_dot[k];
+                x0.d[k] = lo - P.kap_lo * (hi - lo); dx.d[k] = (hi - lo) * (1.0 + P.kap_lo + P.kap_hi) / n_lines;
+            }
+        }
+        D5 xl, wl;
+        line_node_d(P.flags, n_lines, line, x0, dx, xl, wl);
         D5 U, S, f; bool edge, clipped;
         D5 rho_d = d5_const(rho);
 #pragma unroll
         for (int k = 0; k < UL_NT; ++k) rho_d.d[k] = T.drho[k];
-        if (P.flags & UL_PATCH_SCAN_R) {
-            double th = P.th0 + (line + 0.5) * P.dth;
-            shoot_col_d<N, LD>(L, T, wcx, wcy, rho, th, r0, dr, P.n_r, U, S, edge);
+        if (scan_r) {
+            shoot_col_d<N, LD>(L, T, wcx, wcy, rho, xl, d5_const(P.r0), d5_const(P.dr), P.n_r, U, S, edge);
             f = U * (1.0 - u1);
             if (LD) f += (S / rho_d) * u1;
-            f = f * P.dth;
-            clipped = edge || (!(P.flags & UL_PATCH_PERIODIC) && (line < 1 || line >= P.n_th - 1) && U.v > 0.0);
+            f = f * wl;
+            clipped = edge || (!periodic && (line < 1 || line >= P.n_th - 1) && U.v > 0.0);
         } else {
-            D5 r = r0 + dr * (line + 0.5);
-            bool periodic = (P.flags & UL_PATCH_PERIODIC) != 0;
-            shoot_ring_d<N, LD>(L, T, wcx, wcy, rho, r, P.th0, P.dth, P.n_th, periodic, U, S, edge);
+            shoot_ring_d<N, LD>(L, T, wcx, wcy, rho, xl, P.th0, P.dth, P.n_th, periodic, U, S, edge);
             f = U * (1.0 - u1);
             if (LD) f += (S / rho_d) * u1;
-            f = r * f * dr * P.dth;
+            f = xl * f * wl * P.dth;
             clipped = edge || ((line < 1 || line >= P.n_r - 1) && U.v > 0.0 && P.r0 > 0.0);
         }
         double tot = warp_sum(f.v);

@@ -58,6 +58,7 @@ struct Patch {
     int unit0;           // first 32-ring work unit of this patch in the unit arrays
     int flags;           // UL_PATCH_*: periodic in theta (full ring); scan lines are radial (lanes = theta); sin-spaced rings
     int n_units;         // 32-line work units
+    double kap_lo, kap_hi; // across-line margins as fractions of the image extent (the dual variant moves them with it)
 };
 
 #define UL_PATCH_PERIODIC 1

@@ -91,7 +91,7 @@ UL_HD D5 zeta_m32_d(const D5& u)
 // and, through the moving ray, dw = dz + g conj(dz) (Eq. 1 differentiated; g = sum eps_i / conj(z - a_i)^2).
 template <int N>
 UL_HD D5 ray_F_dual(const Lens& L, const TangentTable& T, const D5& r, double c, double s, double wcx, double wcy,
-                    double rho)
+                    double rho, const double* thdot = nullptr)
 {
     const double x = r.v * c, y = r.v * s;
     double px[N], py[N], qx[N], qy[N];
@@ -109,6 +109,7 @@ UL_HD D5 ray_F_dual(const Lens& L, const TangentTable& T, const D5& r, double c,
 #pragma unroll
     for (int k = 0; k < UL_NT; ++k) {
         double zdx = r.d[k] * c, zdy = r.d[k] * s;
+        if (thdot) { zdx -= r.v * thdot[k] * s; zdy += r.v * thdot[k] * c; }     // the scan line itself turns
         double edx = zdx - T.dwx[k], edy = zdy - T.dwy[k];
 #pragma unroll
         for (int i = 0; i < N; ++i) {
@@ -203,17 +204,17 @@ UL_HD void shoot_ring_d(const Lens& L, const TangentTable& T, double wcx, double
 
 // shoot_col of ulens_core.cuh with tangents: radial line at fixed theta, nodes r0 + (i + 1/2) dr with dual r0, dr.
 template <int N, bool LD>
-UL_HD void shoot_col_d(const Lens& L, const TangentTable& T, double wcx, double wcy, double rho, double th,
+UL_HD void shoot_col_d(const Lens& L, const TangentTable& T, double wcx, double wcy, double rho, const D5& th,
                        const D5& r0, const D5& dr, int n_r, D5& U_out, D5& S_out, bool& edge)
 {
-    double c = cos(th), s = sin(th);
+    double c = cos(th.v), s = sin(th.v);
     D5 big = d5_const(UL_BIG);
     D5 f0 = big, f1 = big, f2 = big, f3;
     D5 U = d5_const(0.0), S = d5_const(0.0), U2 = d5_const(0.0);
     edge = false;
     for (int i = -2; i <= n_r + 1; ++i) {
         D5 r = r0 + dr * (i + 0.5);
-        f3 = ray_F_dual<N>(L, T, r, c, s, wcx, wcy, rho);
+        f3 = ray_F_dual<N>(L, T, r, c, s, wcx, wcy, rho, th.d);
         if (i >= 0 && i < n_r && f3.v < 0.0) {
             U += r;
             if (LD) S += r * d5_sqrt(-f3);
@@ -239,12 +240,24 @@ UL_HD void shoot_col_d(const Lens& L, const TangentTable& T, double wcx, double 
     U_out = U * dr + U2; S_out = S * dr;
 }
 
+// line_node of ulens_core.cuh for a span [x0, x0 + n dx] that moves with the parameters
+UL_HD void line_node_d(int flags, int n, int line, const D5& x0, const D5& dx, D5& x, D5& w)
+{
+    if (flags & UL_PATCH_SINR) {
+        double ph = (line + 0.5) * (UL_PI / n), sn = sin(ph), cs = cos(ph);
+        D5 h = dx * (0.5 * n);
+        x = x0 + h * (1.0 - cs);
+        w = h * (sn * (UL_PI / n));
+    } else { x = x0 + dx * (line + 0.5); w = dx; }
+}
+
 // d z / d p_k of an image point z of the limb point w_c + rho e^{i phi}: Eq. 1 differentiated at fixed phi,
 // dz + g conj(dz) = b_k,  b_k = dw_c + drho e^{i phi} + sum_i [ deps_i / conj(d_i) + eps_i conj(da_i) / conj(d_i)^2 ]
 // => dz = (b - g conj(b)) / (1 - |g|^2)   (P:163-175 by the implicit-function theorem, here on Eq. 1 itself).
 // Returns d|z|/dp_k in out[k]; the tangents are capped (they only have to follow the edge).
 template <int N>
-UL_HD void limb_point_rdot(const Lens& L, const TangentTable& T, double zx, double zy, double phi, double* out)
+UL_HD void limb_point_rdot(const Lens& L, const TangentTable& T, double zx, double zy, double phi, double* out,
+                           double* out_theta = nullptr)
 {
     double gx = 0.0, gy = 0.0, px[N], py[N], qx[N], qy[N];
 #pragma unroll
@@ -273,7 +286,12 @@ UL_HD void limb_point_rdot(const Lens& L, const TangentTable& T, double zx, doub
         double dzx = (bx - hx) / det, dzy = (by - hy) / det;
         double v = rr > 0.0 ? (zx * dzx + zy * dzy) / rr : 0.0;
         if (!(fabs(v) < 1e3)) v = 0.0;                            // on a critical curve: give up following
-        out[k] = v;
+        if (out) out[k] = v;
+        if (out_theta) {
+            double tv = rr > 0.0 ? (zx * dzy - zy * dzx) / (rr * rr) : 0.0;
+            if (!(fabs(tv) < 1e3)) tv = 0.0;
+            out_theta[k] = tv;
+        }
     }
 }
 

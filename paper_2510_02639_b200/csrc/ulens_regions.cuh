@@ -45,11 +45,14 @@ struct RegionParams {
 struct BoxExt {
     double lo_r, lo_x, lo_y, lo_ph;
     double hi_r, hi_x, hi_y, hi_ph;
+    double tlo_t, tlo_x, tlo_y, tlo_ph;     // smallest / largest unwrapped theta along the arc
+    double thi_t, thi_x, thi_y, thi_ph;
 };
 
 // dual variant only: how a sector's radial bounds move (d r_lo / d p_k, d r_hi / d p_k)
 struct PatchTan {
     double rlo_dot[UL_NT], rhi_dot[UL_NT];
+    double tlo_dot[UL_NT], thi_dot[UL_NT];
 };
 
 template <int DEG>
@@ -151,7 +154,8 @@ UL_HDN void regions_phaseA(int lane, const Lens& L, const LensPoly& T, double wc
     unsigned valid_prev = 0, faint_prev = 0;
 #pragma unroll
     BoxExt* E = W.ext ? &W.ext[lane * DEG] : nullptr;
-    if (E) for (int j = 0; j < DEG; ++j) { E[j].lo_r = 1e300; E[j].hi_r = -1.0; E[j].lo_x = E[j].lo_y = E[j].lo_ph = E[j].hi_x = E[j].hi_y = E[j].hi_ph = 0.0; }
+    if (E) for (int j = 0; j < DEG; ++j) { E[j].lo_r = 1e300; E[j].hi_r = -1.0; E[j].lo_x = E[j].lo_y = E[j].lo_ph = E[j].hi_x = E[j].hi_y = E[j].hi_ph = 0.0;
+        E[j].tlo_t = 1e300; E[j].thi_t = -1e300; E[j].tlo_x = E[j].tlo_y = E[j].tlo_ph = E[j].thi_x = E[j].thi_y = E[j].thi_ph = 0.0; }
 #pragma unroll
     for (int j = 0; j < DEG; ++j) { B[j].r_lo = 1.0; B[j].r_hi = -1.0; B[j].t_lo = B[j].t_hi = 0.0; B[j].hr = B[j].ht = B[j].cr = B[j].ct = 1e300; t_cur[j] = 0.0; pvx[j] = pvy[j] = 0.0; }
 
@@ -324,6 +328,8 @@ UL_HDN void regions_phaseA(int lane, const Lens& L, const LensPoly& T, double wc
                 double rr = sqrt(px[j] * px[j] + py[j] * py[j]);
                 if (rr < E[bi].lo_r) { E[bi].lo_r = rr; E[bi].lo_x = px[j]; E[bi].lo_y = py[j]; E[bi].lo_ph = ph_new; }
                 if (rr > E[bi].hi_r) { E[bi].hi_r = rr; E[bi].hi_x = px[j]; E[bi].hi_y = py[j]; E[bi].hi_ph = ph_new; }
+                if (t_cur[bi] < E[bi].tlo_t) { E[bi].tlo_t = t_cur[bi]; E[bi].tlo_x = px[j]; E[bi].tlo_y = py[j]; E[bi].tlo_ph = ph_new; }
+                if (t_cur[bi] > E[bi].thi_t) { E[bi].thi_t = t_cur[bi]; E[bi].thi_x = px[j]; E[bi].thi_y = py[j]; E[bi].thi_ph = ph_new; }
             }
         }
         // links: a slot that switched off (its last point) or on (its first point) between s-1 and s is one
@@ -420,10 +426,14 @@ UL_HDN void regions_phaseB(int lane, RegionWork<DEG>& W)
 template <int N>
 UL_HD void patch_tangents(const Lens& L, const TangentTable& T, const BoxExt& x, bool from_origin, PatchTan& out)
 {
-    for (int k = 0; k < UL_NT; ++k) { out.rlo_dot[k] = 0.0; out.rhi_dot[k] = 0.0; }
+    for (int k = 0; k < UL_NT; ++k) { out.rlo_dot[k] = 0.0; out.rhi_dot[k] = 0.0; out.tlo_dot[k] = 0.0; out.thi_dot[k] = 0.0; }
     if (x.hi_r < 0.0) return;                           // no own point (links only): frozen
     if (!from_origin) limb_point_rdot<N>(L, T, x.lo_x, x.lo_y, x.lo_ph, out.rlo_dot);
     limb_point_rdot<N>(L, T, x.hi_x, x.hi_y, x.hi_ph, out.rhi_dot);
+    if (x.thi_t > -1e299 && !from_origin) {             // theta ends (used by sectors scanned along radial lines)
+        limb_point_rdot<N>(L, T, x.tlo_x, x.tlo_y, x.tlo_ph, nullptr, out.tlo_dot);
+        limb_point_rdot<N>(L, T, x.thi_x, x.thi_y, x.thi_ph, nullptr, out.thi_dot);
+    }
 }
 
 // ---------------------------------------------------------------------------------------------- phase C
@@ -441,6 +451,7 @@ UL_HD void emit_patch(Patch& out, const RegionParams& P, int point, double rl, d
 {
     double r_ext = rh - rl;
     double t_ext = periodic ? 2.0 * UL_PI : (th - tl);
+    out.kap_lo = out.kap_hi = 0.0;
     // lines: spaced by the projected half-extent / n_r; nodes on a line: by the half-chord / n_theta
     double hr = ul_min(scan_r ? cr_ : hr_, 0.5 * r_ext);
     double ht = ul_min(scan_r ? ht_ : ct_, 0.5 * t_ext * rh);
@@ -459,7 +470,8 @@ UL_HD void emit_patch(Patch& out, const RegionParams& P, int point, double rl, d
         // ALONG the scan lines a generous margin costs only a few nodes: 3 cells for the cubic stencil + 5 % of
         // the span; ACROSS the lines the sector must end where the image ends (sin-spaced lines): no margin
         double e_lo = ul_min(3.0 * dth + 0.05 * t_ext, 0.45 * gap_t_lo), e_hi = ul_min(3.0 * dth + 0.05 * t_ext, 0.45 * gap_t_hi);
-        if (scan_r) e_lo = e_hi = 0.0;
+        if (scan_r) { e_lo = ul_min(0.002 * t_ext, 0.45 * gap_t_lo); e_hi = ul_min(0.002 * t_ext, 0.45 * gap_t_hi); }   // tips thinner than a parabola
+        if (scan_r) { out.kap_lo = e_lo / t_ext; out.kap_hi = e_hi / t_ext; }
         tl -= e_lo;
         span_t = t_ext + e_lo + e_hi;
         const double span = span_t;
@@ -472,7 +484,8 @@ UL_HD void emit_patch(Patch& out, const RegionParams& P, int point, double rl, d
     {
         // radial scan lines need 3 empty nodes per side for the cubic stencil; rings need none
         double e_lo = ul_min(3.0 * dr + 0.05 * r_ext, 0.45 * gap_r_lo), e_hi = ul_min(3.0 * dr + 0.05 * r_ext, 0.45 * gap_r_hi);
-        if (!scan_r) e_lo = e_hi = 0.0;
+        if (!scan_r) { e_lo = ul_min(0.002 * r_ext, 0.45 * gap_r_lo); e_hi = ul_min(0.002 * r_ext, 0.45 * gap_r_hi); }
+        if (!scan_r) { out.kap_lo = e_lo / r_ext; out.kap_hi = e_hi / r_ext; }
         if (rl <= 0.0) e_lo = 0.0;
         rl -= e_lo;
         span_r = r_ext + e_lo + e_hi;
@@ -572,6 +585,7 @@ UL_HDN int regions_phaseC(RegionWork<N * N + 1>& W, const RegionParams& P, int p
             // filled ring / disk: one full-ring sector scanned along radial lines
             double hr = 1e300, ht = 1e300, cr = 1e300, ct = 1e300;
             BoxExt xlo; xlo.lo_r = 1e300; xlo.hi_r = -1.0; xlo.lo_x = xlo.lo_y = xlo.lo_ph = xlo.hi_x = xlo.hi_y = xlo.hi_ph = 0.0;
+            xlo.tlo_t = 1e300; xlo.thi_t = -1e300; xlo.tlo_x = xlo.tlo_y = xlo.tlo_ph = xlo.thi_x = xlo.thi_y = xlo.thi_ph = 0.0;   // full ring: theta frozen
             for (int i = 0; i < n; ++i) {
                 const SubBox& b = W.box[i];
                 if (b.r_lo > b.r_hi) continue;
@@ -627,7 +641,8 @@ UL_HDN int regions_phaseC(RegionWork<N * N + 1>& W, const RegionParams& P, int p
         // ---- tight bounds of each theta-group's members
         double c_rl[UL_MAXG], c_rh[UL_MAXG], c_tl[UL_MAXG], c_th[UL_MAXG], c_hr[UL_MAXG], c_ht[UL_MAXG], c_cr[UL_MAXG], c_ct[UL_MAXG];
         BoxExt c_ext[UL_MAXG];
-        for (int g = 0; g < ngt; ++g) { c_ext[g].lo_r = 1e300; c_ext[g].hi_r = -1.0; c_ext[g].lo_x = c_ext[g].lo_y = c_ext[g].lo_ph = c_ext[g].hi_x = c_ext[g].hi_y = c_ext[g].hi_ph = 0.0; }
+        for (int g = 0; g < ngt; ++g) { c_ext[g].lo_r = 1e300; c_ext[g].hi_r = -1.0; c_ext[g].lo_x = c_ext[g].lo_y = c_ext[g].lo_ph = c_ext[g].hi_x = c_ext[g].hi_y = c_ext[g].hi_ph = 0.0;
+            c_ext[g].tlo_t = 1e300; c_ext[g].thi_t = -1e300; c_ext[g].tlo_x = c_ext[g].tlo_y = c_ext[g].tlo_ph = c_ext[g].thi_x = c_ext[g].thi_y = c_ext[g].thi_ph = 0.0; }
         for (int g = 0; g < ngt; ++g) { c_rl[g] = 1e300; c_rh[g] = -1e300; c_tl[g] = 1e300; c_th[g] = -1e300; c_hr[g] = c_ht[g] = c_cr[g] = c_ct[g] = 1e300; }
         for (int i = 0; i < n; ++i) {
             const SubBox& b = W.box[i];
@@ -652,6 +667,9 @@ UL_HDN int regions_phaseC(RegionWork<N * N + 1>& W, const RegionParams& P, int p
                 BoxExt& x = c_ext[c];
                 if (e.lo_r < x.lo_r) { x.lo_r = e.lo_r; x.lo_x = e.lo_x; x.lo_y = e.lo_y; x.lo_ph = e.lo_ph; }
                 if (e.hi_r > x.hi_r) { x.hi_r = e.hi_r; x.hi_x = e.hi_x; x.hi_y = e.hi_y; x.hi_ph = e.hi_ph; }
+                // theta ends in the cell's own unwrapping: this box's interval is [tl, th] after the shifts above
+                if (tl < x.tlo_t) { x.tlo_t = tl; x.tlo_x = e.tlo_x; x.tlo_y = e.tlo_y; x.tlo_ph = e.tlo_ph; }
+                if (th > x.thi_t) { x.thi_t = th; x.thi_x = e.thi_x; x.thi_y = e.thi_y; x.thi_ph = e.thi_ph; }
             }
         }
         for (int c = 0; c < ngt; ++c) {
@@ -689,7 +707,7 @@ UL_HDN int regions_phaseC(RegionWork<N * N + 1>& W, const RegionParams& P, int p
             rl = ul_min(rl, a1); rh = ul_max(rh, a2); hr = ul_min(hr, b.hr); ht = ul_min(ht, b.ht); cr = ul_min(cr, b.cr); ct = ul_min(ct, b.ct);
         }
         np = 0; units_left = P.max_units_pt;
-        for (int k = 0; k < UL_NT; ++k) { W.ptan[0].rlo_dot[k] = 0.0; W.ptan[0].rhi_dot[k] = 0.0; }
+        for (int k = 0; k < UL_NT; ++k) { W.ptan[0].rlo_dot[k] = 0.0; W.ptan[0].rhi_dot[k] = 0.0; W.ptan[0].tlo_dot[k] = 0.0; W.ptan[0].thi_dot[k] = 0.0; }
         emit_patch(W.patch[np++], P, point, rl, rh, -UL_PI, UL_PI, hr, ht, cr, ct, true, false, rl, 1e300, 0.0, 0.0,
                    units_left, status);
     }
