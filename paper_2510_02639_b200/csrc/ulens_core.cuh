@@ -18,9 +18,11 @@
 #if defined(__CUDACC__)
 #define UL_HD __host__ __device__ __forceinline__
 #define UL_HDN __host__ __device__
+#define UL_HDNI __host__ __device__ __noinline__
 #else
 #define UL_HD inline
 #define UL_HDN inline
+#define UL_HDNI inline
 #endif
 
 namespace ulens {
@@ -345,6 +347,28 @@ UL_HD void match_roots(const double* ozr, const double* ozi, double* zr, double*
 #pragma unroll
         for (int j = 0; j < DEG; ++j) { zr[j] = nr[j]; zi[j] = ni[j]; }
     }
+}
+
+// Out-of-line copies for the region builder: k_regions calls these from several places inside loops over
+// the root slots; inlined and unrolled they made a 0.5-1 MB kernel that stalled on instruction fetch
+// (ncu: stall_no_instruction 11.8 per issue). The arithmetic is the same.
+template <int DEG>
+UL_HDNI int ea_iterate_ni(const double* br, const double* bi, double* zr, double* zi, int max_it, double tol2)
+{
+    return ea_iterate<DEG>(br, bi, zr, zi, max_it, tol2);
+}
+template <int DEG>
+UL_HDNI void ea_init_ni(const double* br, const double* bi, double* zr, double* zi) { ea_init<DEG>(br, bi, zr, zi); }
+template <int N>
+UL_HDNI bool polish_image_ni(const Lens& L, double wx, double wy, double& zx, double& zy, int max_it,
+                             double tol, double& detJ, double& resid, double& gx, double& gy)
+{
+    return polish_image<N>(L, wx, wy, zx, zy, max_it, tol, detJ, resid, gx, gy);
+}
+template <int N>
+UL_HDNI void poly_coeffs_ni(const Lens& L, const LensPoly& T, double wx, double wy, double* br, double* bi)
+{
+    poly_coeffs<N>(L, T, wx, wy, br, bi);
 }
 
 // ------------------------------------------------------------------------------------------------

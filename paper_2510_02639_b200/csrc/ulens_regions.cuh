@@ -152,7 +152,6 @@ UL_HDN void regions_phaseA(int lane, const Lens& L, const LensPoly& T, double wc
     double zr[DEG], zi[DEG], ozr[DEG], ozi[DEG], pvx[DEG], pvy[DEG];
     double br[DEG + 1], bi[DEG + 1];
     unsigned valid_prev = 0, faint_prev = 0;
-#pragma unroll
     BoxExt* E = W.ext ? &W.ext[lane * DEG] : nullptr;
     if (E) for (int j = 0; j < DEG; ++j) { E[j].lo_r = 1e300; E[j].hi_r = -1.0; E[j].lo_x = E[j].lo_y = E[j].lo_ph = E[j].hi_x = E[j].hi_y = E[j].hi_ph = 0.0;
         E[j].tlo_t = 1e300; E[j].thi_t = -1e300; E[j].tlo_x = E[j].tlo_y = E[j].tlo_ph = E[j].thi_x = E[j].thi_y = E[j].thi_ph = 0.0; }
@@ -176,15 +175,25 @@ UL_HDN void regions_phaseA(int lane, const Lens& L, const LensPoly& T, double wc
         if (ph + st_try > ph_end - 1e-9 * dphi) st_try = ph_end - ph;      // land exactly on the arc's end
         const double ph_new = first ? ph0 : ph + st_try;
         double wx = wcx + rho * cos(ph_new), wy = wcy + rho * sin(ph_new);      // Eq. 8 (G2)
-        poly_coeffs<N>(L, T, wx, wy, br, bi);
-        // limb solves only have to land in the basin of the Eq.-1 polish: relative step 1e-7
+        poly_coeffs_ni<N>(L, T, wx, wy, br, bi);
+        // limb solves only have to land in the basin of the Eq.-1 polish: relative step 1e-7.
+        // Warm start from the previous limb point (cap 24); cold restart from the Cauchy circle (cap 64) for the
+        // arc's first point or when the warm solve hits its cap. One call site each (code size).
         int it;
-        if (first) { ea_init<DEG>(br, bi, zr, zi); it = ea_iterate<DEG>(br, bi, zr, zi, 64, 1e-14); }
-        else {
+        bool cold = first;
+        if (!first) {
 #pragma unroll
             for (int j = 0; j < DEG; ++j) { ozr[j] = zr[j]; ozi[j] = zi[j]; }
-            it = ea_iterate<DEG>(br, bi, zr, zi, 24, 1e-14);
-            if (it > 24) { ea_init<DEG>(br, bi, zr, zi); it = ea_iterate<DEG>(br, bi, zr, zi, 64, 1e-14); if (it <= 64) it = 1; }
+        }
+#pragma unroll 1
+        for (;;) {
+            if (cold) ea_init_ni<DEG>(br, bi, zr, zi);
+            it = ea_iterate_ni<DEG>(br, bi, zr, zi, cold ? 64 : 24, 1e-14);
+            if (cold || it <= 24) break;
+            cold = true;
+        }
+        if (!first) {
+            if (cold && it <= 64) it = 1;
             match_roots<DEG>(ozr, ozi, zr, zi);          // slot j keeps following the same root
         }
         ++n_solves;
@@ -192,14 +201,14 @@ UL_HDN void regions_phaseA(int lane, const Lens& L, const LensPoly& T, double wc
 
         unsigned valid = 0, faint = 0;
         double px[DEG], py[DEG], hrr[DEG], htt[DEG], crr[DEG], ctt[DEG];
-#pragma unroll
+#pragma unroll 1
         for (int j = 0; j < DEG; ++j) {
             double zx = zr[j], zy = zi[j], detJ, resid, gx, gy;
             // distance of the EA root to the nearest lens bounds how far the polish may move it
             double dm2 = 1e300;
 #pragma unroll
             for (int i = 0; i < N; ++i) { double dx = zx - L.ax[i], dy = zy - L.ay[i]; dm2 = ul_min(dm2, dx * dx + dy * dy); }
-            bool ok = polish_image<N>(L, wx, wy, zx, zy, 6, 1e-9, detJ, resid, gx, gy);
+            bool ok = polish_image_ni<N>(L, wx, wy, zx, zy, 6, 1e-9, detJ, resid, gx, gy);
             // along the limb a slot must follow ONE image continuously: a polish that carries the EA root
             // further than 10 % of its distance to the nearest lens has jumped to some other image
             double mv2 = (zx - zr[j]) * (zx - zr[j]) + (zy - zi[j]) * (zy - zi[j]);
@@ -208,7 +217,7 @@ UL_HDN void regions_phaseA(int lane, const Lens& L, const LensPoly& T, double wc
             // resolve the root clusters next to a light lens in double) is re-polished from that image
             if (!ok && (valid_prev & (1u << j))) {
                 zx = pvx[j]; zy = pvy[j];
-                ok = polish_image<N>(L, wx, wy, zx, zy, 10, 1e-9, detJ, resid, gx, gy);
+                ok = polish_image_ni<N>(L, wx, wy, zx, zy, 10, 1e-9, detJ, resid, gx, gy);
                 double jx = zx - pvx[j], jy = zy - pvy[j];
                 ok = ok && (jx * jx + jy * jy <= 0.0016 * ul_max(zx * zx + zy * zy, 0.04));
             }
@@ -236,11 +245,11 @@ UL_HDN void regions_phaseA(int lane, const Lens& L, const LensPoly& T, double wc
             // unrestricted polish, duplicates removed, faint images seeded): damped Newton on Eq. 1 for this
             // limb point from each of them. Whatever it converges to is an image of the limb point; if no
             // slot holds it yet it takes a free one.
-#pragma unroll
+#pragma unroll 1
             for (int m = 0; m < DEG; ++m) {
                 if (!(cmask & (1u << m))) continue;
                 double zx = czr[m], zy = czi[m], detJ, resid, gx, gy;
-                if (!polish_image<N>(L, wx, wy, zx, zy, 12, 1e-9, detJ, resid, gx, gy)) continue;
+                if (!polish_image_ni<N>(L, wx, wy, zx, zy, 12, 1e-9, detJ, resid, gx, gy)) continue;
                 bool dup = false;
                 int free_slot = -1;
 #pragma unroll
@@ -280,7 +289,7 @@ UL_HDN void regions_phaseA(int lane, const Lens& L, const LensPoly& T, double wc
         if (lane == UL_DEBUG_PHASEA) { printf("lane %d ph %.6f step %.3g it %d valid %x:", lane, ph_new / dphi, st_try / dphi, it, valid); for (int j = 0; j < DEG; ++j) printf(" (%.6f,%.6f)", px[j], py[j]); printf("\n"); }
 #endif
         // own points
-#pragma unroll
+#pragma unroll 1
         for (int j = 0; j < DEG; ++j) {
             if (!(valid & ~faint & (1u << j))) continue;
             // A box holds ONE arc. If this slot's image is nowhere near the last point of its box (the slot
@@ -343,11 +352,11 @@ UL_HDN void regions_phaseA(int lane, const Lens& L, const LensPoly& T, double wc
                 double ex[DEG], ey[DEG];
 #pragma unroll
                 for (int a = 0; a < DEG; ++a) { ex[a] = (off & (1u << a)) ? pvx[a] : px[a]; ey[a] = (off & (1u << a)) ? pvy[a] : py[a]; }
-#pragma unroll
+#pragma unroll 1
                 for (int a = 0; a < DEG; ++a) {
                     if (!(grp & ~(faint | faint_prev) & (1u << a))) continue;
                     int nb = -1; double bd = 0.25;
-#pragma unroll
+#pragma unroll 1
                     for (int b = 0; b < DEG; ++b) {
                         if (b == a || !(grp & ~(faint | faint_prev) & (1u << b))) continue;
                         double dx = ex[a] - ex[b], dy = ey[a] - ey[b];
