@@ -38,6 +38,9 @@ UNIT = "magnifications/s"
 # the lens map with one reciprocal per ray, the rotation recurrence, d^2 and the inside test; the limb-
 # darkened figure adds the square root of the inside rays (about half of all rays).
 FP64_INSTR_PER_RAY = {(1, False): 27, (1, True): 32, (2, False): 35, (2, True): 40, (3, False): 47, (3, True): 52}
+# Forward-mode variant (binary, 5 intrinsic tangents): per tangent the moving ray dz (2), g conj(dz) (4), the explicit
+# lens-parameter term (0..8, mean 3), dF (4), accumulation (1) = 14, plus g itself (4 per ray): + 74 per ray.
+FP64_INSTR_PER_RAY_DUAL_EXTRA = 74
 # FP64 FMA pipe of one B200: 148 SMs x 64 DFMA lanes / clk x 1.965 GHz (clocks.max.sm) -- DESIGN.md
 FP64_PEAK_DFMA = 148 * 64 * 1.965e9
 
@@ -195,6 +198,7 @@ def main_ours(args, rank, local_rank, world):
     lenses = gpu_lenses(binding, wl)
     n = wl.n_cfg * wl.n_pts
     ctx = binding.Context(local_rank)
+    dual = args.config == 4                                          # C4: trajectory parameters in, A and dA/d(7) out
     w_re = torch.tensor(np.ascontiguousarray(wl.w.real), device=dev)
     w_im = torch.tensor(np.ascontiguousarray(wl.w.imag), device=dev)
     A = torch.empty((wl.n_cfg, wl.n_pts), dtype=torch.float64, device=dev)
@@ -202,8 +206,15 @@ def main_ours(args, rank, local_rank, world):
     st = torch.empty((wl.n_cfg, wl.n_pts), dtype=torch.int32, device=dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)    # > 126 MB L2
 
+    if dual:
+        t_dev = torch.tensor(wl.t.copy(), device=dev)
+        dA = torch.empty((wl.n_cfg, wl.n_pts, 7), dtype=torch.float64, device=dev)
+
     def step():
-        ctx.ulens_mag(lenses, wl.rho, wl.u1, w_re, w_im, A, err, st)
+        if dual:
+            ctx.ulens_lightcurve_binary(wl.theta, float(wl.u1[0]), t_dev, out=(A, dA, err, st))
+        else:
+            ctx.ulens_mag(lenses, wl.rho, wl.u1, w_re, w_im, A, err, st)
 
     def barrier():
         if world > 1:
@@ -243,11 +254,25 @@ def main_ours(args, rank, local_rank, world):
     h_err = torch.empty((wl.n_cfg, wl.n_pts), dtype=torch.float64).pin_memory()
     h_st = torch.empty((wl.n_cfg, wl.n_pts), dtype=torch.int32).pin_memory()
     e2e_steps = max(1, min(args.steps, 3))
-    ctx.ulens_mag_host(lenses, wl.rho, wl.u1, h_re.numpy(), h_im.numpy(), h_A.numpy(), h_err.numpy(), h_st.numpy())
+    if dual:
+        h_t = torch.tensor(wl.t.copy()).pin_memory()
+        h_dA = torch.empty((wl.n_cfg, wl.n_pts, 7), dtype=torch.float64).pin_memory()
+
+        def e2e_step():
+            ctx.ulens_lightcurve_binary_host(wl.theta, float(wl.u1[0]), h_t.numpy(), h_A.numpy(), h_dA.numpy(),
+                                             h_err.numpy(), h_st.numpy())
+        h2d, d2h = 8 * wl.n_pts + 56 * wl.n_cfg, (8 + 56 + 8 + 4) * n
+        e2e_api = "ulens_lightcurve_binary_host (pinned host buffers)"
+    else:
+        def e2e_step():
+            ctx.ulens_mag_host(lenses, wl.rho, wl.u1, h_re.numpy(), h_im.numpy(), h_A.numpy(), h_err.numpy(), h_st.numpy())
+        h2d, d2h = 16 * n, 20 * n
+        e2e_api = "ulens_mag_host (pinned host buffers)"
+    e2e_step()
     barrier()
     t0 = time.perf_counter()
     for _ in range(e2e_steps):
-        ctx.ulens_mag_host(lenses, wl.rho, wl.u1, h_re.numpy(), h_im.numpy(), h_A.numpy(), h_err.numpy(), h_st.numpy())
+        e2e_step()
     barrier()
     e2e_s = time.perf_counter() - t0
     assert np.array_equal(h_A.numpy(), A_host, equal_nan=True), "host entry and device entry disagree"
@@ -267,11 +292,12 @@ def main_ours(args, rank, local_rank, world):
         shoot_ms, shoot_n = kms["k_shoot"]
         rays_per_step = stats["n_rays"] / args.steps
         rays_per_launch = stats["n_rays"] / max(shoot_n, 1)
-        ipr = FP64_INSTR_PER_RAY[(n_lens, ld)]
+        ipr = FP64_INSTR_PER_RAY[(n_lens, ld)] + (FP64_INSTR_PER_RAY_DUAL_EXTRA if dual else 0)
         shoot_avg_s = shoot_ms * 1e-3 / max(shoot_n, 1)
         achieved = 2.0 * ipr * rays_per_launch / shoot_avg_s / 1e12
         peak_measured = ctx.ulens_fp64_peak(200.0)
         roofline = {"bound": "alu", "kernel": "k_shoot", "achieved": achieved, "peak": 2.0 * FP64_PEAK_DFMA / 1e12,
+                    "variant": "k_shoot_dual (value + 5 tangents per ray)" if dual else "k_shoot",
                     "unit": "TFLOP/s", "frac": achieved / (2.0 * FP64_PEAK_DFMA / 1e12), "traffic": None,
                     "peak_source": "derived: 148 SM x 64 DFMA/clk x 1.965 GHz x 2 flop (DESIGN.md); "
                                    "MEASURED_PEAKS.json has no FP64 entry",
@@ -290,8 +316,8 @@ def main_ours(args, rank, local_rank, world):
                 "kernel_ms_per_step": {k: v[0] / args.steps for k, v in kms.items()},
                 "flagged_points": int(((status & 0xff) != 0).sum()), "nan_points": int(np.isnan(A_host).sum()),
                 "roofline": roofline,
-                "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 16 * n, "d2h_bytes_per_step": 20 * n,
-                        "steps": e2e_steps, "api": "ulens_mag_host (pinned host buffers)"},
+                "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                        "steps": e2e_steps, "api": e2e_api},
                 "gpu_launches": launches_per_step * args.steps,
                 "clocks": clk}
         if not args.no_cpu_baseline and world == 1:
@@ -312,7 +338,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=1, help="BASELINE.json config index 0..3 (default 1)")
+    ap.add_argument("--config", type=int, default=1, help="BASELINE.json config index 0..4 (default 1; 4 = light curves with forward-mode derivatives)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

@@ -133,6 +133,14 @@ int  ulens_lightcurve_binary(ulens_ctx* ctx, int n_cfg, int n_epochs,
                const double* theta_host, double u1, const double* t,
                double* A_out, double* dA_out, double* err_out, uint32_t* status_out, void* stream);
 
+/* Same with HOST arrays for t, A_out, dA_out (may be NULL), err_out (may be NULL), status_out (may be NULL):
+ * copies t in, computes, copies the results out and synchronises the stream before returning
+ * (the end-to-end entry point of the light-curve / derivative path, BASELINE.json configs[4]). */
+int  ulens_lightcurve_binary_host(ulens_ctx* ctx, int n_cfg, int n_epochs,
+               const double* theta_host, double u1, const double* t_host,
+               double* A_out_host, double* dA_out_host, double* err_out_host, uint32_t* status_out_host,
+               void* stream);
+
 /* (iii) Root export (Eq. 4, Eq. 7): all N^2+1 roots of the lens polynomial for
  * each source position and which of them are images (validated on Eq. 1; images are polished
  * on Eq. 1). roots_re/im device [n_pts][n_deg], is_image device [n_pts][n_deg] bytes, n_deg = N^2+1. */

@@ -20,7 +20,7 @@ ST_NIMG_SHIFT = 8
 KERNEL_NAMES = ["k_traj", "k_roots", "k_regions", "k_shoot", "k_finalize"]     # ULENS_K_* order
 
 EXPORTS = ["ulens_create", "ulens_destroy", "ulens_lens_binary", "ulens_lens_triple", "ulens_mag", "ulens_mag_grad",
-           "ulens_mag_host", "ulens_lightcurve_binary", "ulens_roots", "ulens_get_stats",
+           "ulens_mag_host", "ulens_lightcurve_binary", "ulens_lightcurve_binary_host", "ulens_roots", "ulens_get_stats",
            "ulens_reset_stats", "ulens_last_launch_count", "ulens_set_timing", "ulens_get_kernel_ms", "ulens_fp64_peak", "ulens_strerror",
            "ulens_last_cuda_error"]
 
@@ -64,6 +64,7 @@ def lib() -> C.CDLL:
         L.ulens_mag_grad.argtypes = [vp, ip, ip, C.POINTER(ulens_lens), dp, dp, vp, vp, vp, vp, vp, vp, vp]
         L.ulens_mag_host.argtypes = [vp, ip, ip, C.POINTER(ulens_lens), dp, dp, vp, vp, vp, vp, vp, vp]
         L.ulens_lightcurve_binary.argtypes = [vp, ip, ip, dp, C.c_double, vp, vp, vp, vp, vp, vp]
+        L.ulens_lightcurve_binary_host.argtypes = [vp, ip, ip, dp, C.c_double, vp, vp, vp, vp, vp, vp]
         L.ulens_roots.argtypes = [vp, C.POINTER(ulens_lens), ip, vp, vp, vp, vp, vp, vp]
         L.ulens_get_stats.argtypes = [vp, C.POINTER(ulens_stats)]
         L.ulens_reset_stats.argtypes = [vp]
@@ -215,21 +216,42 @@ class Context:
                                     st.ctypes.data_as(C.c_void_p), self._stream(stream)), self._h)
         return A, err, st
 
-    def ulens_lightcurve_binary(self, theta, u1, t, want_dA=False, stream=None):
-        """theta: host [n_cfg, 7] (t0,u0,tE,s,q,rho,alpha); t: CUDA float64 [n_epochs]."""
+    def ulens_lightcurve_binary(self, theta, u1, t, want_dA=False, stream=None, out=None):
+        """theta: host [n_cfg, 7] (t0,u0,tE,s,q,rho,alpha); t: CUDA float64 [n_epochs];
+        out: optional caller-owned CUDA tensors (A, dA, err, st) to write into."""
         torch = self._torch
         theta = np.ascontiguousarray(theta, dtype=np.float64).reshape(-1, 7)
         n_cfg, n_ep = theta.shape[0], t.numel()
         dev = t.device
-        A = torch.empty((n_cfg, n_ep), dtype=torch.float64, device=dev)
-        err = torch.empty((n_cfg, n_ep), dtype=torch.float64, device=dev)
-        st = torch.empty((n_cfg, n_ep), dtype=torch.int32, device=dev)
-        dA = torch.empty((n_cfg, n_ep, 7), dtype=torch.float64, device=dev) if want_dA else None
+        if out is not None:
+            A, dA, err, st = out
+            want_dA = dA is not None
+        else:
+            A = torch.empty((n_cfg, n_ep), dtype=torch.float64, device=dev)
+            err = torch.empty((n_cfg, n_ep), dtype=torch.float64, device=dev)
+            st = torch.empty((n_cfg, n_ep), dtype=torch.int32, device=dev)
+            dA = torch.empty((n_cfg, n_ep, 7), dtype=torch.float64, device=dev) if want_dA else None
         _check(lib().ulens_lightcurve_binary(self._h, n_cfg, n_ep, _dptr(theta), float(u1),
                                              _dev(t, torch.float64, n_ep), _dev(A, torch.float64, n_cfg * n_ep),
                                              _dev(dA, torch.float64, n_cfg * n_ep * 7) if want_dA else None,
                                              _dev(err, torch.float64, n_cfg * n_ep),
                                              _dev(st, torch.int32, n_cfg * n_ep), self._stream(stream)), self._h)
+        return A, dA, err, st
+
+    def ulens_lightcurve_binary_host(self, theta, u1, t, A, dA=None, err=None, st=None, stream=None):
+        """Host numpy arrays in / out (e.g. views of pinned tensors): t [n_epochs]; A, err [n_cfg, n_epochs];
+        dA [n_cfg, n_epochs, 7] or None; st 32-bit. The copies and the synchronisation happen inside the C call."""
+        theta = np.ascontiguousarray(theta, dtype=np.float64).reshape(-1, 7)
+        t = np.ascontiguousarray(t, dtype=np.float64)
+        n_cfg, n_ep = theta.shape[0], t.size
+        for a, k in ((A, 1), (dA, 7), (err, 1)):
+            if a is not None and (a.dtype != np.float64 or not a.flags.c_contiguous or a.size != k * n_cfg * n_ep):
+                raise UlensError("output arrays must be C-contiguous float64 of the documented size")
+        if st is not None and (st.dtype.itemsize != 4 or not st.flags.c_contiguous or st.size != n_cfg * n_ep):
+            raise UlensError("status array must be C-contiguous 32-bit of n_cfg*n_epochs elements")
+        p = lambda a: a.ctypes.data_as(C.c_void_p) if a is not None else None
+        _check(lib().ulens_lightcurve_binary_host(self._h, n_cfg, n_ep, _dptr(theta), float(u1), p(t), p(A), p(dA),
+                                                  p(err), p(st), self._stream(stream)), self._h)
         return A, dA, err, st
 
     def ulens_roots(self, lens, w_re, w_im, stream=None):

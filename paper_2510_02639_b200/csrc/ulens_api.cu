@@ -181,8 +181,11 @@ __global__ void k_roots(int n, int pt_base, int n_pts_per_cfg, const PointCfg* _
 }
 
 // One warp per source point.
+#ifndef UL_REGIONS_MINB
+#define UL_REGIONS_MINB 2
+#endif
 template <int N>
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(128, UL_REGIONS_MINB)
 k_regions(int n, int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cfg, const LensPoly* __restrict__ poly,
           const double* __restrict__ w_re, const double* __restrict__ w_im, RegionParams rp,
           Patch* __restrict__ patches, int* __restrict__ n_patch, unsigned* __restrict__ status,
@@ -210,6 +213,8 @@ k_regions(int n, int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cf
     regions_phaseA<N>(lane, L, poly[c], wcx, wcy, rho, rp, W, st, n_solves, c_zr + (long long)i * 10, c_zi + (long long)i * 10, c_mask[i]);
     st = __reduce_or_sync(0xffffffffu, st);
     const int tot_solves = __reduce_add_sync(0xffffffffu, n_solves);
+    __syncwarp();
+    regions_phaseB_keys<DEG>(lane, W);
     __syncwarp();
     regions_phaseB<DEG>(lane, W);
     __syncwarp();
@@ -809,6 +814,36 @@ extern "C" int ulens_lightcurve_binary(ulens_ctx* ctx, int n_cfg, int n_epochs, 
         CK(cudaGetLastError());
     }
     return rc;
+}
+
+extern "C" int ulens_lightcurve_binary_host(ulens_ctx* ctx, int n_cfg, int n_epochs, const double* theta_host, double u1,
+                                            const double* t_host, double* A_out_host, double* dA_out_host,
+                                            double* err_out_host, uint32_t* status_out_host, void* stream)
+{
+    if (!ctx || n_cfg < 0 || n_epochs < 0) return ULENS_EINVAL;
+    if (n_cfg == 0 || n_epochs == 0) return ULENS_OK;
+    if (!theta_host || !t_host || !A_out_host) return ULENS_EINVAL;
+    CK(cudaSetDevice(ctx->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t n = (size_t)n_cfg * n_epochs;
+    const size_t need = (size_t)n_epochs + n * (3 + (dA_out_host ? 7 : 0));   // t, A, err, status (8-byte slots), dA
+    if (need > ctx->io_cap) {
+        cudaFree(ctx->io_buf); ctx->io_buf = nullptr; ctx->io_cap = 0;
+        if (cudaMalloc(&ctx->io_buf, sizeof(double) * need) != cudaSuccess) return ULENS_ENOMEM;
+        ctx->io_cap = need;
+    }
+    double* d_t = ctx->io_buf; double* d_A = d_t + n_epochs; double* d_err = d_A + n;
+    unsigned* d_st = reinterpret_cast<unsigned*>(d_err + n);
+    double* d_dA = dA_out_host ? d_err + 2 * n : nullptr;
+    CK(cudaMemcpyAsync(d_t, t_host, sizeof(double) * n_epochs, cudaMemcpyHostToDevice, st));
+    int rc = ulens_lightcurve_binary(ctx, n_cfg, n_epochs, theta_host, u1, d_t, d_A, d_dA, d_err, d_st, stream);
+    if (rc != ULENS_OK) return rc;
+    CK(cudaMemcpyAsync(A_out_host, d_A, sizeof(double) * n, cudaMemcpyDeviceToHost, st));
+    if (dA_out_host) CK(cudaMemcpyAsync(dA_out_host, d_dA, sizeof(double) * 7 * n, cudaMemcpyDeviceToHost, st));
+    if (err_out_host) CK(cudaMemcpyAsync(err_out_host, d_err, sizeof(double) * n, cudaMemcpyDeviceToHost, st));
+    if (status_out_host) CK(cudaMemcpyAsync(status_out_host, d_st, sizeof(unsigned) * n, cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    return ULENS_OK;
 }
 
 extern "C" int ulens_roots(ulens_ctx* ctx, const ulens_lens* lens_host, int n_pts, const double* w_re, const double* w_im,

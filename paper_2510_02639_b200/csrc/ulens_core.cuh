@@ -352,10 +352,57 @@ UL_HD void match_roots(const double* ozr, const double* ozi, double* zr, double*
 // Out-of-line copies for the region builder: k_regions calls these from several places inside loops over
 // the root slots; inlined and unrolled they made a 0.5-1 MB kernel that stalled on instruction fetch
 // (ncu: stall_no_instruction 11.8 per issue). The arithmetic is the same.
+// ea_iterate with the loop over the roots kept rolled (the root arrays are indexed dynamically and live in
+// local memory, L1-resident): one fifth / one tenth of the code of the unrolled form, same arithmetic.
 template <int DEG>
-UL_HDNI int ea_iterate_ni(const double* br, const double* bi, double* zr, double* zi, int max_it, double tol2)
+UL_HDNI int ea_iterate_ni(const double* br_, const double* bi_, double* zr, double* zi, int max_it, double tol2)
 {
-    return ea_iterate<DEG>(br, bi, zr, zi, max_it, tol2);
+    double br[DEG + 1], bi[DEG + 1], prev[DEG];
+#pragma unroll
+    for (int l = 0; l <= DEG; ++l) { br[l] = br_[l]; bi[l] = bi_[l]; }
+#pragma unroll
+    for (int k = 0; k < DEG; ++k) prev[k] = 1e300;
+    unsigned done = 0;
+    const unsigned all = (1u << DEG) - 1u;
+    for (int it = 1; it <= max_it; ++it) {
+        bool bad = false;
+#pragma unroll 1
+        for (int k = 0; k < DEG; ++k) {
+            if (done & (1u << k)) continue;
+            const double zkr = zr[k], zki = zi[k];
+            double pr, pi, dr, di;
+            horner2<DEG>(br, bi, zkr, zki, pr, pi, dr, di);
+            double p2 = pr * pr + pi * pi;
+            if (p2 == 0.0) { done |= 1u << k; continue; }
+            double d2 = dr * dr + di * di;
+            double nx, ny;
+            if (d2 > 0.0) { double id = 1.0 / d2; nx = (pr * dr + pi * di) * id; ny = (pi * dr - pr * di) * id; }
+            else { nx = 1e-3; ny = 1e-3; }
+            double sx = 0.0, sy = 0.0;
+#pragma unroll 1
+            for (int j = 0; j < DEG; ++j) {
+                if (j == k) continue;
+                double ux = zkr - zr[j], uy = zki - zi[j];
+                double u2 = ux * ux + uy * uy;
+                if (u2 > 0.0) { double iu = 1.0 / u2; sx += ux * iu; sy -= uy * iu; }
+            }
+            double ax = 1.0 - (nx * sx - ny * sy), ay = -(nx * sy + ny * sx);
+            double a2 = ax * ax + ay * ay;
+            double stx, sty;
+            if (a2 > 1e-300) { double ia = 1.0 / a2; stx = (nx * ax + ny * ay) * ia; sty = (ny * ax - nx * ay) * ia; }
+            else { stx = nx; sty = ny; }
+            const double nzr = zkr - stx, nzi = zki - sty;
+            zr[k] = nzr; zi[k] = nzi;
+            double z2 = nzr * nzr + nzi * nzi;
+            double rel = (stx * stx + sty * sty) / (z2 + 1e-12);
+            if (!(rel == rel)) bad = true;
+            if (rel < tol2 || (rel < 1e-6 && rel > 0.5 * prev[k])) done |= 1u << k;
+            prev[k] = rel;
+        }
+        if (bad) return max_it + 1;
+        if (done == all) return it;
+    }
+    return max_it + 1;
 }
 template <int DEG>
 UL_HDNI void ea_init_ni(const double* br, const double* bi, double* zr, double* zi) { ea_init<DEG>(br, bi, zr, zi); }

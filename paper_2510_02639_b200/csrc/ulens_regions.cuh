@@ -60,6 +60,7 @@ struct RegionWork {
     BoxExt* ext;            // [32 * DEG] or nullptr (primal run)
     PatchTan ptan[UL_MAXP];
     SubBox box[32 * DEG];
+    double key_r[32 * DEG], key_t[32 * DEG];   // lower r / lower theta of the expanded boxes (sort keys; empty: 1e300)
     short order_r[32 * DEG], order_t[32 * DEG];
     int n_sorted;
     unsigned status;
@@ -75,7 +76,7 @@ UL_HD double wrap_pi(double a)      // to (-pi, pi]
 }
 
 // add an image-limb point to a slot box (polar coordinates about the origin, G8)
-UL_HD void box_add(SubBox& b, double& t_cur, double r, double th, double hr, double ht, double cr, double ct, bool advance)
+UL_HDNI void box_add(SubBox& b, double& t_cur, double r, double th, double hr, double ht, double cr, double ct, bool advance)
 {
     if (b.r_lo > b.r_hi) {               // first point
         b.r_lo = b.r_hi = r; b.t_lo = b.t_hi = th; b.hr = hr; b.ht = ht; b.cr = cr; b.ct = ct; t_cur = th;
@@ -93,7 +94,7 @@ UL_HD void box_add(SubBox& b, double& t_cur, double r, double th, double hr, dou
 // extreme of the parabola through three consecutive boundary samples (x = limb angle, y = r or theta), if the
 // middle sample is a local extreme: the image boundary bulges beyond its samples by ~ (step)^2 / 8 x curvature,
 // which matters now that the sector margins are tight
-UL_HD bool parabola_vertex(double x0, double y0, double x1, double y1, double x2, double y2, double& yv)
+UL_HDNI bool parabola_vertex(double x0, double y0, double x1, double y1, double x2, double y2, double& yv)
 {
     if (!((y1 >= y0 && y1 >= y2) || (y1 <= y0 && y1 <= y2))) return false;
     double h0 = x1 - x0, h1 = x2 - x1;
@@ -112,7 +113,7 @@ UL_HD bool parabola_vertex(double x0, double y0, double x1, double y1, double x2
 // radius rho is an ellipse with semi-axes rho/(1+|g|) (along arg(g)/2) and rho/|1-|g|| (perpendicular);
 // hr, ht = its half-extents (projections) along the radial / azimuthal direction at z; cr, ct = its
 // half-chords through the centre along those directions.
-UL_HD void local_extents(double zx, double zy, double gx, double gy, double rho, double& hr, double& ht,
+UL_HDNI void local_extents(double zx, double zy, double gx, double gy, double rho, double& hr, double& ht,
                          double& cr, double& ct)
 {
     double ga = sqrt(gx * gx + gy * gy);
@@ -409,20 +410,29 @@ UL_HD void box_expanded(const SubBox& b, double& rl, double& rh, double& tl, dou
 
 // ---------------------------------------------------------------------------------------------- phase B
 template <int DEG>
-UL_HDN void regions_phaseB(int lane, RegionWork<DEG>& W)
+UL_HDN void regions_phaseB_keys(int lane, RegionWork<DEG>& W)
 {
     const int n = 32 * DEG;
     for (int i = lane; i < n; i += 32) {
         const SubBox& b = W.box[i];
-        if (b.r_lo > b.r_hi) continue;
-        double rl, rh, tl, th;
-        box_expanded(b, rl, rh, tl, th);
+        double rl = 1e300, rh, tl = 1e300, th;
+        if (!(b.r_lo > b.r_hi)) box_expanded(b, rl, rh, tl, th);
+        W.key_r[i] = rl; W.key_t[i] = tl;
+    }
+}
+
+// rank sort on the cached keys (call regions_phaseB_keys first, then synchronise the warp)
+template <int DEG>
+UL_HDN void regions_phaseB(int lane, RegionWork<DEG>& W)
+{
+    const int n = 32 * DEG;
+    for (int i = lane; i < n; i += 32) {
+        const double rl = W.key_r[i], tl = W.key_t[i];
+        if (rl >= 1e300) continue;
         int rank_r = 0, rank_t = 0;
         for (int j = 0; j < n; ++j) {
-            const SubBox& c = W.box[j];
-            if (c.r_lo > c.r_hi || j == i) continue;
-            double rl2, rh2, tl2, th2;
-            box_expanded(c, rl2, rh2, tl2, th2);
+            const double rl2 = W.key_r[j], tl2 = W.key_t[j];
+            if (rl2 >= 1e300 || j == i) continue;
             rank_r += (rl2 < rl) || (rl2 == rl && j < i);
             rank_t += (tl2 < tl) || (tl2 == tl && j < i);
         }

@@ -23,7 +23,7 @@ def declared_symbols():
 
 def test_header_declares_the_boundary():
     syms = declared_symbols()
-    for s in ["ulens_create", "ulens_destroy", "ulens_mag", "ulens_mag_host", "ulens_lightcurve_binary", "ulens_roots",
+    for s in ["ulens_create", "ulens_destroy", "ulens_mag", "ulens_mag_host", "ulens_lightcurve_binary", "ulens_lightcurve_binary_host", "ulens_roots",
               "ulens_get_stats", "ulens_strerror", "ulens_lens_binary", "ulens_lens_triple", "ulens_fp64_peak"]:
         assert s in syms
 
