@@ -41,6 +41,10 @@ FP64_INSTR_PER_RAY = {(1, False): 27, (1, True): 32, (2, False): 35, (2, True): 
 # Forward-mode variant (binary, 5 intrinsic tangents): per tangent the moving ray dz (2), g conj(dz) (4), the explicit
 # lens-parameter term (0..8, mean 3), dF (4), accumulation (1) = 14, plus g itself (4 per ray): + 74 per ray.
 FP64_INSTR_PER_RAY_DUAL_EXTRA = 74
+# k_regions: algorithmic FP64-pipe instructions per limb solve: coefficients ~26 DEG, warm-started
+# Ehrlich-Aberth 3 iterations x DEG roots x (8 DEG Horner + 12 (DEG-1) repulsion + 24), Eq.-1 polish of the
+# N+1..DEG images 2.5 iterations x (17 N + 25), boxes ~100.
+FP64_INSTR_PER_LIMB_SOLVE = {1: 600, 2: 2400, 3: 8300}
 # FP64 FMA pipe of one B200: 148 SMs x 64 DFMA lanes / clk x 1.965 GHz (clocks.max.sm) -- DESIGN.md
 FP64_PEAK_DFMA = 148 * 64 * 1.965e9
 
@@ -185,7 +189,7 @@ def main_reference(args, rank, world):
 def main_ours(args, rank, local_rank, world):
     import torch
     import torch.distributed as dist
-    from paper_2510_02639_b200 import binding, inputs
+    from paper_2510_02639_b200 import binding, inputs, replicas
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device -- the hot path has no CPU fallback")
@@ -278,13 +282,10 @@ def main_ours(args, rank, local_rank, world):
     assert np.array_equal(h_A.numpy(), A_host, equal_nan=True), "host entry and device entry disagree"
 
     # ---- max over ranks
-    t = torch.tensor([ms, e2e_s], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms, e2e_s = float(t[0]), float(t[1])
+    ms, e2e_s = replicas.max_over_ranks([ms, e2e_s], dev)
     ms_per_step = ms / args.steps
-    value = world * n / (ms_per_step * 1e-3)
-    e2e_value = world * n / (e2e_s / e2e_steps)
+    value = replicas.aggregate_throughput(n, world, ms_per_step)
+    e2e_value = replicas.aggregate_throughput(n, world, 1e3 * e2e_s / e2e_steps)
 
     if rank == 0:
         n_lens = 2 if wl.kind == "binary" else 3
@@ -305,6 +306,14 @@ def main_ours(args, rank, local_rank, world):
                     "frac_of_measured": achieved / (2.0 * peak_measured / 1e12),
                     "fp64_instr_per_ray": ipr, "rays_per_launch": rays_per_launch,
                     "kernel_ms_avg": 1e3 * shoot_avg_s, "share_of_step": shoot_ms / ms}
+        reg_ms, reg_n = kms["k_regions"]
+        solves_per_launch = stats["n_limb_solves"] / max(reg_n, 1)
+        reg_ach = 2.0 * FP64_INSTR_PER_LIMB_SOLVE[n_lens] * solves_per_launch / (reg_ms * 1e-3 / max(reg_n, 1)) / 1e12
+        roofline_regions = {"bound": "alu", "kernel": "k_regions", "achieved": reg_ach, "peak": 2.0 * FP64_PEAK_DFMA / 1e12,
+                            "unit": "TFLOP/s", "frac": reg_ach / (2.0 * FP64_PEAK_DFMA / 1e12), "traffic": None,
+                            "fp64_instr_per_limb_solve": FP64_INSTR_PER_LIMB_SOLVE[n_lens],
+                            "limb_solves_per_point": stats["n_limb_solves"] / args.steps / n,
+                            "kernel_ms_avg": reg_ms / max(reg_n, 1), "share_of_step": reg_ms / ms}
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -315,7 +324,7 @@ def main_ours(args, rank, local_rank, world):
                 "rays_per_point": rays_per_step / n,
                 "kernel_ms_per_step": {k: v[0] / args.steps for k, v in kms.items()},
                 "flagged_points": int(((status & 0xff) != 0).sum()), "nan_points": int(np.isnan(A_host).sum()),
-                "roofline": roofline,
+                "roofline": roofline, "roofline_regions": roofline_regions,
                 "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                         "steps": e2e_steps, "api": e2e_api},
                 "gpu_launches": launches_per_step * args.steps,

@@ -117,7 +117,7 @@ UL_HD void lens_resid(const Lens& L, double zx, double zy, double wx, double wy,
 // (or the last Newton step) is below tol * max(1, |z|); z is updated in place; detJ = 1 - |g|^2 (Eq. 3).
 template <int N>
 UL_HD bool polish_image(const Lens& L, double wx, double wy, double& zx, double& zy, int max_it,
-                        double tol, double& detJ, double& resid, double& gx, double& gy)
+                        double tol, double& detJ, double& resid, double& gx, double& gy, double reject_frac2 = 0.0)
 {
     double fx, fy, dmin2;
     bool ok = false;
@@ -136,6 +136,9 @@ UL_HD bool polish_image(const Lens& L, double wx, double wy, double& zx, double&
         double qx = gx * bx + gy * by, qy = gy * bx - gx * by;
         double sx = (bx - qx) / detJ, sy = (by - qy) / detJ;
         double s2 = sx * sx + sy * sy;
+        // region builder only: a start whose FIRST Newton step already exceeds sqrt(reject_frac2) of its distance
+        // to the nearest lens is a spurious root of the polynomial, not an image known to ~1e-7
+        if (it == 0 && reject_frac2 > 0.0 && s2 > reject_frac2 * dmin2) return false;
         double lim2 = 0.25 * dmin2;
         if (s2 > lim2) { double k = sqrt(lim2 / s2); sx *= k; sy *= k; }
         zx += sx; zy += sy;
@@ -408,9 +411,9 @@ template <int DEG>
 UL_HDNI void ea_init_ni(const double* br, const double* bi, double* zr, double* zi) { ea_init<DEG>(br, bi, zr, zi); }
 template <int N>
 UL_HDNI bool polish_image_ni(const Lens& L, double wx, double wy, double& zx, double& zy, int max_it,
-                             double tol, double& detJ, double& resid, double& gx, double& gy)
+                             double tol, double& detJ, double& resid, double& gx, double& gy, double reject_frac2 = 0.0)
 {
-    return polish_image<N>(L, wx, wy, zx, zy, max_it, tol, detJ, resid, gx, gy);
+    return polish_image<N>(L, wx, wy, zx, zy, max_it, tol, detJ, resid, gx, gy, reject_frac2);
 }
 template <int N>
 UL_HDNI void poly_coeffs_ni(const Lens& L, const LensPoly& T, double wx, double wy, double* br, double* bi)
@@ -628,24 +631,32 @@ UL_HD void shoot_ring(const Lens& L, double wcx, double wcy, double rho2, double
     double U = 0.0, S = 0.0;
     edge = false;
     const int j_first = periodic ? 2 : 1;
-    for (int j = -2; j <= n_th + 1; ++j) {
-        f3 = ray_F<N>(L, r * c, r * s, wcx, wcy, rho2);
+    // per ray: count it, then close the pair (j-2, j-1) = (f1, f2) once its stencil (f0..f3) is complete
+    auto node = [&](int j, double f3) {
         if (j >= 0 && j < n_th && f3 < 0.0) {
             U += 1.0;
             if (LD) S += sqrt(-f3);
             if (!periodic && (j < 2 || j >= n_th - 2)) edge = true;
         }
-        // pair (j-2, j-1) = (f1, f2), stencil complete once f0 = F_{j-3} exists (j >= 1). In a periodic
-        // sector pair (-1, 0) is pair (n_th-1, n_th) again: take it once.
+        // stencil complete once f0 = F_{j-3} exists (j >= 1). In a periodic sector pair (-1, 0) is pair
+        // (n_th-1, n_th) again: take it once.
         if (j >= j_first && ((f1 < 0.0) != (f2 < 0.0))) {
             double u, dS; bool en;
             edge_event(f0, f1, f2, f3, LD, 0.0, u, en, dS);
             U += u - 0.5; S += dS;
         }
         f0 = f1; f1 = f2; f2 = f3;
-        double cn = c * cd - s * sd;
-        s = s * cd + c * sd;
-        c = cn;
+    };
+    // two rays in flight per iteration: their lens maps are independent, which doubles the FP64 pipe's
+    // instruction-level parallelism (the rotation recurrence is the only loop-carried chain)
+    for (int j = -2; j <= n_th + 1; j += 2) {
+        const double c2 = c * cd - s * sd, s2 = s * cd + c * sd;
+        const double fa = ray_F<N>(L, r * c, r * s, wcx, wcy, rho2);
+        const double fb = ray_F<N>(L, r * c2, r * s2, wcx, wcy, rho2);
+        node(j, fa);
+        if (j + 1 <= n_th + 1) node(j + 1, fb);
+        c = c2 * cd - s2 * sd;
+        s = s2 * cd + c2 * sd;
     }
     U_out = U; S_out = S;
 }
@@ -679,9 +690,7 @@ UL_HD void shoot_col(const Lens& L, double wcx, double wcy, double rho2, double 
     double f0 = UL_BIG, f1 = UL_BIG, f2 = UL_BIG, f3;
     double U = 0.0, S = 0.0, U2 = 0.0;
     edge = false;
-    for (int i = -2; i <= n_r + 1; ++i) {
-        double r = r0 + (i + 0.5) * dr;
-        f3 = ray_F<N>(L, r * c, r * s, wcx, wcy, rho2);
+    auto node = [&](int i, double r, double f3) {
         if (i >= 0 && i < n_r && f3 < 0.0) {
             U += r;
             if (LD) S += r * sqrt(-f3);
@@ -703,6 +712,13 @@ UL_HD void shoot_col(const Lens& L, double wcx, double wcy, double rho2, double 
             }
         }
         f0 = f1; f1 = f2; f2 = f3;
+    };
+    for (int i = -2; i <= n_r + 1; i += 2) {               // two rays in flight (see shoot_ring)
+        const double ra = r0 + (i + 0.5) * dr, rb = r0 + (i + 1.5) * dr;
+        const double fa = ray_F<N>(L, ra * c, ra * s, wcx, wcy, rho2);
+        const double fb = ray_F<N>(L, rb * c, rb * s, wcx, wcy, rho2);
+        node(i, ra, fa);
+        if (i + 1 <= n_r + 1) node(i + 1, rb, fb);
     }
     U_out = U * dr + U2; S_out = S * dr;
 }

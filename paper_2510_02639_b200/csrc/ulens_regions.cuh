@@ -209,7 +209,9 @@ UL_HDN void regions_phaseA(int lane, const Lens& L, const LensPoly& T, double wc
             double dm2 = 1e300;
 #pragma unroll
             for (int i = 0; i < N; ++i) { double dx = zx - L.ax[i], dy = zy - L.ay[i]; dm2 = ul_min(dm2, dx * dx + dy * dy); }
-            bool ok = polish_image_ni<N>(L, wx, wy, zx, zy, 6, 1e-9, detJ, resid, gx, gy);
+            // (0.04: the acceptance test below allows a total move of 10 % of that distance, so a first step
+            // beyond 20 % is rejected either way -- after one iteration instead of six)
+            bool ok = polish_image_ni<N>(L, wx, wy, zx, zy, 6, 1e-9, detJ, resid, gx, gy, 0.04);
             // along the limb a slot must follow ONE image continuously: a polish that carries the EA root
             // further than 10 % of its distance to the nearest lens has jumped to some other image
             double mv2 = (zx - zr[j]) * (zx - zr[j]) + (zy - zi[j]) * (zy - zi[j]);

@@ -120,7 +120,7 @@ def test_config4_derivatives_vs_oracle_fd(ctx, torch_cuda, oracle):
     seeded subsample (2 parameter vectors x 7 epochs spanning the peak)."""
     from paper_2510_02639_b200 import inputs
     torch = torch_cuda
-    wl = inputs.get(4, n_cfg=4, n_epochs=2000)
+    wl = inputs.get(4)                                     # the full C4 workload; vectors 0 and 3 of its 1,024
     sel = np.array([600, 800, 900, 950, 1050, 1100, 1300])
     t = torch.tensor(wl.t[sel].copy(), device="cuda:0")
     n_used = n_ok = 0

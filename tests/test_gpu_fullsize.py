@@ -1,0 +1,100 @@
+"""BASELINE.json's full-size workloads in the launch configuration bench.py times (one call over every point
+of the config, 65,536-point chunks), checked on sampled outputs and on properties that hold at any size.
+
+The sampled outputs are compared with a separate call on just the sample -- the call test_gpu_parity /
+test_gpu_dual compare with the oracle point by point -- so the full-size launch is tied to the oracle through
+values the oracle has checked. A point's result does not depend on its batch: same sectors, same rays, same
+(ordered) reduction, so the two calls must agree to the last bit.
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    return torch
+
+
+@pytest.fixture(scope="module")
+def ctx(torch_cuda):
+    from paper_2510_02639_b200 import binding, build
+    build.build()
+    c = binding.Context(0)
+    yield c
+    c.close()
+
+
+def _lenses(binding, wl, cs):
+    f = binding.ulens_lens_binary if wl.kind == "binary" else binding.ulens_lens_triple
+    return [f(*wl.lens_params[c]) for c in cs]
+
+
+@pytest.mark.parametrize("cfg,n_cfg_used,n_per_cfg", [(1, 8, 24), (2, 6, 16), (3, 4, 16)])
+def test_full_config_sampled_outputs_and_invariants(ctx, torch_cuda, cfg, n_cfg_used, n_per_cfg):
+    from paper_2510_02639_b200 import binding, inputs
+    torch = torch_cuda
+    wl = inputs.get(cfg)
+    dev = "cuda:0"
+    w_re = torch.tensor(np.ascontiguousarray(wl.w.real), device=dev)
+    w_im = torch.tensor(np.ascontiguousarray(wl.w.imag), device=dev)
+    A, err, st = ctx.ulens_mag(_lenses(binding, wl, range(wl.n_cfg)), wl.rho, wl.u1, w_re, w_im)
+    torch.cuda.synchronize()
+    A = A.cpu().numpy(); st = st.cpu().numpy().astype(np.uint32); err = err.cpu().numpy()
+    assert A.shape == (wl.n_cfg, wl.n_pts)
+    # properties at any size: finite; a point-mass lens never demagnifies the total flux (A >= 1);
+    # image count parity N+1 (mod 2) and range wherever the point is not flagged
+    assert np.all(np.isfinite(A))
+    assert A.min() >= 1.0 - 1e-4
+    n_img = (st >> 8) & 0xf
+    n_lens = 2 if wl.kind == "binary" else 3
+    clean = (st & 0xff) == 0
+    assert clean.mean() > 0.98
+    assert np.all((n_img[clean] % 2) == ((n_lens + 1) % 2))
+    assert np.all((n_img[clean] >= n_lens + 1) & (n_img[clean] <= n_lens * n_lens + 1))
+    assert np.all(err[clean] <= 1e-4)
+    # the same sample test_config_subsample compares with the oracle
+    idx = inputs.subsample(wl, n_per_cfg, seed=cfg)
+    cs = list(range(0, wl.n_cfg, wl.n_cfg // n_cfg_used))[:n_cfg_used]
+    w = np.stack([wl.w[c][idx[c]] for c in cs])
+    s_re = torch.tensor(np.ascontiguousarray(w.real), device=dev)
+    s_im = torch.tensor(np.ascontiguousarray(w.imag), device=dev)
+    A_s, _, _ = ctx.ulens_mag(_lenses(binding, wl, cs), wl.rho[cs], wl.u1[cs], s_re, s_im)
+    torch.cuda.synchronize()
+    A_full_sample = np.stack([A[c][idx[c]] for c in cs])
+    assert np.array_equal(A_s.cpu().numpy(), A_full_sample)
+
+
+def test_full_config4_with_derivatives(ctx, torch_cuda):
+    """C4 at full size (1,024 parameter vectors x 2,000 epochs, A and 7 derivatives each)."""
+    from paper_2510_02639_b200 import inputs
+    torch = torch_cuda
+    wl = inputs.get(4)
+    t = torch.tensor(wl.t.copy(), device="cuda:0")
+    A, dA, err, st = ctx.ulens_lightcurve_binary(wl.theta, 0.5, t, want_dA=True)
+    torch.cuda.synchronize()
+    A = A.cpu().numpy(); dA = dA.cpu().numpy(); st = st.cpu().numpy().astype(np.uint32)
+    assert A.shape == (1024, 2000) and dA.shape == (1024, 2000, 7)
+    assert np.all(np.isfinite(A)) and np.all(np.isfinite(dA))
+    assert A.min() >= 1.0 - 1e-4
+    assert ((st & 0xff) == 0).mean() > 0.98
+    # the curve only shifts with t0, so dA/dt0 = -dA/dt: integrated over each wing of the first curve (trapezoid
+    # rule on the 2,000 epochs; differencing neighbouring epochs instead would amplify the 1e-5 quadrature noise)
+    c = 0
+    tau = (wl.t - wl.theta[c, 0]) / wl.theta[c, 2]
+    for wing in (np.flatnonzero(tau < -0.5), np.flatnonzero(tau > 0.5)):
+        g = dA[c, wing, 0]
+        integral = np.sum(0.5 * (g[1:] + g[:-1]) * np.diff(wl.t[wing]))
+        delta = A[c, wing[-1]] - A[c, wing[0]]
+        assert abs(integral + delta) <= 1e-3 * abs(delta) + 1e-5
+    # sampled outputs: the epochs test_config4_derivatives_vs_oracle_fd compares with the oracle, recomputed alone
+    sel = np.array([600, 800, 900, 950, 1050, 1100, 1300])
+    for c in (0, 3):
+        A1, dA1, _, _ = ctx.ulens_lightcurve_binary(wl.theta[c][None, :], 0.5, t[torch.as_tensor(sel, device="cuda:0")].contiguous(),
+                                                    want_dA=True)
+        torch.cuda.synchronize()
+        assert np.array_equal(A1.cpu().numpy()[0], A[c, sel])
+        assert np.array_equal(dA1.cpu().numpy()[0], dA[c, sel])
