@@ -240,8 +240,11 @@ k_regions(int n, int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cf
 }
 
 // One warp per 32-ring work unit, one lane per ring (Sec. 3.3; App. A). Units are pulled from a device counter.
+#ifndef UL_SHOOT_MINB
+#define UL_SHOOT_MINB 5
+#endif
 template <int N, bool LD>
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(128, UL_SHOOT_MINB)
 k_shoot(int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cfg, const double* __restrict__ w_re,
         const double* __restrict__ w_im, const Patch* __restrict__ patches, const unsigned* __restrict__ unit_desc,
         double* __restrict__ unit_sum, double* __restrict__ unit_odd, unsigned* __restrict__ status,
@@ -339,7 +342,7 @@ k_shoot_dual(int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cfg, c
              const double* __restrict__ w_re, const double* __restrict__ w_im, const Patch* __restrict__ patches,
              const PatchTan* __restrict__ ptans, const unsigned* __restrict__ unit_desc, double* __restrict__ unit_sum,
              double* __restrict__ unit_odd, double* __restrict__ unit_tan, unsigned* __restrict__ status,
-             ChunkCounters* cc, DevCounters* ctr, unsigned cap_units)
+             ChunkCounters* cc, DevCounters* ctr, unsigned cap_units, int n_theta_opt)
 {
     const int lane = threadIdx.x & 31;
     const unsigned n_units = min(cc->n_units, cap_units);
@@ -378,14 +381,55 @@ k_shoot_dual(int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cfg, c
         D5 rho_d = d5_const(rho);
 #pragma unroll
         for (int k = 0; k < UL_NT; ++k) rho_d.d[k] = T.drho[k];
+        if (scan_r) shoot_col_d<N, LD>(L, T, wcx, wcy, rho, xl, d5_const(P.r0), d5_const(P.dr), P.n_r, U, S, edge);
+        else shoot_ring_d<N, LD>(L, T, wcx, wcy, rho, xl, P.th0, P.dth, P.n_th, periodic, U, S, edge);
+        if (P.flags & UL_PATCH_SINR) {
+            // Tip caps. The sin-spaced lines crowd towards the two tips of the image, where a line
+            // cuts a chord shorter than a few node spacings: harmless for the value (those lines weigh ~phi^2),
+            // but the edge terms of a chord the nodes do not resolve are (small)/(small) and can be arbitrarily
+            // wrong. Near a tip the boundary is a parabola in co-moving coordinates, so the line integrals of the
+            // cap lines all scale with the parameters by ONE common factor (U ~ sqrt(h/kappa), S ~ h b/sqrt(a),
+            // times a function of the line index only): a line whose chord spans < 3 node spacings takes its
+            // relative tangents from the nearest resolved line on the side away from the tip (same warp);
+            // if there is none in this unit its tangents are dropped (bounded: such lines carry < 1e-3 of the flux).
+            const double cells = scan_r ? U.v / ((P.r0 + 0.5 * P.n_r * P.dr) * P.dr) : U.v;
+            const unsigned m_ne = __ballot_sync(0xffffffffu, cells > 0.0);
+            const unsigned m_res = __ballot_sync(0xffffffffu, cells >= 3.0);
+            const unsigned below = (1u << lane) - 1u, above = ~((2u << lane) - 1u);   // (2u << 31) == 0: no lanes above
+            int src = lane;
+            const bool unresolved = cells > 0.0 && cells < 3.0;
+            if (unresolved) {
+                const unsigned res_dn = m_res & below, emp_dn = ~m_ne & below;
+                const unsigned res_up = m_res & above, emp_up = ~m_ne & above;
+                const int s_dn = res_dn ? 31 - __clz(res_dn) : -1, e_dn = emp_dn ? 31 - __clz(emp_dn) : -1;
+                const int s_up = res_up ? __ffs(res_up) - 1 : 32, e_up = emp_up ? __ffs(emp_up) - 1 : 32;
+                // unit edges: line -1 and line n_lines count as empty (the sector ends there)
+                const bool tip_below = (e_dn > s_dn) || (s_dn < 0 && blk == 0);
+                const bool tip_above = (e_up < s_up) || (s_up > 31 && blk == P.n_units - 1);
+                if (tip_below && !tip_above && s_up <= 31) src = s_up;
+                else if (tip_above && !tip_below && s_dn >= 0) src = s_dn;
+                else src = -1;
+            }
+            const int from = src < 0 ? lane : src;
+            D5 Uc, Sc;
+            Uc.v = __shfl_sync(0xffffffffu, U.v, from); Sc.v = __shfl_sync(0xffffffffu, S.v, from);
+#pragma unroll
+            for (int k = 0; k < UL_NT; ++k) {
+                Uc.d[k] = __shfl_sync(0xffffffffu, U.d[k], from); Sc.d[k] = __shfl_sync(0xffffffffu, S.d[k], from);
+            }
+            if (unresolved) {
+                const double ku = (src >= 0 && Uc.v > 0.0) ? U.v / Uc.v : 0.0;
+                const double ks = (src >= 0 && Sc.v > 0.0) ? S.v / Sc.v : 0.0;
+#pragma unroll
+                for (int k = 0; k < UL_NT; ++k) { U.d[k] = ku * Uc.d[k]; S.d[k] = ks * Sc.d[k]; }
+            }
+        }
         if (scan_r) {
-            shoot_col_d<N, LD>(L, T, wcx, wcy, rho, xl, d5_const(P.r0), d5_const(P.dr), P.n_r, U, S, edge);
             f = U * (1.0 - u1);
             if (LD) f += (S / rho_d) * u1;
             f = f * wl;
             clipped = edge || (!periodic && (line < 1 || line >= P.n_th - 1) && U.v > 0.0);
         } else {
-            shoot_ring_d<N, LD>(L, T, wcx, wcy, rho, xl, P.th0, P.dth, P.n_th, periodic, U, S, edge);
             f = U * (1.0 - u1);
             if (LD) f += (S / rho_d) * u1;
             f = xl * f * wl * P.dth;
@@ -627,18 +671,25 @@ static int run_chunks(ulens_ctx* ctx, long long n_total, int n_pts, bool ld, con
                                                          ctx->patches, ctx->n_patch, ctx->status_ws, ctx->unit_desc,
                                                          (unsigned)ctx->cap_units, ctx->cc, ctx->counters, ctx->c_zr, ctx->c_zi, ctx->c_mask, tans, ctx->ptans);
         }
-        int grid = sm_count * 4;
+        // persistent grid: as many CTAs as are resident at once (occupancy API; 4-6 per SM by register count)
+        int per_sm = 4;
+        if (!dual) {
+            if (ld) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_shoot<N, true>, 128, 0);
+            else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_shoot<N, false>, 128, 0);
+            if (per_sm < 1) per_sm = 1;
+        }
+        int grid = sm_count * per_sm;
         {
             KTimer kt(ctx, ULENS_K_SHOOT, st);
             if constexpr (N < 3) {
                 if (dual && ld)
                     k_shoot_dual<N, true><<<grid, 128, 0, st>>>((int)base, n_pts, ctx->cfg_dev, tans, w_re, w_im, ctx->patches, ctx->ptans,
                                                                 ctx->unit_desc, ctx->unit_sum, ctx->unit_odd, ctx->unit_tan, ctx->status_ws,
-                                                                ctx->cc, ctx->counters, (unsigned)ctx->cap_units);
+                                                                ctx->cc, ctx->counters, (unsigned)ctx->cap_units, ctx->rp.n_theta);
                 else if (dual)
                     k_shoot_dual<N, false><<<grid, 128, 0, st>>>((int)base, n_pts, ctx->cfg_dev, tans, w_re, w_im, ctx->patches, ctx->ptans,
                                                                  ctx->unit_desc, ctx->unit_sum, ctx->unit_odd, ctx->unit_tan, ctx->status_ws,
-                                                                 ctx->cc, ctx->counters, (unsigned)ctx->cap_units);
+                                                                 ctx->cc, ctx->counters, (unsigned)ctx->cap_units, ctx->rp.n_theta);
             }
             if (dual) {}
             else if (ld)

@@ -19,7 +19,8 @@ namespace ulens {
 
 #define UL_NT 5          // tangent directions: w_cx, w_cy, s, q, rho
 
-// how the inputs of Eq. 1 / Eq. 5 move in each direction (filled on the host per configuration)
+// how the inputs of Eq. 1 / Eq. 5 move in each direction (filled on the host per configuration by
+// upload_tangents, whose structure -- which entries can be non-zero -- ray_F_dual relies on)
 struct TangentTable {
     double dwx[UL_NT], dwy[UL_NT], drho[UL_NT];
     double deps[UL_NT][3], dax[UL_NT][3], day[UL_NT][3];
@@ -93,33 +94,42 @@ template <int N>
 UL_HD D5 ray_F_dual(const Lens& L, const TangentTable& T, const D5& r, double c, double s, double wcx, double wcy,
                     double rho, const double* thdot = nullptr)
 {
+    // The five directions have a fixed structure (upload_tangents in ulens_api.cu is the only writer of T):
+    //   k = 0, 1  source centre: dw_c = 1, i            k = 4  rho
+    //   k = 2     s: real displacements da_i = T.dax[2][i]
+    //   k = 3     q: d eps_i = T.deps[3][i] and real displacements da_i = T.dax[3][i]
+    // so per ray: g once, the moving-ray response h = e + g conj(e) once (e = unit vector of the line), and two
+    // explicit lens-parameter terms; every tangent is then one FMA on top of the value's reciprocals.
     const double x = r.v * c, y = r.v * s;
-    double px[N], py[N], qx[N], qy[N];
     double ex = x - wcx, ey = y - wcy;
+    double gx = 0.0, gy = 0.0, s2x = 0.0, s2y = 0.0, s3x = 0.0, s3y = 0.0;
 #pragma unroll
     for (int i = 0; i < N; ++i) {
         double dx = x - L.ax[i], dy = y - L.ay[i];
         double inv = 1.0 / (dx * dx + dy * dy);
-        px[i] = dx * inv; py[i] = dy * inv;                       // 1/conj(d) = d/|d|^2
-        qx[i] = px[i] * px[i] - py[i] * py[i]; qy[i] = 2.0 * px[i] * py[i];   // 1/conj(d)^2
-        ex -= L.eps[i] * px[i]; ey -= L.eps[i] * py[i];
+        double px = dx * inv, py = dy * inv;                      // 1/conj(d) = d/|d|^2
+        double qx = px * px - py * py, qy = 2.0 * px * py;        // 1/conj(d)^2
+        ex -= L.eps[i] * px; ey -= L.eps[i] * py;
+        gx += L.eps[i] * qx; gy += L.eps[i] * qy;
+        if (N > 1) {
+            // - d eps_i / conj(d_i)  -  eps_i conj(d a_i) / conj(d_i)^2     (Eq. 1 differentiated at fixed z)
+            const double e2 = L.eps[i] * T.dax[2][i], e3 = L.eps[i] * T.dax[3][i];
+            s2x -= e2 * qx; s2y -= e2 * qy;
+            s3x -= T.deps[3][i] * px + e3 * qx; s3y -= T.deps[3][i] * py + e3 * qy;
+        }
     }
     D5 F;
     F.v = ex * ex + ey * ey - rho * rho;
+    const double ex2 = 2.0 * ex, ey2 = 2.0 * ey;
+    // dz = a (c, s): dz + g conj(dz) = a h
+    const double H = ex2 * (c + gx * c + gy * s) + ey2 * (s + gy * c - gx * s);
+    const double expl[UL_NT] = {-ex2, -ey2, ex2 * s2x + ey2 * s2y, ex2 * s3x + ey2 * s3y, -2.0 * rho};
 #pragma unroll
-    for (int k = 0; k < UL_NT; ++k) {
-        double zdx = r.d[k] * c, zdy = r.d[k] * s;
-        if (thdot) { zdx -= r.v * thdot[k] * s; zdy += r.v * thdot[k] * c; }     // the scan line itself turns
-        double edx = zdx - T.dwx[k], edy = zdy - T.dwy[k];
+    for (int k = 0; k < UL_NT; ++k) F.d[k] = r.d[k] * H + expl[k];
+    if (thdot) {                                                  // the scan line itself turns: dz += r thdot (-s, c)
+        const double Hp = r.v * (ex2 * (-s - gx * s + gy * c) + ey2 * (c - gy * s - gx * c));
 #pragma unroll
-        for (int i = 0; i < N; ++i) {
-            edx -= T.deps[k][i] * px[i]; edy -= T.deps[k][i] * py[i];
-            double ddx = zdx - T.dax[k][i], ddy = zdy - T.day[k][i];       // d(z - a_i)
-            // - eps_i d(1/conj d) = + eps_i conj(dd) / conj(d)^2
-            edx += L.eps[i] * (ddx * qx[i] + ddy * qy[i]);
-            edy += L.eps[i] * (ddx * qy[i] - ddy * qx[i]);
-        }
-        F.d[k] = 2.0 * (ex * edx + ey * edy) - 2.0 * rho * T.drho[k];
+        for (int k = 0; k < UL_NT; ++k) F.d[k] += thdot[k] * Hp;
     }
     if (!(F.v < UL_BIG)) { F = d5_const(UL_BIG); }               // ray on a lens: outside, never NaN
     return F;

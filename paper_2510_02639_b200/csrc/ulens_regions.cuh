@@ -31,6 +31,9 @@ struct SubBox {
     double cr, ct;          // smallest local half-chord of the image along r / along theta: node spacing on a line
 };
 
+#ifndef UL_EA_LIMB_TOL2
+#define UL_EA_LIMB_TOL2 1e-10   // squared relative step at which a limb root is settled (the Eq.-1 polish follows)
+#endif
 #define UL_MAXP 12          // sector cap per point ("capped based on the maximum expected number of images")
 #define UL_MAXG 16          // groups per axis
 
@@ -189,7 +192,7 @@ UL_HDN void regions_phaseA(int lane, const Lens& L, const LensPoly& T, double wc
 #pragma unroll 1
         for (;;) {
             if (cold) ea_init_ni<DEG>(br, bi, zr, zi);
-            it = ea_iterate_ni<DEG>(br, bi, zr, zi, cold ? 64 : 24, 1e-14);
+            it = ea_iterate_ni<DEG>(br, bi, zr, zi, cold ? 64 : 24, UL_EA_LIMB_TOL2);
             if (cold || it <= 24) break;
             cold = true;
         }
