@@ -45,6 +45,10 @@ FP64_INSTR_PER_RAY_DUAL_EXTRA = 74
 # Ehrlich-Aberth 3 iterations x DEG roots x (8 DEG Horner + 12 (DEG-1) repulsion + 24), Eq.-1 polish of the
 # N+1..DEG images 2.5 iterations x (17 N + 25), boxes ~100.
 FP64_INSTR_PER_LIMB_SOLVE = {1: 600, 2: 2400, 3: 8300}
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the roofline kernel, from the `ncu --set full`
+# captures summarised in profiles/r01b_ncu_k_shoot_c1.md (C1) and profiles/r01b_ncu_k_shoot_dual_c4.md (C4);
+# configs without a capture report null.
+NCU_TRAFFIC_BYTES_PER_LAUNCH = {1: 27.4112e6 + 0.6766e6, 4: 61.8944e6 + 33.8424e6}
 # FP64 FMA pipe of one B200: 148 SMs x 64 DFMA lanes / clk x 1.965 GHz (clocks.max.sm) -- DESIGN.md
 FP64_PEAK_DFMA = 148 * 64 * 1.965e9
 
@@ -299,7 +303,9 @@ def main_ours(args, rank, local_rank, world):
         peak_measured = ctx.ulens_fp64_peak(200.0)
         roofline = {"bound": "alu", "kernel": "k_shoot", "achieved": achieved, "peak": 2.0 * FP64_PEAK_DFMA / 1e12,
                     "variant": "k_shoot_dual (value + 5 tangents per ray)" if dual else "k_shoot",
-                    "unit": "TFLOP/s", "frac": achieved / (2.0 * FP64_PEAK_DFMA / 1e12), "traffic": None,
+                    "unit": "TFLOP/s", "frac": achieved / (2.0 * FP64_PEAK_DFMA / 1e12),
+                    "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH.get(args.config),
+                    "traffic_note": "DRAM bytes of one launch (ncu capture in profiles/); the path is ALU-bound",
                     "peak_source": "derived: 148 SM x 64 DFMA/clk x 1.965 GHz x 2 flop (DESIGN.md); "
                                    "MEASURED_PEAKS.json has no FP64 entry",
                     "peak_measured_dfma_microbench": 2.0 * peak_measured / 1e12,

@@ -141,6 +141,14 @@ int  ulens_lightcurve_binary_host(ulens_ctx* ctx, int n_cfg, int n_epochs,
                double* A_out_host, double* dA_out_host, double* err_out_host, uint32_t* status_out_host,
                void* stream);
 
+/* Point-source magnification (Eq. 2-3): A = sum over the images of 1/|det J|, det J = 1 - |sum_i eps_i/conj(z - a_i)^2|^2,
+ * from the validated, polished images of step a2 (one thread per source position). Layout as ulens_mag
+ * (lenses host, w_re/w_im device [n_cfg][n_pts], A_out device, status_out device or NULL: image count in
+ * bits 8-11, ULENS_ST_EA_NOCONV / ULENS_ST_IMG_PARITY). On a caustic det J -> 0 and A diverges, as it must.
+ * This is the building block of the point-source / finite-source switch for far epochs, SURVEY 8.f-2. */
+int  ulens_mag_point(ulens_ctx* ctx, int n_cfg, int n_pts, const ulens_lens* lenses_host,
+               const double* w_re, const double* w_im, double* A_out, uint32_t* status_out, void* stream);
+
 /* (iii) Root export (Eq. 4, Eq. 7): all N^2+1 roots of the lens polynomial for
  * each source position and which of them are images (validated on Eq. 1; images are polished
  * on Eq. 1). roots_re/im device [n_pts][n_deg], is_image device [n_pts][n_deg] bytes, n_deg = N^2+1. */

@@ -20,7 +20,7 @@ ST_NIMG_SHIFT = 8
 KERNEL_NAMES = ["k_traj", "k_roots", "k_regions", "k_shoot", "k_finalize"]     # ULENS_K_* order
 
 EXPORTS = ["ulens_create", "ulens_destroy", "ulens_lens_binary", "ulens_lens_triple", "ulens_mag", "ulens_mag_grad",
-           "ulens_mag_host", "ulens_lightcurve_binary", "ulens_lightcurve_binary_host", "ulens_roots", "ulens_get_stats",
+           "ulens_mag_host", "ulens_lightcurve_binary", "ulens_lightcurve_binary_host", "ulens_mag_point", "ulens_roots", "ulens_get_stats",
            "ulens_reset_stats", "ulens_last_launch_count", "ulens_set_timing", "ulens_get_kernel_ms", "ulens_fp64_peak", "ulens_strerror",
            "ulens_last_cuda_error"]
 
@@ -65,6 +65,7 @@ def lib() -> C.CDLL:
         L.ulens_mag_host.argtypes = [vp, ip, ip, C.POINTER(ulens_lens), dp, dp, vp, vp, vp, vp, vp, vp]
         L.ulens_lightcurve_binary.argtypes = [vp, ip, ip, dp, C.c_double, vp, vp, vp, vp, vp, vp]
         L.ulens_lightcurve_binary_host.argtypes = [vp, ip, ip, dp, C.c_double, vp, vp, vp, vp, vp, vp]
+        L.ulens_mag_point.argtypes = [vp, ip, ip, C.POINTER(ulens_lens), vp, vp, vp, vp, vp]
         L.ulens_roots.argtypes = [vp, C.POINTER(ulens_lens), ip, vp, vp, vp, vp, vp, vp]
         L.ulens_get_stats.argtypes = [vp, C.POINTER(ulens_stats)]
         L.ulens_reset_stats.argtypes = [vp]
@@ -237,6 +238,20 @@ class Context:
                                              _dev(err, torch.float64, n_cfg * n_ep),
                                              _dev(st, torch.int32, n_cfg * n_ep), self._stream(stream)), self._h)
         return A, dA, err, st
+
+    def ulens_mag_point(self, lenses, w_re, w_im, stream=None):
+        """Point-source magnification sum 1/|det J| (Eq. 2-3): returns (A [n_cfg, n_pts], status)."""
+        torch = self._torch
+        lenses = list(lenses)
+        n_cfg = len(lenses)
+        arr = (ulens_lens * n_cfg)(*lenses)
+        n_pts = w_re.numel() // max(n_cfg, 1)
+        n = n_cfg * n_pts
+        A = torch.empty((n_cfg, n_pts), dtype=torch.float64, device=w_re.device)
+        st = torch.empty((n_cfg, n_pts), dtype=torch.int32, device=w_re.device)
+        _check(lib().ulens_mag_point(self._h, n_cfg, n_pts, arr, _dev(w_re, torch.float64, n), _dev(w_im, torch.float64, n),
+                                     _dev(A, torch.float64, n), _dev(st, torch.int32, n), self._stream(stream)), self._h)
+        return A, st
 
     def ulens_lightcurve_binary_host(self, theta, u1, t, A, dA=None, err=None, st=None, stream=None):
         """Host numpy arrays in / out (e.g. views of pinned tensors): t [n_epochs]; A, err [n_cfg, n_epochs];

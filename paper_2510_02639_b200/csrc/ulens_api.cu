@@ -152,7 +152,8 @@ __global__ void k_roots(int n, int pt_base, int n_pts_per_cfg, const PointCfg* _
                         const LensPoly* __restrict__ poly, const double* __restrict__ w_re,
                         const double* __restrict__ w_im, double* __restrict__ out_re, double* __restrict__ out_im,
                         uint8_t* __restrict__ out_img, unsigned* __restrict__ status,
-                        double* __restrict__ c_zr, double* __restrict__ c_zi, unsigned* __restrict__ c_mask)
+                        double* __restrict__ c_zr, double* __restrict__ c_zi, unsigned* __restrict__ c_mask,
+                        double* __restrict__ A_ps = nullptr, unsigned* __restrict__ status_global = nullptr)
 {
     constexpr int DEG = N * N + 1;
     int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -165,6 +166,19 @@ __global__ void k_roots(int n, int pt_base, int n_pts_per_cfg, const PointCfg* _
     unsigned mask = 0;
     unsigned st = centre_images<N>(L, poly[c], wx, wy, zr, zi, mask);
     if (status) status[i] = st;
+    if (A_ps) {
+        // point-source magnification (Eq. 2-3): A = sum over the images of 1 / |det J|, det J = 1 - |g|^2
+        double a = 0.0;
+#pragma unroll
+        for (int k = 0; k < DEG; ++k) {
+            if (!((mask >> k) & 1u)) continue;
+            double fx, fy, gx, gy, dm2;
+            lens_resid<N>(L, zr[k], zi[k], wx, wy, fx, fy, gx, gy, dm2);
+            a += 1.0 / fabs(1.0 - (gx * gx + gy * gy));
+        }
+        A_ps[gp] = a;
+        if (status_global) status_global[gp] = st;
+    }
     if (c_zr) {
 #pragma unroll
         for (int k = 0; k < DEG; ++k) { c_zr[(long long)i * 10 + k] = zr[k]; c_zi[(long long)i * 10 + k] = zi[k]; }
@@ -894,6 +908,31 @@ extern "C" int ulens_lightcurve_binary_host(ulens_ctx* ctx, int n_cfg, int n_epo
     if (err_out_host) CK(cudaMemcpyAsync(err_out_host, d_err, sizeof(double) * n, cudaMemcpyDeviceToHost, st));
     if (status_out_host) CK(cudaMemcpyAsync(status_out_host, d_st, sizeof(unsigned) * n, cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
+    return ULENS_OK;
+}
+
+extern "C" int ulens_mag_point(ulens_ctx* ctx, int n_cfg, int n_pts, const ulens_lens* lenses_host, const double* w_re,
+                               const double* w_im, double* A_out, uint32_t* status_out, void* stream)
+{
+    if (!ctx || n_cfg < 0 || n_pts < 0) return ULENS_EINVAL;
+    if (n_cfg == 0 || n_pts == 0) return ULENS_OK;
+    if (!lenses_host || !w_re || !w_im || !A_out) return ULENS_EINVAL;
+    CK(cudaSetDevice(ctx->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    std::vector<double> rho(n_cfg, 1.0), u1(n_cfg, 0.0);       // unused by the point-source sum
+    int N = 0; bool ld = false;
+    int rc = upload_cfgs(ctx, n_cfg, lenses_host, rho.data(), u1.data(), st, &N, &ld);
+    if (rc != ULENS_OK) return rc;
+    long long n_total = (long long)n_cfg * n_pts;
+    if (n_total > 0x7fffffffLL) return ULENS_EUNSUPPORTED;
+    const int n = (int)n_total, grid = (n + 127) / 128;
+    switch (N) {
+        case 1: k_roots<1><<<grid, 128, 0, st>>>(n, 0, n_pts, ctx->cfg_dev, ctx->poly_dev, w_re, w_im, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, A_out, status_out); break;
+        case 2: k_roots<2><<<grid, 128, 0, st>>>(n, 0, n_pts, ctx->cfg_dev, ctx->poly_dev, w_re, w_im, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, A_out, status_out); break;
+        default: k_roots<3><<<grid, 128, 0, st>>>(n, 0, n_pts, ctx->cfg_dev, ctx->poly_dev, w_re, w_im, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, A_out, status_out); break;
+    }
+    ctx->last_launches = 1;
+    CK(cudaGetLastError());
     return ULENS_OK;
 }
 
