@@ -327,13 +327,14 @@ UL_HD int ea_iterate(const double* br, const double* bi, double* zr, double* zi,
 // slot j's previous position (greedy in slot order). Roots move continuously with w, so after this a slot
 // can only confuse roots that are closer to each other than one step of the path.
 template <int DEG>
-UL_HD void match_roots(const double* ozr, const double* ozi, double* zr, double* zi)
+UL_HD void match_roots(const double* ozr, const double* ozi, double* zr, double* zi, unsigned fixed = 0)
 {
     double nr[DEG], ni[DEG];
-    unsigned used = 0;
+    unsigned used = fixed;               // slots in `fixed` keep their root (continued images)
     bool ident = true;
 #pragma unroll
     for (int j = 0; j < DEG; ++j) {
+        if (fixed & (1u << j)) { nr[j] = zr[j]; ni[j] = zi[j]; continue; }
         int best = -1; double bd = 1e300;
 #pragma unroll
         for (int k = 0; k < DEG; ++k) {
@@ -358,15 +359,17 @@ UL_HD void match_roots(const double* ozr, const double* ozi, double* zr, double*
 // ea_iterate with the loop over the roots kept rolled (the root arrays are indexed dynamically and live in
 // local memory, L1-resident): one fifth / one tenth of the code of the unrolled form, same arithmetic.
 template <int DEG>
-UL_HDNI int ea_iterate_ni(const double* br_, const double* bi_, double* zr, double* zi, int max_it, double tol2)
+UL_HDNI int ea_iterate_ni(const double* br_, const double* bi_, double* zr, double* zi, int max_it, double tol2,
+                          unsigned done0 = 0)
 {
     double br[DEG + 1], bi[DEG + 1], prev[DEG];
 #pragma unroll
     for (int l = 0; l <= DEG; ++l) { br[l] = br_[l]; bi[l] = bi_[l]; }
 #pragma unroll
     for (int k = 0; k < DEG; ++k) prev[k] = 1e300;
-    unsigned done = 0;
+    unsigned done = done0;               // roots known exactly beforehand: frozen, but still repelling the others
     const unsigned all = (1u << DEG) - 1u;
+    if (done == all) return 1;
     for (int it = 1; it <= max_it; ++it) {
         bool bad = false;
 #pragma unroll 1
