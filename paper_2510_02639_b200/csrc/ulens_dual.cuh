@@ -67,7 +67,8 @@ UL_HD D5 zeta_m12_d(const D5& u)
     for (int i = 8; i >= 0; --i) { dp = dp * u.v + p; p = p * u.v + c[i]; }
     D5 r; double su = sqrt(u.v);
     r.v = su + p;
-    double g = (u.v > 0.0 ? 0.5 / su : 0.0) + dp;
+    // d sqrt(u)/du is singular at u = 0 (a node exactly on the edge: the rule is not differentiable there): dropped
+    double g = (u.v > 1e-8 ? 0.5 / su : 0.0) + dp;
     for (int k = 0; k < UL_NT; ++k) r.d[k] = g * u.d[k];
     return r;
 }
@@ -179,6 +180,25 @@ UL_HD void edge_event_d(const D5& f0, const D5& f1, const D5& f2, const D5& f3, 
     }
 }
 
+// Edge events in the dual loops are DEFERRED and BATCHED. An event costs ~600 instructions in D5 arithmetic and each
+// of the 32 lines of a work unit meets the image edge at its own node: evaluated on the spot, 1-2 lanes were
+// active in edge_event_d and the events took two thirds of the kernel (ncu: 15 of 32 lanes active on average).
+// Now the loop keeps only the VALUES of the 4-node window; a lane that sees a sign change remembers the node
+// index, and the warp evaluates all pending events together -- at the latest UL_DEFER_D nodes later --
+// recomputing the four window rays with their tangents (4 ray_F_dual, also batched).
+#ifndef UL_DEFER_D
+#define UL_DEFER_D 16
+#endif
+
+// The recomputed window may differ from the loop's values in the last bit (another rounding path), which can flip
+// the sign of a node sitting exactly on the edge: the loop's classification (entering: node 1 outside, node 2
+// inside) is authoritative, a disagreeing node is moved onto the edge.
+UL_HD void enforce_crossing(D5& w1, D5& w2, bool entering)
+{
+    if (entering) { if (w1.v < 0.0) w1.v = 0.0; if (!(w2.v < 0.0)) w2.v = -1e-9 * fabs(w1.v) - 1e-300; }
+    else { if (!(w1.v < 0.0)) w1.v = -1e-9 * fabs(w2.v) - 1e-300; if (w2.v < 0.0) w2.v = 0.0; }
+}
+
 // shoot_ring of ulens_core.cuh with tangents. r = ring radius (dual); theta grid frozen.
 template <int N, bool LD>
 UL_HD void shoot_ring_d(const Lens& L, const TangentTable& T, double wcx, double wcy, double rho, const D5& r,
@@ -187,28 +207,52 @@ UL_HD void shoot_ring_d(const Lens& L, const TangentTable& T, double wcx, double
     double cd = cos(dth), sd = sin(dth);
     double t = th0 - 1.5 * dth;
     double c = cos(t), s = sin(t);
-    D5 big = d5_const(UL_BIG);
-    D5 f0 = big, f1 = big, f2 = big, f3;
+    double f0 = UL_BIG, f1 = UL_BIG, f2 = UL_BIG;
     D5 U = d5_const(0.0), S = d5_const(0.0);
     edge = false;
     const int j_first = periodic ? 2 : 1;
+    bool pend = false, pen = false; int pj = 0;
+    auto flush = [&]() {
+        if (pend) {
+            // window nodes pj-3 .. pj at angles th0 + (k + 1/2) dth
+            double a = th0 + (pj - 2.5) * dth, wc = cos(a), ws = sin(a);
+            D5 w[4];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                w[k] = ray_F_dual<N>(L, T, r, wc, ws, wcx, wcy, rho);
+                double cn = wc * cd - ws * sd; ws = ws * cd + wc * sd; wc = cn;
+            }
+#ifdef UL_DEBUG_FLUSH
+            printf("ring flush pj %d pen %d w %.6g %.6g %.6g %.6g  loop f1 f2 ? r %.12g\n", pj, (int)pen, w[0].v, w[1].v, w[2].v, w[3].v, r.v);
+#endif
+            enforce_crossing(w[1], w[2], pen);
+            D5 u, dS; bool en;
+            edge_event_d(w[0], w[1], w[2], w[3], LD, 0.0, u, en, dS);
+#ifdef UL_DEBUG_FLUSH
+            printf("   u %.6g du0 %.6g dS %.6g dS0 %.6g\n", u.v, u.d[0], dS.v, dS.d[0]);
+#endif
+            U += u - 0.5; S += dS;
+            pend = false;
+        }
+    };
     for (int j = -2; j <= n_th + 1; ++j) {
-        f3 = ray_F_dual<N>(L, T, r, c, s, wcx, wcy, rho);
+        D5 f3 = ray_F_dual<N>(L, T, r, c, s, wcx, wcy, rho);
         if (j >= 0 && j < n_th && f3.v < 0.0) {
             U.v += 1.0;
             if (LD) S += d5_sqrt(-f3);
             if (!periodic && (j < 2 || j >= n_th - 2)) edge = true;
         }
-        if (j >= j_first && ((f1.v < 0.0) != (f2.v < 0.0))) {
-            D5 u, dS; bool en;
-            edge_event_d(f0, f1, f2, f3, LD, 0.0, u, en, dS);
-            U += u - 0.5; S += dS;
-        }
-        f0 = f1; f1 = f2; f2 = f3;
+        const bool ev = j >= j_first && ((f1 < 0.0) != (f2 < 0.0));
+        if (ev && pend) flush();                                       // second crossing before the batch: rare
+        if (UL_WARP_ANY(pend && j - pj >= UL_DEFER_D)) flush();
+        if (ev) { pj = j; pend = true; pen = !(f1 < 0.0); }
+        f0 = f1; f1 = f2; f2 = f3.v;
         double cn = c * cd - s * sd;
         s = s * cd + c * sd;
         c = cn;
     }
+    flush();
+    (void)f0;
     U_out = U; S_out = S;
 }
 
@@ -218,35 +262,47 @@ UL_HD void shoot_col_d(const Lens& L, const TangentTable& T, double wcx, double 
                        const D5& r0, const D5& dr, int n_r, D5& U_out, D5& S_out, bool& edge)
 {
     double c = cos(th.v), s = sin(th.v);
-    D5 big = d5_const(UL_BIG);
-    D5 f0 = big, f1 = big, f2 = big, f3;
+    double f0 = UL_BIG, f1 = UL_BIG, f2 = UL_BIG;
     D5 U = d5_const(0.0), S = d5_const(0.0), U2 = d5_const(0.0);
     edge = false;
+    bool pend = false, pen = false; int pi = 0;
+    auto flush = [&]() {
+        if (pend) {
+            D5 w[4];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) w[k] = ray_F_dual<N>(L, T, r0 + dr * (pi - 3 + k + 0.5), c, s, wcx, wcy, rho, th.d);
+            enforce_crossing(w[1], w[2], pen);
+            D5 r1 = r0 + dr * (pi - 1.5);
+            D5 rh = r1 + dr * 0.5;
+            D5 u, dS; bool en;
+            bool ent = pen;
+            D5 rin = ent ? r1 + dr : r1;
+            double t2x = dr.v / ul_max(rin.v, 0.5 * dr.v);
+            edge_event_d(w[0], w[1], w[2], w[3], LD, t2x, u, en, dS);
+            D5 rc = en ? (r1 + dr) - u * dr : r1 + u * dr;
+            if (rc.v < 0.0) rc = d5_const(0.0);
+            U2 += en ? (rh * rh - rc * rc) * 0.5 : (rc * rc - rh * rh) * 0.5;
+            S += dS * rc;
+            pend = false;
+        }
+    };
     for (int i = -2; i <= n_r + 1; ++i) {
         D5 r = r0 + dr * (i + 0.5);
-        f3 = ray_F_dual<N>(L, T, r, c, s, wcx, wcy, rho, th.d);
+        D5 f3 = ray_F_dual<N>(L, T, r, c, s, wcx, wcy, rho, th.d);
         if (i >= 0 && i < n_r && f3.v < 0.0) {
             U += r;
             if (LD) S += r * d5_sqrt(-f3);
             if ((i < 2 && r0.v > 0.0) || i >= n_r - 2) edge = true;
         }
-        if (i >= 1 && ((f1.v < 0.0) != (f2.v < 0.0))) {
-            D5 r1 = r0 + dr * (i - 1.5);
-            D5 rh = r1 + dr * 0.5;
-            if (rh.v > 0.0) {
-                D5 u, dS; bool en;
-                bool ent = !(f1.v < 0.0);
-                D5 rin = ent ? r1 + dr : r1;
-                double t2x = dr.v / ul_max(rin.v, 0.5 * dr.v);
-                edge_event_d(f0, f1, f2, f3, LD, t2x, u, en, dS);
-                D5 rc = en ? (r1 + dr) - u * dr : r1 + u * dr;
-                if (rc.v < 0.0) rc = d5_const(0.0);
-                U2 += en ? (rh * rh - rc * rc) * 0.5 : (rc * rc - rh * rh) * 0.5;
-                S += dS * rc;
-            }
-        }
-        f0 = f1; f1 = f2; f2 = f3;
+        // pair (i-2, i-1) = (f1, f2); the cell face between the pair must lie at r > 0
+        const bool ev = i >= 1 && ((f1 < 0.0) != (f2 < 0.0)) && (r0.v + dr.v * (i - 1.0) > 0.0);
+        if (ev && pend) flush();
+        if (UL_WARP_ANY(pend && i - pi >= UL_DEFER_D)) flush();
+        if (ev) { pi = i; pend = true; pen = !(f1 < 0.0); }
+        f0 = f1; f1 = f2; f2 = f3.v;
     }
+    flush();
+    (void)f0;
     U_out = U * dr + U2; S_out = S * dr;
 }
 
