@@ -184,10 +184,10 @@ UL_HD void edge_event_d(const D5& f0, const D5& f1, const D5& f2, const D5& f3, 
 // of the 32 lines of a work unit meets the image edge at its own node: evaluated on the spot, 1-2 lanes were
 // active in edge_event_d and the events took two thirds of the kernel (ncu: 15 of 32 lanes active on average).
 // Now the loop keeps only the VALUES of the 4-node window; a lane that sees a sign change remembers the node
-// index, and the warp evaluates all pending events together -- at the latest UL_DEFER_D nodes later --
+// index, and the warp evaluates all pending events together -- at the latest UL_DEFER_D nodes later, or when one of the lanes meets its next crossing --
 // recomputing the four window rays with their tangents (4 ray_F_dual, also batched).
 #ifndef UL_DEFER_D
-#define UL_DEFER_D 16
+#define UL_DEFER_D 32
 #endif
 
 // The recomputed window may differ from the loop's values in the last bit (another rounding path), which can flip
@@ -243,8 +243,8 @@ UL_HD void shoot_ring_d(const Lens& L, const TangentTable& T, double wcx, double
             if (!periodic && (j < 2 || j >= n_th - 2)) edge = true;
         }
         const bool ev = j >= j_first && ((f1 < 0.0) != (f2 < 0.0));
-        if (ev && pend) flush();                                       // second crossing before the batch: rare
-        if (UL_WARP_ANY(pend && j - pj >= UL_DEFER_D)) flush();
+        // flush for the whole warp when a pending event is old enough or its lane meets its next crossing
+        if (UL_WARP_ANY(pend && (ev || j - pj >= UL_DEFER_D))) flush();
         if (ev) { pj = j; pend = true; pen = !(f1 < 0.0); }
         f0 = f1; f1 = f2; f2 = f3.v;
         double cn = c * cd - s * sd;
@@ -296,8 +296,7 @@ UL_HD void shoot_col_d(const Lens& L, const TangentTable& T, double wcx, double 
         }
         // pair (i-2, i-1) = (f1, f2); the cell face between the pair must lie at r > 0
         const bool ev = i >= 1 && ((f1 < 0.0) != (f2 < 0.0)) && (r0.v + dr.v * (i - 1.0) > 0.0);
-        if (ev && pend) flush();
-        if (UL_WARP_ANY(pend && i - pi >= UL_DEFER_D)) flush();
+        if (UL_WARP_ANY(pend && (ev || i - pi >= UL_DEFER_D))) flush();
         if (ev) { pi = i; pend = true; pen = !(f1 < 0.0); }
         f0 = f1; f1 = f2; f2 = f3.v;
     }
