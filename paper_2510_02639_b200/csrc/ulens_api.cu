@@ -667,7 +667,10 @@ static int run_chunks(ulens_ctx* ctx, long long n_total, int n_pts, bool ld, con
         if (cudaMalloc(&ctx->ptans, sizeof(PatchTan) * UL_MAXP * (size_t)ctx->chunk) != cudaSuccess) return ULENS_ENOMEM;
         if (cudaMalloc(&ctx->unit_tan, sizeof(double) * UL_NT * ctx->cap_units) != cudaSuccess) return ULENS_ENOMEM;
     }
-    const size_t smem = 4 * sizeof(RegionWork<DEG>) + (dual ? 4 * 32 * DEG * sizeof(BoxExt) : 0);
+    // warps (= source points) per CTA of k_regions: the degree-10 work area is 30 KB per warp, so 4 warps per CTA
+    // would leave one CTA per SM; 2 per CTA lets three CTAs share the SM's shared memory (measured on C3)
+    const int wpc = (N == 3) ? 2 : 4;
+    const size_t smem = wpc * sizeof(RegionWork<DEG>) + (dual ? wpc * 32 * DEG * sizeof(BoxExt) : 0);
     CK(cudaFuncSetAttribute(k_regions<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int sm_count = 148;
     cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, ctx->device);
@@ -681,7 +684,7 @@ static int run_chunks(ulens_ctx* ctx, long long n_total, int n_pts, bool ld, con
         }
         {
             KTimer kt(ctx, ULENS_K_REGIONS, st);
-            k_regions<N><<<(n + 3) / 4, 128, smem, st>>>(n, (int)base, n_pts, ctx->cfg_dev, ctx->poly_dev, w_re, w_im, ctx->rp,
+            k_regions<N><<<(n + wpc - 1) / wpc, 32 * wpc, smem, st>>>(n, (int)base, n_pts, ctx->cfg_dev, ctx->poly_dev, w_re, w_im, ctx->rp,
                                                          ctx->patches, ctx->n_patch, ctx->status_ws, ctx->unit_desc,
                                                          (unsigned)ctx->cap_units, ctx->cc, ctx->counters, ctx->c_zr, ctx->c_zi, ctx->c_mask, tans, ctx->ptans);
         }
