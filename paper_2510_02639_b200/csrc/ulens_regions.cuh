@@ -32,7 +32,7 @@ struct SubBox {
 };
 
 #ifndef UL_EA_LIMB_TOL2
-#define UL_EA_LIMB_TOL2 1e-10   // squared relative step at which a limb root is settled (the Eq.-1 polish follows)
+#define UL_EA_LIMB_TOL2 1e-8    // squared relative step at which a limb root is settled (the Eq.-1 polish follows)
 #endif
 #define UL_MAXP 12          // sector cap per point ("capped based on the maximum expected number of images")
 #define UL_MAXG 16          // groups per axis
