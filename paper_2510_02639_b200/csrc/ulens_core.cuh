@@ -125,35 +125,42 @@ UL_HD void lens_resid(const Lens& L, double zx, double zy, double wx, double wy,
 // (or the last Newton step) is below tol * max(1, |z|); z is updated in place; detJ = 1 - |g|^2 (Eq. 3).
 template <int N>
 UL_HD bool polish_image(const Lens& L, double wx, double wy, double& zx, double& zy, int max_it,
-                        double tol, double& detJ, double& resid, double& gx, double& gy, double reject_frac2 = 0.0)
+                        double tol, double& detJ, double& resid, double& gx, double& gy, double reject_frac2 = 0.0,
+                        bool refine = true)
 {
     double fx, fy, dmin2;
     bool ok = false;
-    resid = 1e300; detJ = 0.0;
+    double r2 = 1e300;
+    detJ = 0.0;
+    const double tol2 = tol * tol;
     for (int it = 0; it <= max_it; ++it) {
         lens_resid<N>(L, zx, zy, wx, wy, fx, fy, gx, gy, dmin2);
         detJ = 1.0 - (gx * gx + gy * gy);
-        resid = sqrt(fx * fx + fy * fy);
-        double scale = ul_max(1.0, sqrt(zx * zx + zy * zy));
-        if (!(resid == resid)) return false;
-        if (resid <= tol * scale) { ok = true; if (resid <= 4e-16 * scale) break; }
+        r2 = fx * fx + fy * fy;
+        const double scale2 = ul_max(1.0, zx * zx + zy * zy);       // compared squared: no square roots in the loop
+        if (!(r2 == r2)) { resid = r2; return false; }
+        // refine: keep iterating down to the rounding floor (step a2: images to 1e-15); the limb solves of the
+        // region builder stop as soon as the residual is below tol
+        if (r2 <= tol2 * scale2) { ok = true; if (!refine || r2 <= 1.6e-31 * scale2) break; }
         if (it == max_it) break;
         if (fabs(detJ) < 1e-14) break;
         double bx = -fx, by = -fy;
         // g conj(b)
         double qx = gx * bx + gy * by, qy = gy * bx - gx * by;
-        double sx = (bx - qx) / detJ, sy = (by - qy) / detJ;
+        const double idet = 1.0 / detJ;
+        double sx = (bx - qx) * idet, sy = (by - qy) * idet;
         double s2 = sx * sx + sy * sy;
         // region builder only: a start whose FIRST Newton step already exceeds sqrt(reject_frac2) of its distance
         // to the nearest lens is a spurious root of the polynomial, not an image known to ~1e-7
-        if (it == 0 && reject_frac2 > 0.0 && s2 > reject_frac2 * dmin2) return false;
+        if (it == 0 && reject_frac2 > 0.0 && s2 > reject_frac2 * dmin2) { resid = sqrt(r2); return false; }
         double lim2 = 0.25 * dmin2;
         if (s2 > lim2) { double k = sqrt(lim2 / s2); sx *= k; sy *= k; }
         zx += sx; zy += sy;
         // converged in POSITION: next to a light lens |g| ~ 1e5 and the rounding floor of the residual
         // (~1e-16 |a| |g|) is far above tol although the image is located to ~1e-16
-        if (s2 <= tol * tol * scale * scale && resid <= 1e-6 * scale) { ok = true; break; }
+        if (s2 <= tol2 * scale2 && r2 <= 1e-12 * scale2) { ok = true; break; }
     }
+    resid = sqrt(r2);
     return ok;
 }
 
@@ -424,7 +431,7 @@ template <int N>
 UL_HDNI bool polish_image_ni(const Lens& L, double wx, double wy, double& zx, double& zy, int max_it,
                              double tol, double& detJ, double& resid, double& gx, double& gy, double reject_frac2 = 0.0)
 {
-    return polish_image<N>(L, wx, wy, zx, zy, max_it, tol, detJ, resid, gx, gy, reject_frac2);
+    return polish_image<N>(L, wx, wy, zx, zy, max_it, tol, detJ, resid, gx, gy, reject_frac2, false);
 }
 template <int N>
 UL_HDNI void poly_coeffs_ni(const Lens& L, const LensPoly& T, double wx, double wy, double* br, double* bi)
