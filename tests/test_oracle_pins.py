@@ -5,6 +5,7 @@ brute-force evaluation written in this file (mpmath / numpy) -- never from the C
 from the oracle itself.
 """
 import math
+import os
 
 import mpmath as mp
 import numpy as np
@@ -207,7 +208,11 @@ def test_lens_geometry(oracle):
     assert abs(L.eps[0] + L.eps[1] - 1) < 1e-15 and abs(L.eps[1] / L.eps[0] - q) < 1e-15
     assert abs(L.eps[0] * L.ax[0] + L.eps[1] * L.ax[1]) < 1e-15      # barycentre at the origin
     assert abs((L.ax[1] - L.ax[0]) - s) < 1e-15 and L.ax[0] < 0 < L.ax[1]  # reading G4
-    q3, r3, psi = 0.03, 1.24, math.radians(76.0)                      # Fig. 2 values
+    # Fig. 2 values, read from the fixture
+    fig2 = dict(l.split() for l in open(os.path.join(os.path.dirname(__file__), "golden", "fig2_triple_lens.txt"))
+                if l.strip() and not l.startswith("#"))
+    q3, r3, psi = float(fig2["q3"]), float(fig2["r3"]), math.radians(float(fig2["psi"]))
+    assert (q3, r3) == (0.03, 1.24)
     T = oracle.lens_triple(s, q, q3, r3, psi)
     assert abs(sum(T.eps[:3]) - 1) < 1e-15 and abs(T.eps[2] / T.eps[0] - q3) < 1e-15
     mid = 0.5 * (T.ax[0] + T.ax[1])
