@@ -54,6 +54,7 @@ extern "C" {
 #define ULENS_ST_ERR_HIGH    0x0040u  /* half-resolution self-check differs by more than rel_tol */
 #define ULENS_ST_NO_IMAGE    0x0080u  /* no image-limb point found (A = NaN) */
 #define ULENS_ST_NIMG_SHIFT  8        /* bits 8..11: number of images of the source centre */
+#define ULENS_ST_POINT_SRC   0x1000u  /* ulens_lightcurve_binary_ext: the epoch took the point-source value (Eq. 2-3) */
 
 typedef struct ulens_ctx ulens_ctx;
 
@@ -140,6 +141,26 @@ int  ulens_lightcurve_binary_host(ulens_ctx* ctx, int n_cfg, int n_epochs,
                const double* theta_host, double u1, const double* t_host,
                double* A_out_host, double* dA_out_host, double* err_out_host, uint32_t* status_out_host,
                void* stream);
+
+/* Light-curve driver with the point-source / finite-source switch (Sec. 3.4 (iii): "For extended-source
+ * treatment, only a preselected set of N_ext epochs (e.g., near caustics) are modeled").
+ * Every epoch gets the point-source magnification of its source centre (Eq. 2-3; with dA_out its
+ * derivatives by implicit differentiation of Eq. 1 at the images); the N_ext selected epochs are then
+ * gathered and recomputed by the finite-source path (a2-a8) exactly as ulens_lightcurve_binary does, and
+ * scattered back. Arguments as ulens_lightcurve_binary, plus:
+ *   ext_mask  device uint8 [n_cfg][n_epochs], non-zero = finite-source epoch (the caller's preselection), or NULL:
+ *             the library selects ([proposal]): A_ps at 8 points of the source limb; an epoch keeps
+ *             the point-source value when all 8 have as many images as the centre and the quadrupole estimate
+ *             |mean_8 - A_c|/2 plus the hexadecapole guard |mean_axes - mean_diagonals| is <= sel_tol * A_c.
+ *   sel_tol   tolerance of that test (ignored with ext_mask; <= 0 selects the default 2e-5).
+ *   n_ext_out host int*, may be NULL: N_ext, the number of epochs that took the finite-source path.
+ * Point-source epochs carry ULENS_ST_POINT_SRC in status_out and 0 in err_out. The call synchronises the stream
+ * once (N_ext sizes the finite-source launches); the results are stream-ordered as everywhere else. */
+int  ulens_lightcurve_binary_ext(ulens_ctx* ctx, int n_cfg, int n_epochs,
+               const double* theta_host, double u1, const double* t,
+               const uint8_t* ext_mask, double sel_tol,
+               double* A_out, double* dA_out, double* err_out, uint32_t* status_out,
+               int* n_ext_out, void* stream);
 
 /* Point-source magnification (Eq. 2-3): A = sum over the images of 1/|det J|, det J = 1 - |sum_i eps_i/conj(z - a_i)^2|^2,
  * from the validated, polished images of step a2 (one thread per source position). Layout as ulens_mag

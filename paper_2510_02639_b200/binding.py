@@ -20,7 +20,7 @@ ST_NIMG_SHIFT = 8
 KERNEL_NAMES = ["k_traj", "k_roots", "k_regions", "k_shoot", "k_finalize"]     # ULENS_K_* order
 
 EXPORTS = ["ulens_create", "ulens_destroy", "ulens_lens_binary", "ulens_lens_triple", "ulens_mag", "ulens_mag_grad",
-           "ulens_mag_host", "ulens_lightcurve_binary", "ulens_lightcurve_binary_host", "ulens_mag_point", "ulens_roots", "ulens_get_stats",
+           "ulens_mag_host", "ulens_lightcurve_binary", "ulens_lightcurve_binary_host", "ulens_lightcurve_binary_ext", "ulens_mag_point", "ulens_roots", "ulens_get_stats",
            "ulens_reset_stats", "ulens_last_launch_count", "ulens_set_timing", "ulens_get_kernel_ms", "ulens_fp64_peak", "ulens_strerror",
            "ulens_last_cuda_error"]
 
@@ -65,6 +65,8 @@ def lib() -> C.CDLL:
         L.ulens_mag_host.argtypes = [vp, ip, ip, C.POINTER(ulens_lens), dp, dp, vp, vp, vp, vp, vp, vp]
         L.ulens_lightcurve_binary.argtypes = [vp, ip, ip, dp, C.c_double, vp, vp, vp, vp, vp, vp]
         L.ulens_lightcurve_binary_host.argtypes = [vp, ip, ip, dp, C.c_double, vp, vp, vp, vp, vp, vp]
+        L.ulens_lightcurve_binary_ext.argtypes = [vp, ip, ip, dp, C.c_double, vp, vp, C.c_double, vp, vp, vp, vp,
+                                                  C.POINTER(C.c_int), vp]
         L.ulens_mag_point.argtypes = [vp, ip, ip, C.POINTER(ulens_lens), vp, vp, vp, vp, vp]
         L.ulens_roots.argtypes = [vp, C.POINTER(ulens_lens), ip, vp, vp, vp, vp, vp, vp]
         L.ulens_get_stats.argtypes = [vp, C.POINTER(ulens_stats)]
@@ -238,6 +240,28 @@ class Context:
                                              _dev(err, torch.float64, n_cfg * n_ep),
                                              _dev(st, torch.int32, n_cfg * n_ep), self._stream(stream)), self._h)
         return A, dA, err, st
+
+    def ulens_lightcurve_binary_ext(self, theta, u1, t, ext_mask=None, sel_tol=0.0, want_dA=False, stream=None):
+        """Light curve with the point-source / finite-source switch. ext_mask: CUDA uint8 [n_cfg, n_epochs]
+        (non-zero = finite-source epoch) or None (the library selects with sel_tol). Returns (A, dA, err, st, n_ext)."""
+        torch = self._torch
+        theta = np.ascontiguousarray(theta, dtype=np.float64).reshape(-1, 7)
+        n_cfg, n_ep = theta.shape[0], t.numel()
+        dev = t.device
+        A = torch.empty((n_cfg, n_ep), dtype=torch.float64, device=dev)
+        err = torch.empty((n_cfg, n_ep), dtype=torch.float64, device=dev)
+        st = torch.empty((n_cfg, n_ep), dtype=torch.int32, device=dev)
+        dA = torch.empty((n_cfg, n_ep, 7), dtype=torch.float64, device=dev) if want_dA else None
+        n_ext = C.c_int(0)
+        _check(lib().ulens_lightcurve_binary_ext(self._h, n_cfg, n_ep, _dptr(theta), float(u1),
+                                                 _dev(t, torch.float64, n_ep),
+                                                 _dev(ext_mask, torch.uint8, n_cfg * n_ep) if ext_mask is not None else None,
+                                                 float(sel_tol), _dev(A, torch.float64, n_cfg * n_ep),
+                                                 _dev(dA, torch.float64, n_cfg * n_ep * 7) if want_dA else None,
+                                                 _dev(err, torch.float64, n_cfg * n_ep),
+                                                 _dev(st, torch.int32, n_cfg * n_ep), C.byref(n_ext),
+                                                 self._stream(stream)), self._h)
+        return A, dA, err, st, n_ext.value
 
     def ulens_mag_point(self, lenses, w_re, w_im, stream=None):
         """Point-source magnification sum 1/|det J| (Eq. 2-3): returns (A [n_cfg, n_pts], status)."""

@@ -60,6 +60,8 @@ struct ulens_ctx {
     PointCfg* cfg_dev; LensPoly* poly_dev; size_t cfg_cap;
     double* traj_w; size_t traj_cap;    // lightcurve entry: source centres [2][n]
     double* io_buf; size_t io_cap;      // *_host entry: staging
+    // point-source / finite-source switch (ulens_lightcurve_binary_ext): flags, block offsets, gather map
+    unsigned char* ext_flag; int* ext_map; unsigned* ext_blk; size_t ext_cap;
     int last_launches;
     // optional per-kernel device timing (ulens_set_timing): event pairs recorded on the caller's stream
     int timing_on;
@@ -153,12 +155,13 @@ __global__ void k_roots(int n, int pt_base, int n_pts_per_cfg, const PointCfg* _
                         const double* __restrict__ w_im, double* __restrict__ out_re, double* __restrict__ out_im,
                         uint8_t* __restrict__ out_img, unsigned* __restrict__ status,
                         double* __restrict__ c_zr, double* __restrict__ c_zi, unsigned* __restrict__ c_mask,
-                        double* __restrict__ A_ps = nullptr, unsigned* __restrict__ status_global = nullptr)
+                        double* __restrict__ A_ps = nullptr, unsigned* __restrict__ status_global = nullptr,
+                        const int* __restrict__ pmap = nullptr)
 {
     constexpr int DEG = N * N + 1;
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
-    long long gp = (long long)pt_base + i;
+    long long gp = pmap ? (long long)pmap[pt_base + i] : (long long)pt_base + i;
     int c = (int)(gp / n_pts_per_cfg);
     Lens L = cfg[c].lens;
     double wx = w_re[gp], wy = w_im[gp];
@@ -194,6 +197,187 @@ __global__ void k_roots(int n, int pt_base, int n_pts_per_cfg, const PointCfg* _
     }
 }
 
+
+// ------------------------------------------------------------------------------------------------
+// Point-source / finite-source switch ("(iii) ... only a preselected set of N_ext epochs
+// (e.g., near caustics) are modeled" with the extended source; the other epochs take Eq. 2-3).
+// ------------------------------------------------------------------------------------------------
+
+// Point-source magnification of one source position, A = sum_j 1/|D_j|, D = det J = 1 - |g|^2 (Eq. 2-3), from the
+// images already found (zr, zi, mask) and, if tt != nullptr, its tangents in the UL_NT intrinsic directions by
+// implicit differentiation of Eq. 1 at every image (P:163-175 does this through the polynomial; the lens
+// equation itself is better conditioned). With d_i = z - a_i, g_i = eps_i/conj(d_i)^2, g = sum_i g_i:
+//   delta w = dz + g conj(dz) - sum_i g_i conj(da_i) - sum_i deps_i/conj(d_i)
+//   =>  dz = (R - g conj(R))/D,   R = dw + sum_i g_i conj(da_i) + sum_i deps_i/conj(d_i)
+//   dg = sum_i deps_i/conj(d_i)^2 - 2 sum_i eps_i conj(dz - da_i)/conj(d_i)^3
+//   dA_j = sign(D) d|g|^2/D^2,   d|g|^2 = 2 Re(conj(g) dg)
+template <int N>
+__device__ double point_mag(const Lens& L, const TangentTable* tt, const double* zr, const double* zi, unsigned mask,
+                            double* g5)
+{
+    constexpr int DEG = N * N + 1;
+    double A = 0.0;
+    if (g5) for (int k = 0; k < UL_NT; ++k) g5[k] = 0.0;
+#pragma unroll 1
+    for (int j = 0; j < DEG; ++j) {
+        if (!((mask >> j) & 1u)) continue;
+        double qx[N], qy[N];        // 1/conj(d_i) = d_i/|d_i|^2
+        double gx = 0.0, gy = 0.0;
+#pragma unroll
+        for (int i = 0; i < N; ++i) {
+            double dx = zr[j] - L.ax[i], dy = zi[j] - L.ay[i];
+            double inv = 1.0 / (dx * dx + dy * dy);
+            qx[i] = dx * inv; qy[i] = dy * inv;
+            gx += L.eps[i] * (qx[i] * qx[i] - qy[i] * qy[i]);
+            gy += L.eps[i] * (2.0 * qx[i] * qy[i]);
+        }
+        const double D = 1.0 - (gx * gx + gy * gy);
+        A += 1.0 / fabs(D);
+        if (!g5) continue;
+        const double sD = (D >= 0.0 ? 1.0 : -1.0) / (D * D);
+#pragma unroll 1
+        for (int k = 0; k < UL_NT; ++k) {
+            double Rx = tt->dwx[k], Ry = tt->dwy[k];
+#pragma unroll
+            for (int i = 0; i < N; ++i) {
+                double q2x = qx[i] * qx[i] - qy[i] * qy[i], q2y = 2.0 * qx[i] * qy[i];      // 1/conj(d)^2
+                double gix = L.eps[i] * q2x, giy = L.eps[i] * q2y;
+                double ax = tt->dax[k][i], ay = -tt->day[k][i];                             // conj(da_i)
+                Rx += gix * ax - giy * ay + tt->deps[k][i] * qx[i];
+                Ry += gix * ay + giy * ax + tt->deps[k][i] * qy[i];
+            }
+            // dz = (R - g conj(R))/D
+            double dzx = (Rx - (gx * Rx + gy * Ry)) / D;
+            double dzy = (Ry - (gy * Rx - gx * Ry)) / D;
+            double dgx = 0.0, dgy = 0.0;
+#pragma unroll
+            for (int i = 0; i < N; ++i) {
+                double q2x = qx[i] * qx[i] - qy[i] * qy[i], q2y = 2.0 * qx[i] * qy[i];
+                double q3x = q2x * qx[i] - q2y * qy[i], q3y = q2x * qy[i] + q2y * qx[i];    // 1/conj(d)^3
+                double cx = dzx - tt->dax[k][i], cy = -(dzy - tt->day[k][i]);               // conj(dz - da_i)
+                dgx += tt->deps[k][i] * q2x - 2.0 * L.eps[i] * (cx * q3x - cy * q3y);
+                dgy += tt->deps[k][i] * q2y - 2.0 * L.eps[i] * (cx * q3y + cy * q3x);
+            }
+            g5[k] += sD * 2.0 * (gx * dgx + gy * dgy);
+        }
+    }
+    return A;
+}
+
+// One thread per epoch: point-source A (and tangents) of the source centre, and the decision which path the epoch takes.
+//   mask_in != nullptr: the caller preselected the finite-source epochs (the paper's reading).
+//   mask_in == nullptr: [proposal] multipole probe. A_ps is evaluated at 8 points of the limb (4 on the axes,
+//     4 on the diagonals). For a source that no caustic touches, the disk average of A_ps differs from A_ps(centre)
+//     by rho^2/8 lap A + O(rho^4) (uniform; less when limb-darkened) and the mean over the 8 limb points by
+//     rho^2/4 lap A + O(rho^4), so  Q = |mean_8 - A_c|/2  estimates the finite-source correction and
+//     H = |mean_axes - mean_diagonals| the size of the fourth-order term. The epoch keeps the point-source value
+//     when every probe has as many images as the centre (no caustic between them) and Q + H <= sel_tol * A_c.
+template <int N>
+__global__ void k_point_ext(int n, int n_pts_per_cfg, const PointCfg* __restrict__ cfg, const LensPoly* __restrict__ poly,
+                            const TangentTable* __restrict__ tans, const double* __restrict__ w_re,
+                            const double* __restrict__ w_im, const unsigned char* __restrict__ mask_in, double sel_tol,
+                            double* __restrict__ A_out, double* __restrict__ err_out, unsigned* __restrict__ status_out,
+                            double* __restrict__ grad5, unsigned char* __restrict__ flag_out)
+{
+    constexpr int DEG = N * N + 1;
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    int c = i / n_pts_per_cfg;
+    Lens L = cfg[c].lens;
+    const double rho = cfg[c].rho;
+    const double wx = w_re[i], wy = w_im[i];
+    double zr[DEG], zi[DEG], g5[UL_NT];
+    double A_c = 0.0, s_axes = 0.0, s_diag = 0.0;
+    unsigned st_c = 0;
+    bool ext = mask_in ? (mask_in[i] != 0) : false;
+    const int n_probe = mask_in ? 1 : 9;
+#pragma unroll 1
+    for (int p = 0; p < n_probe; ++p) {
+        double px = wx, py = wy;
+        if (p > 0) {
+            const double r = (p > 4) ? rho * 0.70710678118654752 : rho;
+            const int k = (p - 1) & 3;
+            const double ex = (k == 0) ? 1.0 : (k == 2) ? -1.0 : 0.0, ey = (k == 1) ? 1.0 : (k == 3) ? -1.0 : 0.0;
+            if (p > 4) { px += r * (ex - ey); py += r * (ex + ey); }     // diagonals: e rotated by pi/4, |.| = rho
+            else { px += r * ex; py += r * ey; }
+        }
+        unsigned mask = 0;
+        unsigned st = centre_images<N>(L, poly[c], px, py, zr, zi, mask);
+        if (p == 0) {
+            st_c = st;
+            A_c = point_mag<N>(L, grad5 ? &tans[c] : nullptr, zr, zi, mask, grad5 ? g5 : nullptr);
+            if (st & (UL_ST_EA_NOCONV | UL_ST_IMG_PARITY)) ext = ext || !mask_in;     // doubtful centre: integrate
+        } else {
+            double a = point_mag<N>(L, nullptr, zr, zi, mask, nullptr);
+            if (((st ^ st_c) >> 8) & 0xfu) ext = true;                              // image count changed
+            if (st & (UL_ST_EA_NOCONV | UL_ST_IMG_PARITY)) ext = true;
+            if (p > 4) s_diag += a; else s_axes += a;
+        }
+    }
+    if (!mask_in && !ext) {
+        const double Q = 0.5 * fabs(0.125 * (s_axes + s_diag) - A_c);
+        const double H = 0.25 * fabs(s_axes - s_diag);
+        if (!(Q + H <= sel_tol * A_c)) ext = true;
+    }
+    flag_out[i] = ext ? 1 : 0;
+    A_out[i] = A_c;
+    if (err_out) err_out[i] = 0.0;
+    if (status_out) status_out[i] = st_c | UL_ST_POINT_SRC;
+    if (grad5) for (int k = 0; k < UL_NT; ++k) grad5[(long long)i * UL_NT + k] = g5[k];
+}
+
+// ordered stream compaction of the flagged epochs into the gather map (three small kernels, 1024 epochs per block)
+__global__ void k_ext_count(int n, const unsigned char* __restrict__ flag, unsigned* __restrict__ blk)
+{
+    __shared__ unsigned wsum[32];
+    int i = blockIdx.x * 1024 + threadIdx.x;
+    unsigned b = __ballot_sync(0xffffffffu, i < n && flag[i]);
+    if ((threadIdx.x & 31) == 0) wsum[threadIdx.x >> 5] = __popc(b);
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        unsigned v = wsum[threadIdx.x];
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if (threadIdx.x == 0) blk[blockIdx.x] = v;
+    }
+}
+// exclusive scan of the block counts by one block (n_blk <= a few thousand); blk[n_blk] = total
+__global__ void k_ext_scan(int n_blk, unsigned* __restrict__ blk)
+{
+    __shared__ unsigned part[1024];
+    const int per = (n_blk + 1023) / 1024;
+    const int lo = threadIdx.x * per, hi = min(lo + per, n_blk);
+    unsigned s = 0;
+    for (int j = lo; j < hi; ++j) s += blk[j];
+    part[threadIdx.x] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        unsigned run = 0;
+        for (int j = 0; j < 1024; ++j) { unsigned v = part[j]; part[j] = run; run += v; }
+        blk[n_blk] = run;
+    }
+    __syncthreads();
+    unsigned run = part[threadIdx.x];
+    for (int j = lo; j < hi; ++j) { unsigned v = blk[j]; blk[j] = run; run += v; }
+}
+__global__ void k_ext_scatter(int n, const unsigned char* __restrict__ flag, const unsigned* __restrict__ blk,
+                              int* __restrict__ map)
+{
+    __shared__ unsigned wsum[32];
+    int i = blockIdx.x * 1024 + threadIdx.x;
+    const bool f = i < n && flag[i];
+    unsigned b = __ballot_sync(0xffffffffu, f);
+    const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+    if (l == 0) wsum[w] = __popc(b);
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        unsigned v = wsum[threadIdx.x], inc = v;
+        for (int o = 1; o < 32; o <<= 1) { unsigned t = __shfl_up_sync(0xffffffffu, inc, o); if (threadIdx.x >= o) inc += t; }
+        wsum[threadIdx.x] = inc - v;
+    }
+    __syncthreads();
+    if (f) map[blk[blockIdx.x] + wsum[w] + __popc(b & ((1u << l) - 1u))] = i;
+}
+
 // One warp per source point.
 #ifndef UL_REGIONS_MINB
 #define UL_REGIONS_MINB 2
@@ -205,7 +389,7 @@ k_regions(int n, int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cf
           Patch* __restrict__ patches, int* __restrict__ n_patch, unsigned* __restrict__ status,
           unsigned* __restrict__ unit_desc, unsigned cap_units, ChunkCounters* cc, DevCounters* ctr,
           const double* __restrict__ c_zr, const double* __restrict__ c_zi, const unsigned* __restrict__ c_mask,
-          const TangentTable* __restrict__ tans, PatchTan* __restrict__ ptans)
+          const TangentTable* __restrict__ tans, PatchTan* __restrict__ ptans, const int* __restrict__ pmap = nullptr)
 {
     constexpr int DEG = N * N + 1;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -218,7 +402,7 @@ k_regions(int n, int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cf
     RegionWork<DEG>& W = Wall[warp];
     if (lane == 0) W.ext = tans ? ext_all + warp * 32 * DEG : nullptr;
     __syncwarp();
-    long long gp = (long long)pt_base + i;
+    long long gp = pmap ? (long long)pmap[pt_base + i] : (long long)pt_base + i;
     int c = (int)(gp / n_pts_per_cfg);
     Lens L = cfg[c].lens;
     double rho = cfg[c].rho;
@@ -262,7 +446,7 @@ __global__ void __launch_bounds__(128, UL_SHOOT_MINB)
 k_shoot(int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cfg, const double* __restrict__ w_re,
         const double* __restrict__ w_im, const Patch* __restrict__ patches, const unsigned* __restrict__ unit_desc,
         double* __restrict__ unit_sum, double* __restrict__ unit_odd, unsigned* __restrict__ status,
-        ChunkCounters* cc, DevCounters* ctr, unsigned cap_units)
+        ChunkCounters* cc, DevCounters* ctr, unsigned cap_units, const int* __restrict__ pmap = nullptr)
 {
     const int lane = threadIdx.x & 31;
     const unsigned n_units = min(cc->n_units, cap_units);       // an overflowing point allocated nothing (UL_ST_UNIT_OVF)
@@ -275,7 +459,7 @@ k_shoot(int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cfg, const 
         unsigned d = unit_desc[u];
         const Patch P = patches[d >> 11];
         int blk = (int)(d & 0x7ffu);
-        long long gp = (long long)pt_base + P.point;
+        long long gp = pmap ? (long long)pmap[pt_base + P.point] : (long long)pt_base + P.point;
         int c = (int)(gp / n_pts_per_cfg);
         Lens L = cfg[c].lens;
         double rho = cfg[c].rho, u1 = cfg[c].u1;
@@ -314,11 +498,11 @@ __global__ void k_finalize(int n, int pt_base, int n_pts_per_cfg, const PointCfg
                            const double* __restrict__ unit_sum, const double* __restrict__ unit_odd,
                            const unsigned* __restrict__ status_ws, double rel_tol,
                            double* __restrict__ A_out, double* __restrict__ err_out, unsigned* __restrict__ status_out,
-                           DevCounters* ctr)
+                           DevCounters* ctr, const int* __restrict__ pmap = nullptr)
 {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
-    long long gp = (long long)pt_base + i;
+    long long gp = pmap ? (long long)pmap[pt_base + i] : (long long)pt_base + i;
     int c = (int)(gp / n_pts_per_cfg);
     double rho = cfg[c].rho, u1 = cfg[c].u1;
     double F0 = UL_PI * rho * rho * (1.0 - u1 / 3.0);
@@ -356,7 +540,7 @@ k_shoot_dual(int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cfg, c
              const double* __restrict__ w_re, const double* __restrict__ w_im, const Patch* __restrict__ patches,
              const PatchTan* __restrict__ ptans, const unsigned* __restrict__ unit_desc, double* __restrict__ unit_sum,
              double* __restrict__ unit_odd, double* __restrict__ unit_tan, unsigned* __restrict__ status,
-             ChunkCounters* cc, DevCounters* ctr, unsigned cap_units, int n_theta_opt)
+             ChunkCounters* cc, DevCounters* ctr, unsigned cap_units, int n_theta_opt, const int* __restrict__ pmap = nullptr)
 {
     const int lane = threadIdx.x & 31;
     const unsigned n_units = min(cc->n_units, cap_units);
@@ -370,7 +554,7 @@ k_shoot_dual(int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cfg, c
         const Patch P = patches[d >> 11];
         const PatchTan PT = ptans[d >> 11];
         int blk = (int)(d & 0x7ffu);
-        long long gp = (long long)pt_base + P.point;
+        long long gp = pmap ? (long long)pmap[pt_base + P.point] : (long long)pt_base + P.point;
         int c = (int)(gp / n_pts_per_cfg);
         Lens L = cfg[c].lens;
         const TangentTable& T = tans[c];
@@ -472,11 +656,11 @@ k_shoot_dual(int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cfg, c
 __global__ void k_finalize_dual(int n, int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cfg,
                                 const TangentTable* __restrict__ tans, const Patch* __restrict__ patches,
                                 const int* __restrict__ n_patch, const double* __restrict__ unit_sum,
-                                const double* __restrict__ unit_tan, double* __restrict__ grad5)
+                                const double* __restrict__ unit_tan, double* __restrict__ grad5, const int* __restrict__ pmap = nullptr)
 {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
-    long long gp = (long long)pt_base + i;
+    long long gp = pmap ? (long long)pmap[pt_base + i] : (long long)pt_base + i;
     int c = (int)(gp / n_pts_per_cfg);
     double rho = cfg[c].rho, u1 = cfg[c].u1;
     double F0 = UL_PI * rho * rho * (1.0 - u1 / 3.0);
@@ -608,6 +792,7 @@ extern "C" void ulens_destroy(ulens_ctx* ctx)
     cudaFree(ctx->patches); cudaFree(ctx->n_patch); cudaFree(ctx->status_ws); cudaFree(ctx->unit_desc);
     cudaFree(ctx->unit_sum); cudaFree(ctx->unit_odd); cudaFree(ctx->cc); cudaFree(ctx->counters);
     cudaFree(ctx->cfg_dev); cudaFree(ctx->poly_dev); cudaFree(ctx->traj_w); cudaFree(ctx->io_buf);
+    cudaFree(ctx->ext_flag); cudaFree(ctx->ext_map); cudaFree(ctx->ext_blk);
     if (ctx->timed) {
         for (auto& t : *ctx->timed) { cudaEventDestroy(t.a); cudaEventDestroy(t.b); }
         delete ctx->timed;
@@ -657,7 +842,8 @@ static int upload_cfgs(ulens_ctx* ctx, int n_cfg, const ulens_lens* lenses, cons
 
 template <int N>
 static int run_chunks(ulens_ctx* ctx, long long n_total, int n_pts, bool ld, const double* w_re, const double* w_im,
-                      double* A_out, double* err_out, unsigned* status_out, cudaStream_t st, double* grad5_out = nullptr)
+                      double* A_out, double* err_out, unsigned* status_out, cudaStream_t st, double* grad5_out = nullptr,
+                      const int* pmap = nullptr)
 {
     constexpr int DEG = N * N + 1;
     const bool dual = grad5_out != nullptr;
@@ -680,13 +866,13 @@ static int run_chunks(ulens_ctx* ctx, long long n_total, int n_pts, bool ld, con
         {
             KTimer kt(ctx, ULENS_K_ROOTS, st);
             k_roots<N><<<(n + 127) / 128, 128, 0, st>>>(n, (int)base, n_pts, ctx->cfg_dev, ctx->poly_dev, w_re, w_im,
-                                                        nullptr, nullptr, nullptr, ctx->status_ws, ctx->c_zr, ctx->c_zi, ctx->c_mask);
+                                                        nullptr, nullptr, nullptr, ctx->status_ws, ctx->c_zr, ctx->c_zi, ctx->c_mask, nullptr, nullptr, pmap);
         }
         {
             KTimer kt(ctx, ULENS_K_REGIONS, st);
             k_regions<N><<<(n + wpc - 1) / wpc, 32 * wpc, smem, st>>>(n, (int)base, n_pts, ctx->cfg_dev, ctx->poly_dev, w_re, w_im, ctx->rp,
                                                          ctx->patches, ctx->n_patch, ctx->status_ws, ctx->unit_desc,
-                                                         (unsigned)ctx->cap_units, ctx->cc, ctx->counters, ctx->c_zr, ctx->c_zi, ctx->c_mask, tans, ctx->ptans);
+                                                         (unsigned)ctx->cap_units, ctx->cc, ctx->counters, ctx->c_zr, ctx->c_zi, ctx->c_mask, tans, ctx->ptans, pmap);
         }
         // persistent grid: as many CTAs as are resident at once (occupancy API; 4-6 per SM by register count)
         int per_sm = 4;
@@ -702,28 +888,28 @@ static int run_chunks(ulens_ctx* ctx, long long n_total, int n_pts, bool ld, con
                 if (dual && ld)
                     k_shoot_dual<N, true><<<grid, 128, 0, st>>>((int)base, n_pts, ctx->cfg_dev, tans, w_re, w_im, ctx->patches, ctx->ptans,
                                                                 ctx->unit_desc, ctx->unit_sum, ctx->unit_odd, ctx->unit_tan, ctx->status_ws,
-                                                                ctx->cc, ctx->counters, (unsigned)ctx->cap_units, ctx->rp.n_theta);
+                                                                ctx->cc, ctx->counters, (unsigned)ctx->cap_units, ctx->rp.n_theta, pmap);
                 else if (dual)
                     k_shoot_dual<N, false><<<grid, 128, 0, st>>>((int)base, n_pts, ctx->cfg_dev, tans, w_re, w_im, ctx->patches, ctx->ptans,
                                                                  ctx->unit_desc, ctx->unit_sum, ctx->unit_odd, ctx->unit_tan, ctx->status_ws,
-                                                                 ctx->cc, ctx->counters, (unsigned)ctx->cap_units, ctx->rp.n_theta);
+                                                                 ctx->cc, ctx->counters, (unsigned)ctx->cap_units, ctx->rp.n_theta, pmap);
             }
             if (dual) {}
             else if (ld)
                 k_shoot<N, true><<<grid, 128, 0, st>>>((int)base, n_pts, ctx->cfg_dev, w_re, w_im, ctx->patches, ctx->unit_desc,
-                                                       ctx->unit_sum, ctx->unit_odd, ctx->status_ws, ctx->cc, ctx->counters, (unsigned)ctx->cap_units);
+                                                       ctx->unit_sum, ctx->unit_odd, ctx->status_ws, ctx->cc, ctx->counters, (unsigned)ctx->cap_units, pmap);
             else
                 k_shoot<N, false><<<grid, 128, 0, st>>>((int)base, n_pts, ctx->cfg_dev, w_re, w_im, ctx->patches, ctx->unit_desc,
-                                                        ctx->unit_sum, ctx->unit_odd, ctx->status_ws, ctx->cc, ctx->counters, (unsigned)ctx->cap_units);
+                                                        ctx->unit_sum, ctx->unit_odd, ctx->status_ws, ctx->cc, ctx->counters, (unsigned)ctx->cap_units, pmap);
         }
         {
             KTimer kt(ctx, ULENS_K_FINALIZE, st);
             k_finalize<<<(n + 127) / 128, 128, 0, st>>>(n, (int)base, n_pts, ctx->cfg_dev, ctx->patches, ctx->n_patch,
                                                         ctx->unit_sum, ctx->unit_odd, ctx->status_ws, ctx->opt.rel_tol,
-                                                        A_out, err_out, status_out, ctx->counters);
+                                                        A_out, err_out, status_out, ctx->counters, pmap);
             if (dual) {
                 k_finalize_dual<<<(n + 127) / 128, 128, 0, st>>>(n, (int)base, n_pts, ctx->cfg_dev, tans, ctx->patches, ctx->n_patch,
-                                                                 ctx->unit_sum, ctx->unit_tan, grad5_out);
+                                                                 ctx->unit_sum, ctx->unit_tan, grad5_out, pmap);
                 ctx->last_launches += 1;
             }
         }
@@ -882,6 +1068,89 @@ extern "C" int ulens_lightcurve_binary(ulens_ctx* ctx, int n_cfg, int n_epochs, 
         CK(cudaGetLastError());
     }
     return rc;
+}
+
+extern "C" int ulens_lightcurve_binary_ext(ulens_ctx* ctx, int n_cfg, int n_epochs, const double* theta_host, double u1,
+                                           const double* t, const uint8_t* ext_mask, double sel_tol, double* A_out,
+                                           double* dA_out, double* err_out, uint32_t* status_out, int* n_ext_out,
+                                           void* stream)
+{
+    if (n_ext_out) *n_ext_out = 0;
+    if (!ctx || n_cfg < 0 || n_epochs < 0) return ULENS_EINVAL;
+    if (n_cfg == 0 || n_epochs == 0) return ULENS_OK;
+    if (!theta_host || !t || !A_out || !(u1 >= 0.0 && u1 <= 1.0) || !isfinite(sel_tol)) return ULENS_EINVAL;
+    if (!(sel_tol > 0.0)) sel_tol = 2e-5;
+    CK(cudaSetDevice(ctx->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    std::vector<ulens_lens> lenses(n_cfg);
+    std::vector<double> rho(n_cfg), u1v(n_cfg, u1);
+    for (int c = 0; c < n_cfg; ++c) {
+        const double* th = theta_host + 7 * c;
+        for (int k = 0; k < 7; ++k) if (!isfinite(th[k])) return ULENS_EINVAL;
+        if (!(th[2] > 0.0)) return ULENS_EINVAL;
+        int rc = ulens_lens_binary(&lenses[c], th[3], th[4]);
+        if (rc != ULENS_OK) return rc;
+        rho[c] = th[5];
+    }
+    const size_t n = (size_t)n_cfg * n_epochs;
+    if (n > 0x7fffffffULL) return ULENS_EUNSUPPORTED;
+    size_t need = 2 * n + 7 * (size_t)n_cfg + (dA_out ? UL_NT * n : 0);
+    if (need > ctx->traj_cap) {
+        cudaFree(ctx->traj_w); ctx->traj_w = nullptr; ctx->traj_cap = 0;
+        if (cudaMalloc(&ctx->traj_w, sizeof(double) * need) != cudaSuccess) return ULENS_ENOMEM;
+        ctx->traj_cap = need;
+    }
+    const int n_blk = (int)((n + 1023) / 1024);
+    if (n > ctx->ext_cap) {
+        cudaFree(ctx->ext_flag); cudaFree(ctx->ext_map); cudaFree(ctx->ext_blk);
+        ctx->ext_flag = nullptr; ctx->ext_map = nullptr; ctx->ext_blk = nullptr; ctx->ext_cap = 0;
+        if (cudaMalloc(&ctx->ext_flag, n) != cudaSuccess) return ULENS_ENOMEM;
+        if (cudaMalloc(&ctx->ext_map, sizeof(int) * n) != cudaSuccess) return ULENS_ENOMEM;
+        if (cudaMalloc(&ctx->ext_blk, sizeof(unsigned) * ((size_t)n_blk + 1)) != cudaSuccess) return ULENS_ENOMEM;
+        ctx->ext_cap = n;
+    }
+    double* w_re = ctx->traj_w; double* w_im = w_re + n; double* th_dev = w_im + n;
+    double* g5 = dA_out ? th_dev + 7 * (size_t)n_cfg : nullptr;
+    CK(cudaMemcpyAsync(th_dev, theta_host, sizeof(double) * 7 * n_cfg, cudaMemcpyHostToDevice, st));
+    {
+        KTimer kt(ctx, ULENS_K_TRAJ, st);
+        k_traj<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(n_cfg, n_epochs, th_dev, t, w_re, w_im);
+    }
+    CK(cudaGetLastError());
+    int N = 0; bool ld = false;
+    int rc = upload_cfgs(ctx, n_cfg, lenses.data(), rho.data(), u1v.data(), st, &N, &ld);
+    if (rc != ULENS_OK) return rc;
+    if (dA_out) {
+        rc = upload_tangents(ctx, n_cfg, lenses.data(), st);
+        if (rc != ULENS_OK) return rc;
+    }
+    ctx->last_launches = 1;
+    // every epoch: point-source value (and tangents) + the decision; then the ordered gather map of the N_ext epochs
+    {
+        KTimer kt(ctx, ULENS_K_ROOTS, st);
+        k_point_ext<2><<<(unsigned)((n + 127) / 128), 128, 0, st>>>((int)n, n_epochs, ctx->cfg_dev, ctx->poly_dev,
+                                                                    dA_out ? ctx->tan_dev : nullptr, w_re, w_im, ext_mask, sel_tol,
+                                                                    A_out, err_out, status_out, g5, ctx->ext_flag);
+    }
+    k_ext_count<<<n_blk, 1024, 0, st>>>((int)n, ctx->ext_flag, ctx->ext_blk);
+    k_ext_scan<<<1, 1024, 0, st>>>(n_blk, ctx->ext_blk);
+    k_ext_scatter<<<n_blk, 1024, 0, st>>>((int)n, ctx->ext_flag, ctx->ext_blk, ctx->ext_map);
+    ctx->last_launches += 4;
+    CK(cudaGetLastError());
+    unsigned n_ext = 0;
+    CK(cudaMemcpyAsync(&n_ext, ctx->ext_blk + n_blk, sizeof(unsigned), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    if (n_ext_out) *n_ext_out = (int)n_ext;
+    if (n_ext > 0) {
+        rc = run_chunks<2>(ctx, (long long)n_ext, n_epochs, ld, w_re, w_im, A_out, err_out, status_out, st, g5, ctx->ext_map);
+        if (rc != ULENS_OK) return rc;
+    }
+    if (dA_out) {
+        k_chain7<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(n_cfg, n_epochs, th_dev, t, w_re, w_im, g5, dA_out);
+        ctx->last_launches += 1;
+        CK(cudaGetLastError());
+    }
+    return ULENS_OK;
 }
 
 extern "C" int ulens_lightcurve_binary_host(ulens_ctx* ctx, int n_cfg, int n_epochs, const double* theta_host, double u1,

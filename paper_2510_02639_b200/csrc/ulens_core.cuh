@@ -84,6 +84,7 @@ struct Patch {
 #define UL_ST_UNIT_OVF   0x0020u
 #define UL_ST_ERR_HIGH   0x0040u
 #define UL_ST_NO_IMAGE   0x0080u
+#define UL_ST_POINT_SRC  0x1000u
 
 #define UL_PI 3.14159265358979323846
 #define UL_BIG 1e100
