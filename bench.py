@@ -218,9 +218,15 @@ def main_ours(args, rank, local_rank, world):
         t_dev = torch.tensor(wl.t.copy(), device=dev)
         dA = torch.empty((wl.n_cfg, wl.n_pts, 7), dtype=torch.float64, device=dev)
 
+    n_ext = n
+
     def step():
         if dual:
-            ctx.ulens_lightcurve_binary(wl.theta, float(wl.u1[0]), t_dev, out=(A, dA, err, st))
+            if args.switch:
+                nonlocal n_ext, A, dA, err, st
+                A, dA, err, st, n_ext = ctx.ulens_lightcurve_binary_ext(wl.theta, float(wl.u1[0]), t_dev, want_dA=True)
+            else:
+                ctx.ulens_lightcurve_binary(wl.theta, float(wl.u1[0]), t_dev, out=(A, dA, err, st))
         else:
             ctx.ulens_mag(lenses, wl.rho, wl.u1, w_re, w_im, A, err, st)
 
@@ -267,10 +273,14 @@ def main_ours(args, rank, local_rank, world):
         h_dA = torch.empty((wl.n_cfg, wl.n_pts, 7), dtype=torch.float64).pin_memory()
 
         def e2e_step():
-            ctx.ulens_lightcurve_binary_host(wl.theta, float(wl.u1[0]), h_t.numpy(), h_A.numpy(), h_dA.numpy(),
-                                             h_err.numpy(), h_st.numpy())
+            if args.switch:
+                ctx.ulens_lightcurve_binary_ext_host(wl.theta, float(wl.u1[0]), h_t.numpy(), h_A.numpy(), h_dA.numpy(),
+                                                     h_err.numpy(), h_st.numpy())
+            else:
+                ctx.ulens_lightcurve_binary_host(wl.theta, float(wl.u1[0]), h_t.numpy(), h_A.numpy(), h_dA.numpy(),
+                                                 h_err.numpy(), h_st.numpy())
         h2d, d2h = 8 * wl.n_pts + 56 * wl.n_cfg, (8 + 56 + 8 + 4) * n
-        e2e_api = "ulens_lightcurve_binary_host (pinned host buffers)"
+        e2e_api = ("ulens_lightcurve_binary_ext_host" if args.switch else "ulens_lightcurve_binary_host") + " (pinned host buffers)"
     else:
         def e2e_step():
             ctx.ulens_mag_host(lenses, wl.rho, wl.u1, h_re.numpy(), h_im.numpy(), h_A.numpy(), h_err.numpy(), h_st.numpy())
@@ -335,6 +345,10 @@ def main_ours(args, rank, local_rank, world):
                         "steps": e2e_steps, "api": e2e_api},
                 "gpu_launches": launches_per_step * args.steps,
                 "clocks": clk}
+        if dual and args.switch:
+            line["config"]["switch"] = {"api": "ulens_lightcurve_binary_ext", "selection": "library (sel_tol default 2e-5)",
+                                        "n_ext": int(n_ext), "n_epochs_total": int(n),
+                                        "note": "SURVEY 8.f-2 driver: the other epochs take the point-source value (P:153)"}
         if not args.no_cpu_baseline and world == 1:
             npts, dt, nev, cores = run_oracle_sample(wl, inputs)
             line["cpu_baseline"] = {"value": npts / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
@@ -356,7 +370,12 @@ def main():
     ap.add_argument("--config", type=int, default=1, help="BASELINE.json config index 0..4 (default 1; 4 = light curves with forward-mode derivatives)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--switch", action="store_true",
+                    help="config 4 only: ulens_lightcurve_binary_ext (point-source value for the far epochs, P:153; "
+                         "library selection at the default tolerance) instead of the finite-source path on every epoch")
     args = ap.parse_args()
+    if args.switch and args.config != 4:
+        ap.error("--switch needs --config 4")
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))

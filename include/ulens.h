@@ -162,6 +162,14 @@ int  ulens_lightcurve_binary_ext(ulens_ctx* ctx, int n_cfg, int n_epochs,
                double* A_out, double* dA_out, double* err_out, uint32_t* status_out,
                int* n_ext_out, void* stream);
 
+/* Same with HOST arrays for t, ext_mask (may be NULL), A_out, dA_out (may be NULL), err_out (may be NULL),
+ * status_out (may be NULL): copies in, computes, copies out and synchronises the stream before returning. */
+int  ulens_lightcurve_binary_ext_host(ulens_ctx* ctx, int n_cfg, int n_epochs,
+               const double* theta_host, double u1, const double* t_host,
+               const uint8_t* ext_mask_host, double sel_tol,
+               double* A_out_host, double* dA_out_host, double* err_out_host, uint32_t* status_out_host,
+               int* n_ext_out, void* stream);
+
 /* Point-source magnification (Eq. 2-3): A = sum over the images of 1/|det J|, det J = 1 - |sum_i eps_i/conj(z - a_i)^2|^2,
  * from the validated, polished images of step a2 (one thread per source position). Layout as ulens_mag
  * (lenses host, w_re/w_im device [n_cfg][n_pts], A_out device, status_out device or NULL: image count in

@@ -20,7 +20,7 @@ ST_NIMG_SHIFT = 8
 KERNEL_NAMES = ["k_traj", "k_roots", "k_regions", "k_shoot", "k_finalize"]     # ULENS_K_* order
 
 EXPORTS = ["ulens_create", "ulens_destroy", "ulens_lens_binary", "ulens_lens_triple", "ulens_mag", "ulens_mag_grad",
-           "ulens_mag_host", "ulens_lightcurve_binary", "ulens_lightcurve_binary_host", "ulens_lightcurve_binary_ext", "ulens_mag_point", "ulens_roots", "ulens_get_stats",
+           "ulens_mag_host", "ulens_lightcurve_binary", "ulens_lightcurve_binary_host", "ulens_lightcurve_binary_ext", "ulens_lightcurve_binary_ext_host", "ulens_mag_point", "ulens_roots", "ulens_get_stats",
            "ulens_reset_stats", "ulens_last_launch_count", "ulens_set_timing", "ulens_get_kernel_ms", "ulens_fp64_peak", "ulens_strerror",
            "ulens_last_cuda_error"]
 
@@ -67,6 +67,8 @@ def lib() -> C.CDLL:
         L.ulens_lightcurve_binary_host.argtypes = [vp, ip, ip, dp, C.c_double, vp, vp, vp, vp, vp, vp]
         L.ulens_lightcurve_binary_ext.argtypes = [vp, ip, ip, dp, C.c_double, vp, vp, C.c_double, vp, vp, vp, vp,
                                                   C.POINTER(C.c_int), vp]
+        L.ulens_lightcurve_binary_ext_host.argtypes = [vp, ip, ip, dp, C.c_double, vp, vp, C.c_double, vp, vp, vp, vp,
+                                                       C.POINTER(C.c_int), vp]
         L.ulens_mag_point.argtypes = [vp, ip, ip, C.POINTER(ulens_lens), vp, vp, vp, vp, vp]
         L.ulens_roots.argtypes = [vp, C.POINTER(ulens_lens), ip, vp, vp, vp, vp, vp, vp]
         L.ulens_get_stats.argtypes = [vp, C.POINTER(ulens_stats)]
@@ -292,6 +294,27 @@ class Context:
         _check(lib().ulens_lightcurve_binary_host(self._h, n_cfg, n_ep, _dptr(theta), float(u1), p(t), p(A), p(dA),
                                                   p(err), p(st), self._stream(stream)), self._h)
         return A, dA, err, st
+
+    def ulens_lightcurve_binary_ext_host(self, theta, u1, t, A, dA=None, err=None, st=None, ext_mask=None, sel_tol=0.0,
+                                         stream=None):
+        """Host numpy arrays in / out as ulens_lightcurve_binary_host; ext_mask uint8 [n_cfg, n_epochs] or None
+        (library selection). Returns (A, dA, err, st, n_ext)."""
+        theta = np.ascontiguousarray(theta, dtype=np.float64).reshape(-1, 7)
+        t = np.ascontiguousarray(t, dtype=np.float64)
+        n_cfg, n_ep = theta.shape[0], t.size
+        for a, k in ((A, 1), (dA, 7), (err, 1)):
+            if a is not None and (a.dtype != np.float64 or not a.flags.c_contiguous or a.size != k * n_cfg * n_ep):
+                raise UlensError("output arrays must be C-contiguous float64 of the documented size")
+        if st is not None and (st.dtype.itemsize != 4 or not st.flags.c_contiguous or st.size != n_cfg * n_ep):
+            raise UlensError("status array must be C-contiguous 32-bit of n_cfg*n_epochs elements")
+        if ext_mask is not None and (ext_mask.dtype != np.uint8 or not ext_mask.flags.c_contiguous or ext_mask.size != n_cfg * n_ep):
+            raise UlensError("ext_mask must be C-contiguous uint8 of n_cfg*n_epochs elements")
+        p = lambda a: a.ctypes.data_as(C.c_void_p) if a is not None else None
+        n_ext = C.c_int(0)
+        _check(lib().ulens_lightcurve_binary_ext_host(self._h, n_cfg, n_ep, _dptr(theta), float(u1), p(t), p(ext_mask),
+                                                      float(sel_tol), p(A), p(dA), p(err), p(st), C.byref(n_ext),
+                                                      self._stream(stream)), self._h)
+        return A, dA, err, st, n_ext.value
 
     def ulens_roots(self, lens, w_re, w_im, stream=None):
         """All N^2+1 roots per source position and the image flags: (roots complex [n, deg], is_image bool)."""

@@ -1183,6 +1183,42 @@ extern "C" int ulens_lightcurve_binary_host(ulens_ctx* ctx, int n_cfg, int n_epo
     return ULENS_OK;
 }
 
+extern "C" int ulens_lightcurve_binary_ext_host(ulens_ctx* ctx, int n_cfg, int n_epochs, const double* theta_host, double u1,
+                                                const double* t_host, const uint8_t* ext_mask_host, double sel_tol,
+                                                double* A_out_host, double* dA_out_host, double* err_out_host,
+                                                uint32_t* status_out_host, int* n_ext_out, void* stream)
+{
+    if (n_ext_out) *n_ext_out = 0;
+    if (!ctx || n_cfg < 0 || n_epochs < 0) return ULENS_EINVAL;
+    if (n_cfg == 0 || n_epochs == 0) return ULENS_OK;
+    if (!theta_host || !t_host || !A_out_host) return ULENS_EINVAL;
+    CK(cudaSetDevice(ctx->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t n = (size_t)n_cfg * n_epochs;
+    // t, A, err, status (8-byte slots), dA, mask (bytes, rounded up to 8-byte slots)
+    const size_t need = (size_t)n_epochs + n * (3 + (dA_out_host ? 7 : 0)) + (ext_mask_host ? (n + 7) / 8 : 0);
+    if (need > ctx->io_cap) {
+        cudaFree(ctx->io_buf); ctx->io_buf = nullptr; ctx->io_cap = 0;
+        if (cudaMalloc(&ctx->io_buf, sizeof(double) * need) != cudaSuccess) return ULENS_ENOMEM;
+        ctx->io_cap = need;
+    }
+    double* d_t = ctx->io_buf; double* d_A = d_t + n_epochs; double* d_err = d_A + n;
+    unsigned* d_st = reinterpret_cast<unsigned*>(d_err + n);
+    double* d_dA = dA_out_host ? d_err + 2 * n : nullptr;
+    uint8_t* d_mask = ext_mask_host ? reinterpret_cast<uint8_t*>(d_err + 2 * n + (dA_out_host ? 7 * n : 0)) : nullptr;
+    CK(cudaMemcpyAsync(d_t, t_host, sizeof(double) * n_epochs, cudaMemcpyHostToDevice, st));
+    if (d_mask) CK(cudaMemcpyAsync(d_mask, ext_mask_host, n, cudaMemcpyHostToDevice, st));
+    int rc = ulens_lightcurve_binary_ext(ctx, n_cfg, n_epochs, theta_host, u1, d_t, d_mask, sel_tol, d_A, d_dA, d_err, d_st,
+                                         n_ext_out, stream);
+    if (rc != ULENS_OK) return rc;
+    CK(cudaMemcpyAsync(A_out_host, d_A, sizeof(double) * n, cudaMemcpyDeviceToHost, st));
+    if (dA_out_host) CK(cudaMemcpyAsync(dA_out_host, d_dA, sizeof(double) * 7 * n, cudaMemcpyDeviceToHost, st));
+    if (err_out_host) CK(cudaMemcpyAsync(err_out_host, d_err, sizeof(double) * n, cudaMemcpyDeviceToHost, st));
+    if (status_out_host) CK(cudaMemcpyAsync(status_out_host, d_st, sizeof(unsigned) * n, cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    return ULENS_OK;
+}
+
 extern "C" int ulens_mag_point(ulens_ctx* ctx, int n_cfg, int n_pts, const ulens_lens* lenses_host, const double* w_re,
                                const double* w_im, double* A_out, uint32_t* status_out, void* stream)
 {

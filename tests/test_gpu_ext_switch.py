@@ -176,3 +176,21 @@ def test_ext_edge_cases(ctx, torch_cuda):
         torch.cuda.synchronize()
         st1 = _np(st1)
         assert n_ext == 1 and not (st1[0, pos] & ST_POINT_SRC) and ((st1[0] & ST_POINT_SRC) != 0).sum() == 63
+
+
+def test_ext_host_entry_matches_device_entry(ctx, torch_cuda):
+    """ulens_lightcurve_binary_ext_host (host arrays, mask copied in) against the device entry, bit for bit."""
+    torch = torch_cuda
+    theta, t = _case(2, 400)
+    rng = np.random.default_rng(17)
+    m = (rng.random((2, 400)) < 0.3).astype(np.uint8)
+    td = torch.tensor(t, device="cuda:0")
+    for mask_h in (m, None):
+        mask_d = torch.tensor(m, device="cuda:0") if mask_h is not None else None
+        A0, dA0, err0, st0, n0 = ctx.ulens_lightcurve_binary_ext(theta, 0.5, td, ext_mask=mask_d, want_dA=True)
+        torch.cuda.synchronize()
+        A = np.empty((2, 400)); dA = np.empty((2, 400, 7)); err = np.empty((2, 400)); st = np.empty((2, 400), dtype=np.int32)
+        _, _, _, _, n1 = ctx.ulens_lightcurve_binary_ext_host(theta, 0.5, t, A, dA, err, st, ext_mask=mask_h)
+        assert n0 == n1 and (mask_h is None or n1 == int(m.sum()))
+        assert np.array_equal(A, _np(A0)) and np.array_equal(dA, _np(dA0), equal_nan=True)
+        assert np.array_equal(err, _np(err0)) and np.array_equal(st, _np(st0))
