@@ -56,7 +56,12 @@ FP64_PEAK_DFMA = 148 * 64 * 1.965e9
 # the seed was fixed once so that the oracle's work on the sample is a few 1e8 lens-map evaluations.
 CPU_SAMPLE_SEED = 2
 CPU_SAMPLE_CFGS = 8
-CPU_SAMPLE_PER_CFG = 16
+CPU_SAMPLE_PER_CFG_BY_WL = {"C0": 500, "C1": 64, "C2": 256, "C3": 32, "C4": 256}   # sized for ~2-10 s of wall time on 16 cores
+
+
+def sample_per_cfg(wl):
+    return min(CPU_SAMPLE_PER_CFG_BY_WL.get(wl.name, 16), wl.n_pts)
+
 # The parity tests run the oracle at (n_rho, ss) = (100, 8); a near-caustic point of C1 (A of a few hundred)
 # then costs ~1e9 lens-map evaluations = minutes of ONE core (the oracle parallelises over points only), which
 # no 10-30 s sample can hold. The timed baseline therefore runs the same oracle at (50, 4): 16x less work,
@@ -131,7 +136,7 @@ def oracle_lenses(O, wl, cs):
 
 def cpu_sample(wl, inputs):
     """(config indices, point indices [n_cfg_used, k]) of the bounded oracle sample."""
-    idx = inputs.subsample(wl, CPU_SAMPLE_PER_CFG, seed=CPU_SAMPLE_SEED)
+    idx = inputs.subsample(wl, sample_per_cfg(wl), seed=CPU_SAMPLE_SEED)
     n_used = min(CPU_SAMPLE_CFGS, wl.n_cfg)
     cs = list(range(0, wl.n_cfg, max(1, wl.n_cfg // n_used)))[:n_used]
     return cs, idx
@@ -175,7 +180,7 @@ def main_reference(args, rank, world):
         tot_t += dt; tot_pts += n; tot_ev += ev
     value = tot_pts / tot_t
     sample = "%d seeded points per step (%d configs x %d, half near-caustic, seed %d) at oracle n_rho=%d ss=%d" % (
-        tot_pts // max(args.steps, 1), CPU_SAMPLE_CFGS, CPU_SAMPLE_PER_CFG, CPU_SAMPLE_SEED, ORACLE_N_RHO, ORACLE_SS)
+        tot_pts // max(args.steps, 1), min(CPU_SAMPLE_CFGS, wl.n_cfg), sample_per_cfg(wl), CPU_SAMPLE_SEED, ORACLE_N_RHO, ORACLE_SS)
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": min(args.warmup, 1), "ms_per_step": 1e3 * tot_t / max(args.steps, 1),
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -353,7 +358,7 @@ def main_ours(args, rank, local_rank, world):
             npts, dt, nev, cores = run_oracle_sample(wl, inputs)
             line["cpu_baseline"] = {"value": npts / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
                                     "sample": "%d seeded points (%d configs x %d, half near-caustic, seed %d), oracle n_rho=%d ss=%d, %.1f s"
-                                              % (npts, CPU_SAMPLE_CFGS, CPU_SAMPLE_PER_CFG, CPU_SAMPLE_SEED, ORACLE_N_RHO, ORACLE_SS, dt),
+                                              % (npts, min(CPU_SAMPLE_CFGS, wl.n_cfg), sample_per_cfg(wl), CPU_SAMPLE_SEED, ORACLE_N_RHO, ORACLE_SS, dt),
                                     "rays_per_s": nev / dt}
         print(json.dumps(line), flush=True)
     ctx.close()
