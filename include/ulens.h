@@ -54,9 +54,13 @@ extern "C" {
 #define ULENS_ST_ERR_HIGH    0x0040u  /* half-resolution self-check differs by more than rel_tol */
 #define ULENS_ST_NO_IMAGE    0x0080u  /* no image-limb point found (A = NaN) */
 #define ULENS_ST_NIMG_SHIFT  8        /* bits 8..11: number of images of the source centre */
+#define ULENS_ST_RETRIED     0x2000u  /* the first result was doubtful (EA_NOCONV, PATCH_CAP, CLIPPED, ERR_HIGH or NO_IMAGE): this is the
+                                         result and status of the retry pass with twice the limb samples */
 #define ULENS_ST_POINT_SRC   0x1000u  /* ulens_lightcurve_binary_ext: the epoch took the point-source value (Eq. 2-3) */
 
 typedef struct ulens_ctx ulens_ctx;
+
+#define ULENS_OPT_NO_RETRY   0x1      /* ulens_options.flags: do not re-integrate doubtful points (see ULENS_ST_RETRIED) */
 
 /* Tunables; a zeroed struct (or NULL) selects the defaults in brackets. */
 typedef struct {
@@ -65,7 +69,7 @@ typedef struct {
     int    n_theta;       /* rays per image half-chord along a scan line (P:139 N_theta)         [48]    */
     double rel_tol;       /* self-check threshold for ULENS_ST_ERR_HIGH                          [1e-4]  */
     int    chunk_pts;     /* points processed per internal pass (workspace size)                 [65536] */
-    int    flags;         /* reserved, 0 */
+    int    flags;         /* ULENS_OPT_* bits                                                    [0]     */
 } ulens_options;
 
 /* Lens: n_lens in {1,2,3}; eps sums to 1; positions in Einstein radii of the total mass. */

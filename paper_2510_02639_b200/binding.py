@@ -25,6 +25,11 @@ EXPORTS = ["ulens_create", "ulens_destroy", "ulens_lens_binary", "ulens_lens_tri
            "ulens_last_cuda_error"]
 
 
+ULENS_OPT_NO_RETRY = 0x1
+ULENS_ST_RETRIED = 0x2000
+ULENS_ST_POINT_SRC = 0x1000
+
+
 class ulens_options(C.Structure):
     _fields_ = [("n_limb", C.c_int), ("n_r", C.c_int), ("n_theta", C.c_int), ("rel_tol", C.c_double),
                 ("chunk_pts", C.c_int), ("flags", C.c_int)]
@@ -129,13 +134,13 @@ class Context:
     """ulens_ctx: one device, one stream at a time. Methods mirror the C entry points."""
 
     def __init__(self, device: int = 0, n_limb: int = 0, n_r: int = 0, n_theta: int = 0, rel_tol: float = 0.0,
-                 chunk_pts: int = 0):
+                 chunk_pts: int = 0, flags: int = 0):
         import torch
         if not torch.cuda.is_available():
             raise UlensError("no CUDA device: the ulens hot path has no CPU fallback")
         self._torch = torch
         self.device = device
-        opt = ulens_options(n_limb, n_r, n_theta, rel_tol, chunk_pts, 0)
+        opt = ulens_options(n_limb, n_r, n_theta, rel_tol, chunk_pts, flags)
         self._h = C.c_void_p()
         _check(lib().ulens_create(C.byref(self._h), device, C.byref(opt)))
 

@@ -62,6 +62,7 @@ struct ulens_ctx {
     double* io_buf; size_t io_cap;      // *_host entry: staging
     // point-source / finite-source switch (ulens_lightcurve_binary_ext): flags, block offsets, gather map
     unsigned char* ext_flag; int* ext_map; unsigned* ext_blk; size_t ext_cap;
+    unsigned* st_all; size_t st_all_cap;    // status of every point when the caller passes none (the retry pass reads it)
     int last_launches;
     // optional per-kernel device timing (ulens_set_timing): event pairs recorded on the caller's stream
     int timing_on;
@@ -156,10 +157,11 @@ __global__ void k_roots(int n, int pt_base, int n_pts_per_cfg, const PointCfg* _
                         uint8_t* __restrict__ out_img, unsigned* __restrict__ status,
                         double* __restrict__ c_zr, double* __restrict__ c_zi, unsigned* __restrict__ c_mask,
                         double* __restrict__ A_ps = nullptr, unsigned* __restrict__ status_global = nullptr,
-                        const int* __restrict__ pmap = nullptr)
+                        const int* __restrict__ pmap = nullptr, const unsigned* __restrict__ n_dev = nullptr)
 {
     constexpr int DEG = N * N + 1;
     int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (n_dev) n = min(n, (int)*n_dev);              // retry pass: the point count lives on the device
     if (i >= n) return;
     long long gp = pmap ? (long long)pmap[pt_base + i] : (long long)pt_base + i;
     int c = (int)(gp / n_pts_per_cfg);
@@ -326,6 +328,17 @@ __global__ void k_point_ext(int n, int n_pts_per_cfg, const PointCfg* __restrict
     if (grad5) for (int k = 0; k < UL_NT; ++k) grad5[(long long)i * UL_NT + k] = g5[k];
 }
 
+// which points the retry pass takes: a doubtful finite-source result (not the centre's image parity, which is
+// informational, nor a resolution cap, which more limb points cannot lift); never a point-source epoch
+#define UL_ST_RETRY_MASK (UL_ST_EA_NOCONV | UL_ST_PATCH_CAP | UL_ST_CLIPPED | UL_ST_ERR_HIGH | UL_ST_NO_IMAGE)
+__global__ void k_retry_flag(int n, const unsigned* __restrict__ status, unsigned char* __restrict__ flag)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    unsigned st = status[i];
+    flag[i] = ((st & UL_ST_RETRY_MASK) && !(st & UL_ST_POINT_SRC)) ? 1 : 0;
+}
+
 // ordered stream compaction of the flagged epochs into the gather map (three small kernels, 1024 epochs per block)
 __global__ void k_ext_count(int n, const unsigned char* __restrict__ flag, unsigned* __restrict__ blk)
 {
@@ -389,7 +402,8 @@ k_regions(int n, int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cf
           Patch* __restrict__ patches, int* __restrict__ n_patch, unsigned* __restrict__ status,
           unsigned* __restrict__ unit_desc, unsigned cap_units, ChunkCounters* cc, DevCounters* ctr,
           const double* __restrict__ c_zr, const double* __restrict__ c_zi, const unsigned* __restrict__ c_mask,
-          const TangentTable* __restrict__ tans, PatchTan* __restrict__ ptans, const int* __restrict__ pmap = nullptr)
+          const TangentTable* __restrict__ tans, PatchTan* __restrict__ ptans, const int* __restrict__ pmap = nullptr,
+          const unsigned* __restrict__ n_dev = nullptr)
 {
     constexpr int DEG = N * N + 1;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -398,6 +412,7 @@ k_regions(int n, int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cf
     BoxExt* ext_all = reinterpret_cast<BoxExt*>(smem_raw + (blockDim.x >> 5) * sizeof(RegionWork<DEG>));
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     int i = blockIdx.x * (blockDim.x >> 5) + warp;
+    if (n_dev) n = min(n, (int)*n_dev);
     if (i >= n) return;                                  // whole warp leaves together
     RegionWork<DEG>& W = Wall[warp];
     if (lane == 0) W.ext = tans ? ext_all + warp * 32 * DEG : nullptr;
@@ -498,9 +513,11 @@ __global__ void k_finalize(int n, int pt_base, int n_pts_per_cfg, const PointCfg
                            const double* __restrict__ unit_sum, const double* __restrict__ unit_odd,
                            const unsigned* __restrict__ status_ws, double rel_tol,
                            double* __restrict__ A_out, double* __restrict__ err_out, unsigned* __restrict__ status_out,
-                           DevCounters* ctr, const int* __restrict__ pmap = nullptr)
+                           DevCounters* ctr, const int* __restrict__ pmap = nullptr,
+                           const unsigned* __restrict__ n_dev = nullptr, unsigned st_or = 0)
 {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (n_dev) n = min(n, (int)*n_dev);
     if (i >= n) return;
     long long gp = pmap ? (long long)pmap[pt_base + i] : (long long)pt_base + i;
     int c = (int)(gp / n_pts_per_cfg);
@@ -515,7 +532,7 @@ __global__ void k_finalize(int n, int pt_base, int n_pts_per_cfg, const PointCfg
         nu_tot += nu;
         for (int b = 0; b < nu; ++b) { s += unit_sum[P.unit0 + b]; so += unit_odd[P.unit0 + b]; }
     }
-    unsigned st = status_ws[i];
+    unsigned st = status_ws[i] | st_or;
     double A = s / F0, Ao = so / F0;
     if (np == 0) { A = nan(""); Ao = A; }
     // half-resolution self check: the radial rule errs like dr^1.5 (square-root ring ends), so the error
@@ -526,8 +543,12 @@ __global__ void k_finalize(int n, int pt_base, int n_pts_per_cfg, const PointCfg
     if (err_out) err_out[gp] = err;
     if (status_out) status_out[gp] = st;
     atomicAdd(&ctr->n_units, nu_tot);
-    if (i == 0) atomicAdd(&ctr->n_points, (unsigned long long)n);
-    if (st & 0xffu) atomicAdd(&ctr->n_flagged, 1ull);
+    if (st_or) {                                         // retry pass: the point was counted (and counted as flagged) before
+        if (!(st & 0xffu)) atomicAdd(&ctr->n_flagged, ~0ull);
+    } else {
+        if (i == 0) atomicAdd(&ctr->n_points, (unsigned long long)n);
+        if (st & 0xffu) atomicAdd(&ctr->n_flagged, 1ull);
+    }
 }
 
 // ------------------------------------------------------------------------------------------------ forward-mode variant (a8)
@@ -656,9 +677,11 @@ k_shoot_dual(int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cfg, c
 __global__ void k_finalize_dual(int n, int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cfg,
                                 const TangentTable* __restrict__ tans, const Patch* __restrict__ patches,
                                 const int* __restrict__ n_patch, const double* __restrict__ unit_sum,
-                                const double* __restrict__ unit_tan, double* __restrict__ grad5, const int* __restrict__ pmap = nullptr)
+                                const double* __restrict__ unit_tan, double* __restrict__ grad5, const int* __restrict__ pmap = nullptr,
+                                const unsigned* __restrict__ n_dev = nullptr)
 {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (n_dev) n = min(n, (int)*n_dev);
     if (i >= n) return;
     long long gp = pmap ? (long long)pmap[pt_base + i] : (long long)pt_base + i;
     int c = (int)(gp / n_pts_per_cfg);
@@ -792,7 +815,7 @@ extern "C" void ulens_destroy(ulens_ctx* ctx)
     cudaFree(ctx->patches); cudaFree(ctx->n_patch); cudaFree(ctx->status_ws); cudaFree(ctx->unit_desc);
     cudaFree(ctx->unit_sum); cudaFree(ctx->unit_odd); cudaFree(ctx->cc); cudaFree(ctx->counters);
     cudaFree(ctx->cfg_dev); cudaFree(ctx->poly_dev); cudaFree(ctx->traj_w); cudaFree(ctx->io_buf);
-    cudaFree(ctx->ext_flag); cudaFree(ctx->ext_map); cudaFree(ctx->ext_blk);
+    cudaFree(ctx->ext_flag); cudaFree(ctx->ext_map); cudaFree(ctx->ext_blk); cudaFree(ctx->st_all);
     if (ctx->timed) {
         for (auto& t : *ctx->timed) { cudaEventDestroy(t.a); cudaEventDestroy(t.b); }
         delete ctx->timed;
@@ -843,8 +866,10 @@ static int upload_cfgs(ulens_ctx* ctx, int n_cfg, const ulens_lens* lenses, cons
 template <int N>
 static int run_chunks(ulens_ctx* ctx, long long n_total, int n_pts, bool ld, const double* w_re, const double* w_im,
                       double* A_out, double* err_out, unsigned* status_out, cudaStream_t st, double* grad5_out = nullptr,
-                      const int* pmap = nullptr)
+                      const int* pmap = nullptr, const unsigned* n_dev = nullptr, const RegionParams* rp_override = nullptr,
+                      unsigned st_or = 0)
 {
+    const RegionParams rp = rp_override ? *rp_override : ctx->rp;
     constexpr int DEG = N * N + 1;
     const bool dual = grad5_out != nullptr;
     const TangentTable* tans = dual ? ctx->tan_dev : nullptr;
@@ -866,13 +891,13 @@ static int run_chunks(ulens_ctx* ctx, long long n_total, int n_pts, bool ld, con
         {
             KTimer kt(ctx, ULENS_K_ROOTS, st);
             k_roots<N><<<(n + 127) / 128, 128, 0, st>>>(n, (int)base, n_pts, ctx->cfg_dev, ctx->poly_dev, w_re, w_im,
-                                                        nullptr, nullptr, nullptr, ctx->status_ws, ctx->c_zr, ctx->c_zi, ctx->c_mask, nullptr, nullptr, pmap);
+                                                        nullptr, nullptr, nullptr, ctx->status_ws, ctx->c_zr, ctx->c_zi, ctx->c_mask, nullptr, nullptr, pmap, n_dev);
         }
         {
             KTimer kt(ctx, ULENS_K_REGIONS, st);
-            k_regions<N><<<(n + wpc - 1) / wpc, 32 * wpc, smem, st>>>(n, (int)base, n_pts, ctx->cfg_dev, ctx->poly_dev, w_re, w_im, ctx->rp,
+            k_regions<N><<<(n + wpc - 1) / wpc, 32 * wpc, smem, st>>>(n, (int)base, n_pts, ctx->cfg_dev, ctx->poly_dev, w_re, w_im, rp,
                                                          ctx->patches, ctx->n_patch, ctx->status_ws, ctx->unit_desc,
-                                                         (unsigned)ctx->cap_units, ctx->cc, ctx->counters, ctx->c_zr, ctx->c_zi, ctx->c_mask, tans, ctx->ptans, pmap);
+                                                         (unsigned)ctx->cap_units, ctx->cc, ctx->counters, ctx->c_zr, ctx->c_zi, ctx->c_mask, tans, ctx->ptans, pmap, n_dev);
         }
         // persistent grid: as many CTAs as are resident at once (occupancy API; 4-6 per SM by register count)
         int per_sm = 4;
@@ -888,11 +913,11 @@ static int run_chunks(ulens_ctx* ctx, long long n_total, int n_pts, bool ld, con
                 if (dual && ld)
                     k_shoot_dual<N, true><<<grid, 128, 0, st>>>((int)base, n_pts, ctx->cfg_dev, tans, w_re, w_im, ctx->patches, ctx->ptans,
                                                                 ctx->unit_desc, ctx->unit_sum, ctx->unit_odd, ctx->unit_tan, ctx->status_ws,
-                                                                ctx->cc, ctx->counters, (unsigned)ctx->cap_units, ctx->rp.n_theta, pmap);
+                                                                ctx->cc, ctx->counters, (unsigned)ctx->cap_units, rp.n_theta, pmap);
                 else if (dual)
                     k_shoot_dual<N, false><<<grid, 128, 0, st>>>((int)base, n_pts, ctx->cfg_dev, tans, w_re, w_im, ctx->patches, ctx->ptans,
                                                                  ctx->unit_desc, ctx->unit_sum, ctx->unit_odd, ctx->unit_tan, ctx->status_ws,
-                                                                 ctx->cc, ctx->counters, (unsigned)ctx->cap_units, ctx->rp.n_theta, pmap);
+                                                                 ctx->cc, ctx->counters, (unsigned)ctx->cap_units, rp.n_theta, pmap);
             }
             if (dual) {}
             else if (ld)
@@ -906,10 +931,10 @@ static int run_chunks(ulens_ctx* ctx, long long n_total, int n_pts, bool ld, con
             KTimer kt(ctx, ULENS_K_FINALIZE, st);
             k_finalize<<<(n + 127) / 128, 128, 0, st>>>(n, (int)base, n_pts, ctx->cfg_dev, ctx->patches, ctx->n_patch,
                                                         ctx->unit_sum, ctx->unit_odd, ctx->status_ws, ctx->opt.rel_tol,
-                                                        A_out, err_out, status_out, ctx->counters, pmap);
+                                                        A_out, err_out, status_out, ctx->counters, pmap, n_dev, st_or);
             if (dual) {
                 k_finalize_dual<<<(n + 127) / 128, 128, 0, st>>>(n, (int)base, n_pts, ctx->cfg_dev, tans, ctx->patches, ctx->n_patch,
-                                                                 ctx->unit_sum, ctx->unit_tan, grad5_out, pmap);
+                                                                 ctx->unit_sum, ctx->unit_tan, grad5_out, pmap, n_dev);
                 ctx->last_launches += 1;
             }
         }
@@ -917,6 +942,44 @@ static int run_chunks(ulens_ctx* ctx, long long n_total, int n_pts, bool ld, con
         CK(cudaGetLastError());
     }
     return ULENS_OK;
+}
+
+static int ensure_ext_buffers(ulens_ctx* ctx, size_t n)
+{
+    if (n <= ctx->ext_cap) return ULENS_OK;
+    cudaFree(ctx->ext_flag); cudaFree(ctx->ext_map); cudaFree(ctx->ext_blk);
+    ctx->ext_flag = nullptr; ctx->ext_map = nullptr; ctx->ext_blk = nullptr; ctx->ext_cap = 0;
+    if (cudaMalloc(&ctx->ext_flag, n) != cudaSuccess) return ULENS_ENOMEM;
+    if (cudaMalloc(&ctx->ext_map, sizeof(int) * n) != cudaSuccess) return ULENS_ENOMEM;
+    if (cudaMalloc(&ctx->ext_blk, sizeof(unsigned) * ((n + 1023) / 1024 + 1)) != cudaSuccess) return ULENS_ENOMEM;
+    ctx->ext_cap = n;
+    return ULENS_OK;
+}
+
+// Retry pass. The points whose finite-source result came back doubtful (UL_ST_RETRY_MASK: an inside
+// ray on a sector border, self-check above rel_tol, sector cap, EA cap, no image-limb point) are gathered and
+// integrated once more with twice the limb samples (Eq. 8), which moves every sector border; the new result and
+// status (| ULENS_ST_RETRIED) replace the old ones. Their number stays on the device -- the launches are sized for
+// the worst case (one chunk; further flagged points keep their first result) -- so nothing synchronises.
+template <int N>
+static int retry_flagged(ulens_ctx* ctx, long long n_total, int n_pts, bool ld, const double* w_re, const double* w_im,
+                         double* A_out, double* err_out, unsigned* status, cudaStream_t st, double* grad5_out)
+{
+    if (ctx->opt.flags & ULENS_OPT_NO_RETRY) return ULENS_OK;
+    int rc = ensure_ext_buffers(ctx, (size_t)n_total);
+    if (rc != ULENS_OK) return rc;
+    const int n = (int)n_total, n_blk = (n + 1023) / 1024;
+    k_retry_flag<<<(n + 255) / 256, 256, 0, st>>>(n, status, ctx->ext_flag);
+    k_ext_count<<<n_blk, 1024, 0, st>>>(n, ctx->ext_flag, ctx->ext_blk);
+    k_ext_scan<<<1, 1024, 0, st>>>(n_blk, ctx->ext_blk);
+    k_ext_scatter<<<n_blk, 1024, 0, st>>>(n, ctx->ext_flag, ctx->ext_blk, ctx->ext_map);
+    ctx->last_launches += 4;
+    CK(cudaGetLastError());
+    RegionParams rp2 = ctx->rp;
+    rp2.n_limb = ctx->rp.n_limb * 2 > 8192 ? 8192 : ctx->rp.n_limb * 2;
+    const long long n_max = n_total < ctx->chunk ? n_total : ctx->chunk;
+    return run_chunks<N>(ctx, n_max, n_pts, ld, w_re, w_im, A_out, err_out, status, st, grad5_out, ctx->ext_map,
+                         ctx->ext_blk + n_blk, &rp2, UL_ST_RETRIED);
 }
 
 // tangent tables of the UL_NT intrinsic directions (w_cx, w_cy, s, q, rho). The lens-parameter directions
@@ -964,10 +1027,24 @@ static int mag_device(ulens_ctx* ctx, int n_cfg, int n_pts, const ulens_lens* le
     long long n_total = (long long)n_cfg * n_pts;
     if (n_total > 0x7fffffffLL) return ULENS_EUNSUPPORTED;
     ctx->last_launches = 0;
+    if (!status_out) {                                   // the retry pass needs every point's status
+        if ((size_t)n_total > ctx->st_all_cap) {
+            cudaFree(ctx->st_all); ctx->st_all = nullptr; ctx->st_all_cap = 0;
+            if (cudaMalloc(&ctx->st_all, sizeof(unsigned) * (size_t)n_total) != cudaSuccess) return ULENS_ENOMEM;
+            ctx->st_all_cap = (size_t)n_total;
+        }
+        status_out = ctx->st_all;
+    }
     switch (N) {
-        case 1: rc = run_chunks<1>(ctx, n_total, n_pts, ld, w_re, w_im, A_out, err_out, status_out, st, grad5_out); break;
-        case 2: rc = run_chunks<2>(ctx, n_total, n_pts, ld, w_re, w_im, A_out, err_out, status_out, st, grad5_out); break;
-        default: rc = run_chunks<3>(ctx, n_total, n_pts, ld, w_re, w_im, A_out, err_out, status_out, st, grad5_out); break;
+        case 1: rc = run_chunks<1>(ctx, n_total, n_pts, ld, w_re, w_im, A_out, err_out, status_out, st, grad5_out);
+                if (rc == ULENS_OK) rc = retry_flagged<1>(ctx, n_total, n_pts, ld, w_re, w_im, A_out, err_out, status_out, st, grad5_out);
+                break;
+        case 2: rc = run_chunks<2>(ctx, n_total, n_pts, ld, w_re, w_im, A_out, err_out, status_out, st, grad5_out);
+                if (rc == ULENS_OK) rc = retry_flagged<2>(ctx, n_total, n_pts, ld, w_re, w_im, A_out, err_out, status_out, st, grad5_out);
+                break;
+        default: rc = run_chunks<3>(ctx, n_total, n_pts, ld, w_re, w_im, A_out, err_out, status_out, st, grad5_out);
+                if (rc == ULENS_OK) rc = retry_flagged<3>(ctx, n_total, n_pts, ld, w_re, w_im, A_out, err_out, status_out, st, grad5_out);
+                break;
     }
     return rc;
 }
@@ -1101,13 +1178,17 @@ extern "C" int ulens_lightcurve_binary_ext(ulens_ctx* ctx, int n_cfg, int n_epoc
         ctx->traj_cap = need;
     }
     const int n_blk = (int)((n + 1023) / 1024);
-    if (n > ctx->ext_cap) {
-        cudaFree(ctx->ext_flag); cudaFree(ctx->ext_map); cudaFree(ctx->ext_blk);
-        ctx->ext_flag = nullptr; ctx->ext_map = nullptr; ctx->ext_blk = nullptr; ctx->ext_cap = 0;
-        if (cudaMalloc(&ctx->ext_flag, n) != cudaSuccess) return ULENS_ENOMEM;
-        if (cudaMalloc(&ctx->ext_map, sizeof(int) * n) != cudaSuccess) return ULENS_ENOMEM;
-        if (cudaMalloc(&ctx->ext_blk, sizeof(unsigned) * ((size_t)n_blk + 1)) != cudaSuccess) return ULENS_ENOMEM;
-        ctx->ext_cap = n;
+    {
+        int rc = ensure_ext_buffers(ctx, n);
+        if (rc != ULENS_OK) return rc;
+    }
+    if (!status_out) {
+        if (n > ctx->st_all_cap) {
+            cudaFree(ctx->st_all); ctx->st_all = nullptr; ctx->st_all_cap = 0;
+            if (cudaMalloc(&ctx->st_all, sizeof(unsigned) * n) != cudaSuccess) return ULENS_ENOMEM;
+            ctx->st_all_cap = n;
+        }
+        status_out = ctx->st_all;
     }
     double* w_re = ctx->traj_w; double* w_im = w_re + n; double* th_dev = w_im + n;
     double* g5 = dA_out ? th_dev + 7 * (size_t)n_cfg : nullptr;
@@ -1143,6 +1224,7 @@ extern "C" int ulens_lightcurve_binary_ext(ulens_ctx* ctx, int n_cfg, int n_epoc
     if (n_ext_out) *n_ext_out = (int)n_ext;
     if (n_ext > 0) {
         rc = run_chunks<2>(ctx, (long long)n_ext, n_epochs, ld, w_re, w_im, A_out, err_out, status_out, st, g5, ctx->ext_map);
+        if (rc == ULENS_OK) rc = retry_flagged<2>(ctx, (long long)n, n_epochs, ld, w_re, w_im, A_out, err_out, status_out, st, g5);
         if (rc != ULENS_OK) return rc;
     }
     if (dA_out) {

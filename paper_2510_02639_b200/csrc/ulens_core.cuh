@@ -85,8 +85,12 @@ struct Patch {
 #define UL_ST_ERR_HIGH   0x0040u
 #define UL_ST_NO_IMAGE   0x0080u
 #define UL_ST_POINT_SRC  0x1000u
+#define UL_ST_RETRIED    0x2000u
 
 #define UL_PI 3.14159265358979323846
+// the 8 directions k pi/4 (seeds on a light lens's Einstein ring)
+#define UL_RING8_X(k) ((k) == 0 ? 1.0 : (k) == 4 ? -1.0 : ((k) == 2 || (k) == 6) ? 0.0 : ((k) == 1 || (k) == 7) ? 0.70710678118654752 : -0.70710678118654752)
+#define UL_RING8_Y(k) ((k) == 2 ? 1.0 : (k) == 6 ? -1.0 : ((k) == 0 || (k) == 4) ? 0.0 : ((k) == 1 || (k) == 3) ? 0.70710678118654752 : -0.70710678118654752)
 #define UL_BIG 1e100
 
 UL_HD double ul_min(double a, double b) { return a < b ? a : b; }
@@ -512,6 +516,39 @@ UL_HDN unsigned centre_images(const Lens& L, const LensPoly& T, double wx, doubl
                     if (mask & (1u << k)) continue;
                     double ddx = zr[k] - zx, ddy = zi[k] - zy, d = ddx * ddx + ddy * ddy;
                     if (d < bd) { bd = d; slot = k; }
+                }
+                if (slot < 0) continue;
+                ix[n_img] = zx; iy[n_img] = zy; ++n_img; mask |= 1u << slot; zr[slot] = zx; zi[slot] = zy;
+            }
+        }
+    }
+    // Still the wrong parity: images next to a LIGHT lens (eps_a < 1e-2: the pair a planetary caustic adds, of ordinary
+    // brightness) hide in the same unresolved cluster (seen on C3 with q3 ~ 1e-5: A off by 10-40 %).
+    // Seed Eq. 1 from 8 points of that lens's own Einstein ring |z - a| = sqrt(eps_a), where those images live.
+    if constexpr (N > 1) {
+#pragma unroll 1
+        for (int a = 0; a < N; ++a) {
+            if (!(((n_img - (N + 1)) & 1) != 0 || n_img < N + 1)) break;
+            if (!(L.eps[a] < 1e-2)) continue;
+            const double re = sqrt(L.eps[a]);
+#pragma unroll 1
+            for (int k = 0; k < 8; ++k) {
+                double zx = L.ax[a] + re * UL_RING8_X(k), zy = L.ay[a] + re * UL_RING8_Y(k);
+                double detJ, resid, gx, gy;
+                bool ok = polish_image<N>(L, wx, wy, zx, zy, 12, 1e-13, detJ, resid, gx, gy);
+                if (ok) {
+                    double sc = ul_max(1.0, zx * zx + zy * zy);
+                    for (int q = 0; q < n_img; ++q) {
+                        double ddx = zx - ix[q], ddy = zy - iy[q];
+                        if (ddx * ddx + ddy * ddy < 1e-18 * sc) ok = false;
+                    }
+                }
+                if (!ok || n_img >= DEG) continue;
+                int slot = -1; double bd = 1e300;
+                for (int m = 0; m < DEG; ++m) {
+                    if (mask & (1u << m)) continue;
+                    double ddx = zr[m] - zx, ddy = zi[m] - zy, d = ddx * ddx + ddy * ddy;
+                    if (d < bd) { bd = d; slot = m; }
                 }
                 if (slot < 0) continue;
                 ix[n_img] = zx; iy[n_img] = zy; ++n_img; mask |= 1u << slot; zr[slot] = zx; zi[slot] = zy;

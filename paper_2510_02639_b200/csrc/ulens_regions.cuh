@@ -168,6 +168,25 @@ UL_HDN void regions_phaseA(int lane, const Lens& L, const LensPoly& T, double wc
     // cusp the image boundary races along a long arc within a fraction of dphi and uniform limb sampling
     // would leave most of that arc unsampled -- and (down to dphi / 8) when the set of images
     // changed, which localises the creation / destruction of an image pair on a caustic.
+    // light lenses (eps_a < 1e-2) whose planetary caustic -- centred on w_a = a_a - sum_{b != a} eps_b/conj(a_a - a_b),
+    // a few sqrt(eps_a) across -- the source overlaps or nearly so
+    unsigned near_light = 0;
+    if (N == 3) {
+#pragma unroll
+        for (int a = 0; a < N; ++a) {
+            if (!(L.eps[a] < 1e-2)) continue;
+            double tx = L.ax[a] - wcx, ty = L.ay[a] - wcy;
+#pragma unroll
+            for (int b = 0; b < N; ++b) {
+                if (b == a) continue;
+                double dx = L.ax[a] - L.ax[b], dy = L.ay[a] - L.ay[b];
+                double i2 = L.eps[b] / (dx * dx + dy * dy);
+                tx -= dx * i2; ty -= dy * i2;
+            }
+            const double R = 8.0 * sqrt(L.eps[a]) + 2.0 * rho;
+            if (tx * tx + ty * ty < R * R) near_light |= 1u << a;
+        }
+    }
     const double dphi = 2.0 * UL_PI / P.n_limb;
     const double ph0 = dphi * (lane * chunk), ph_end = dphi * (lane * chunk + chunk);
     double ph = ph0, step = dphi;
@@ -303,6 +322,47 @@ UL_HDN void regions_phaseA(int lane, const Lens& L, const LensPoly& T, double wc
                 valid |= 1u << q; px[q] = zx; py[q] = zy; zr[q] = zx; zi[q] = zy;
                 local_extents(zx, zy, gx, gy, rho, hrr[q], htt[q], crr[q], ctt[q]);
                 if (fabs(detJ) > 1e7) faint |= 1u << q;
+            }
+        }
+        if (N == 3) {
+            // Wrong image parity at this limb point: images next to a light lens are hidden in the root cluster
+            // EA cannot resolve (see centre_images). Seed Eq. 1 from that lens's Einstein ring; whatever converges to
+            // an image no slot holds yet takes a free slot and is tracked by continuation from here on.
+            int nv = 0;
+#pragma unroll
+            for (int j = 0; j < DEG; ++j) nv += (valid >> j) & 1u;
+            const bool bad_parity = (((nv - (N + 1)) & 1) != 0 || nv < N + 1);
+            // A missing PAIR leaves the parity right. Where the source sits on the planetary caustic of a light lens
+            // (near_light, below) the ring is therefore seeded at every limb point.
+            if (bad_parity || near_light) {
+#pragma unroll 1
+                for (int a = 0; a < N; ++a) {
+                    if (!(L.eps[a] < 1e-2)) continue;
+                    if (!bad_parity && !(near_light & (1u << a))) continue;
+                    const double re = sqrt(L.eps[a]);
+#pragma unroll 1
+                    // all 8 directions at the arc's first point and on a wrong parity; otherwise the even and the odd
+                    // four on alternate limb points (an image, once found, is tracked by continuation)
+                    const int k_step = (first || bad_parity) ? 1 : 2, k_0 = (first || bad_parity) ? 0 : (n_solves & 1);
+                    for (int k = k_0; k < 8; k += k_step) {
+                        double zx = L.ax[a] + re * UL_RING8_X(k), zy = L.ay[a] + re * UL_RING8_Y(k), detJ, resid, gx, gy;
+                        if (!polish_image_ni<N>(L, wx, wy, zx, zy, 12, 1e-9, detJ, resid, gx, gy)) continue;
+                        bool dup = false;
+                        int free_slot = -1;
+#pragma unroll 1
+                        for (int q = 0; q < DEG; ++q) {
+                            if (valid & (1u << q)) {
+                                double ddx = zx - px[q], ddy = zy - py[q];
+                                if (ddx * ddx + ddy * ddy < 1e-10 * ul_max(1.0, zx * zx + zy * zy)) dup = true;
+                            } else if (free_slot < 0) free_slot = q;
+                        }
+                        if (dup || free_slot < 0) continue;
+                        const int q = free_slot;
+                        valid |= 1u << q; px[q] = zx; py[q] = zy; zr[q] = zx; zi[q] = zy;
+                        local_extents(zx, zy, gx, gy, rho, hrr[q], htt[q], crr[q], ctt[q]);
+                        if (fabs(detJ) > 1e7) faint |= 1u << q;
+                    }
+                }
             }
         }
         if (!first && ++guard < 4096) {
