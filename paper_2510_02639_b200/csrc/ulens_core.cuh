@@ -528,9 +528,23 @@ UL_HDN unsigned centre_images(const Lens& L, const LensPoly& T, double wx, doubl
     if constexpr (N > 1) {
 #pragma unroll 1
         for (int a = 0; a < N; ++a) {
-            if (!(((n_img - (N + 1)) & 1) != 0 || n_img < N + 1)) break;
             if (!(L.eps[a] < 1e-2)) continue;
             const double re = sqrt(L.eps[a]);
+            // a missing PAIR leaves the parity right: where the source sits on this lens's planetary caustic (centre
+            // w_a = a_a - sum_{b != a} eps_b/conj(a_a - a_b), a few sqrt(eps_a) across) the ring is seeded regardless
+            bool near = false;
+            if (N == 3) {
+                double tx = L.ax[a] - wx, ty = L.ay[a] - wy;
+#pragma unroll
+                for (int b = 0; b < N; ++b) {
+                    if (b == a) continue;
+                    double dx = L.ax[a] - L.ax[b], dy = L.ay[a] - L.ay[b];
+                    double i2 = L.eps[b] / (dx * dx + dy * dy);
+                    tx -= dx * i2; ty -= dy * i2;
+                }
+                near = tx * tx + ty * ty < 64.0 * L.eps[a];
+            }
+            if (!near && !(((n_img - (N + 1)) & 1) != 0 || n_img < N + 1)) continue;
 #pragma unroll 1
             for (int k = 0; k < 8; ++k) {
                 double zx = L.ax[a] + re * UL_RING8_X(k), zy = L.ay[a] + re * UL_RING8_Y(k);
