@@ -46,9 +46,9 @@ FP64_INSTR_PER_RAY_DUAL_EXTRA = 74
 # N+1..DEG images 2.5 iterations x (17 N + 25), boxes ~100.
 FP64_INSTR_PER_LIMB_SOLVE = {1: 600, 2: 2400, 3: 8300}
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the roofline kernel, from the `ncu --set full`
-# captures summarised in profiles/r01d_ncu_k_shoot_c1.md (C1) and profiles/r01c_ncu_k_shoot_dual_c4.md (C4);
+# captures summarised in profiles/r01g_ncu_k_shoot_c1.md (C1) and profiles/r01c_ncu_k_shoot_dual_c4.md (C4);
 # configs without a capture report null.
-NCU_TRAFFIC_BYTES_PER_LAUNCH = {1: 27.4040e6 + 0.5501e6, 4: 63.2251e6 + 203.0922e6}
+NCU_TRAFFIC_BYTES_PER_LAUNCH = {1: 27.3631e6 + 0.8640e6, 4: 63.2251e6 + 203.0922e6}
 # FP64 FMA pipe of one B200: 148 SMs x 64 DFMA lanes / clk x 1.965 GHz (clocks.max.sm) -- DESIGN.md
 FP64_PEAK_DFMA = 148 * 64 * 1.965e9
 
