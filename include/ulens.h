@@ -174,6 +174,20 @@ int  ulens_lightcurve_binary_ext_host(ulens_ctx* ctx, int n_cfg, int n_epochs,
                double* A_out_host, double* dA_out_host, double* err_out_host, uint32_t* status_out_host,
                int* n_ext_out, void* stream);
 
+/* Marginalised-flux negative log-likelihood of n_cfg model light curves against ONE data set, and its gradient
+ * (App. B.2, Eqs. B17-B23). Model (B20): F_i = (A_i - 1) F_S + F_base; the two linear flux
+ * parameters carry Gaussian priors N(mu_fs, var_fs), N(mu_fb, var_fb) and are integrated out (B15); the noise is
+ * independent Gaussian, C = diag(sigma_i^2). Per light curve c:
+ *   NLL_c = 1/2 r^T B^-1 r + 1/2 ln|B|,  r = F - M mu,  B = C + M Lambda M^T,  M_i = (A_ci - 1, 1)        (B17, B21-B23)
+ * evaluated through the 2x2 Woodbury forms B18-B19 (the constant n/2 ln 2 pi is left out, as in B17), and
+ *   grad_c[k] = sum_i dNLL_c/dA_ci * dA_ci/dtheta_k   for the 7 parameters of dA (forward-mode output of a8).
+ * A device [n_cfg][n_epochs]; dA device [n_cfg][n_epochs][7] (needed iff grad_out != NULL); flux, sigma device [n_epochs];
+ * nll_out device [n_cfg]; grad_out device [n_cfg][7] or NULL. One CTA per light curve, sums in a fixed order
+ * (deterministic). EINVAL: NULL where not allowed, n_epochs == 0 with n_cfg > 0, non-finite means, variances <= 0. */
+int  ulens_nll_marginal(ulens_ctx* ctx, int n_cfg, int n_epochs, const double* A, const double* dA,
+               const double* flux, const double* sigma, double mu_fs, double mu_fb, double var_fs, double var_fb,
+               double* nll_out, double* grad_out, void* stream);
+
 /* Point-source magnification (Eq. 2-3): A = sum over the images of 1/|det J|, det J = 1 - |sum_i eps_i/conj(z - a_i)^2|^2,
  * from the validated, polished images of step a2 (one thread per source position). Layout as ulens_mag
  * (lenses host, w_re/w_im device [n_cfg][n_pts], A_out device, status_out device or NULL: image count in

@@ -20,7 +20,7 @@ ST_NIMG_SHIFT = 8
 KERNEL_NAMES = ["k_traj", "k_roots", "k_regions", "k_shoot", "k_finalize"]     # ULENS_K_* order
 
 EXPORTS = ["ulens_create", "ulens_destroy", "ulens_lens_binary", "ulens_lens_triple", "ulens_mag", "ulens_mag_grad",
-           "ulens_mag_host", "ulens_lightcurve_binary", "ulens_lightcurve_binary_host", "ulens_lightcurve_binary_ext", "ulens_lightcurve_binary_ext_host", "ulens_mag_point", "ulens_roots", "ulens_get_stats",
+           "ulens_mag_host", "ulens_lightcurve_binary", "ulens_lightcurve_binary_host", "ulens_lightcurve_binary_ext", "ulens_lightcurve_binary_ext_host", "ulens_nll_marginal", "ulens_mag_point", "ulens_roots", "ulens_get_stats",
            "ulens_reset_stats", "ulens_last_launch_count", "ulens_set_timing", "ulens_get_kernel_ms", "ulens_fp64_peak", "ulens_strerror",
            "ulens_last_cuda_error"]
 
@@ -74,6 +74,7 @@ def lib() -> C.CDLL:
                                                   C.POINTER(C.c_int), vp]
         L.ulens_lightcurve_binary_ext_host.argtypes = [vp, ip, ip, dp, C.c_double, vp, vp, C.c_double, vp, vp, vp, vp,
                                                        C.POINTER(C.c_int), vp]
+        L.ulens_nll_marginal.argtypes = [vp, ip, ip, vp, vp, vp, vp] + [C.c_double] * 4 + [vp, vp, vp]
         L.ulens_mag_point.argtypes = [vp, ip, ip, C.POINTER(ulens_lens), vp, vp, vp, vp, vp]
         L.ulens_roots.argtypes = [vp, C.POINTER(ulens_lens), ip, vp, vp, vp, vp, vp, vp]
         L.ulens_get_stats.argtypes = [vp, C.POINTER(ulens_stats)]
@@ -320,6 +321,20 @@ class Context:
                                                       float(sel_tol), p(A), p(dA), p(err), p(st), C.byref(n_ext),
                                                       self._stream(stream)), self._h)
         return A, dA, err, st, n_ext.value
+
+    def ulens_nll_marginal(self, A, dA, flux, sigma, mu_fs, mu_fb, var_fs, var_fb, stream=None):
+        """Marginalised-flux NLL per light curve (App. B.2) and, with dA, its gradient: (nll [n_cfg], grad [n_cfg, 7] or None)."""
+        torch = self._torch
+        n_cfg, n_ep = A.shape
+        nll = torch.empty(n_cfg, dtype=torch.float64, device=A.device)
+        grad = torch.empty((n_cfg, 7), dtype=torch.float64, device=A.device) if dA is not None else None
+        _check(lib().ulens_nll_marginal(self._h, n_cfg, n_ep, _dev(A, torch.float64, n_cfg * n_ep),
+                                        _dev(dA, torch.float64, n_cfg * n_ep * 7) if dA is not None else None,
+                                        _dev(flux, torch.float64, n_ep), _dev(sigma, torch.float64, n_ep),
+                                        float(mu_fs), float(mu_fb), float(var_fs), float(var_fb),
+                                        _dev(nll, torch.float64, n_cfg), _dev(grad, torch.float64, n_cfg * 7) if grad is not None else None,
+                                        self._stream(stream)), self._h)
+        return nll, grad
 
     def ulens_roots(self, lens, w_re, w_im, stream=None):
         """All N^2+1 roots per source position and the image flags: (roots complex [n, deg], is_image bool)."""

@@ -727,6 +727,71 @@ __global__ void k_chain7(int n_cfg, int n_ep, const double* __restrict__ theta, 
     o[6] = -g[0] * w_im[i] + g[1] * w_re[i];
 }
 
+
+// ------------------------------------------------------------------------------------------------
+// Marginalised-flux negative log-likelihood and its gradient (App. B.2, Eqs. B17-B23).
+// One CTA per light curve. With m_i = A_i - 1, M_i = (m_i, 1), r = F - M mu, C = diag(sigma_i^2), Lambda = diag(l1, l2):
+//   S = Lambda^-1 + M^T C^-1 M (2x2),  v = M^T C^-1 r,
+//   NLL = 1/2 [ sum r_i^2/sigma_i^2 - v^T S^-1 v ] + 1/2 [ sum ln sigma_i^2 + ln l1 + ln l2 + ln det S ]      (B17-B19)
+// and, with alpha = B^-1 r, bm = B^-1 m (B = C + M Lambda M^T, both through B18),
+//   dNLL/dA_i = -(mu_1 + l1 m.alpha) alpha_i + l1 bm_i,     grad_k = sum_i dNLL/dA_i dA_i/dtheta_k.
+// ------------------------------------------------------------------------------------------------
+template <int NV>
+__device__ __forceinline__ void block_sum(double (&v)[NV], double* sh)
+{
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = blockDim.x >> 5;
+#pragma unroll
+    for (int k = 0; k < NV; ++k) v[k] = warp_sum(v[k]);
+    __syncthreads();
+    if (lane == 0) for (int k = 0; k < NV; ++k) sh[w * NV + k] = v[k];
+    __syncthreads();
+    // every thread adds the warp partials in the same order: deterministic, and all threads hold the totals
+#pragma unroll
+    for (int k = 0; k < NV; ++k) { double t = 0.0; for (int j = 0; j < nw; ++j) t += sh[j * NV + k]; v[k] = t; }
+}
+
+__global__ void __launch_bounds__(256)
+k_nll(int n_ep, const double* __restrict__ A, const double* __restrict__ dA, const double* __restrict__ flux,
+      const double* __restrict__ sigma, double mu1, double mu2, double l1, double l2,
+      double* __restrict__ nll_out, double* __restrict__ grad_out)
+{
+    __shared__ double sh[8 * 15];
+    const int c = blockIdx.x;
+    const double* Ac = A + (size_t)c * n_ep;
+    double a[7] = {0, 0, 0, 0, 0, 0, 0};       // S11', S12, S22', v1, v2, sum r^2/s^2, sum ln s^2
+    for (int i = threadIdx.x; i < n_ep; i += blockDim.x) {
+        const double m = Ac[i] - 1.0, s2 = sigma[i] * sigma[i], iw = 1.0 / s2;
+        const double r = flux[i] - m * mu1 - mu2;
+        a[0] += m * m * iw; a[1] += m * iw; a[2] += iw; a[3] += m * r * iw; a[4] += r * iw; a[5] += r * r * iw; a[6] += log(s2);
+    }
+    block_sum<7>(a, sh);
+    const double S11 = 1.0 / l1 + a[0], S12 = a[1], S22 = 1.0 / l2 + a[2];
+    const double det = S11 * S22 - S12 * S12;
+    // S^-1 v and S^-1 u,  u = M^T C^-1 m = (a0, a1)
+    const double x1 = (S22 * a[3] - S12 * a[4]) / det, x2 = (S11 * a[4] - S12 * a[3]) / det;
+    const double y1 = (S22 * a[0] - S12 * a[1]) / det, y2 = (S11 * a[1] - S12 * a[0]) / det;
+    if (threadIdx.x == 0)
+        nll_out[c] = 0.5 * (a[5] - (a[3] * x1 + a[4] * x2)) + 0.5 * (a[6] + log(l1) + log(l2) + log(det));
+    if (!grad_out) return;
+    const double* dAc = dA + (size_t)c * n_ep * 7;
+    double g[15];                                // m.alpha, P_k = sum alpha_i dA_ik, Q_k = sum bm_i dA_ik
+#pragma unroll
+    for (int k = 0; k < 15; ++k) g[k] = 0.0;
+    for (int i = threadIdx.x; i < n_ep; i += blockDim.x) {
+        const double m = Ac[i] - 1.0, iw = 1.0 / (sigma[i] * sigma[i]);
+        const double r = flux[i] - m * mu1 - mu2;
+        const double al = (r - (m * x1 + x2)) * iw, bm = (m - (m * y1 + y2)) * iw;
+        g[0] += m * al;
+#pragma unroll
+        for (int k = 0; k < 7; ++k) { const double d = dAc[(size_t)i * 7 + k]; g[1 + k] += al * d; g[8 + k] += bm * d; }
+    }
+    block_sum<15>(g, sh);
+    if (threadIdx.x < 7) {
+        const int k = threadIdx.x;
+        grad_out[(size_t)c * 7 + k] = -(mu1 + l1 * g[0]) * g[1 + k] + l1 * g[8 + k];
+    }
+}
+
 // FP64 FMA peak: 8 independent chains per thread
 __global__ void k_dfma_peak(int iters, double* out)
 {
@@ -1298,6 +1363,21 @@ extern "C" int ulens_lightcurve_binary_ext_host(ulens_ctx* ctx, int n_cfg, int n
     if (err_out_host) CK(cudaMemcpyAsync(err_out_host, d_err, sizeof(double) * n, cudaMemcpyDeviceToHost, st));
     if (status_out_host) CK(cudaMemcpyAsync(status_out_host, d_st, sizeof(unsigned) * n, cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
+    return ULENS_OK;
+}
+
+extern "C" int ulens_nll_marginal(ulens_ctx* ctx, int n_cfg, int n_epochs, const double* A, const double* dA,
+                                  const double* flux, const double* sigma, double mu_fs, double mu_fb, double var_fs,
+                                  double var_fb, double* nll_out, double* grad_out, void* stream)
+{
+    if (!ctx || n_cfg < 0 || n_epochs < 0) return ULENS_EINVAL;
+    if (n_cfg == 0) return ULENS_OK;
+    if (n_epochs == 0 || !A || !flux || !sigma || !nll_out || (grad_out && !dA)) return ULENS_EINVAL;
+    if (!isfinite(mu_fs) || !isfinite(mu_fb) || !finite_pos(var_fs) || !finite_pos(var_fb)) return ULENS_EINVAL;
+    CK(cudaSetDevice(ctx->device));
+    k_nll<<<n_cfg, 256, 0, (cudaStream_t)stream>>>(n_epochs, A, dA, flux, sigma, mu_fs, mu_fb, var_fs, var_fb, nll_out, grad_out);
+    ctx->last_launches = 1;
+    CK(cudaGetLastError());
     return ULENS_OK;
 }
 
