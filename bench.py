@@ -1,25 +1,29 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the ICRS hot path on B200 (contract: see the task statement / DESIGN.md "Measurement").
 
-One "step" = one pass of the whole hot path (k_roots -> k_regions -> k_shoot -> k_finalize, SURVEY 8.a rows
-a2..a7; a1 too for light-curve workloads) over one batch of synthetic input = every source point of the
-workload. Default workload: BASELINE.json configs[1] ("C1": binary lens, u1 = 0.5, rho = 1e-3, 64 lens
-configurations x 2,048 source points, half of them within 3 rho of a caustic; seeded).
+One "step" = one pass of the whole hot path (k_traj -> k_roots -> k_regions -> k_shoot[_dual] -> k_finalize, SURVEY 8.a
+rows a1..a8) over one batch of synthetic input = every source point of the workload. Default workload: the largest
+single-GPU configuration of BASELINE.json, configs[4] ("C4": 1,024 parameter vectors x 2,000 epochs, binary lens,
+rho = 5e-3, u1 = 0.5; trajectory parameters in, A and the 7 forward-mode derivatives out; every epoch takes the
+finite-source path -- the point-source / finite-source switch of SURVEY 8.f-2 rides along under "c4_switch").
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl ours|reference]
 
 prints ONE JSON line on rank 0:
-  value      finite-source magnifications / s, inputs resident in HBM, CUDA events, max over ranks
-  e2e        the same through ulens_mag_host (pinned HOST buffers, H2D + D2H inside the timed region)
-  roofline   k_shoot (the dominant kernel) against the FP64 FMA pipe
-  cpu_baseline  the CPU oracle, as it stands, on a bounded seeded sample of the same workload
-N > 1 runs N independent replicas (the path has no exchange step: DESIGN.md "Multi-GPU: replicas only").
+  value        finite-source magnifications / s, inputs resident in HBM, CUDA events, max over ranks
+  e2e          the same through the *_host entry (pinned HOST buffers, H2D + D2H inside the timed region)
+  roofline     the ray-shooting kernel (k_shoot_dual for C4, k_shoot otherwise) against the FP64 FMA pipe
+  cpu_baseline the CPU oracle, as it stands, on a bounded seeded sample of the same workload
+  all_configs  value / roofline fractions of the other BASELINE configs (short runs, same code path)
+N > 1 runs N independent replicas (the path has no exchange step: DESIGN.md "Multi-GPU: replicas only"); a plain
+`python bench.py --gpus N` re-launches itself under torch.distributed.run with N ranks.
 """
 from __future__ import annotations
 
 import argparse
 import json
 import os
+import socket
 import subprocess
 import sys
 import threading
@@ -45,10 +49,6 @@ FP64_INSTR_PER_RAY_DUAL_EXTRA = 74
 # Ehrlich-Aberth 3 iterations x DEG roots x (8 DEG Horner + 12 (DEG-1) repulsion + 24), Eq.-1 polish of the
 # N+1..DEG images 2.5 iterations x (17 N + 25), boxes ~100.
 FP64_INSTR_PER_LIMB_SOLVE = {1: 600, 2: 2400, 3: 8300}
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the roofline kernel, from the `ncu --set full`
-# captures summarised in profiles/r01g_ncu_k_shoot_c1.md (C1) and profiles/r01c_ncu_k_shoot_dual_c4.md (C4);
-# configs without a capture report null.
-NCU_TRAFFIC_BYTES_PER_LAUNCH = {1: 27.3631e6 + 0.8640e6, 4: 63.2251e6 + 203.0922e6}
 # FP64 FMA pipe of one B200: 148 SMs x 64 DFMA lanes / clk x 1.965 GHz (clocks.max.sm) -- DESIGN.md
 FP64_PEAK_DFMA = 148 * 64 * 1.965e9
 
@@ -184,7 +184,8 @@ def main_reference(args, rank, world):
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": min(args.warmup, 1), "ms_per_step": 1e3 * tot_t / max(args.steps, 1),
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": workload_name(wl), "note": "CPU oracle (oracle/), bounded sample per step"},
+            "config": {"workload": workload_name(wl), "note": "CPU oracle (oracle/), bounded sample per step; values only "
+                       "(the oracle's derivative reference is finite differences: 29 evaluations per point)"},
             "rays_per_s": tot_ev / tot_t,
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
                              "rays_per_s": tot_ev / tot_t},
@@ -194,6 +195,159 @@ def main_reference(args, rank, world):
 
 
 # ----------------------------------------------------------------------------------------------- our arm
+
+class Env:
+    """What every measurement of this process shares."""
+    def __init__(self, torch, dist, binding, inputs, replicas, ctx, dev, local_rank, world):
+        self.torch, self.dist, self.binding, self.inputs, self.replicas = torch, dist, binding, inputs, replicas
+        self.ctx, self.dev, self.local_rank, self.world = ctx, dev, local_rank, world
+        self.flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)    # > 126 MB L2
+
+    def barrier(self):
+        if self.world > 1:
+            self.dist.barrier()
+        self.torch.cuda.synchronize()
+
+
+def measure_config(env: Env, cfg: int, steps: int, warmup: int, switch: bool = False, with_e2e: bool = True,
+                   with_clocks: bool = False) -> dict:
+    """W warm-up steps, K timed steps (CUDA events on the launch stream, L2 flushed before each), per-kernel
+    device times from the library's own event pairs, optionally the end-to-end leg; max over ranks."""
+    torch, ctx, dev, binding, inputs, replicas = env.torch, env.ctx, env.dev, env.binding, env.inputs, env.replicas
+    wl = inputs.get(cfg)                                             # every rank: the same seeded workload (replica)
+    lenses = gpu_lenses(binding, wl)
+    n = wl.n_cfg * wl.n_pts
+    dual = cfg == 4                                                  # C4: trajectory parameters in, A and dA/d(7) out
+    A = torch.empty((wl.n_cfg, wl.n_pts), dtype=torch.float64, device=dev)
+    err = torch.empty_like(A)
+    st = torch.empty((wl.n_cfg, wl.n_pts), dtype=torch.int32, device=dev)
+    if dual:
+        t_dev = torch.tensor(wl.t.copy(), device=dev)
+        dA = torch.empty((wl.n_cfg, wl.n_pts, 7), dtype=torch.float64, device=dev)
+    else:
+        w_re = torch.tensor(np.ascontiguousarray(wl.w.real), device=dev)
+        w_im = torch.tensor(np.ascontiguousarray(wl.w.imag), device=dev)
+    box = {"n_ext": n, "A": A, "st": st}
+
+    def step():
+        if dual and switch:
+            a_, d_, e_, s_, box["n_ext"] = ctx.ulens_lightcurve_binary_ext(wl.theta, float(wl.u1[0]), t_dev, want_dA=True)
+            box["A"], box["st"] = a_, s_
+        elif dual:
+            ctx.ulens_lightcurve_binary(wl.theta, float(wl.u1[0]), t_dev, out=(A, dA, err, st))
+        else:
+            ctx.ulens_mag(lenses, wl.rho, wl.u1, w_re, w_im, A, err, st)
+
+    for _ in range(warmup):
+        step()
+    env.barrier()
+    launches_per_step = ctx.ulens_last_launch_count()
+
+    # ---- timed region 1: inputs resident in HBM
+    ctx.ulens_reset_stats()
+    ctx.ulens_set_timing(True)
+    clocks = ClockSampler(env.local_rank) if with_clocks else None
+    if clocks:
+        clocks.start()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    env.barrier()
+    for a, b in ev:
+        env.flush.fill_(1)                                           # L2 flush between timed iterations (untimed)
+        a.record()
+        step()
+        b.record()
+    env.barrier()
+    clk = clocks.stop() if clocks else None
+    ms = sum(a.elapsed_time(b) for a, b in ev)
+    kms = ctx.ulens_get_kernel_ms()
+    ctx.ulens_set_timing(False)
+    stats = ctx.ulens_get_stats()
+    status = box["st"].cpu().numpy().astype(np.uint32)
+    A_host = box["A"].cpu().numpy()
+
+    # ---- timed region 2: end to end through the C ABI with pinned HOST buffers
+    e2e = None
+    if with_e2e:
+        h_A = torch.empty((wl.n_cfg, wl.n_pts), dtype=torch.float64).pin_memory()
+        h_err = torch.empty((wl.n_cfg, wl.n_pts), dtype=torch.float64).pin_memory()
+        h_st = torch.empty((wl.n_cfg, wl.n_pts), dtype=torch.int32).pin_memory()
+        e2e_steps = max(1, min(steps, 3))
+        if dual:
+            h_t = torch.tensor(wl.t.copy()).pin_memory()
+            h_dA = torch.empty((wl.n_cfg, wl.n_pts, 7), dtype=torch.float64).pin_memory()
+
+            def e2e_step():
+                f = ctx.ulens_lightcurve_binary_ext_host if switch else ctx.ulens_lightcurve_binary_host
+                f(wl.theta, float(wl.u1[0]), h_t.numpy(), h_A.numpy(), h_dA.numpy(), h_err.numpy(), h_st.numpy())
+            h2d, d2h = 8 * wl.n_pts + 56 * wl.n_cfg, (8 + 56 + 8 + 4) * n
+            e2e_api = ("ulens_lightcurve_binary_ext_host" if switch else "ulens_lightcurve_binary_host") + " (pinned host buffers)"
+        else:
+            h_re = torch.tensor(np.ascontiguousarray(wl.w.real)).pin_memory()
+            h_im = torch.tensor(np.ascontiguousarray(wl.w.imag)).pin_memory()
+
+            def e2e_step():
+                ctx.ulens_mag_host(lenses, wl.rho, wl.u1, h_re.numpy(), h_im.numpy(), h_A.numpy(), h_err.numpy(), h_st.numpy())
+            h2d, d2h = 16 * n, 20 * n
+            e2e_api = "ulens_mag_host (pinned host buffers)"
+        e2e_step()
+        env.barrier()
+        t0 = time.perf_counter()
+        for _ in range(e2e_steps):
+            e2e_step()
+        env.barrier()
+        e2e_s = time.perf_counter() - t0
+        assert np.array_equal(h_A.numpy(), A_host, equal_nan=True), "host entry and device entry disagree"
+        (e2e_s,) = replicas.max_over_ranks([e2e_s], dev)
+        e2e = {"value": replicas.aggregate_throughput(n, env.world, 1e3 * e2e_s / e2e_steps), "unit": UNIT,
+               "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": e2e_steps, "api": e2e_api}
+
+    # ---- max over ranks
+    (ms,) = replicas.max_over_ranks([ms], dev)
+    ms_per_step = ms / steps
+    value = replicas.aggregate_throughput(n, env.world, ms_per_step)
+
+    n_lens = 2 if wl.kind == "binary" else 3
+    ld = bool(np.any(wl.u1 > 0))
+    shoot_ms, shoot_n = kms["k_shoot"]
+    rays_per_step = stats["n_rays"] / steps
+    rays_per_launch = stats["n_rays"] / max(shoot_n, 1)
+    ipr = FP64_INSTR_PER_RAY[(n_lens, ld)] + (FP64_INSTR_PER_RAY_DUAL_EXTRA if dual else 0)
+    shoot_avg_s = shoot_ms * 1e-3 / max(shoot_n, 1)
+    achieved = 2.0 * ipr * rays_per_launch / shoot_avg_s / 1e12
+    peak = 2.0 * FP64_PEAK_DFMA / 1e12
+    roofline = {"bound": "alu", "kernel": "k_shoot_dual" if dual else "k_shoot", "achieved": achieved, "peak": peak,
+                "variant": "k_shoot_dual (value + 5 tangents per ray)" if dual else "k_shoot",
+                "unit": "TFLOP/s", "frac": achieved / peak, "traffic": None,
+                "traffic_note": "the path is ALU-bound; DRAM bytes of one launch are in the ncu captures under profiles/",
+                "peak_source": "derived: 148 SM x 64 DFMA/clk x 1.965 GHz x 2 flop (DESIGN.md); "
+                               "MEASURED_PEAKS.json has no FP64 entry",
+                "fp64_instr_per_ray": ipr, "rays_per_launch": rays_per_launch,
+                "kernel_ms_avg": 1e3 * shoot_avg_s, "share_of_step": shoot_ms / ms}
+    reg_ms, reg_n = kms["k_regions"]
+    solves_per_launch = stats["n_limb_solves"] / max(reg_n, 1)
+    reg_ach = 2.0 * FP64_INSTR_PER_LIMB_SOLVE[n_lens] * solves_per_launch / (reg_ms * 1e-3 / max(reg_n, 1)) / 1e12
+    roofline_regions = {"bound": "alu", "kernel": "k_regions", "achieved": reg_ach, "peak": peak,
+                        "unit": "TFLOP/s", "frac": reg_ach / peak, "traffic": None,
+                        "fp64_instr_per_limb_solve": FP64_INSTR_PER_LIMB_SOLVE[n_lens],
+                        "limb_solves_per_point": stats["n_limb_solves"] / steps / n,
+                        "kernel_ms_avg": reg_ms / max(reg_n, 1), "share_of_step": reg_ms / ms}
+    out = {"wl": wl, "n": n, "value": value, "ms_per_step": ms_per_step, "e2e": e2e, "roofline": roofline,
+           "roofline_regions": roofline_regions, "rays_per_s": env.world * rays_per_step / (ms_per_step * 1e-3),
+           "rays_per_point": rays_per_step / n, "kernel_ms_per_step": {k: v[0] / steps for k, v in kms.items()},
+           "flagged_points": int(((status & 0xff) != 0).sum()), "nan_points": int(np.isnan(A_host).sum()),
+           "gpu_launches": launches_per_step * steps, "clocks": clk, "n_ext": int(box["n_ext"]), "steps": steps, "warmup": warmup}
+    return out
+
+
+def summary(r: dict) -> dict:
+    """One config's short entry under all_configs."""
+    return {"workload": workload_name(r["wl"]), "value": r["value"], "unit": UNIT, "ms_per_step": r["ms_per_step"],
+            "steps": r["steps"], "warmup": r["warmup"], "rays_per_s": r["rays_per_s"], "rays_per_point": r["rays_per_point"],
+            "roofline_kernel": r["roofline"]["kernel"], "roofline_frac": r["roofline"]["frac"],
+            "roofline_share_of_step": r["roofline"]["share_of_step"],
+            "regions_frac": r["roofline_regions"]["frac"], "regions_share_of_step": r["roofline_regions"]["share_of_step"],
+            "flagged_points": r["flagged_points"], "nan_points": r["nan_points"]}
+
 
 def main_ours(args, rank, local_rank, world):
     import torch
@@ -206,158 +360,53 @@ def main_ours(args, rank, local_rank, world):
     dev = torch.device("cuda", local_rank)
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
-
-    wl = inputs.get(args.config)                                     # every rank: the same seeded workload (replica)
-    lenses = gpu_lenses(binding, wl)
-    n = wl.n_cfg * wl.n_pts
     ctx = binding.Context(local_rank)
-    dual = args.config == 4                                          # C4: trajectory parameters in, A and dA/d(7) out
-    w_re = torch.tensor(np.ascontiguousarray(wl.w.real), device=dev)
-    w_im = torch.tensor(np.ascontiguousarray(wl.w.imag), device=dev)
-    A = torch.empty((wl.n_cfg, wl.n_pts), dtype=torch.float64, device=dev)
-    err = torch.empty_like(A)
-    st = torch.empty((wl.n_cfg, wl.n_pts), dtype=torch.int32, device=dev)
-    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)    # > 126 MB L2
+    env = Env(torch, dist, binding, inputs, replicas, ctx, dev, local_rank, world)
 
-    if dual:
-        t_dev = torch.tensor(wl.t.copy(), device=dev)
-        dA = torch.empty((wl.n_cfg, wl.n_pts, 7), dtype=torch.float64, device=dev)
-
-    n_ext = n
-
-    def step():
-        if dual:
-            if args.switch:
-                nonlocal n_ext, A, dA, err, st
-                A, dA, err, st, n_ext = ctx.ulens_lightcurve_binary_ext(wl.theta, float(wl.u1[0]), t_dev, want_dA=True)
-            else:
-                ctx.ulens_lightcurve_binary(wl.theta, float(wl.u1[0]), t_dev, out=(A, dA, err, st))
-        else:
-            ctx.ulens_mag(lenses, wl.rho, wl.u1, w_re, w_im, A, err, st)
-
-    def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    for _ in range(args.warmup):
-        step()
-    barrier()
-    launches_per_step = ctx.ulens_last_launch_count()
-
-    # ---- timed region 1: inputs resident in HBM
-    ctx.ulens_reset_stats()
-    ctx.ulens_set_timing(True)
-    clocks = ClockSampler(local_rank)
-    clocks.start()
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    barrier()
-    for a, b in ev:
-        flush.fill_(1)                                               # L2 flush between timed iterations (untimed)
-        a.record()
-        step()
-        b.record()
-    barrier()
-    clk = clocks.stop()
-    ms = sum(a.elapsed_time(b) for a, b in ev)
-    kms = ctx.ulens_get_kernel_ms()
-    ctx.ulens_set_timing(False)
-    stats = ctx.ulens_get_stats()
-    status = st.cpu().numpy().astype(np.uint32)
-    A_host = A.cpu().numpy()
-
-    # ---- timed region 2: end to end through the C ABI with pinned HOST buffers
-    h_re = torch.tensor(np.ascontiguousarray(wl.w.real)).pin_memory()
-    h_im = torch.tensor(np.ascontiguousarray(wl.w.imag)).pin_memory()
-    h_A = torch.empty((wl.n_cfg, wl.n_pts), dtype=torch.float64).pin_memory()
-    h_err = torch.empty((wl.n_cfg, wl.n_pts), dtype=torch.float64).pin_memory()
-    h_st = torch.empty((wl.n_cfg, wl.n_pts), dtype=torch.int32).pin_memory()
-    e2e_steps = max(1, min(args.steps, 3))
-    if dual:
-        h_t = torch.tensor(wl.t.copy()).pin_memory()
-        h_dA = torch.empty((wl.n_cfg, wl.n_pts, 7), dtype=torch.float64).pin_memory()
-
-        def e2e_step():
-            if args.switch:
-                ctx.ulens_lightcurve_binary_ext_host(wl.theta, float(wl.u1[0]), h_t.numpy(), h_A.numpy(), h_dA.numpy(),
-                                                     h_err.numpy(), h_st.numpy())
-            else:
-                ctx.ulens_lightcurve_binary_host(wl.theta, float(wl.u1[0]), h_t.numpy(), h_A.numpy(), h_dA.numpy(),
-                                                 h_err.numpy(), h_st.numpy())
-        h2d, d2h = 8 * wl.n_pts + 56 * wl.n_cfg, (8 + 56 + 8 + 4) * n
-        e2e_api = ("ulens_lightcurve_binary_ext_host" if args.switch else "ulens_lightcurve_binary_host") + " (pinned host buffers)"
-    else:
-        def e2e_step():
-            ctx.ulens_mag_host(lenses, wl.rho, wl.u1, h_re.numpy(), h_im.numpy(), h_A.numpy(), h_err.numpy(), h_st.numpy())
-        h2d, d2h = 16 * n, 20 * n
-        e2e_api = "ulens_mag_host (pinned host buffers)"
-    e2e_step()
-    barrier()
-    t0 = time.perf_counter()
-    for _ in range(e2e_steps):
-        e2e_step()
-    barrier()
-    e2e_s = time.perf_counter() - t0
-    assert np.array_equal(h_A.numpy(), A_host, equal_nan=True), "host entry and device entry disagree"
-
-    # ---- max over ranks
-    ms, e2e_s = replicas.max_over_ranks([ms, e2e_s], dev)
-    ms_per_step = ms / args.steps
-    value = replicas.aggregate_throughput(n, world, ms_per_step)
-    e2e_value = replicas.aggregate_throughput(n, world, 1e3 * e2e_s / e2e_steps)
+    r = measure_config(env, args.config, args.steps, args.warmup, switch=args.switch, with_e2e=True, with_clocks=True)
+    others = {}
+    if args.all_configs and world == 1:
+        # the other BASELINE configs through the same code path, short runs (W = 3 warm-up, 2 timed steps)
+        for c in range(5):
+            if c != args.config:
+                others["C%d" % c] = summary(measure_config(env, c, 2, 3, with_e2e=False))
+        if args.config == 4 and not args.switch:
+            rs = measure_config(env, 4, 2, 3, switch=True, with_e2e=False)
+            others["C4_switch"] = dict(summary(rs), n_ext=rs["n_ext"], n_epochs_total=rs["n"],
+                                       api="ulens_lightcurve_binary_ext, library selection (sel_tol default 2e-5): the other "
+                                           "epochs take the point-source value (P:153, SURVEY 8.f-2)")
 
     if rank == 0:
-        n_lens = 2 if wl.kind == "binary" else 3
-        ld = bool(np.any(wl.u1 > 0))
-        shoot_ms, shoot_n = kms["k_shoot"]
-        rays_per_step = stats["n_rays"] / args.steps
-        rays_per_launch = stats["n_rays"] / max(shoot_n, 1)
-        ipr = FP64_INSTR_PER_RAY[(n_lens, ld)] + (FP64_INSTR_PER_RAY_DUAL_EXTRA if dual else 0)
-        shoot_avg_s = shoot_ms * 1e-3 / max(shoot_n, 1)
-        achieved = 2.0 * ipr * rays_per_launch / shoot_avg_s / 1e12
+        wl = r["wl"]
         peak_measured = ctx.ulens_fp64_peak(200.0)
-        roofline = {"bound": "alu", "kernel": "k_shoot", "achieved": achieved, "peak": 2.0 * FP64_PEAK_DFMA / 1e12,
-                    "variant": "k_shoot_dual (value + 5 tangents per ray)" if dual else "k_shoot",
-                    "unit": "TFLOP/s", "frac": achieved / (2.0 * FP64_PEAK_DFMA / 1e12),
-                    "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH.get(args.config),
-                    "traffic_note": "DRAM bytes of one launch (ncu capture in profiles/); the path is ALU-bound",
-                    "peak_source": "derived: 148 SM x 64 DFMA/clk x 1.965 GHz x 2 flop (DESIGN.md); "
-                                   "MEASURED_PEAKS.json has no FP64 entry",
-                    "peak_measured_dfma_microbench": 2.0 * peak_measured / 1e12,
-                    "frac_of_measured": achieved / (2.0 * peak_measured / 1e12),
-                    "fp64_instr_per_ray": ipr, "rays_per_launch": rays_per_launch,
-                    "kernel_ms_avg": 1e3 * shoot_avg_s, "share_of_step": shoot_ms / ms}
-        reg_ms, reg_n = kms["k_regions"]
-        solves_per_launch = stats["n_limb_solves"] / max(reg_n, 1)
-        reg_ach = 2.0 * FP64_INSTR_PER_LIMB_SOLVE[n_lens] * solves_per_launch / (reg_ms * 1e-3 / max(reg_n, 1)) / 1e12
-        roofline_regions = {"bound": "alu", "kernel": "k_regions", "achieved": reg_ach, "peak": 2.0 * FP64_PEAK_DFMA / 1e12,
-                            "unit": "TFLOP/s", "frac": reg_ach / (2.0 * FP64_PEAK_DFMA / 1e12), "traffic": None,
-                            "fp64_instr_per_limb_solve": FP64_INSTR_PER_LIMB_SOLVE[n_lens],
-                            "limb_solves_per_point": stats["n_limb_solves"] / args.steps / n,
-                            "kernel_ms_avg": reg_ms / max(reg_n, 1), "share_of_step": reg_ms / ms}
-        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-                "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+        for k in ("roofline", "roofline_regions"):
+            r[k]["peak_measured_dfma_microbench"] = 2.0 * peak_measured / 1e12
+            r[k]["frac_of_measured"] = r[k]["achieved"] / (2.0 * peak_measured / 1e12)
+        dual = args.config == 4
+        line = {"metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": r["ms_per_step"], "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f64", "data": "synthetic",
                 "config": {"workload": workload_name(wl), "rho": [float(wl.rho.min()), float(wl.rho.max())],
-                           "u1": [float(wl.u1.min()), float(wl.u1.max())], "l2": "flushed between timed steps (256 MiB fill)",
+                           "u1": [float(wl.u1.min()), float(wl.u1.max())],
+                           "outputs": "A and dA/d(t0,u0,tE,s,q,rho,alpha) per epoch (forward-mode variant, step a8)" if dual else "A per point",
+                           "switch": bool(args.switch),
+                           "l2": "flushed between timed steps (256 MiB fill)",
                            "parallelism": "replicas" if world > 1 else "1 GPU"},
-                "rays_per_s": world * rays_per_step / (ms_per_step * 1e-3),
-                "rays_per_point": rays_per_step / n,
-                "kernel_ms_per_step": {k: v[0] / args.steps for k, v in kms.items()},
-                "flagged_points": int(((status & 0xff) != 0).sum()), "nan_points": int(np.isnan(A_host).sum()),
-                "roofline": roofline, "roofline_regions": roofline_regions,
-                "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                        "steps": e2e_steps, "api": e2e_api},
-                "gpu_launches": launches_per_step * args.steps,
-                "clocks": clk}
+                "rays_per_s": r["rays_per_s"], "rays_per_point": r["rays_per_point"],
+                "kernel_ms_per_step": r["kernel_ms_per_step"],
+                "flagged_points": r["flagged_points"], "nan_points": r["nan_points"],
+                "roofline": r["roofline"], "roofline_regions": r["roofline_regions"],
+                "e2e": r["e2e"], "gpu_launches": r["gpu_launches"], "clocks": r["clocks"]}
         if dual and args.switch:
-            line["config"]["switch"] = {"api": "ulens_lightcurve_binary_ext", "selection": "library (sel_tol default 2e-5)",
-                                        "n_ext": int(n_ext), "n_epochs_total": int(n),
-                                        "note": "SURVEY 8.f-2 driver: the other epochs take the point-source value (P:153)"}
+            line["config"]["switch_detail"] = {"api": "ulens_lightcurve_binary_ext", "selection": "library (sel_tol default 2e-5)",
+                                               "n_ext": r["n_ext"], "n_epochs_total": r["n"]}
+        if others:
+            line["all_configs"] = others
         if not args.no_cpu_baseline and world == 1:
             npts, dt, nev, cores = run_oracle_sample(wl, inputs)
             line["cpu_baseline"] = {"value": npts / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
-                                    "sample": "%d seeded points (%d configs x %d, half near-caustic, seed %d), oracle n_rho=%d ss=%d, %.1f s"
+                                    "sample": "%d seeded points (%d configs x %d, half near-caustic, seed %d), oracle n_rho=%d ss=%d, %.1f s; "
+                                              "values only (no derivatives)"
                                               % (npts, min(CPU_SAMPLE_CFGS, wl.n_cfg), sample_per_cfg(wl), CPU_SAMPLE_SEED, ORACLE_N_RHO, ORACLE_SS, dt),
                                     "rays_per_s": nev / dt}
         print(json.dumps(line), flush=True)
@@ -367,25 +416,72 @@ def main_ours(args, rank, local_rank, world):
         dist.destroy_process_group()
 
 
+def main_stub(args, rank, world):
+    """TEST HOOK (tests/test_replicas_gloo.py): the N > 1 plumbing of main_ours -- rendezvous from the launcher's
+    environment, barrier, per-rank timing, max over ranks, whole-job aggregate, one line on rank 0 -- on CPU ranks
+    over gloo, with the CUDA step replaced by a sleep. The line is marked "stub" and carries no metric."""
+    import torch.distributed as dist
+    from paper_2510_02639_b200 import replicas
+    if world > 1:
+        dist.init_process_group("gloo")
+    units = 1000
+    if world > 1:
+        dist.barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        time.sleep(0.02 * (rank + 1))                           # rank r is (r + 1) x slower: the max must win
+    ms_own = 1e3 * (time.perf_counter() - t0)
+    (ms,) = replicas.max_over_ranks([ms_own])
+    value = replicas.aggregate_throughput(units, world, ms / args.steps)
+    if rank == 0:
+        print(json.dumps({"stub": True, "metric": "stub", "n_gpus": world, "steps": args.steps, "ms_per_step": ms / args.steps,
+                          "ms_per_step_rank0": ms_own / args.steps, "value": value, "scaling": "weak"}), flush=True)
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def relaunch_under_torchrun(n: int) -> int:
+    """`python bench.py --gpus N` outside a launcher: start N ranks on this node and return their exit code."""
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(n),
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=1, help="BASELINE.json config index 0..4 (default 1; 4 = light curves with forward-mode derivatives)")
+    ap.add_argument("--config", type=int, default=4, help="BASELINE.json config index 0..4 (default 4: the largest single-GPU "
+                    "configuration, light curves with forward-mode derivatives)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-all-configs", dest="all_configs", action="store_false",
+                    help="skip the short runs of the other BASELINE configs (the all_configs key)")
     ap.add_argument("--switch", action="store_true",
                     help="config 4 only: ulens_lightcurve_binary_ext (point-source value for the far epochs, P:153; "
                          "library selection at the default tolerance) instead of the finite-source path on every epoch")
+    ap.add_argument("--stub", action="store_true", help=argparse.SUPPRESS)
     args = ap.parse_args()
     if args.switch and args.config != 4:
         ap.error("--switch needs --config 4")
+    if args.gpus < 1:
+        ap.error("--gpus must be >= 1")
+    if "WORLD_SIZE" not in os.environ and args.gpus > 1 and args.impl != "reference":
+        raise SystemExit(relaunch_under_torchrun(args.gpus))    # (the oracle arm runs on rank 0's host cores only)
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.impl != "reference" and world != args.gpus:
+        raise SystemExit("bench.py: --gpus %d but the launcher started WORLD_SIZE=%d ranks" % (args.gpus, world))
     if args.impl == "reference":
         main_reference(args, rank, world)
+    elif args.stub:
+        main_stub(args, rank, world)
     else:
         main_ours(args, rank, local_rank, world)
 

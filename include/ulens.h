@@ -20,8 +20,11 @@
  *     never frees or keeps them beyond the work it enqueues. "host" pointers are ordinary memory, read
  *     (or written, for *_host entry points) before the call returns.
  *   - all device work is enqueued on the caller's stream (a cudaStream_t passed as void*, NULL = the
- *     legacy default stream) and the call does NOT synchronise, except the *_host entry points, the
- *     stats/peak calls and ulens_destroy, which say so.
+ *     legacy default stream) and the call does NOT synchronise, except the *_host entry points,
+ *     ulens_lightcurve_binary_ext (once, to read N_ext), the stats/peak calls and ulens_destroy, which say so.
+ *     Host tables (lenses, rho, u1, theta) are copied into context-owned pinned staging during the call and
+ *     uploaded stream-ordered; an array identical to the previous call's is not rebuilt or uploaded again.
+ *     (A call that has to GROW a workspace buffer frees the old one, which waits for the device: first calls only.)
  *   - one context = one device = one stream at a time (the context owns the workspace the kernels share).
  *   - lengths are in Einstein radii of the TOTAL lens mass; complex numbers are passed as
  *     separate re / im arrays (SoA); doubles are IEEE binary64.
@@ -50,12 +53,15 @@ extern "C" {
 #define ULENS_ST_PATCH_CAP   0x0004u  /* more sectors than the cap: merged into one */
 #define ULENS_ST_RES_CAP     0x0008u  /* a sector wanted more rings / rays than the cap allows */
 #define ULENS_ST_CLIPPED     0x0010u  /* an inside ray sat on a sector border (margin too small) */
-#define ULENS_ST_UNIT_OVF    0x0020u  /* work-queue overflow: point not integrated, A = NaN */
+#define ULENS_ST_UNIT_OVF    0x0020u  /* work-queue refusal: point not integrated, A = NaN (cannot happen with the built-in
+                                         per-point unit cap: the queue holds chunk_pts x that cap) */
 #define ULENS_ST_ERR_HIGH    0x0040u  /* half-resolution self-check differs by more than rel_tol */
 #define ULENS_ST_NO_IMAGE    0x0080u  /* no image-limb point found (A = NaN) */
 #define ULENS_ST_NIMG_SHIFT  8        /* bits 8..11: number of images of the source centre */
-#define ULENS_ST_RETRIED     0x2000u  /* the first result was doubtful (EA_NOCONV, PATCH_CAP, CLIPPED, ERR_HIGH or NO_IMAGE): this is the
-                                         result and status of the retry pass with twice the limb samples */
+#define ULENS_ST_RETRIED     0x2000u  /* the first result was doubtful (EA_NOCONV, PATCH_CAP, CLIPPED, ERR_HIGH or NO_IMAGE) and the retry pass
+                                         with twice the limb samples gave a finite result that is no worse (fewer of those bits, or as many
+                                         and a smaller self-error): this is the retry's result and status. A doubtful point without this
+                                         bit kept its first result (retry not better, or beyond the two chunks the retry pass covers) */
 #define ULENS_ST_POINT_SRC   0x1000u  /* ulens_lightcurve_binary_ext: the epoch took the point-source value (Eq. 2-3) */
 
 typedef struct ulens_ctx ulens_ctx;
@@ -128,6 +134,12 @@ int  ulens_mag_host(ulens_ctx* ctx, int n_cfg, int n_pts,
                const ulens_lens* lenses_host, const double* rho_host, const double* u1_host,
                const double* w_re_host, const double* w_im_host,
                double* A_out_host, double* err_out_host, uint32_t* status_out_host, void* stream);
+
+/* Step a1 alone: trajectory parameters -> source centres (reading G3). theta_host [n_cfg][7] as below (only t0, u0,
+ * tE, alpha are read), t device [n_epochs]; w_re_out, w_im_out device [n_cfg][n_epochs]:
+ *   tau = (t - t0)/tE,  w_c = (tau cos a - u0 sin a) + i (tau sin a + u0 cos a).   EINVAL unless tE > 0 and all finite. */
+int  ulens_trajectory(ulens_ctx* ctx, int n_cfg, int n_epochs, const double* theta_host, const double* t,
+               double* w_re_out, double* w_im_out, void* stream);
 
 /* (ii) Trajectory parameters in -> light curve out (binary lens, reading G3):
  *   theta_host [n_cfg][7] = (t0, u0, tE, s, q, rho, alpha), host; u1 shared; t device [n_epochs].

@@ -20,7 +20,7 @@ ST_NIMG_SHIFT = 8
 KERNEL_NAMES = ["k_traj", "k_roots", "k_regions", "k_shoot", "k_finalize"]     # ULENS_K_* order
 
 EXPORTS = ["ulens_create", "ulens_destroy", "ulens_lens_binary", "ulens_lens_triple", "ulens_mag", "ulens_mag_grad",
-           "ulens_mag_host", "ulens_lightcurve_binary", "ulens_lightcurve_binary_host", "ulens_lightcurve_binary_ext", "ulens_lightcurve_binary_ext_host", "ulens_nll_marginal", "ulens_mag_point", "ulens_roots", "ulens_get_stats",
+           "ulens_mag_host", "ulens_trajectory", "ulens_lightcurve_binary", "ulens_lightcurve_binary_host", "ulens_lightcurve_binary_ext", "ulens_lightcurve_binary_ext_host", "ulens_nll_marginal", "ulens_mag_point", "ulens_roots", "ulens_get_stats",
            "ulens_reset_stats", "ulens_last_launch_count", "ulens_set_timing", "ulens_get_kernel_ms", "ulens_fp64_peak", "ulens_strerror",
            "ulens_last_cuda_error"]
 
@@ -68,6 +68,7 @@ def lib() -> C.CDLL:
         L.ulens_mag.argtypes = [vp, ip, ip, C.POINTER(ulens_lens), dp, dp, vp, vp, vp, vp, vp, vp]
         L.ulens_mag_grad.argtypes = [vp, ip, ip, C.POINTER(ulens_lens), dp, dp, vp, vp, vp, vp, vp, vp, vp]
         L.ulens_mag_host.argtypes = [vp, ip, ip, C.POINTER(ulens_lens), dp, dp, vp, vp, vp, vp, vp, vp]
+        L.ulens_trajectory.argtypes = [vp, ip, ip, dp, vp, vp, vp, vp]
         L.ulens_lightcurve_binary.argtypes = [vp, ip, ip, dp, C.c_double, vp, vp, vp, vp, vp, vp]
         L.ulens_lightcurve_binary_host.argtypes = [vp, ip, ip, dp, C.c_double, vp, vp, vp, vp, vp, vp]
         L.ulens_lightcurve_binary_ext.argtypes = [vp, ip, ip, dp, C.c_double, vp, vp, C.c_double, vp, vp, vp, vp,
@@ -226,6 +227,18 @@ class Context:
                                     A.ctypes.data_as(C.c_void_p), err.ctypes.data_as(C.c_void_p),
                                     st.ctypes.data_as(C.c_void_p), self._stream(stream)), self._h)
         return A, err, st
+
+    def ulens_trajectory(self, theta, t, stream=None):
+        """Step a1 alone: theta host [n_cfg, 7], t CUDA float64 [n_epochs] -> (w_re, w_im) CUDA [n_cfg, n_epochs]."""
+        torch = self._torch
+        theta = np.ascontiguousarray(theta, dtype=np.float64).reshape(-1, 7)
+        n_cfg, n_ep = theta.shape[0], t.numel()
+        w_re = torch.empty((n_cfg, n_ep), dtype=torch.float64, device=t.device)
+        w_im = torch.empty((n_cfg, n_ep), dtype=torch.float64, device=t.device)
+        _check(lib().ulens_trajectory(self._h, n_cfg, n_ep, _dptr(theta), _dev(t, torch.float64, n_ep),
+                                      _dev(w_re, torch.float64, n_cfg * n_ep), _dev(w_im, torch.float64, n_cfg * n_ep),
+                                      self._stream(stream)), self._h)
+        return w_re, w_im
 
     def ulens_lightcurve_binary(self, theta, u1, t, want_dA=False, stream=None, out=None):
         """theta: host [n_cfg, 7] (t0,u0,tE,s,q,rho,alpha); t: CUDA float64 [n_epochs];

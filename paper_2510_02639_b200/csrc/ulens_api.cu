@@ -35,6 +35,8 @@ struct ChunkCounters {          // reset per chunk
     unsigned int next_unit;     // dynamic scheduler of k_shoot
 };
 
+#define UL_N_STAGE 8
+#define UL_MAX_POINTS (0x7fffffffLL - 4096)    // grid arithmetic (n + 1023) stays inside int
 struct ulens_ctx {
     int device;
     ulens_options opt;
@@ -64,6 +66,14 @@ struct ulens_ctx {
     unsigned char* ext_flag; int* ext_map; unsigned* ext_blk; size_t ext_cap;
     unsigned* st_all; size_t st_all_cap;    // status of every point when the caller passes none (the retry pass reads it)
     int last_launches;
+    // host -> device uploads of the per-configuration tables go through context-owned PINNED staging buffers
+    // (a pageable cudaMemcpyAsync would synchronise the stream first); a slot is reused only after the copy
+    // that read it has completed (its event), so no entry point has to wait for the stream
+    struct Stage { void* host; size_t cap; cudaEvent_t ev; bool used; };
+    Stage stage[UL_N_STAGE]; int stage_next;
+    // the tables of the last call: an identical (lenses, rho, u1) array is neither rebuilt nor uploaded again
+    std::vector<ulens_lens>* last_lenses; std::vector<double>* last_rho; std::vector<double>* last_u1;
+    int last_N; bool last_ld; bool last_tan_valid;
     // optional per-kernel device timing (ulens_set_timing): event pairs recorded on the caller's stream
     int timing_on;
     struct TimedLaunch { cudaEvent_t a, b; int which; };
@@ -161,7 +171,7 @@ __global__ void k_roots(int n, int pt_base, int n_pts_per_cfg, const PointCfg* _
 {
     constexpr int DEG = N * N + 1;
     int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (n_dev) n = min(n, (int)*n_dev);              // retry pass: the point count lives on the device
+    if (n_dev) n = min(n, (int)*n_dev - pt_base);    // retry pass: the point count lives on the device
     if (i >= n) return;
     long long gp = pmap ? (long long)pmap[pt_base + i] : (long long)pt_base + i;
     int c = (int)(gp / n_pts_per_cfg);
@@ -412,7 +422,7 @@ k_regions(int n, int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cf
     BoxExt* ext_all = reinterpret_cast<BoxExt*>(smem_raw + (blockDim.x >> 5) * sizeof(RegionWork<DEG>));
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     int i = blockIdx.x * (blockDim.x >> 5) + warp;
-    if (n_dev) n = min(n, (int)*n_dev);
+    if (n_dev) n = min(n, (int)*n_dev - pt_base);
     if (i >= n) return;                                  // whole warp leaves together
     RegionWork<DEG>& W = Wall[warp];
     if (lane == 0) W.ext = tans ? ext_all + warp * 32 * DEG : nullptr;
@@ -435,8 +445,17 @@ k_regions(int n, int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cf
     if (lane == 0) {
         np = regions_phaseC<N>(W, rp, i, L, wcx, wcy, rho, st, tans ? &tans[c] : nullptr);
         for (int p = 0; p < np; ++p) total_units += W.patch[p].n_units;
-        base = atomicAdd(&cc->n_units, (unsigned)total_units);
-        if ((unsigned long long)base + total_units > cap_units) { st |= UL_ST_UNIT_OVF; np = 0; total_units = 0; }
+        // claim the units with a compare-and-swap that REFUSES instead of overshooting, so the queue never holds an
+        // unwritten descriptor (the queue holds chunk x max_units_pt units: a refusal needs hand-made options)
+        {
+            unsigned cur = *(volatile unsigned*)&cc->n_units;
+            for (;;) {
+                if ((unsigned long long)cur + (unsigned)total_units > cap_units) { st |= UL_ST_UNIT_OVF; np = 0; total_units = 0; break; }
+                const unsigned prev = atomicCAS(&cc->n_units, cur, cur + (unsigned)total_units);
+                if (prev == cur) { base = cur; break; }
+                cur = prev;
+            }
+        }
         int u = base;
         for (int p = 0; p < np; ++p) { W.patch[p].unit0 = u; u += W.patch[p].n_units; patches[(long long)i * UL_MAXP + p] = W.patch[p]; if (tans) ptans[(long long)i * UL_MAXP + p] = W.ptan[p]; }
         n_patch[i] = np;
@@ -517,7 +536,7 @@ __global__ void k_finalize(int n, int pt_base, int n_pts_per_cfg, const PointCfg
                            const unsigned* __restrict__ n_dev = nullptr, unsigned st_or = 0)
 {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (n_dev) n = min(n, (int)*n_dev);
+    if (n_dev) n = min(n, (int)*n_dev - pt_base);
     if (i >= n) return;
     long long gp = pmap ? (long long)pmap[pt_base + i] : (long long)pt_base + i;
     int c = (int)(gp / n_pts_per_cfg);
@@ -539,11 +558,20 @@ __global__ void k_finalize(int n, int pt_base, int n_pts_per_cfg, const PointCfg
     // of the full sum is about |A - A_half| / (2^1.5 - 1)
     double err = fabs(A - Ao) / (1.8284271247461903 * fabs(A));
     if (!(err <= rel_tol)) st |= UL_ST_ERR_HIGH;
+    atomicAdd(&ctr->n_units, nu_tot);
+    if (st_or) {
+        // retry pass: the new result replaces the first one only if it is finite and no worse (fewer doubtful
+        // bits, or as many and a smaller self-error); a point that keeps its first result keeps its first status
+        const unsigned st0 = status_out[gp];
+        const int b0 = __popc(st0 & UL_ST_RETRY_MASK), b1 = __popc(st & UL_ST_RETRY_MASK);
+        const double err0 = err_out ? err_out[gp] : 1e300;
+        const bool better = (A == A) && (b1 < b0 || (b1 == b0 && !(err > err0)));
+        if (!better) return;
+    }
     A_out[gp] = A;
     if (err_out) err_out[gp] = err;
     if (status_out) status_out[gp] = st;
-    atomicAdd(&ctr->n_units, nu_tot);
-    if (st_or) {                                         // retry pass: the point was counted (and counted as flagged) before
+    if (st_or) {                                         // the point was counted (and counted as flagged) before
         if (!(st & 0xffu)) atomicAdd(&ctr->n_flagged, ~0ull);
     } else {
         if (i == 0) atomicAdd(&ctr->n_points, (unsigned long long)n);
@@ -678,12 +706,13 @@ __global__ void k_finalize_dual(int n, int pt_base, int n_pts_per_cfg, const Poi
                                 const TangentTable* __restrict__ tans, const Patch* __restrict__ patches,
                                 const int* __restrict__ n_patch, const double* __restrict__ unit_sum,
                                 const double* __restrict__ unit_tan, double* __restrict__ grad5, const int* __restrict__ pmap = nullptr,
-                                const unsigned* __restrict__ n_dev = nullptr)
+                                const unsigned* __restrict__ n_dev = nullptr, const unsigned* __restrict__ status_retry = nullptr)
 {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (n_dev) n = min(n, (int)*n_dev);
+    if (n_dev) n = min(n, (int)*n_dev - pt_base);
     if (i >= n) return;
     long long gp = pmap ? (long long)pmap[pt_base + i] : (long long)pt_base + i;
+    if (status_retry && !(status_retry[gp] & UL_ST_RETRIED)) return;     // retry pass: k_finalize kept the first result
     int c = (int)(gp / n_pts_per_cfg);
     double rho = cfg[c].rho, u1 = cfg[c].u1;
     double F0 = UL_PI * rho * rho * (1.0 - u1 / 3.0);
@@ -835,7 +864,13 @@ extern "C" int ulens_create(ulens_ctx** out, int cuda_device, const ulens_option
     memset(ctx, 0, sizeof *ctx);
     ctx->device = cuda_device;
     ctx->timed = new (std::nothrow) std::vector<ulens_ctx::TimedLaunch>();
-    if (!ctx->timed) { delete ctx; return ULENS_ENOMEM; }
+    ctx->last_lenses = new (std::nothrow) std::vector<ulens_lens>();
+    ctx->last_rho = new (std::nothrow) std::vector<double>();
+    ctx->last_u1 = new (std::nothrow) std::vector<double>();
+    if (!ctx->timed || !ctx->last_lenses || !ctx->last_rho || !ctx->last_u1) {
+        delete ctx->timed; delete ctx->last_lenses; delete ctx->last_rho; delete ctx->last_u1; delete ctx;
+        return ULENS_ENOMEM;
+    }
     ulens_options o; memset(&o, 0, sizeof o);
     if (opt) o = *opt;
     if (o.n_limb <= 0) o.n_limb = 512;
@@ -846,11 +881,12 @@ extern "C" int ulens_create(ulens_ctx** out, int cuda_device, const ulens_option
     if (!(o.rel_tol > 0.0)) o.rel_tol = 1e-4;
     if (o.chunk_pts <= 0) o.chunk_pts = 65536;
     if (o.chunk_pts > (1 << 21) / UL_MAXP) o.chunk_pts = (1 << 21) / UL_MAXP;
+    if (o.chunk_pts > 0x7fffff00 / 1024) o.chunk_pts = 0x7fffff00 / 1024;
     ctx->opt = o;
     ctx->rp.n_limb = o.n_limb; ctx->rp.n_r = o.n_r; ctx->rp.n_theta = o.n_theta;
     ctx->rp.max_nr = 8192; ctx->rp.max_nth = 32768; ctx->rp.max_units_pt = 1024;
     ctx->chunk = o.chunk_pts;
-    ctx->cap_units = (size_t)ctx->chunk * 192;
+    ctx->cap_units = (size_t)ctx->chunk * ctx->rp.max_units_pt;     // a full chunk of points at the per-point cap fits: no overflow
     if (ctx->cap_units > 0x7fffff00u) ctx->cap_units = 0x7fffff00u;
     cudaError_t e = cudaSetDevice(cuda_device);
     if (e == cudaSuccess) e = cudaMalloc(&ctx->patches, sizeof(Patch) * UL_MAXP * (size_t)ctx->chunk);
@@ -885,7 +921,34 @@ extern "C" void ulens_destroy(ulens_ctx* ctx)
         for (auto& t : *ctx->timed) { cudaEventDestroy(t.a); cudaEventDestroy(t.b); }
         delete ctx->timed;
     }
+    for (int k = 0; k < UL_N_STAGE; ++k) {
+        if (ctx->stage[k].host) cudaFreeHost(ctx->stage[k].host);
+        if (ctx->stage[k].ev) cudaEventDestroy(ctx->stage[k].ev);
+    }
+    delete ctx->last_lenses; delete ctx->last_rho; delete ctx->last_u1;
     delete ctx;
+}
+
+// copy `bytes` from ordinary host memory to the device through a pinned staging slot, stream-ordered, no sync
+static int stage_upload(ulens_ctx* ctx, void* dst_dev, const void* src_host, size_t bytes, cudaStream_t st)
+{
+    if (bytes == 0) return ULENS_OK;
+    ulens_ctx::Stage& S = ctx->stage[ctx->stage_next];
+    ctx->stage_next = (ctx->stage_next + 1) % UL_N_STAGE;
+    if (S.used) CK(cudaEventSynchronize(S.ev));          // the copy issued UL_N_STAGE uploads ago: long finished
+    if (!S.ev) CK(cudaEventCreateWithFlags(&S.ev, cudaEventDisableTiming));
+    if (bytes > S.cap) {
+        if (S.host) cudaFreeHost(S.host);
+        S.host = nullptr; S.cap = 0;
+        size_t cap = bytes + bytes / 4 + 4096;
+        if (cudaHostAlloc(&S.host, cap, cudaHostAllocDefault) != cudaSuccess) return ULENS_ENOMEM;
+        S.cap = cap;
+    }
+    memcpy(S.host, src_host, bytes);
+    CK(cudaMemcpyAsync(dst_dev, S.host, bytes, cudaMemcpyHostToDevice, st));
+    CK(cudaEventRecord(S.ev, st));
+    S.used = true;
+    return ULENS_OK;
 }
 
 static int upload_cfgs(ulens_ctx* ctx, int n_cfg, const ulens_lens* lenses, const double* rho, const double* u1,
@@ -893,6 +956,15 @@ static int upload_cfgs(ulens_ctx* ctx, int n_cfg, const ulens_lens* lenses, cons
 {
     int N = lenses[0].n_lens;
     if (N < 1 || N > 3) return ULENS_EINVAL;
+    // same tables as the last call (an HMC chain re-evaluates the same lens array many times): nothing to do
+    if (ctx->last_lenses->size() == (size_t)n_cfg && ctx->cfg_dev &&
+        memcmp(ctx->last_lenses->data(), lenses, sizeof(ulens_lens) * n_cfg) == 0 &&
+        memcmp(ctx->last_rho->data(), rho, sizeof(double) * n_cfg) == 0 &&
+        memcmp(ctx->last_u1->data(), u1, sizeof(double) * n_cfg) == 0) {
+        *n_lens_out = ctx->last_N; *any_ld = ctx->last_ld;
+        return ULENS_OK;
+    }
+    ctx->last_lenses->clear(); ctx->last_tan_valid = false;
     std::vector<PointCfg> cfg(n_cfg);
     std::vector<LensPoly> poly(n_cfg);
     *any_ld = false;
@@ -920,10 +992,12 @@ static int upload_cfgs(ulens_ctx* ctx, int n_cfg, const ulens_lens* lenses, cons
         if (cudaMalloc(&ctx->poly_dev, sizeof(LensPoly) * cap) != cudaSuccess) return ULENS_ENOMEM;
         ctx->cfg_cap = cap;
     }
-    // pageable source: the runtime stages the bytes before returning, so the vectors may die here
-    CK(cudaMemcpyAsync(ctx->cfg_dev, cfg.data(), sizeof(PointCfg) * n_cfg, cudaMemcpyHostToDevice, st));
-    CK(cudaMemcpyAsync(ctx->poly_dev, poly.data(), sizeof(LensPoly) * n_cfg, cudaMemcpyHostToDevice, st));
-    CK(cudaStreamSynchronize(st));
+    int rc = stage_upload(ctx, ctx->cfg_dev, cfg.data(), sizeof(PointCfg) * n_cfg, st);
+    if (rc == ULENS_OK) rc = stage_upload(ctx, ctx->poly_dev, poly.data(), sizeof(LensPoly) * n_cfg, st);
+    if (rc != ULENS_OK) return rc;
+    ctx->last_lenses->assign(lenses, lenses + n_cfg);
+    ctx->last_rho->assign(rho, rho + n_cfg); ctx->last_u1->assign(u1, u1 + n_cfg);
+    ctx->last_N = N; ctx->last_ld = *any_ld;
     *n_lens_out = N;
     return ULENS_OK;
 }
@@ -999,7 +1073,7 @@ static int run_chunks(ulens_ctx* ctx, long long n_total, int n_pts, bool ld, con
                                                         A_out, err_out, status_out, ctx->counters, pmap, n_dev, st_or);
             if (dual) {
                 k_finalize_dual<<<(n + 127) / 128, 128, 0, st>>>(n, (int)base, n_pts, ctx->cfg_dev, tans, ctx->patches, ctx->n_patch,
-                                                                 ctx->unit_sum, ctx->unit_tan, grad5_out, pmap, n_dev);
+                                                                 ctx->unit_sum, ctx->unit_tan, grad5_out, pmap, n_dev, st_or ? status_out : nullptr);
                 ctx->last_launches += 1;
             }
         }
@@ -1033,8 +1107,8 @@ static int retry_flagged(ulens_ctx* ctx, long long n_total, int n_pts, bool ld, 
     if (ctx->opt.flags & ULENS_OPT_NO_RETRY) return ULENS_OK;
     int rc = ensure_ext_buffers(ctx, (size_t)n_total);
     if (rc != ULENS_OK) return rc;
-    const int n = (int)n_total, n_blk = (n + 1023) / 1024;
-    k_retry_flag<<<(n + 255) / 256, 256, 0, st>>>(n, status, ctx->ext_flag);
+    const int n = (int)n_total, n_blk = (int)((n_total + 1023) / 1024);
+    k_retry_flag<<<(unsigned)((n_total + 255) / 256), 256, 0, st>>>(n, status, ctx->ext_flag);
     k_ext_count<<<n_blk, 1024, 0, st>>>(n, ctx->ext_flag, ctx->ext_blk);
     k_ext_scan<<<1, 1024, 0, st>>>(n_blk, ctx->ext_blk);
     k_ext_scatter<<<n_blk, 1024, 0, st>>>(n, ctx->ext_flag, ctx->ext_blk, ctx->ext_map);
@@ -1042,7 +1116,9 @@ static int retry_flagged(ulens_ctx* ctx, long long n_total, int n_pts, bool ld, 
     CK(cudaGetLastError());
     RegionParams rp2 = ctx->rp;
     rp2.n_limb = ctx->rp.n_limb * 2 > 8192 ? 8192 : ctx->rp.n_limb * 2;
-    const long long n_max = n_total < ctx->chunk ? n_total : ctx->chunk;
+    // launches are sized for two chunks of doubtful points (their number stays on the device); any beyond that keep
+    // their first result and status, without ULENS_ST_RETRIED
+    const long long n_max = n_total < 2LL * ctx->chunk ? n_total : 2LL * ctx->chunk;
     return run_chunks<N>(ctx, n_max, n_pts, ld, w_re, w_im, A_out, err_out, status, st, grad5_out, ctx->ext_map,
                          ctx->ext_blk + n_blk, &rp2, UL_ST_RETRIED);
 }
@@ -1051,6 +1127,7 @@ static int retry_flagged(ulens_ctx* ctx, long long n_total, int n_pts, bool ld, 
 // exist for a binary in the geometry of ulens_lens_binary (G4): s = a_2 - a_1, q = eps_2 / eps_1.
 static int upload_tangents(ulens_ctx* ctx, int n_cfg, const ulens_lens* lenses, cudaStream_t st)
 {
+    if (ctx->last_tan_valid && ctx->tan_dev) return ULENS_OK;       // same lens array as the last call (upload_cfgs checked)
     std::vector<TangentTable> tt(n_cfg);
     for (int c = 0; c < n_cfg; ++c) {
         TangentTable& T = tt[c];
@@ -1072,8 +1149,9 @@ static int upload_tangents(ulens_ctx* ctx, int n_cfg, const ulens_lens* lenses, 
         if (cudaMalloc(&ctx->tan_dev, sizeof(TangentTable) * ((size_t)n_cfg + 64)) != cudaSuccess) return ULENS_ENOMEM;
         ctx->tan_cap = (size_t)n_cfg + 64;
     }
-    CK(cudaMemcpyAsync(ctx->tan_dev, tt.data(), sizeof(TangentTable) * n_cfg, cudaMemcpyHostToDevice, st));
-    CK(cudaStreamSynchronize(st));
+    int rc = stage_upload(ctx, ctx->tan_dev, tt.data(), sizeof(TangentTable) * n_cfg, st);
+    if (rc != ULENS_OK) return rc;
+    ctx->last_tan_valid = true;
     return ULENS_OK;
 }
 
@@ -1090,7 +1168,7 @@ static int mag_device(ulens_ctx* ctx, int n_cfg, int n_pts, const ulens_lens* le
         if (rc != ULENS_OK) return rc;
     }
     long long n_total = (long long)n_cfg * n_pts;
-    if (n_total > 0x7fffffffLL) return ULENS_EUNSUPPORTED;
+    if (n_total > UL_MAX_POINTS) return ULENS_EUNSUPPORTED;
     ctx->last_launches = 0;
     if (!status_out) {                                   // the retry pass needs every point's status
         if ((size_t)n_total > ctx->st_all_cap) {
@@ -1167,6 +1245,34 @@ extern "C" int ulens_mag_host(ulens_ctx* ctx, int n_cfg, int n_pts, const ulens_
     return ULENS_OK;
 }
 
+extern "C" int ulens_trajectory(ulens_ctx* ctx, int n_cfg, int n_epochs, const double* theta_host, const double* t,
+                                double* w_re_out, double* w_im_out, void* stream)
+{
+    if (!ctx || n_cfg < 0 || n_epochs < 0) return ULENS_EINVAL;
+    if (n_cfg == 0 || n_epochs == 0) return ULENS_OK;
+    if (!theta_host || !t || !w_re_out || !w_im_out) return ULENS_EINVAL;
+    for (int c = 0; c < n_cfg; ++c) {
+        const double* th = theta_host + 7 * c;
+        if (!isfinite(th[0]) || !isfinite(th[1]) || !isfinite(th[6]) || !finite_pos(th[2])) return ULENS_EINVAL;
+    }
+    CK(cudaSetDevice(ctx->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t n = (size_t)n_cfg * n_epochs;
+    if (n > (size_t)UL_MAX_POINTS) return ULENS_EUNSUPPORTED;
+    const size_t need = 7 * (size_t)n_cfg;
+    if (need > ctx->traj_cap) {
+        cudaFree(ctx->traj_w); ctx->traj_w = nullptr; ctx->traj_cap = 0;
+        if (cudaMalloc(&ctx->traj_w, sizeof(double) * need) != cudaSuccess) return ULENS_ENOMEM;
+        ctx->traj_cap = need;
+    }
+    int rc = stage_upload(ctx, ctx->traj_w, theta_host, sizeof(double) * 7 * n_cfg, st);
+    if (rc != ULENS_OK) return rc;
+    k_traj<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(n_cfg, n_epochs, ctx->traj_w, t, w_re_out, w_im_out);
+    ctx->last_launches = 1;
+    CK(cudaGetLastError());
+    return ULENS_OK;
+}
+
 extern "C" int ulens_lightcurve_binary(ulens_ctx* ctx, int n_cfg, int n_epochs, const double* theta_host, double u1,
                                        const double* t, double* A_out, double* dA_out, double* err_out,
                                        uint32_t* status_out, void* stream)
@@ -1195,7 +1301,10 @@ extern "C" int ulens_lightcurve_binary(ulens_ctx* ctx, int n_cfg, int n_epochs, 
     }
     double* w_re = ctx->traj_w; double* w_im = w_re + n; double* th_dev = w_im + n;
     double* g5 = dA_out ? th_dev + 7 * (size_t)n_cfg : nullptr;
-    CK(cudaMemcpyAsync(th_dev, theta_host, sizeof(double) * 7 * n_cfg, cudaMemcpyHostToDevice, st));
+    {
+        int rcu = stage_upload(ctx, th_dev, theta_host, sizeof(double) * 7 * n_cfg, st);
+        if (rcu != ULENS_OK) return rcu;
+    }
     {
         KTimer kt(ctx, ULENS_K_TRAJ, st);
         k_traj<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(n_cfg, n_epochs, th_dev, t, w_re, w_im);
@@ -1235,7 +1344,7 @@ extern "C" int ulens_lightcurve_binary_ext(ulens_ctx* ctx, int n_cfg, int n_epoc
         rho[c] = th[5];
     }
     const size_t n = (size_t)n_cfg * n_epochs;
-    if (n > 0x7fffffffULL) return ULENS_EUNSUPPORTED;
+    if (n > (size_t)UL_MAX_POINTS) return ULENS_EUNSUPPORTED;
     size_t need = 2 * n + 7 * (size_t)n_cfg + (dA_out ? UL_NT * n : 0);
     if (need > ctx->traj_cap) {
         cudaFree(ctx->traj_w); ctx->traj_w = nullptr; ctx->traj_cap = 0;
@@ -1257,7 +1366,10 @@ extern "C" int ulens_lightcurve_binary_ext(ulens_ctx* ctx, int n_cfg, int n_epoc
     }
     double* w_re = ctx->traj_w; double* w_im = w_re + n; double* th_dev = w_im + n;
     double* g5 = dA_out ? th_dev + 7 * (size_t)n_cfg : nullptr;
-    CK(cudaMemcpyAsync(th_dev, theta_host, sizeof(double) * 7 * n_cfg, cudaMemcpyHostToDevice, st));
+    {
+        int rcu = stage_upload(ctx, th_dev, theta_host, sizeof(double) * 7 * n_cfg, st);
+        if (rcu != ULENS_OK) return rcu;
+    }
     {
         KTimer kt(ctx, ULENS_K_TRAJ, st);
         k_traj<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(n_cfg, n_epochs, th_dev, t, w_re, w_im);
@@ -1394,8 +1506,8 @@ extern "C" int ulens_mag_point(ulens_ctx* ctx, int n_cfg, int n_pts, const ulens
     int rc = upload_cfgs(ctx, n_cfg, lenses_host, rho.data(), u1.data(), st, &N, &ld);
     if (rc != ULENS_OK) return rc;
     long long n_total = (long long)n_cfg * n_pts;
-    if (n_total > 0x7fffffffLL) return ULENS_EUNSUPPORTED;
-    const int n = (int)n_total, grid = (n + 127) / 128;
+    if (n_total > UL_MAX_POINTS) return ULENS_EUNSUPPORTED;
+    const int n = (int)n_total, grid = (int)((n_total + 127) / 128);
     switch (N) {
         case 1: k_roots<1><<<grid, 128, 0, st>>>(n, 0, n_pts, ctx->cfg_dev, ctx->poly_dev, w_re, w_im, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, A_out, status_out); break;
         case 2: k_roots<2><<<grid, 128, 0, st>>>(n, 0, n_pts, ctx->cfg_dev, ctx->poly_dev, w_re, w_im, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, A_out, status_out); break;

@@ -465,13 +465,9 @@ UL_HDN unsigned centre_images(const Lens& L, const LensPoly& T, double wx, doubl
 #pragma unroll
     for (int k = 0; k < DEG; ++k) {
         double zx = zr[k], zy = zi[k], detJ, resid, gx, gy;
-        double dm2 = 1e300;
-#pragma unroll
-        for (int a = 0; a < N; ++a) { double dx = zx - L.ax[a], dy = zy - L.ay[a]; dm2 = ul_min(dm2, dx * dx + dy * dy); }
         // a polish that converges IS an image wherever it started (Eq. 1 is the definition); starts
         // from spurious roots may land on an image already found: the duplicate test below drops those
         bool ok = polish_image<N>(L, wx, wy, zx, zy, 16, 1e-13, detJ, resid, gx, gy);
-        (void)dm2;
         if (ok) {
             double sc = ul_max(1.0, zx * zx + zy * zy);
             for (int q = 0; q < n_img; ++q) {
@@ -746,8 +742,6 @@ UL_HD void line_node(int flags, int n_r, int line, double r0, double dr, double&
     } else { r = r0 + (line + 0.5) * dr; w = dr; }
 }
 
-UL_HD bool en_dummy(double f1) { return !(f1 < 0.0); }
-
 // Integrate one radial line theta over r (filled ring / disk sectors):
 //   U = Int chi r dr,  S = Int chi sqrt(-F) r dr   (length^2 units). Nodes at r0 + (i + 1/2) dr, i = -2 .. n_r+1.
 // A node with r < 0 is the point on the opposite side of the origin: F is smooth along the whole line, so
@@ -772,7 +766,7 @@ UL_HD void shoot_col(const Lens& L, double wcx, double wcy, double rho2, double 
             double rh = r1 + 0.5 * dr;                   // cell face between the pair
             if (rh > 0.0) {
                 double u, dS; bool en;
-                double rin = en_dummy(f1) ? r1 + dr : r1; // first inside node
+                double rin = !(f1 < 0.0) ? r1 + dr : r1;  // first inside node
                 double t2x = dr / ul_max(rin, 0.5 * dr);
                 edge_event(f0, f1, f2, f3, LD, t2x, u, en, dS);
                 double rc = en ? (r1 + dr) - u * dr : r1 + u * dr;

@@ -20,10 +20,6 @@
 
 namespace ulens {
 
-#ifdef UL_EXPERIMENT
-static double g_mscale = 1.0;
-#endif
-
 struct SubBox {
     double r_lo, r_hi;      // r_lo > r_hi: empty
     double t_lo, t_hi;      // unwrapped theta interval, t_lo in [-pi, pi), t_hi - t_lo <= 2 pi
@@ -384,9 +380,6 @@ UL_HDN void regions_phaseA(int lane, const Lens& L, const LensPoly& T, double wc
             }
         }
         if (noconv) status |= UL_ST_EA_NOCONV;
-#ifdef UL_DEBUG_PHASEA
-        if (lane == UL_DEBUG_PHASEA) { printf("lane %d ph %.6f step %.3g it %d valid %x:", lane, ph_new / dphi, st_try / dphi, it, valid); for (int j = 0; j < DEG; ++j) printf(" (%.6f,%.6f)", px[j], py[j]); printf("\n"); }
-#endif
         // own points
 #pragma unroll 1
         for (int j = 0; j < DEG; ++j) {
@@ -496,9 +489,6 @@ UL_HD void box_expanded(const SubBox& b, double& rl, double& rh, double& tl, dou
     // at Chebyshev-like radii r_c + h sin(phi) (emit_patch), which removes the square-root behaviour of the
     // chord length at the radial ends of an image only if the sector ends where the image ends.
     double mr = 0.02 * (0.25 * m + 0.02 * (b.r_hi - b.r_lo));
-#ifdef UL_EXPERIMENT
-    mr *= g_mscale;
-#endif
     double rmid = ul_max(0.5 * (b.r_lo + b.r_hi), 1e-300);
     double mt = 0.02 * (0.25 * m / rmid + 0.02 * (b.t_hi - b.t_lo));   // tight, as in r
     mt = ul_min(mt, 0.5);

@@ -195,3 +195,50 @@ def subsample(wl: Workload, n_per_cfg: int, seed: int = 0) -> np.ndarray:
                                rng.choice(far, k_far, replace=False)])
         out.append(np.sort(pick))
     return np.array(out)
+
+
+def light_body_zone(wl: Workload, c: int, eps_max: float = 1e-3) -> np.ndarray:
+    """Workload points of config c that lie within 8 sqrt(eps_a) + 2 rho of the planetary-caustic centre
+    w_a = a_a - sum_{b != a} eps_b / conj(a_a - a_b) of a light body (eps_a < eps_max): the geometry in which a
+    faint image pair hides next to the light lens. Input selection only; returns a bool mask [n_pts]."""
+    eps, a = lens_geometry(wl.kind, wl.lens_params[c])
+    mask = np.zeros(wl.n_pts, dtype=bool)
+    for i in range(len(a)):
+        if not eps[i] < eps_max:
+            continue
+        others = [b for b in range(len(a)) if b != i]
+        w_a = a[i] - np.sum(eps[others] / np.conj(a[i] - a[others]))
+        mask |= np.abs(wl.w[c] - w_a) < 8.0 * np.sqrt(eps[i]) + 2.0 * wl.rho[c]
+    return mask
+
+
+def golden_sample(wl: Workload, cfg: int, n_total: int = 2048, n_zone: int = 12):
+    """The seeded sample behind tests/golden/oracle_C<cfg>.npz: n_total / n_cfg stratified points of every
+    configuration (subsample(), seed 500 + cfg) plus up to n_zone further points per configuration from
+    light_body_zone(). Returns (cfg_index [m], point_index [m], in_zone [m])."""
+    idx = subsample(wl, n_total // wl.n_cfg, seed=500 + cfg)
+    rng = np.random.default_rng(np.random.SeedSequence([SEED_ROOT, 98, cfg]))
+    cs, ps, zs = [], [], []
+    for c in range(wl.n_cfg):
+        zone = light_body_zone(wl, c)
+        base = idx[c]
+        cand = np.setdiff1d(np.flatnonzero(zone), base)
+        extra = np.sort(rng.choice(cand, min(n_zone, len(cand)), replace=False)) if len(cand) else np.array([], int)
+        p = np.concatenate([base, extra])
+        cs.append(np.full(len(p), c)); ps.append(p); zs.append(zone[p])
+    return np.concatenate(cs), np.concatenate(ps), np.concatenate(zs)
+
+
+def golden_c4_sample(wl: Workload, n_vec: int = 16, n_ep: int = 16):
+    """The seeded (vector, epoch) sample behind tests/golden/oracle_C4_fd.npz: n_vec parameter vectors, and per
+    vector n_ep epochs, half of them from |tau| < 0.15 (the caustic crossing and the peak), half from the rest."""
+    rng = np.random.default_rng(np.random.SeedSequence([SEED_ROOT, 97, 4]))
+    vec = np.sort(rng.choice(wl.n_cfg, n_vec, replace=False))
+    eps_ = []
+    for c in vec:
+        tau = (wl.t - wl.theta[c, 0]) / wl.theta[c, 2]
+        near = np.flatnonzero(np.abs(tau) < 0.15)
+        far = np.flatnonzero(np.abs(tau) >= 0.15)
+        eps_.append(np.sort(np.concatenate([rng.choice(near, n_ep // 2, replace=False),
+                                            rng.choice(far, n_ep - n_ep // 2, replace=False)])))
+    return vec, np.array(eps_)

@@ -17,3 +17,20 @@ def oracle():
     from oracle import oracle as O
     O.build()
     return O
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    return torch
+
+
+@pytest.fixture(scope="module")
+def ctx(torch_cuda):
+    """A default-options context on cuda:0 (one per test module); the library is (re)built if its sources are newer."""
+    from paper_2510_02639_b200 import binding, build
+    build.build()
+    c = binding.Context(0)
+    yield c
+    c.close()

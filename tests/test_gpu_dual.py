@@ -21,22 +21,6 @@ REL = 1e-3
 ABS_A = 1e-4
 
 
-@pytest.fixture(scope="module")
-def torch_cuda():
-    import torch
-    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
-    return torch
-
-
-@pytest.fixture(scope="module")
-def ctx(torch_cuda):
-    from paper_2510_02639_b200 import binding, build
-    build.build()
-    c = binding.Context(0)
-    yield c
-    c.close()
-
-
 def _grad(ctx, torch, lenses, rho, u1, w):
     w = np.atleast_2d(np.asarray(w, dtype=complex))
     wre = torch.tensor(np.ascontiguousarray(w.real), device="cuda:0")

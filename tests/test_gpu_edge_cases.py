@@ -10,22 +10,6 @@ pytestmark = pytest.mark.gpu
 TOL_A = 1e-4
 
 
-@pytest.fixture(scope="module")
-def torch_cuda():
-    import torch
-    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
-    return torch
-
-
-@pytest.fixture(scope="module")
-def ctx(torch_cuda):
-    from paper_2510_02639_b200 import binding, build
-    build.build()
-    c = binding.Context(0)
-    yield c
-    c.close()
-
-
 def _mag(ctx, torch, lenses, rho, u1, w):
     w = np.atleast_2d(np.asarray(w, dtype=complex))
     wre = torch.tensor(np.ascontiguousarray(w.real), device="cuda:0")
@@ -142,3 +126,81 @@ def test_size_limit_and_lightcurve_edge_inputs(ctx, torch_cuda):
                 [0, 0.1, 1.0, 1.0, 0.1, 0.0, 0.3]):
         with pytest.raises(binding.UlensError):
             ctx.ulens_lightcurve_binary(np.array([bad]), 0.5, t1)
+
+
+def test_device_entries_do_not_synchronise(ctx, torch_cuda):
+    """include/ulens.h: 'all device work is enqueued on the caller's stream and the call does NOT synchronise'.
+    The stream is kept busy (a spin kernel of ~0.3 s) before the calls; each call must return while that work is
+    still running, i.e. without waiting for the stream (pinned staging of the host tables, no cudaStreamSynchronize)."""
+    from paper_2510_02639_b200 import binding, inputs
+    torch = torch_cuda
+    wl = inputs.get(0)
+    L = binding.ulens_lens_binary(1.0, 0.01)
+    wre = torch.tensor(np.ascontiguousarray(wl.w.real), device="cuda:0")
+    wim = torch.tensor(np.ascontiguousarray(wl.w.imag), device="cuda:0")
+    t = torch.tensor(wl.t.copy(), device="cuda:0")
+    # warm-up: the first calls grow the workspace (cudaMalloc / cudaFree wait for the device)
+    ctx.ulens_mag([L], wl.rho, wl.u1, wre, wim)
+    ctx.ulens_mag_grad([L], wl.rho, wl.u1, wre, wim)
+    ctx.ulens_lightcurve_binary(wl.theta, 0.0, t, want_dA=True)
+    ctx.ulens_trajectory(wl.theta, t)
+    ctx.ulens_mag_point([L], wre, wim)
+    torch.cuda.synchronize()
+    stream = torch.cuda.current_stream()
+    for name, call in [("ulens_mag", lambda: ctx.ulens_mag([L], wl.rho * 1.01, wl.u1, wre, wim)),
+                       ("ulens_mag_grad", lambda: ctx.ulens_mag_grad([L], wl.rho * 1.02, wl.u1, wre, wim)),
+                       ("ulens_lightcurve_binary", lambda: ctx.ulens_lightcurve_binary(wl.theta * 1.001, 0.0, t, want_dA=True)),
+                       ("ulens_trajectory", lambda: ctx.ulens_trajectory(wl.theta * 1.002, t)),
+                       ("ulens_mag_point", lambda: ctx.ulens_mag_point([binding.ulens_lens_binary(1.0, 0.02)], wre, wim))]:
+        torch.cuda._sleep(int(0.3 * 1.9e9))               # ~0.3 s of spinning on the stream
+        done = torch.cuda.Event()
+        call()
+        done.record()
+        assert not stream.query(), name + " returned only after the stream had drained"
+        assert not done.query(), name
+        torch.cuda.synchronize()
+
+
+def test_trajectory_entry_matches_oracle(ctx, torch_cuda, oracle):
+    """Step a1 directly: k_traj's source centres against oracle.trajectory (pinned in test_oracle_pins.py), to the
+    last bits (the two sides may contract multiply-adds differently: 4 ulp of the largest term)."""
+    from paper_2510_02639_b200 import inputs
+    torch = torch_cuda
+    wl = inputs.get(4)
+    cs = [0, 17, 1023]
+    t = torch.tensor(wl.t.copy(), device="cuda:0")
+    w_re, w_im = ctx.ulens_trajectory(wl.theta[cs], t)
+    torch.cuda.synchronize()
+    w_re, w_im = w_re.cpu().numpy(), w_im.cpu().numpy()
+    for k, c in enumerate(cs):
+        t0, u0, tE, _, _, _, al = wl.theta[c]
+        ox, oy = oracle.trajectory(t0, u0, tE, al, wl.t)
+        scale = np.abs((wl.t - t0) / tE) + abs(u0)
+        assert np.all(np.abs(w_re[k] - ox) <= 1e-15 * scale) and np.all(np.abs(w_im[k] - oy) <= 1e-15 * scale)
+    with pytest.raises(Exception):
+        bad = wl.theta[:1].copy(); bad[0, 2] = 0.0
+        ctx.ulens_trajectory(bad, t)
+
+
+def test_large_sources_fill_the_unit_queue_without_overflow(torch_cuda):
+    """Sources of rho = 0.3 ... 2 need hundreds of 32-line work units per point (the old queue of
+    192 units per point overflowed and left NaNs). The queue now holds chunk_pts x the per-point cap, and units are
+    claimed with a compare-and-swap that refuses rather than overshoots. Single lens, so the reference is the
+    Witt-Mao closed form (test_oracle_pins.A_witt_mao, mpmath); a small chunk makes the call span many chunks."""
+    from paper_2510_02639_b200 import binding
+    from test_oracle_pins import A_witt_mao
+    torch = torch_cuda
+    c = binding.Context(0, chunk_pts=64)
+    rng = np.random.default_rng(5)
+    for rho in (0.3, 0.5, 1.0, 2.0):
+        u = rng.uniform(0.05, 2.5, 150)
+        ph = rng.uniform(0, 2 * np.pi, 150)
+        w = u * np.exp(1j * ph)
+        A, err, st = _mag(c, torch, [binding.lens_single()], [rho], [0.0], [w])
+        assert np.all(np.isfinite(A)), rho
+        assert not np.any(st & binding.ST_UNIT_OVF), rho
+        ref = np.array([float(A_witt_mao(float(x), rho)) for x in u[:40]])
+        assert np.abs(A[0, :40] / ref - 1).max() <= TOL_A, (rho, np.abs(A[0, :40] / ref - 1).max())
+    units = c.ulens_get_stats()["n_units"] / (4 * 150)
+    assert units > 100                                    # the case really is unit-hungry
+    c.close()

@@ -17,22 +17,6 @@ TOL_A = 1e-4
 
 
 @pytest.fixture(scope="module")
-def torch_cuda():
-    import torch
-    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
-    return torch
-
-
-@pytest.fixture(scope="module")
-def ctx(torch_cuda):
-    from paper_2510_02639_b200 import binding, build
-    build.build()
-    c = binding.Context(0)
-    yield c
-    c.close()
-
-
-@pytest.fixture(scope="module")
 def oracle():
     from oracle import oracle as O
     O.build()

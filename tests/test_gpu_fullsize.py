@@ -12,22 +12,6 @@ import pytest
 pytestmark = pytest.mark.gpu
 
 
-@pytest.fixture(scope="module")
-def torch_cuda():
-    import torch
-    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
-    return torch
-
-
-@pytest.fixture(scope="module")
-def ctx(torch_cuda):
-    from paper_2510_02639_b200 import binding, build
-    build.build()
-    c = binding.Context(0)
-    yield c
-    c.close()
-
-
 def _lenses(binding, wl, cs):
     f = binding.ulens_lens_binary if wl.kind == "binary" else binding.ulens_lens_triple
     return [f(*wl.lens_params[c]) for c in cs]

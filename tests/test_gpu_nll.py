@@ -7,22 +7,6 @@ import pytest
 pytestmark = pytest.mark.gpu
 
 
-@pytest.fixture(scope="module")
-def torch_cuda():
-    import torch
-    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
-    return torch
-
-
-@pytest.fixture(scope="module")
-def ctx(torch_cuda):
-    from paper_2510_02639_b200 import binding, build
-    build.build()
-    c = binding.Context(0)
-    yield c
-    c.close()
-
-
 def _data(n_cfg, n_ep, seed):
     """Light-curve-like A (a peak on a baseline), dA random but smooth in scale, noisy fluxes of the first curve."""
     rng = np.random.default_rng(seed)

@@ -14,22 +14,6 @@ TOL_A = 1e-4
 TOL_ROOT = 1e-10
 
 
-@pytest.fixture(scope="module")
-def torch_cuda():
-    import torch
-    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
-    return torch
-
-
-@pytest.fixture(scope="module")
-def ctx(torch_cuda):
-    from paper_2510_02639_b200 import binding, build
-    build.build()
-    c = binding.Context(0)
-    yield c
-    c.close()
-
-
 def _to_dev(torch, w):
     w = np.asarray(w, dtype=complex)
     return (torch.tensor(np.ascontiguousarray(w.real), device="cuda:0"),
@@ -203,14 +187,15 @@ def test_host_entry_matches_device_entry(ctx, torch_cuda):
     assert np.array_equal(A_dev, A_host)                                   # deterministic reduction order
 
 
-def test_lightcurve_entry_matches_positions_entry(ctx, torch_cuda, oracle):
+def test_lightcurve_entry_matches_positions_entry(ctx, torch_cuda):
+    """ulens_lightcurve_binary == ulens_trajectory (step a1, checked against the oracle in
+    test_gpu_edge_cases.test_trajectory_entry_matches_oracle) followed by ulens_mag, bit for bit."""
     from paper_2510_02639_b200 import binding, inputs
     wl = inputs.get(0)
     t = torch_cuda.tensor(wl.t[::5].copy(), device="cuda:0")
     A, dA, err, st = ctx.ulens_lightcurve_binary(wl.theta, 0.0, t)
+    w_re, w_im = ctx.ulens_trajectory(wl.theta, t)
+    A2, _, st2 = ctx.ulens_mag([binding.ulens_lens_binary(1.0, 0.01)], [1e-2], [0.0], w_re, w_im)
     torch_cuda.cuda.synchronize()
-    wx, wy = oracle.trajectory(0.0, 0.05, 1.0, 0.7, wl.t[::5])             # trajectory pinned in test_oracle_pins
-    A2, _, _ = _gpu_mag(ctx, torch_cuda, [binding.ulens_lens_binary(1.0, 0.01)], [1e-2], [0.0], [wx + 1j * wy])
-    # k_traj's w_c differs from the host trajectory in the last bit, which can move a sector border by one
-    # grid cell: two equally valid grids, equal to within the quadrature error
-    assert np.allclose(A.cpu().numpy(), A2, rtol=2e-5)
+    assert np.array_equal(A.cpu().numpy(), A2.cpu().numpy())
+    assert np.array_equal(st.cpu().numpy(), st2.cpu().numpy())

@@ -15,13 +15,6 @@ TOL_A = 1e-4
 
 
 @pytest.fixture(scope="module")
-def torch_cuda():
-    import torch
-    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
-    return torch
-
-
-@pytest.fixture(scope="module")
 def runs(torch_cuda):
     torch = torch_cuda
     from paper_2510_02639_b200 import binding, build, inputs
