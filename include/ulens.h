@@ -120,9 +120,11 @@ int  ulens_mag(ulens_ctx* ctx, int n_cfg, int n_pts,
                double* A_out, double* err_out, uint32_t* status_out, void* stream);
 
 /* (i') The same with forward-mode derivatives (Sec. 3.5) with respect to
- * the intrinsic inputs: dA5_out device [n_cfg*n_pts][5] = dA/d(w_cx, w_cy, s, q, rho). The s and q columns
- * are defined for binary lenses in the geometry of ulens_lens_binary (EUNSUPPORTED otherwise) and are zero
- * for n_lens = 1; n_lens = 3 is EUNSUPPORTED in this build. */
+ * the intrinsic inputs:
+ *   n_lens = 1, 2: dA5_out device [n_cfg*n_pts][5] = dA/d(w_cx, w_cy, s, q, rho)   (s, q columns zero for n_lens = 1)
+ *   n_lens = 3   : dA5_out device [n_cfg*n_pts][8] = dA/d(w_cx, w_cy, s, q, q3, r3, psi, rho)
+ * The lens-parameter columns are defined in the geometry of ulens_lens_binary / ulens_lens_triple (the parameters are
+ * recovered from the lens; any other geometry is EUNSUPPORTED). */
 int  ulens_mag_grad(ulens_ctx* ctx, int n_cfg, int n_pts,
                const ulens_lens* lenses_host, const double* rho_host, const double* u1_host,
                const double* w_re, const double* w_im,
@@ -154,6 +156,18 @@ int  ulens_lightcurve_binary(ulens_ctx* ctx, int n_cfg, int n_epochs,
  * copies t in, computes, copies the results out and synchronises the stream before returning
  * (the end-to-end entry point of the light-curve / derivative path, BASELINE.json configs[4]). */
 int  ulens_lightcurve_binary_host(ulens_ctx* ctx, int n_cfg, int n_epochs,
+               const double* theta_host, double u1, const double* t_host,
+               double* A_out_host, double* dA_out_host, double* err_out_host, uint32_t* status_out_host,
+               void* stream);
+
+/* (ii') The triple-lens light curve (the paper's gradient showcase Fig. 2, is this case):
+ *   theta_host [n_cfg][10] = (t0, u0, tE, s, q, rho, alpha, q3, r3, psi), host; geometry of ulens_lens_triple; trajectory as above.
+ *   A_out device [n_cfg][n_epochs]; dA_out device [n_cfg][n_epochs][10] or NULL: dA/d(theta) in the order of theta.
+ * ulens_lightcurve_triple_host: HOST arrays for t and the outputs, copies and synchronises (as ulens_lightcurve_binary_host). */
+int  ulens_lightcurve_triple(ulens_ctx* ctx, int n_cfg, int n_epochs,
+               const double* theta_host, double u1, const double* t,
+               double* A_out, double* dA_out, double* err_out, uint32_t* status_out, void* stream);
+int  ulens_lightcurve_triple_host(ulens_ctx* ctx, int n_cfg, int n_epochs,
                const double* theta_host, double u1, const double* t_host,
                double* A_out_host, double* dA_out_host, double* err_out_host, uint32_t* status_out_host,
                void* stream);

@@ -20,7 +20,7 @@ ST_NIMG_SHIFT = 8
 KERNEL_NAMES = ["k_traj", "k_roots", "k_regions", "k_shoot", "k_finalize"]     # ULENS_K_* order
 
 EXPORTS = ["ulens_create", "ulens_destroy", "ulens_lens_binary", "ulens_lens_triple", "ulens_mag", "ulens_mag_grad",
-           "ulens_mag_host", "ulens_trajectory", "ulens_lightcurve_binary", "ulens_lightcurve_binary_host", "ulens_lightcurve_binary_ext", "ulens_lightcurve_binary_ext_host", "ulens_nll_marginal", "ulens_mag_point", "ulens_roots", "ulens_get_stats",
+           "ulens_mag_host", "ulens_trajectory", "ulens_lightcurve_binary", "ulens_lightcurve_binary_host", "ulens_lightcurve_triple", "ulens_lightcurve_triple_host", "ulens_lightcurve_binary_ext", "ulens_lightcurve_binary_ext_host", "ulens_nll_marginal", "ulens_mag_point", "ulens_roots", "ulens_get_stats",
            "ulens_reset_stats", "ulens_last_launch_count", "ulens_set_timing", "ulens_get_kernel_ms", "ulens_fp64_peak", "ulens_strerror",
            "ulens_last_cuda_error"]
 
@@ -71,6 +71,8 @@ def lib() -> C.CDLL:
         L.ulens_trajectory.argtypes = [vp, ip, ip, dp, vp, vp, vp, vp]
         L.ulens_lightcurve_binary.argtypes = [vp, ip, ip, dp, C.c_double, vp, vp, vp, vp, vp, vp]
         L.ulens_lightcurve_binary_host.argtypes = [vp, ip, ip, dp, C.c_double, vp, vp, vp, vp, vp, vp]
+        L.ulens_lightcurve_triple.argtypes = [vp, ip, ip, dp, C.c_double, vp, vp, vp, vp, vp, vp]
+        L.ulens_lightcurve_triple_host.argtypes = [vp, ip, ip, dp, C.c_double, vp, vp, vp, vp, vp, vp]
         L.ulens_lightcurve_binary_ext.argtypes = [vp, ip, ip, dp, C.c_double, vp, vp, C.c_double, vp, vp, vp, vp,
                                                   C.POINTER(C.c_int), vp]
         L.ulens_lightcurve_binary_ext_host.argtypes = [vp, ip, ip, dp, C.c_double, vp, vp, C.c_double, vp, vp, vp, vp,
@@ -191,19 +193,21 @@ class Context:
         return A_out, err_out, status_out
 
     def ulens_mag_grad(self, lenses, rho, u1, w_re, w_im, stream=None):
-        """As ulens_mag, plus dA/d(w_cx, w_cy, s, q, rho): returns (A, dA5 [n_cfg, n_pts, 5], err, status)."""
+        """As ulens_mag, plus dA/d(w_cx, w_cy, s, q, rho) (n_lens = 1, 2: [n_cfg, n_pts, 5]) or
+        dA/d(w_cx, w_cy, s, q, q3, r3, psi, rho) (n_lens = 3: [n_cfg, n_pts, 8]): returns (A, dA, err, status)."""
         torch = self._torch
         n_cfg, arr, rho, u1 = self._cfg_arrays(lenses, rho, u1)
         n_pts = w_re.numel() // max(n_cfg, 1)
         n = n_cfg * n_pts
         dev = w_re.device
+        nt = 8 if (n_cfg and arr[0].n_lens == 3) else 5
         A = torch.empty((n_cfg, n_pts), dtype=torch.float64, device=dev)
-        dA = torch.empty((n_cfg, n_pts, 5), dtype=torch.float64, device=dev)
+        dA = torch.empty((n_cfg, n_pts, nt), dtype=torch.float64, device=dev)
         err = torch.empty((n_cfg, n_pts), dtype=torch.float64, device=dev)
         st = torch.empty((n_cfg, n_pts), dtype=torch.int32, device=dev)
         _check(lib().ulens_mag_grad(self._h, n_cfg, n_pts, arr, _dptr(rho), _dptr(u1),
                                     _dev(w_re, torch.float64, n), _dev(w_im, torch.float64, n),
-                                    _dev(A, torch.float64, n), _dev(dA, torch.float64, 5 * n),
+                                    _dev(A, torch.float64, n), _dev(dA, torch.float64, nt * n),
                                     _dev(err, torch.float64, n), _dev(st, torch.int32, n), self._stream(stream)), self._h)
         return A, dA, err, st
 
@@ -260,6 +264,39 @@ class Context:
                                              _dev(dA, torch.float64, n_cfg * n_ep * 7) if want_dA else None,
                                              _dev(err, torch.float64, n_cfg * n_ep),
                                              _dev(st, torch.int32, n_cfg * n_ep), self._stream(stream)), self._h)
+        return A, dA, err, st
+
+    def ulens_lightcurve_triple(self, theta, u1, t, want_dA=False, stream=None):
+        """theta: host [n_cfg, 10] (t0,u0,tE,s,q,rho,alpha,q3,r3,psi); t: CUDA float64 [n_epochs].
+        Returns (A, dA [n_cfg, n_epochs, 10] or None, err, st)."""
+        torch = self._torch
+        theta = np.ascontiguousarray(theta, dtype=np.float64).reshape(-1, 10)
+        n_cfg, n_ep = theta.shape[0], t.numel()
+        dev = t.device
+        A = torch.empty((n_cfg, n_ep), dtype=torch.float64, device=dev)
+        err = torch.empty((n_cfg, n_ep), dtype=torch.float64, device=dev)
+        st = torch.empty((n_cfg, n_ep), dtype=torch.int32, device=dev)
+        dA = torch.empty((n_cfg, n_ep, 10), dtype=torch.float64, device=dev) if want_dA else None
+        _check(lib().ulens_lightcurve_triple(self._h, n_cfg, n_ep, _dptr(theta), float(u1),
+                                             _dev(t, torch.float64, n_ep), _dev(A, torch.float64, n_cfg * n_ep),
+                                             _dev(dA, torch.float64, n_cfg * n_ep * 10) if want_dA else None,
+                                             _dev(err, torch.float64, n_cfg * n_ep),
+                                             _dev(st, torch.int32, n_cfg * n_ep), self._stream(stream)), self._h)
+        return A, dA, err, st
+
+    def ulens_lightcurve_triple_host(self, theta, u1, t, A, dA=None, err=None, st=None, stream=None):
+        """Host numpy arrays in / out: t [n_epochs]; A, err [n_cfg, n_epochs]; dA [n_cfg, n_epochs, 10] or None; st 32-bit."""
+        theta = np.ascontiguousarray(theta, dtype=np.float64).reshape(-1, 10)
+        t = np.ascontiguousarray(t, dtype=np.float64)
+        n_cfg, n_ep = theta.shape[0], t.size
+        for a, k in ((A, 1), (dA, 10), (err, 1)):
+            if a is not None and (a.dtype != np.float64 or not a.flags.c_contiguous or a.size != k * n_cfg * n_ep):
+                raise UlensError("output arrays must be C-contiguous float64 of the documented size")
+        if st is not None and (st.dtype.itemsize != 4 or not st.flags.c_contiguous or st.size != n_cfg * n_ep):
+            raise UlensError("status array must be C-contiguous 32-bit of n_cfg*n_epochs elements")
+        p = lambda a: a.ctypes.data_as(C.c_void_p) if a is not None else None
+        _check(lib().ulens_lightcurve_triple_host(self._h, n_cfg, n_ep, _dptr(theta), float(u1), p(t), p(A), p(dA),
+                                                  p(err), p(st), self._stream(stream)), self._h)
         return A, dA, err, st
 
     def ulens_lightcurve_binary_ext(self, theta, u1, t, ext_mask=None, sel_tol=0.0, want_dA=False, stream=None):

@@ -51,7 +51,7 @@ struct ulens_ctx {
     unsigned* c_mask;           // [chunk]     which of them are images
     // forward-mode variant (allocated on first use)
     PatchTan* ptans;            // [chunk][UL_MAXP] tangents of the sectors' radial bounds
-    double* unit_tan;           // [cap_units][UL_NT] tangent sums of the units
+    double* unit_tan; int unit_tan_nt;  // [cap_units][NT] tangent sums of the units
     double* grad5;              // [chunk][UL_NT] intrinsic gradient dA/d(w_cx, w_cy, s, q, rho)
     TangentTable* tan_dev; size_t tan_cap;
     unsigned* unit_desc;        // [cap_units]  (patch slot << 11) | line block (< 2048)
@@ -581,16 +581,23 @@ __global__ void k_finalize(int n, int pt_base, int n_pts_per_cfg, const PointCfg
 
 // ------------------------------------------------------------------------------------------------ forward-mode variant (a8)
 
-// k_shoot with tangents: same unit queue, same lines; every quantity of the line rule is a dual number with
-// UL_NT tangents (ulens_dual.cuh). The sector's radial grid moves with the image: r0' = r_lo', dr' = (r_hi' - r_lo') / n_r.
+// k_shoot with tangents: same unit queue, same lines. The scan accumulates, per line, the line sums U, S and two
+// tangent-statistic sets (ulens_dual.cuh); the NT directions (5 binary: w_cx, w_cy, s, q, rho; 8 triple: w_cx, w_cy,
+// s, q, q3, r3, psi, rho) only enter per LINE, when the sets are contracted with the configuration's tangent table.
+// The sector's grid moves with the image ACROSS the lines: x0' = lo' - kap_lo (hi' - lo'), dx' = (hi' - lo')(1 + kap_lo + kap_hi) / n.
+#ifndef UL_SHOOT_DUAL_MINB
+#define UL_SHOOT_DUAL_MINB 4
+#endif
 template <int N, bool LD>
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(128, UL_SHOOT_DUAL_MINB)
 k_shoot_dual(int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cfg, const TangentTable* __restrict__ tans,
              const double* __restrict__ w_re, const double* __restrict__ w_im, const Patch* __restrict__ patches,
              const PatchTan* __restrict__ ptans, const unsigned* __restrict__ unit_desc, double* __restrict__ unit_sum,
              double* __restrict__ unit_odd, double* __restrict__ unit_tan, unsigned* __restrict__ status,
-             ChunkCounters* cc, DevCounters* ctr, unsigned cap_units, int n_theta_opt, const int* __restrict__ pmap = nullptr)
+             ChunkCounters* cc, DevCounters* ctr, unsigned cap_units, const int* __restrict__ pmap = nullptr)
 {
+    constexpr int NT = TanDirs<N>::NT;
+    typedef Dual<NT> DN;
     const int lane = threadIdx.x & 31;
     const unsigned n_units = min(cc->n_units, cap_units);
     unsigned long long rays = 0;
@@ -601,7 +608,7 @@ k_shoot_dual(int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cfg, c
         if (u >= n_units) break;
         unsigned d = unit_desc[u];
         const Patch P = patches[d >> 11];
-        const PatchTan PT = ptans[d >> 11];
+        const PatchTan& PT = ptans[d >> 11];
         int blk = (int)(d & 0x7ffu);
         long long gp = pmap ? (long long)pmap[pt_base + P.point] : (long long)pt_base + P.point;
         int c = (int)(gp / n_pts_per_cfg);
@@ -613,23 +620,34 @@ k_shoot_dual(int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cfg, c
         // co-moving grid ACROSS the scan lines: the span's two ends follow the image's extreme
         // limb points; ALONG the lines the nodes are frozen (the margins there are generous)
         const bool scan_r = (P.flags & UL_PATCH_SCAN_R) != 0, periodic = (P.flags & UL_PATCH_PERIODIC) != 0;
-        D5 x0 = d5_const(scan_r ? P.th0 : P.r0), dx = d5_const(scan_r ? P.dth : P.dr);
+        DN x0 = dual_const<NT>(scan_r ? P.th0 : P.r0), dx = dual_const<NT>(scan_r ? P.dth : P.dr);
         const int n_lines = scan_r ? P.n_th : P.n_r;
         if (!(scan_r && periodic)) {
 #pragma unroll
-            for (int k = 0; k < UL_NT; ++k) {
+            for (int k = 0; k < NT; ++k) {
                 double lo = scan_r ? PT.tlo_dot[k] : PT.rlo_dot[k], hi = scan_r ? PT.thi_dot[k] : PT.rhi_dot[k];
                 x0.d[k] = lo - P.kap_lo * (hi - lo); dx.d[k] = (hi - lo) * (1.0 + P.kap_lo + P.kap_hi) / n_lines;
             }
         }
-        D5 xl, wl;
-        line_node_d(P.flags, n_lines, line, x0, dx, xl, wl);
-        D5 U, S, f; bool edge, clipped;
-        D5 rho_d = d5_const(rho);
+        DN xl, wl;
+        line_node_d<NT>(P.flags, n_lines, line, x0, dx, xl, wl);
+        DN U, S, f; bool edge, clipped;
+        {
+            TanStat<N> SU, SS;
+            if (scan_r) {
+                shoot_col_t<N, LD>(L, wcx, wcy, rho * rho, cos(xl.v), sin(xl.v), P.r0, P.dr, P.n_r, U.v, S.v, SU, SS, edge);
+                stat_contract<N, NT>(L, T, rho, SU, xl.d, 1.0, U.d);
+                if (LD) stat_contract<N, NT>(L, T, rho, SS, xl.d, P.dr, S.d);
+            } else {
+                shoot_ring_t<N, LD>(L, wcx, wcy, rho * rho, xl.v, P.th0, P.dth, P.n_th, periodic, U.v, S.v, SU, SS, edge);
+                stat_contract<N, NT>(L, T, rho, SU, xl.d, 1.0, U.d);
+                if (LD) stat_contract<N, NT>(L, T, rho, SS, xl.d, 1.0, S.d);
+            }
+            if (!LD) { S.v = 0.0; for (int k = 0; k < NT; ++k) S.d[k] = 0.0; }
+        }
+        DN rho_d = dual_const<NT>(rho);
 #pragma unroll
-        for (int k = 0; k < UL_NT; ++k) rho_d.d[k] = T.drho[k];
-        if (scan_r) shoot_col_d<N, LD>(L, T, wcx, wcy, rho, xl, d5_const(P.r0), d5_const(P.dr), P.n_r, U, S, edge);
-        else shoot_ring_d<N, LD>(L, T, wcx, wcy, rho, xl, P.th0, P.dth, P.n_th, periodic, U, S, edge);
+        for (int k = 0; k < NT; ++k) rho_d.d[k] = T.drho[k];
         if (P.flags & UL_PATCH_SINR) {
             // Tip caps. The sin-spaced lines crowd towards the two tips of the image, where a line
             // cuts a chord shorter than a few node spacings: harmless for the value (those lines weigh ~phi^2),
@@ -658,41 +676,35 @@ k_shoot_dual(int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cfg, c
                 else src = -1;
             }
             const int from = src < 0 ? lane : src;
-            D5 Uc, Sc;
-            Uc.v = __shfl_sync(0xffffffffu, U.v, from); Sc.v = __shfl_sync(0xffffffffu, S.v, from);
+            const double Ucv = __shfl_sync(0xffffffffu, U.v, from), Scv = __shfl_sync(0xffffffffu, S.v, from);
+            const double ku = (unresolved && src >= 0 && Ucv > 0.0) ? U.v / Ucv : 0.0;
+            const double ks = (unresolved && src >= 0 && Scv > 0.0) ? S.v / Scv : 0.0;
 #pragma unroll
-            for (int k = 0; k < UL_NT; ++k) {
-                Uc.d[k] = __shfl_sync(0xffffffffu, U.d[k], from); Sc.d[k] = __shfl_sync(0xffffffffu, S.d[k], from);
-            }
-            if (unresolved) {
-                const double ku = (src >= 0 && Uc.v > 0.0) ? U.v / Uc.v : 0.0;
-                const double ks = (src >= 0 && Sc.v > 0.0) ? S.v / Sc.v : 0.0;
-#pragma unroll
-                for (int k = 0; k < UL_NT; ++k) { U.d[k] = ku * Uc.d[k]; S.d[k] = ks * Sc.d[k]; }
+            for (int k = 0; k < NT; ++k) {
+                const double ud = __shfl_sync(0xffffffffu, U.d[k], from), sd = __shfl_sync(0xffffffffu, S.d[k], from);
+                if (unresolved) { U.d[k] = ku * ud; S.d[k] = ks * sd; }
             }
         }
+        f = U * (1.0 - u1);
+        if (LD) f = f + (S / rho_d) * u1;
         if (scan_r) {
-            f = U * (1.0 - u1);
-            if (LD) f += (S / rho_d) * u1;
             f = f * wl;
             clipped = edge || (!periodic && (line < 1 || line >= P.n_th - 1) && U.v > 0.0);
         } else {
-            f = U * (1.0 - u1);
-            if (LD) f += (S / rho_d) * u1;
             f = xl * f * wl * P.dth;
             clipped = edge || ((line < 1 || line >= P.n_r - 1) && U.v > 0.0 && P.r0 > 0.0);
         }
         double tot = warp_sum(f.v);
         double odd = warp_sum((lane & 1) ? f.v : 0.0);
-        double tk[UL_NT];
+        double tk[NT];
 #pragma unroll
-        for (int k = 0; k < UL_NT; ++k) tk[k] = warp_sum(f.d[k]);
+        for (int k = 0; k < NT; ++k) tk[k] = warp_sum(f.d[k]);
         unsigned any_clip = __ballot_sync(0xffffffffu, clipped);
         if (lane == 0) {
             unit_sum[u] = tot;
             unit_odd[u] = 2.0 * odd;
 #pragma unroll
-            for (int k = 0; k < UL_NT; ++k) unit_tan[(size_t)u * UL_NT + k] = tk[k];
+            for (int k = 0; k < NT; ++k) unit_tan[(size_t)u * NT + k] = tk[k];
             if (any_clip) atomicOr(&status[P.point], UL_ST_CLIPPED);
             rays += 32ull * (unsigned long long)(((P.flags & UL_PATCH_SCAN_R) ? P.n_r : P.n_th) + 4);
         }
@@ -702,10 +714,11 @@ k_shoot_dual(int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cfg, c
 
 // per point: ordered sum of the units' tangents, normalisation A = flux / F0(rho) differentiated:
 //   dA/dp_k = (dflux_k - A dF0_k) / F0,  F0 = pi rho^2 (1 - u1/3)
+template <int NT>
 __global__ void k_finalize_dual(int n, int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cfg,
                                 const TangentTable* __restrict__ tans, const Patch* __restrict__ patches,
                                 const int* __restrict__ n_patch, const double* __restrict__ unit_sum,
-                                const double* __restrict__ unit_tan, double* __restrict__ grad5, const int* __restrict__ pmap = nullptr,
+                                const double* __restrict__ unit_tan, double* __restrict__ grad, const int* __restrict__ pmap = nullptr,
                                 const unsigned* __restrict__ n_dev = nullptr, const unsigned* __restrict__ status_retry = nullptr)
 {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -717,19 +730,19 @@ __global__ void k_finalize_dual(int n, int pt_base, int n_pts_per_cfg, const Poi
     double rho = cfg[c].rho, u1 = cfg[c].u1;
     double F0 = UL_PI * rho * rho * (1.0 - u1 / 3.0);
     int np = n_patch[i];
-    double s = 0.0, tk[UL_NT];
-    for (int k = 0; k < UL_NT; ++k) tk[k] = 0.0;
+    double s = 0.0, tk[NT];
+    for (int k = 0; k < NT; ++k) tk[k] = 0.0;
     for (int p = 0; p < np; ++p) {
         const Patch& P = patches[(long long)i * UL_MAXP + p];
         for (int b = 0; b < P.n_units; ++b) {
             s += unit_sum[P.unit0 + b];
-            for (int k = 0; k < UL_NT; ++k) tk[k] += unit_tan[(size_t)(P.unit0 + b) * UL_NT + k];
+            for (int k = 0; k < NT; ++k) tk[k] += unit_tan[(size_t)(P.unit0 + b) * NT + k];
         }
     }
     double A = s / F0;
-    for (int k = 0; k < UL_NT; ++k) {
+    for (int k = 0; k < NT; ++k) {
         double dF0 = 2.0 * UL_PI * rho * (1.0 - u1 / 3.0) * tans[c].drho[k];
-        grad5[gp * UL_NT + k] = np ? (tk[k] - A * dF0) / F0 : nan("");
+        grad[gp * NT + k] = np ? (tk[k] - A * dF0) / F0 : nan("");
     }
 }
 
@@ -754,6 +767,47 @@ __global__ void k_chain7(int n_cfg, int n_ep, const double* __restrict__ theta, 
     o[4] = g[3];
     o[5] = g[4];
     o[6] = -g[0] * w_im[i] + g[1] * w_re[i];
+}
+
+
+// the same for the triple lens: (w_cx, w_cy, s, q, q3, r3, psi, rho) -> (t0, u0, tE, s, q, rho, alpha, q3, r3, psi)
+__global__ void k_chain10(int n_cfg, int n_ep, const double* __restrict__ theta, const double* __restrict__ t,
+                          const double* __restrict__ w_re, const double* __restrict__ w_im,
+                          const double* __restrict__ grad8, double* __restrict__ dA)
+{
+    long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= (long long)n_cfg * n_ep) return;
+    int c = (int)(i / n_ep), e = (int)(i % n_ep);
+    const double* th = theta + 10 * c;
+    double tE = th[2], tau = (t[e] - th[0]) / tE;
+    double ca = cos(th[6]), sa = sin(th[6]);
+    const double* g = grad8 + i * 8;
+    double along = g[0] * ca + g[1] * sa;
+    double* o = dA + i * 10;
+    o[0] = -along / tE;
+    o[1] = -g[0] * sa + g[1] * ca;
+    o[2] = -tau * along / tE;
+    o[3] = g[2];
+    o[4] = g[3];
+    o[5] = g[7];
+    o[6] = -g[0] * w_im[i] + g[1] * w_re[i];
+    o[7] = g[4];
+    o[8] = g[5];
+    o[9] = g[6];
+}
+
+// trajectory for the 10-parameter triple-lens vector (t0, u0, tE, s, q, rho, alpha, q3, r3, psi)
+__global__ void k_traj10(int n_cfg, int n_ep, const double* __restrict__ theta, const double* __restrict__ t,
+                         double* __restrict__ w_re, double* __restrict__ w_im)
+{
+    long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= (long long)n_cfg * n_ep) return;
+    int c = (int)(i / n_ep), e = (int)(i % n_ep);
+    const double* th = theta + 10 * c;
+    double tau = (t[e] - th[0]) / th[2];
+    double ca = cos(th[6]), sa = sin(th[6]);
+    w_re[i] = tau * ca - th[1] * sa;
+    w_im[i] = tau * sa + th[1] * ca;
 }
 
 
@@ -1012,10 +1066,14 @@ static int run_chunks(ulens_ctx* ctx, long long n_total, int n_pts, bool ld, con
     constexpr int DEG = N * N + 1;
     const bool dual = grad5_out != nullptr;
     const TangentTable* tans = dual ? ctx->tan_dev : nullptr;
-    if (dual && N == 3) return ULENS_EUNSUPPORTED;
+    constexpr int NT = TanDirs<N>::NT;
     if (dual && !ctx->ptans) {
         if (cudaMalloc(&ctx->ptans, sizeof(PatchTan) * UL_MAXP * (size_t)ctx->chunk) != cudaSuccess) return ULENS_ENOMEM;
-        if (cudaMalloc(&ctx->unit_tan, sizeof(double) * UL_NT * ctx->cap_units) != cudaSuccess) return ULENS_ENOMEM;
+    }
+    if (dual && ctx->unit_tan_nt < NT) {                 // [cap_units][NT]: sized for the widest tangent set seen so far
+        cudaFree(ctx->unit_tan); ctx->unit_tan = nullptr; ctx->unit_tan_nt = 0;
+        if (cudaMalloc(&ctx->unit_tan, sizeof(double) * NT * ctx->cap_units) != cudaSuccess) return ULENS_ENOMEM;
+        ctx->unit_tan_nt = NT;
     }
     // warps (= source points) per CTA of k_regions: the degree-10 work area is 30 KB per warp, so 4 warps per CTA
     // would leave one CTA per SM; 2 per CTA lets three CTAs share the SM's shared memory (measured on C3)
@@ -1040,25 +1098,25 @@ static int run_chunks(ulens_ctx* ctx, long long n_total, int n_pts, bool ld, con
         }
         // persistent grid: as many CTAs as are resident at once (occupancy API; 4-6 per SM by register count)
         int per_sm = 4;
-        if (!dual) {
+        if (dual) {
+            if (ld) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_shoot_dual<N, true>, 128, 0);
+            else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_shoot_dual<N, false>, 128, 0);
+        } else {
             if (ld) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_shoot<N, true>, 128, 0);
             else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_shoot<N, false>, 128, 0);
-            if (per_sm < 1) per_sm = 1;
         }
+        if (per_sm < 1) per_sm = 1;
         int grid = sm_count * per_sm;
         {
             KTimer kt(ctx, ULENS_K_SHOOT, st);
-            if constexpr (N < 3) {
-                if (dual && ld)
-                    k_shoot_dual<N, true><<<grid, 128, 0, st>>>((int)base, n_pts, ctx->cfg_dev, tans, w_re, w_im, ctx->patches, ctx->ptans,
-                                                                ctx->unit_desc, ctx->unit_sum, ctx->unit_odd, ctx->unit_tan, ctx->status_ws,
-                                                                ctx->cc, ctx->counters, (unsigned)ctx->cap_units, rp.n_theta, pmap);
-                else if (dual)
-                    k_shoot_dual<N, false><<<grid, 128, 0, st>>>((int)base, n_pts, ctx->cfg_dev, tans, w_re, w_im, ctx->patches, ctx->ptans,
-                                                                 ctx->unit_desc, ctx->unit_sum, ctx->unit_odd, ctx->unit_tan, ctx->status_ws,
-                                                                 ctx->cc, ctx->counters, (unsigned)ctx->cap_units, rp.n_theta, pmap);
-            }
-            if (dual) {}
+            if (dual && ld)
+                k_shoot_dual<N, true><<<grid, 128, 0, st>>>((int)base, n_pts, ctx->cfg_dev, tans, w_re, w_im, ctx->patches, ctx->ptans,
+                                                            ctx->unit_desc, ctx->unit_sum, ctx->unit_odd, ctx->unit_tan, ctx->status_ws,
+                                                            ctx->cc, ctx->counters, (unsigned)ctx->cap_units, pmap);
+            else if (dual)
+                k_shoot_dual<N, false><<<grid, 128, 0, st>>>((int)base, n_pts, ctx->cfg_dev, tans, w_re, w_im, ctx->patches, ctx->ptans,
+                                                             ctx->unit_desc, ctx->unit_sum, ctx->unit_odd, ctx->unit_tan, ctx->status_ws,
+                                                             ctx->cc, ctx->counters, (unsigned)ctx->cap_units, pmap);
             else if (ld)
                 k_shoot<N, true><<<grid, 128, 0, st>>>((int)base, n_pts, ctx->cfg_dev, w_re, w_im, ctx->patches, ctx->unit_desc,
                                                        ctx->unit_sum, ctx->unit_odd, ctx->status_ws, ctx->cc, ctx->counters, (unsigned)ctx->cap_units, pmap);
@@ -1072,7 +1130,7 @@ static int run_chunks(ulens_ctx* ctx, long long n_total, int n_pts, bool ld, con
                                                         ctx->unit_sum, ctx->unit_odd, ctx->status_ws, ctx->opt.rel_tol,
                                                         A_out, err_out, status_out, ctx->counters, pmap, n_dev, st_or);
             if (dual) {
-                k_finalize_dual<<<(n + 127) / 128, 128, 0, st>>>(n, (int)base, n_pts, ctx->cfg_dev, tans, ctx->patches, ctx->n_patch,
+                k_finalize_dual<NT><<<(n + 127) / 128, 128, 0, st>>>(n, (int)base, n_pts, ctx->cfg_dev, tans, ctx->patches, ctx->n_patch,
                                                                  ctx->unit_sum, ctx->unit_tan, grad5_out, pmap, n_dev, st_or ? status_out : nullptr);
                 ctx->last_launches += 1;
             }
@@ -1123,8 +1181,10 @@ static int retry_flagged(ulens_ctx* ctx, long long n_total, int n_pts, bool ld, 
                          ctx->ext_blk + n_blk, &rp2, UL_ST_RETRIED);
 }
 
-// tangent tables of the UL_NT intrinsic directions (w_cx, w_cy, s, q, rho). The lens-parameter directions
-// exist for a binary in the geometry of ulens_lens_binary (G4): s = a_2 - a_1, q = eps_2 / eps_1.
+// Tangent tables of the intrinsic directions (ulens_dual.cuh): binary / single (w_cx, w_cy, s, q, rho), triple
+// (w_cx, w_cy, s, q, q3, r3, psi, rho). The lens-parameter directions exist in the geometry of ulens_lens_binary
+// (G4: s = a_2 - a_1, q = eps_2 / eps_1, barycentre of M1, M2 at the origin) and ulens_lens_triple (G5: q3 = eps_3 / eps_1,
+// a_3 = midpoint of M1-M2 + r3 e^{i psi}); (s, q, q3, r3, psi) are recovered from the lens and the geometry is checked.
 static int upload_tangents(ulens_ctx* ctx, int n_cfg, const ulens_lens* lenses, cudaStream_t st)
 {
     if (ctx->last_tan_valid && ctx->tan_dev) return ULENS_OK;       // same lens array as the last call (upload_cfgs checked)
@@ -1132,16 +1192,30 @@ static int upload_tangents(ulens_ctx* ctx, int n_cfg, const ulens_lens* lenses, 
     for (int c = 0; c < n_cfg; ++c) {
         TangentTable& T = tt[c];
         memset(&T, 0, sizeof T);
-        T.dwx[0] = 1.0; T.dwy[1] = 1.0; T.drho[4] = 1.0;
         const ulens_lens& L = lenses[c];
-        if (L.n_lens == 2) {
-            double s = L.ax[1] - L.ax[0], q = L.eps[1] / L.eps[0];
+        const int NT = L.n_lens == 3 ? 8 : 5;
+        T.dwx[0] = 1.0; T.dwy[1] = 1.0; T.drho[NT - 1] = 1.0;
+        if (L.n_lens >= 2) {
+            const double s = L.ax[1] - L.ax[0], q = L.eps[1] / L.eps[0];
             if (L.ay[0] != 0.0 || L.ay[1] != 0.0 || fabs(L.eps[0] * L.ax[0] + L.eps[1] * L.ax[1]) > 1e-12 * (1.0 + fabs(s)))
-                return ULENS_EUNSUPPORTED;               // not the ulens_lens_binary geometry
-            double o = 1.0 / (1.0 + q);
+                return ULENS_EUNSUPPORTED;               // not the ulens_lens_binary / ulens_lens_triple geometry
+            const double o = 1.0 / (1.0 + q);
             T.dax[2][0] = -q * o; T.dax[2][1] = o;                       // d/ds
-            T.deps[3][0] = -o * o; T.deps[3][1] = o * o;                 // d/dq
-            T.dax[3][0] = -s * o * o; T.dax[3][1] = -s * o * o;
+            T.dax[3][0] = -s * o * o; T.dax[3][1] = -s * o * o;          // d/dq: positions
+            if (L.n_lens == 2) {
+                T.deps[3][0] = -o * o; T.deps[3][1] = o * o;             // d/dq: masses
+            } else {
+                const double q3 = L.eps[2] / L.eps[0], tot = 1.0 + q + q3, it2 = 1.0 / (tot * tot);
+                const double mid = 0.5 * (L.ax[0] + L.ax[1]);
+                const double r3x = L.ax[2] - mid, r3y = L.ay[2], r3 = sqrt(r3x * r3x + r3y * r3y);
+                if (!(r3 > 0.0)) return ULENS_EUNSUPPORTED;
+                T.dax[2][2] = 0.5 * (1.0 - q) * o;                       // the midpoint moves with s ...
+                T.dax[3][2] = -s * o * o;                                // ... and with q
+                T.deps[3][0] = -it2; T.deps[3][1] = (1.0 + q3) * it2; T.deps[3][2] = -q3 * it2;      // d/dq
+                T.deps[4][0] = -it2; T.deps[4][1] = -q * it2; T.deps[4][2] = (1.0 + q) * it2;        // d/dq3
+                T.dax[5][2] = r3x / r3; T.day[5][2] = r3y / r3;          // d/dr3
+                T.dax[6][2] = -r3y; T.day[6][2] = r3x;                   // d/dpsi
+            }
         }
     }
     if ((size_t)n_cfg > ctx->tan_cap) {
@@ -1163,7 +1237,6 @@ static int mag_device(ulens_ctx* ctx, int n_cfg, int n_pts, const ulens_lens* le
     int rc = upload_cfgs(ctx, n_cfg, lenses, rho, u1, st, &N, &ld);
     if (rc != ULENS_OK) return rc;
     if (grad5_out) {
-        if (N == 3) return ULENS_EUNSUPPORTED;
         rc = upload_tangents(ctx, n_cfg, lenses, st);
         if (rc != ULENS_OK) return rc;
     }
@@ -1319,6 +1392,85 @@ extern "C" int ulens_lightcurve_binary(ulens_ctx* ctx, int n_cfg, int n_epochs, 
         CK(cudaGetLastError());
     }
     return rc;
+}
+
+extern "C" int ulens_lightcurve_triple(ulens_ctx* ctx, int n_cfg, int n_epochs, const double* theta_host, double u1,
+                                       const double* t, double* A_out, double* dA_out, double* err_out,
+                                       uint32_t* status_out, void* stream)
+{
+    if (!ctx || n_cfg < 0 || n_epochs < 0) return ULENS_EINVAL;
+    if (n_cfg == 0 || n_epochs == 0) return ULENS_OK;
+    if (!theta_host || !t || !A_out || !(u1 >= 0.0 && u1 <= 1.0)) return ULENS_EINVAL;
+    CK(cudaSetDevice(ctx->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    std::vector<ulens_lens> lenses(n_cfg);
+    std::vector<double> rho(n_cfg), u1v(n_cfg, u1);
+    for (int c = 0; c < n_cfg; ++c) {
+        const double* th = theta_host + 10 * c;
+        for (int k = 0; k < 10; ++k) if (!isfinite(th[k])) return ULENS_EINVAL;
+        if (!(th[2] > 0.0)) return ULENS_EINVAL;
+        int rc = ulens_lens_triple(&lenses[c], th[3], th[4], th[7], th[8], th[9]);
+        if (rc != ULENS_OK) return rc;
+        rho[c] = th[5];
+    }
+    size_t n = (size_t)n_cfg * n_epochs;
+    if (n > (size_t)UL_MAX_POINTS) return ULENS_EUNSUPPORTED;
+    size_t need = 2 * n + 10 * (size_t)n_cfg + (dA_out ? 8 * n : 0);
+    if (need > ctx->traj_cap) {
+        cudaFree(ctx->traj_w); ctx->traj_w = nullptr; ctx->traj_cap = 0;
+        if (cudaMalloc(&ctx->traj_w, sizeof(double) * need) != cudaSuccess) return ULENS_ENOMEM;
+        ctx->traj_cap = need;
+    }
+    double* w_re = ctx->traj_w; double* w_im = w_re + n; double* th_dev = w_im + n;
+    double* g8 = dA_out ? th_dev + 10 * (size_t)n_cfg : nullptr;
+    {
+        int rcu = stage_upload(ctx, th_dev, theta_host, sizeof(double) * 10 * n_cfg, st);
+        if (rcu != ULENS_OK) return rcu;
+    }
+    {
+        KTimer kt(ctx, ULENS_K_TRAJ, st);
+        k_traj10<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(n_cfg, n_epochs, th_dev, t, w_re, w_im);
+    }
+    CK(cudaGetLastError());
+    int rc = mag_device(ctx, n_cfg, n_epochs, lenses.data(), rho.data(), u1v.data(), w_re, w_im, A_out, err_out, status_out, st, g8);
+    ctx->last_launches += 1;
+    if (rc != ULENS_OK) return rc;
+    if (dA_out) {
+        k_chain10<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(n_cfg, n_epochs, th_dev, t, w_re, w_im, g8, dA_out);
+        ctx->last_launches += 1;
+        CK(cudaGetLastError());
+    }
+    return rc;
+}
+
+extern "C" int ulens_lightcurve_triple_host(ulens_ctx* ctx, int n_cfg, int n_epochs, const double* theta_host, double u1,
+                                            const double* t_host, double* A_out_host, double* dA_out_host,
+                                            double* err_out_host, uint32_t* status_out_host, void* stream)
+{
+    if (!ctx || n_cfg < 0 || n_epochs < 0) return ULENS_EINVAL;
+    if (n_cfg == 0 || n_epochs == 0) return ULENS_OK;
+    if (!theta_host || !t_host || !A_out_host) return ULENS_EINVAL;
+    CK(cudaSetDevice(ctx->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t n = (size_t)n_cfg * n_epochs;
+    const size_t need = (size_t)n_epochs + n * (3 + (dA_out_host ? 10 : 0));   // t, A, err, status (8-byte slots), dA
+    if (need > ctx->io_cap) {
+        cudaFree(ctx->io_buf); ctx->io_buf = nullptr; ctx->io_cap = 0;
+        if (cudaMalloc(&ctx->io_buf, sizeof(double) * need) != cudaSuccess) return ULENS_ENOMEM;
+        ctx->io_cap = need;
+    }
+    double* d_t = ctx->io_buf; double* d_A = d_t + n_epochs; double* d_err = d_A + n;
+    unsigned* d_st = reinterpret_cast<unsigned*>(d_err + n);
+    double* d_dA = dA_out_host ? d_err + 2 * n : nullptr;
+    CK(cudaMemcpyAsync(d_t, t_host, sizeof(double) * n_epochs, cudaMemcpyHostToDevice, st));
+    int rc = ulens_lightcurve_triple(ctx, n_cfg, n_epochs, theta_host, u1, d_t, d_A, d_dA, d_err, d_st, stream);
+    if (rc != ULENS_OK) return rc;
+    CK(cudaMemcpyAsync(A_out_host, d_A, sizeof(double) * n, cudaMemcpyDeviceToHost, st));
+    if (dA_out_host) CK(cudaMemcpyAsync(dA_out_host, d_dA, sizeof(double) * 10 * n, cudaMemcpyDeviceToHost, st));
+    if (err_out_host) CK(cudaMemcpyAsync(err_out_host, d_err, sizeof(double) * n, cudaMemcpyDeviceToHost, st));
+    if (status_out_host) CK(cudaMemcpyAsync(status_out_host, d_st, sizeof(unsigned) * n, cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    return ULENS_OK;
 }
 
 extern "C" int ulens_lightcurve_binary_ext(ulens_ctx* ctx, int n_cfg, int n_epochs, const double* theta_host, double u1,

@@ -574,14 +574,28 @@ UL_HDN unsigned centre_images(const Lens& L, const LensPoly& T, double wx, doubl
 // App. A: ring quadrature along theta
 // ------------------------------------------------------------------------------------------------
 
-// zeta(-1/2, u) and zeta(-3/2, u) for u in (0, 1]: Hurwitz zeta = u^(-s) + zeta(s, 1+u); the smooth
-// part is a degree-9 Chebyshev fit on [0,1] (max error 7e-10 / 2e-10).
+// zeta(-1/2, u) and zeta(-3/2, u) for u in (0, 1]: Hurwitz zeta = u^(-s) + zeta(s, 1+u); the smooth part
+// zeta(s, 1+u) is a degree-9 least-squares fit on Chebyshev nodes of [0,1] (max error 7e-10 / 2e-10). The ONE copy
+// of the tables; paper_2510_02639_b200/csrc/fit_zeta_tables.py regenerates them (mpmath) and tests/test_host_logic.py
+// checks them against mpmath.zeta to 1e-9.
+#define UL_ZETA_M12_COEFFS {-0.207886224314425946, -0.730177387536053191, -0.326542433690562406, \
+                            0.0837832566266219698, -0.0435998186937335486, 0.0271396135617846347, \
+                            -0.0165300041688832568, 0.00823252937110980637, -0.00274063185833692022, \
+                            0.000434876090612478912}
+#define UL_ZETA_M32_COEFFS {-0.0254852020522020475, -0.311829304876540199, -0.547634035662697937, \
+                            -0.163258961591498412, 0.0313415948971861593, -0.0127998326381573904, \
+                            0.00616325441161647825, -0.00268571587959467142, 0.000828839924548779593, \
+                            -0.0001258385180165005}
+// value and derivative of the degree-9 polynomial c[0] + c[1] u + ...
+UL_HD void zeta_poly(const double (&c)[10], double u, double& p, double& dp)
+{
+    p = c[9]; dp = 0.0;
+#pragma unroll
+    for (int i = 8; i >= 0; --i) { dp = dp * u + p; p = p * u + c[i]; }
+}
 UL_HD double zeta_m12(double u)
 {
-    const double c[10] = {-0.207886224314425946, -0.730177387536053191, -0.326542433690562406,
-                          0.0837832566266219698, -0.0435998186937335486, 0.0271396135617846347,
-                          -0.0165300041688832568, 0.00823252937110980637, -0.00274063185833692022,
-                          0.000434876090612478912};
+    const double c[10] = UL_ZETA_M12_COEFFS;
     double p = c[9];
 #pragma unroll
     for (int i = 8; i >= 0; --i) p = p * u + c[i];
@@ -589,14 +603,27 @@ UL_HD double zeta_m12(double u)
 }
 UL_HD double zeta_m32(double u)
 {
-    const double c[10] = {-0.0254852020522020475, -0.311829304876540199, -0.547634035662697937,
-                          -0.163258961591498412, 0.0313415948971861593, -0.0127998326381573904,
-                          0.00616325441161647825, -0.00268571587959467142, 0.000828839924548779593,
-                          -0.0001258385180165005};
+    const double c[10] = UL_ZETA_M32_COEFFS;
     double p = c[9];
 #pragma unroll
     for (int i = 8; i >= 0; --i) p = p * u + c[i];
     return u * sqrt(u) + p;
+}
+// the same with d/du (forward-mode variant). d sqrt(u)/du is singular at u = 0 (a node exactly on the edge: the
+// rule is not differentiable there): that term is dropped below u = 1e-8
+UL_HD void zeta_m12_du(double u, double& z, double& dz)
+{
+    const double c[10] = UL_ZETA_M12_COEFFS;
+    double p, dp; zeta_poly(c, u, p, dp);
+    const double su = sqrt(u);
+    z = su + p; dz = (u > 1e-8 ? 0.5 / su : 0.0) + dp;
+}
+UL_HD void zeta_m32_du(double u, double& z, double& dz)
+{
+    const double c[10] = UL_ZETA_M32_COEFFS;
+    double p, dp; zeta_poly(c, u, p, dp);
+    const double su = sqrt(u);
+    z = u * su + p; dz = 1.5 * su + dp;
 }
 
 // F(z) = |w(z) - w_c|^2 - rho^2  (inside the source image <=> F < 0), one reciprocal per ray.

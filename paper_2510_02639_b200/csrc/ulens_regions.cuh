@@ -50,8 +50,8 @@ struct BoxExt {
 
 // dual variant only: how a sector's radial bounds move (d r_lo / d p_k, d r_hi / d p_k)
 struct PatchTan {
-    double rlo_dot[UL_NT], rhi_dot[UL_NT];
-    double tlo_dot[UL_NT], thi_dot[UL_NT];
+    double rlo_dot[UL_NT_MAX], rhi_dot[UL_NT_MAX];
+    double tlo_dot[UL_NT_MAX], thi_dot[UL_NT_MAX];
 };
 
 template <int DEG>
@@ -533,13 +533,14 @@ UL_HDN void regions_phaseB(int lane, RegionWork<DEG>& W)
 template <int N>
 UL_HD void patch_tangents(const Lens& L, const TangentTable& T, const BoxExt& x, bool from_origin, PatchTan& out)
 {
-    for (int k = 0; k < UL_NT; ++k) { out.rlo_dot[k] = 0.0; out.rhi_dot[k] = 0.0; out.tlo_dot[k] = 0.0; out.thi_dot[k] = 0.0; }
+    constexpr int NT = TanDirs<N>::NT;
+    for (int k = 0; k < UL_NT_MAX; ++k) { out.rlo_dot[k] = 0.0; out.rhi_dot[k] = 0.0; out.tlo_dot[k] = 0.0; out.thi_dot[k] = 0.0; }
     if (x.hi_r < 0.0) return;                           // no own point (links only): frozen
-    if (!from_origin) limb_point_rdot<N>(L, T, x.lo_x, x.lo_y, x.lo_ph, out.rlo_dot);
-    limb_point_rdot<N>(L, T, x.hi_x, x.hi_y, x.hi_ph, out.rhi_dot);
+    if (!from_origin) limb_point_rdot<N, NT>(L, T, x.lo_x, x.lo_y, x.lo_ph, out.rlo_dot);
+    limb_point_rdot<N, NT>(L, T, x.hi_x, x.hi_y, x.hi_ph, out.rhi_dot);
     if (x.thi_t > -1e299 && !from_origin) {             // theta ends (used by sectors scanned along radial lines)
-        limb_point_rdot<N>(L, T, x.tlo_x, x.tlo_y, x.tlo_ph, nullptr, out.tlo_dot);
-        limb_point_rdot<N>(L, T, x.thi_x, x.thi_y, x.thi_ph, nullptr, out.thi_dot);
+        limb_point_rdot<N, NT>(L, T, x.tlo_x, x.tlo_y, x.tlo_ph, nullptr, out.tlo_dot);
+        limb_point_rdot<N, NT>(L, T, x.thi_x, x.thi_y, x.thi_ph, nullptr, out.thi_dot);
     }
 }
 
@@ -814,7 +815,7 @@ UL_HDN int regions_phaseC(RegionWork<N * N + 1>& W, const RegionParams& P, int p
             rl = ul_min(rl, a1); rh = ul_max(rh, a2); hr = ul_min(hr, b.hr); ht = ul_min(ht, b.ht); cr = ul_min(cr, b.cr); ct = ul_min(ct, b.ct);
         }
         np = 0; units_left = P.max_units_pt;
-        for (int k = 0; k < UL_NT; ++k) { W.ptan[0].rlo_dot[k] = 0.0; W.ptan[0].rhi_dot[k] = 0.0; W.ptan[0].tlo_dot[k] = 0.0; W.ptan[0].thi_dot[k] = 0.0; }
+        for (int k = 0; k < UL_NT_MAX; ++k) { W.ptan[0].rlo_dot[k] = 0.0; W.ptan[0].rhi_dot[k] = 0.0; W.ptan[0].tlo_dot[k] = 0.0; W.ptan[0].thi_dot[k] = 0.0; }
         emit_patch(W.patch[np++], P, point, rl, rh, -UL_PI, UL_PI, hr, ht, cr, ct, true, false, rl, 1e300, 0.0, 0.0,
                    units_left, status);
     }
