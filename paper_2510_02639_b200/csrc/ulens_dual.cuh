@@ -178,8 +178,9 @@ UL_HD void stat_contract(const Lens& L, const TangentTable& T, double rho, const
 // in [0, 1]:  dx = - sum_k l_k(x) df_k / p'(x)   (implicit-function theorem: the Reynolds boundary term of P:163-175
 // for the discrete rule);  d p'(x) = sum_k l_k'(x) df_k + p''(x) dx,  d p''(x) = sum_k l_k''(x) df_k + p'''(x) dx;
 // u, sigma, tau and the Hurwitz-zeta end correction are smooth functions of (x, p', p'').
-UL_HD void edge_event_adj(double f0, double f1, double f2, double f3, bool want_S, double t2_extra,
-                          double& u, bool& entering, double& dS, double* au, double* aS)
+// (out of line: an event is rare next to the rays, and inlined at the flush site it costs the scan loops ~60 registers)
+UL_HDNI void edge_event_adj(double f0, double f1, double f2, double f3, bool want_S, double t2_extra,
+                            double& u, bool& entering, double& dS, double* au, double* aS)
 {
     // rows: coefficient of x^0..x^3; columns: f0..f3
     const double M1[4] = {-1.0 / 3.0, -0.5, 1.0, -1.0 / 6.0};
@@ -311,10 +312,12 @@ UL_HD void shoot_ring_t(const Lens& L, double wcx, double wcy, double rho2, doub
             pend = false;
         }
     };
-    for (int j = -2; j <= n_th + 1; ++j) {
+    // (one more pass than there are rays: the last one only flushes what is still pending -- one flush site)
+    for (int j = -2; j <= n_th + 2; ++j) {
+        const bool last = j > n_th + 1;
         RayCore<N> R;
         ray_core<N>(L, r * c, r * s, wcx, wcy, rho2, R);
-        const double f3 = R.F;
+        const double f3 = last ? UL_BIG : R.F;
         if (j >= 0 && j < n_th && f3 < 0.0) {
             U += 1.0;
             if (LD) {
@@ -326,16 +329,15 @@ UL_HD void shoot_ring_t(const Lens& L, double wcx, double wcy, double rho2, doub
             }
             if (!periodic && (j < 2 || j >= n_th - 2)) edge = true;
         }
-        const bool ev = j >= j_first && ((f1 < 0.0) != (f2 < 0.0));
+        const bool ev = !last && j >= j_first && ((f1 < 0.0) != (f2 < 0.0));
         // flush for the whole warp when a pending event is old enough or its lane meets its next crossing
-        if (UL_WARP_ANY(pend && (ev || j - pj >= UL_DEFER_D))) flush();
+        if (UL_WARP_ANY(pend && (ev || last || j - pj >= UL_DEFER_D))) flush();
         if (ev) { pj = j; pend = true; pen = !(f1 < 0.0); }
         f1 = f2; f2 = f3;
         const double cn = c * cd - s * sd;
         s = s * cd + c * sd;
         c = cn;
     }
-    flush();
     U_out = U; S_out = S;
 }
 
@@ -387,11 +389,12 @@ UL_HD void shoot_col_t(const Lens& L, double wcx, double wcy, double rho2, doubl
             pend = false;
         }
     };
-    for (int i = -2; i <= n_r + 1; ++i) {
+    for (int i = -2; i <= n_r + 2; ++i) {                 // (last pass: flush only)
+        const bool last = i > n_r + 1;
         const double r = r0 + dr * (i + 0.5);
         RayCore<N> R;
         ray_core<N>(L, r * c, r * s, wcx, wcy, rho2, R);
-        const double f3 = R.F;
+        const double f3 = last ? UL_BIG : R.F;
         if (i >= 0 && i < n_r && f3 < 0.0) {
             U += r;
             if (LD) {
@@ -404,12 +407,11 @@ UL_HD void shoot_col_t(const Lens& L, double wcx, double wcy, double rho2, doubl
             if ((i < 2 && r0 > 0.0) || i >= n_r - 2) edge = true;
         }
         // pair (i-2, i-1) = (f1, f2); the cell face between the pair must lie at r > 0
-        const bool ev = i >= 1 && ((f1 < 0.0) != (f2 < 0.0)) && (r0 + dr * (i - 1.0) > 0.0);
-        if (UL_WARP_ANY(pend && (ev || i - pi >= UL_DEFER_D))) flush();
+        const bool ev = !last && i >= 1 && ((f1 < 0.0) != (f2 < 0.0)) && (r0 + dr * (i - 1.0) > 0.0);
+        if (UL_WARP_ANY(pend && (ev || last || i - pi >= UL_DEFER_D))) flush();
         if (ev) { pi = i; pend = true; pen = !(f1 < 0.0); }
         f1 = f2; f2 = f3;
     }
-    flush();
     U_out = U * dr + U2; S_out = S * dr;
 }
 
