@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the ICRS hot path on B200 (contract: see the task statement / DESIGN.md "Measurement").
 
-One "step" = one pass of the whole hot path (k_traj -> k_roots -> k_regions -> k_shoot[_dual] -> k_finalize, SURVEY 8.a
+One "step" = one pass of the whole hot path (k_traj -> k_roots -> k_limb -> k_sectors -> k_shoot[_dual] -> k_finalize, SURVEY 8.a
 rows a1..a8) over one batch of synthetic input = every source point of the workload. Default workload: the largest
 single-GPU configuration of BASELINE.json, configs[4] ("C4": 1,024 parameter vectors x 2,000 epochs, binary lens,
 rho = 5e-3, u1 = 0.5; trajectory parameters in, A and the 7 forward-mode derivatives out; every epoch takes the
@@ -45,7 +45,7 @@ FP64_INSTR_PER_RAY = {(1, False): 27, (1, True): 32, (2, False): 35, (2, True): 
 # Forward-mode variant (binary, 5 intrinsic tangents): per tangent the moving ray dz (2), g conj(dz) (4), the explicit
 # lens-parameter term (0..8, mean 3), dF (4), accumulation (1) = 14, plus g itself (4 per ray): + 74 per ray.
 FP64_INSTR_PER_RAY_DUAL_EXTRA = 74
-# k_regions: algorithmic FP64-pipe instructions per limb solve: coefficients ~26 DEG, warm-started
+# k_limb: algorithmic FP64-pipe instructions per limb solve: coefficients ~26 DEG, warm-started
 # Ehrlich-Aberth 3 iterations x DEG roots x (8 DEG Horner + 12 (DEG-1) repulsion + 24), Eq.-1 polish of the
 # N+1..DEG images 2.5 iterations x (17 N + 25), boxes ~100.
 FP64_INSTR_PER_LIMB_SOLVE = {1: 600, 2: 2400, 3: 8300}
@@ -323,14 +323,16 @@ def measure_config(env: Env, cfg: int, steps: int, warmup: int, switch: bool = F
                                "MEASURED_PEAKS.json has no FP64 entry",
                 "fp64_instr_per_ray": ipr, "rays_per_launch": rays_per_launch,
                 "kernel_ms_avg": 1e3 * shoot_avg_s, "share_of_step": shoot_ms / ms}
-    reg_ms, reg_n = kms["k_regions"]
+    reg_ms, reg_n = kms["k_limb"]                          # the limb tracker; k_sectors (thread per point) is reported beside it
+    sec_ms, _ = kms["k_sectors"]
     solves_per_launch = stats["n_limb_solves"] / max(reg_n, 1)
     reg_ach = 2.0 * FP64_INSTR_PER_LIMB_SOLVE[n_lens] * solves_per_launch / (reg_ms * 1e-3 / max(reg_n, 1)) / 1e12
-    roofline_regions = {"bound": "alu", "kernel": "k_regions", "achieved": reg_ach, "peak": peak,
+    roofline_regions = {"bound": "alu", "kernel": "k_limb", "achieved": reg_ach, "peak": peak,
                         "unit": "TFLOP/s", "frac": reg_ach / peak, "traffic": None,
                         "fp64_instr_per_limb_solve": FP64_INSTR_PER_LIMB_SOLVE[n_lens],
                         "limb_solves_per_point": stats["n_limb_solves"] / steps / n,
-                        "kernel_ms_avg": reg_ms / max(reg_n, 1), "share_of_step": reg_ms / ms}
+                        "kernel_ms_avg": reg_ms / max(reg_n, 1), "share_of_step": (reg_ms + sec_ms) / ms,
+                        "share_note": "k_limb + k_sectors (the whole region builder, steps a3 + a4)"}
     out = {"wl": wl, "n": n, "value": value, "ms_per_step": ms_per_step, "e2e": e2e, "roofline": roofline,
            "roofline_regions": roofline_regions, "rays_per_s": env.world * rays_per_step / (ms_per_step * 1e-3),
            "rays_per_point": rays_per_step / n, "kernel_ms_per_step": {k: v[0] / steps for k, v in kms.items()},

@@ -244,10 +244,11 @@ int  ulens_last_launch_count(ulens_ctx* ctx);
  * ulens_set_timing(ctx, 1) call (which also clears the totals). */
 #define ULENS_K_TRAJ     0   /* trajectory -> source centres            (step a1) */
 #define ULENS_K_ROOTS    1   /* centre roots: polynomial, EA, polish    (step a2) */
-#define ULENS_K_REGIONS  2   /* limb images + sector builder            (steps a3, a4) */
-#define ULENS_K_SHOOT    3   /* ray shooting + ring quadrature          (steps a5, a6) */
+#define ULENS_K_LIMB     2   /* limb images -> boxes of the image arcs  (step a3, first half of a4) */
+#define ULENS_K_SHOOT    3   /* ray shooting + ring quadrature          (steps a5, a6; the forward-mode kernel for a8) */
 #define ULENS_K_FINALIZE 4   /* per-point sum, normalisation            (step a7) */
-#define ULENS_K_COUNT    5
+#define ULENS_K_SECTORS  5   /* boxes -> sectors -> work units          (second half of a4) */
+#define ULENS_K_COUNT    6
 int  ulens_set_timing(ulens_ctx* ctx, int on);
 int  ulens_get_kernel_ms(ulens_ctx* ctx, int which, double* ms_total, int* launches);
 

@@ -17,7 +17,7 @@ ULENS_OK, ULENS_EINVAL, ULENS_ECUDA, ULENS_ENOMEM, ULENS_EUNSUPPORTED = 0, -1, -
 ST_EA_NOCONV, ST_IMG_PARITY, ST_PATCH_CAP, ST_RES_CAP = 0x1, 0x2, 0x4, 0x8
 ST_CLIPPED, ST_UNIT_OVF, ST_ERR_HIGH, ST_NO_IMAGE = 0x10, 0x20, 0x40, 0x80
 ST_NIMG_SHIFT = 8
-KERNEL_NAMES = ["k_traj", "k_roots", "k_regions", "k_shoot", "k_finalize"]     # ULENS_K_* order
+KERNEL_NAMES = ["k_traj", "k_roots", "k_limb", "k_shoot", "k_finalize", "k_sectors"]     # ULENS_K_* order
 
 EXPORTS = ["ulens_create", "ulens_destroy", "ulens_lens_binary", "ulens_lens_triple", "ulens_mag", "ulens_mag_grad",
            "ulens_mag_host", "ulens_trajectory", "ulens_lightcurve_binary", "ulens_lightcurve_binary_host", "ulens_lightcurve_triple", "ulens_lightcurve_triple_host", "ulens_lightcurve_binary_ext", "ulens_lightcurve_binary_ext_host", "ulens_nll_marginal", "ulens_mag_point", "ulens_roots", "ulens_get_stats",

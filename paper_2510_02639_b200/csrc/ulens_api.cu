@@ -3,7 +3,8 @@
 // Pipeline per chunk of source points (all on the caller's stream, no host round trip in between):
 //   k_traj      (lightcurve entry only)  trajectory -> source centres
 //   k_roots     thread per point: lens polynomial, Ehrlich-Aberth, validate + polish         Eq. 4, 7
-//   k_regions   warp per point: limb images -> polar sectors -> 32-ring work units           Sec. 3.2
+//   k_limb      CTA per point, lane per root: limb images -> boxes of the image arcs          Sec. 3.2, Eq. 8
+//   k_sectors   thread per point: boxes -> polar sectors -> 32-line work units                 Sec. 3.2
 //   k_shoot     warp per work unit, lane per ring: rays along theta, edge events, ring sums  Sec. 3.3, App. A
 //   k_finalize  thread per point: ordered sum of its units, normalise                        Eq. A5
 //
@@ -18,8 +19,9 @@
 
 #include "../../include/ulens.h"
 #include "ulens_core.cuh"
-#include "ulens_regions.cuh"
 #include "ulens_dual.cuh"
+#include "ulens_regions.cuh"
+#include "ulens_limb.cuh"
 #include "ulens_host.hpp"
 
 using namespace ulens;
@@ -49,6 +51,9 @@ struct ulens_ctx {
     unsigned* status_ws;        // [chunk]
     double* c_zr; double* c_zi; // [chunk][10] roots of the source centre (k_roots -> k_regions)
     unsigned* c_mask;           // [chunk]     which of them are images
+    SubBox* boxes; int boxes_cap;       // [chunk][BoxCap] box lists of the points (k_limb -> k_sectors); boxes_cap = BoxCap allocated
+    BoxExt* exts; int exts_cap;         // forward-mode runs: the boxes' extreme own points
+    int* n_boxes;               // [chunk]
     // forward-mode variant (allocated on first use)
     PatchTan* ptans;            // [chunk][UL_MAXP] tangents of the sectors' radial bounds
     double* unit_tan; int unit_tan_nt;  // [cap_units][NT] tangent sums of the units
@@ -401,74 +406,89 @@ __global__ void k_ext_scatter(int n, const unsigned char* __restrict__ flag, con
     if (f) map[blk[blockIdx.x] + wsum[w] + __popc(b & ((1u << l) - 1u))] = i;
 }
 
-// One warp per source point.
-#ifndef UL_REGIONS_MINB
-#define UL_REGIONS_MINB 2
+// Image-region builder, first half (ulens_limb.cuh): one CTA per source point, a group of N^2+1 lanes per limb arc,
+// one lane per root. Writes the point's box list.
+#ifndef UL_LIMB_MINB
+#define UL_LIMB_MINB 2
 #endif
+template <int N, bool DUAL>
+__global__ void __launch_bounds__(LimbGeom<N>::THREADS, UL_LIMB_MINB)
+k_limb(int n, int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cfg, const LensPoly* __restrict__ poly,
+       const double* __restrict__ w_re, const double* __restrict__ w_im, RegionParams rp,
+       SubBox* __restrict__ boxes, BoxExt* __restrict__ exts, int* __restrict__ n_boxes, unsigned* __restrict__ status,
+       DevCounters* ctr, const double* __restrict__ c_zr, const double* __restrict__ c_zi,
+       const unsigned* __restrict__ c_mask, const int* __restrict__ pmap = nullptr, const unsigned* __restrict__ n_dev = nullptr)
+{
+    __shared__ LimbShared<N> sh;
+    __shared__ LensPoly sT;
+    const int i = blockIdx.x;
+    if (n_dev) n = min(n, (int)*n_dev - pt_base);
+    if (i >= n) return;                                  // whole CTA leaves together
+    const long long gp = pmap ? (long long)pmap[pt_base + i] : (long long)pt_base + i;
+    const int c = (int)(gp / n_pts_per_cfg);
+    if (threadIdx.x == 0) { sh.n_box = 0; sh.status = 0; sh.n_solves = 0; }
+    for (int k = threadIdx.x; k < (int)(sizeof(LensPoly) / sizeof(double)); k += blockDim.x)
+        reinterpret_cast<double*>(&sT)[k] = reinterpret_cast<const double*>(&poly[c])[k];
+    __syncthreads();
+    const Lens L = cfg[c].lens;
+    constexpr int CAP = BoxCap<N>::value;
+    limb_track<N, DUAL>(sh, L, sT, w_re[gp], w_im[gp], cfg[c].rho, rp, c_zr + (long long)i * 10, c_zi + (long long)i * 10,
+                        c_mask[i], boxes + (size_t)i * CAP, DUAL ? exts + (size_t)i * CAP : nullptr, CAP);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        n_boxes[i] = min(sh.n_box, CAP);
+        if (sh.status) status[i] |= sh.status;           // k_roots wrote the word first
+        atomicAdd(&ctr->n_limb_solves, (unsigned long long)sh.n_solves);
+    }
+}
+
+// Image-region builder, second half (ulens_regions.cuh sectors_from_boxes): one thread per source point turns the
+// box list into sectors, sizes their ray grids and claims their 32-line work units in the chunk's queue.
 template <int N>
-__global__ void __launch_bounds__(128, UL_REGIONS_MINB)
-k_regions(int n, int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cfg, const LensPoly* __restrict__ poly,
-          const double* __restrict__ w_re, const double* __restrict__ w_im, RegionParams rp,
-          Patch* __restrict__ patches, int* __restrict__ n_patch, unsigned* __restrict__ status,
+__global__ void __launch_bounds__(128)
+k_sectors(int n, int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cfg, const double* __restrict__ w_re,
+          const double* __restrict__ w_im, RegionParams rp, const SubBox* __restrict__ boxes, const BoxExt* __restrict__ exts,
+          const int* __restrict__ n_boxes, Patch* __restrict__ patches, int* __restrict__ n_patch, unsigned* __restrict__ status,
           unsigned* __restrict__ unit_desc, unsigned cap_units, ChunkCounters* cc, DevCounters* ctr,
-          const double* __restrict__ c_zr, const double* __restrict__ c_zi, const unsigned* __restrict__ c_mask,
           const TangentTable* __restrict__ tans, PatchTan* __restrict__ ptans, const int* __restrict__ pmap = nullptr,
           const unsigned* __restrict__ n_dev = nullptr)
 {
-    constexpr int DEG = N * N + 1;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    RegionWork<DEG>* Wall = reinterpret_cast<RegionWork<DEG>*>(smem_raw);
-    // dual run: the boxes' extreme points live behind the per-warp work areas
-    BoxExt* ext_all = reinterpret_cast<BoxExt*>(smem_raw + (blockDim.x >> 5) * sizeof(RegionWork<DEG>));
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    int i = blockIdx.x * (blockDim.x >> 5) + warp;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (n_dev) n = min(n, (int)*n_dev - pt_base);
-    if (i >= n) return;                                  // whole warp leaves together
-    RegionWork<DEG>& W = Wall[warp];
-    if (lane == 0) W.ext = tans ? ext_all + warp * 32 * DEG : nullptr;
-    __syncwarp();
-    long long gp = pmap ? (long long)pmap[pt_base + i] : (long long)pt_base + i;
-    int c = (int)(gp / n_pts_per_cfg);
-    Lens L = cfg[c].lens;
-    double rho = cfg[c].rho;
-    double wcx = w_re[gp], wcy = w_im[gp];
-    unsigned st = 0; int n_solves = 0;
-    regions_phaseA<N>(lane, L, poly[c], wcx, wcy, rho, rp, W, st, n_solves, c_zr + (long long)i * 10, c_zi + (long long)i * 10, c_mask[i]);
-    st = __reduce_or_sync(0xffffffffu, st);
-    const int tot_solves = __reduce_add_sync(0xffffffffu, n_solves);
-    __syncwarp();
-    regions_phaseB_keys<DEG>(lane, W);
-    __syncwarp();
-    regions_phaseB<DEG>(lane, W);
-    __syncwarp();
-    int np = 0; unsigned base = 0; int total_units = 0;
-    if (lane == 0) {
-        np = regions_phaseC<N>(W, rp, i, L, wcx, wcy, rho, st, tans ? &tans[c] : nullptr);
-        for (int p = 0; p < np; ++p) total_units += W.patch[p].n_units;
-        // claim the units with a compare-and-swap that REFUSES instead of overshooting, so the queue never holds an
-        // unwritten descriptor (the queue holds chunk x max_units_pt units: a refusal needs hand-made options)
-        {
-            unsigned cur = *(volatile unsigned*)&cc->n_units;
-            for (;;) {
-                if ((unsigned long long)cur + (unsigned)total_units > cap_units) { st |= UL_ST_UNIT_OVF; np = 0; total_units = 0; break; }
-                const unsigned prev = atomicCAS(&cc->n_units, cur, cur + (unsigned)total_units);
-                if (prev == cur) { base = cur; break; }
-                cur = prev;
-            }
+    if (i >= n) return;
+    const long long gp = pmap ? (long long)pmap[pt_base + i] : (long long)pt_base + i;
+    const int c = (int)(gp / n_pts_per_cfg);
+    const Lens L = cfg[c].lens;
+    constexpr int CAP = BoxCap<N>::value;
+    Patch* pp = patches + (long long)i * UL_MAXP;
+    PatchTan* pt = tans ? ptans + (long long)i * UL_MAXP : nullptr;
+    unsigned st = 0;
+    int np = sectors_from_boxes<N>(boxes + (size_t)i * CAP, tans ? exts + (size_t)i * CAP : nullptr, n_boxes[i], rp, i, L,
+                                   w_re[gp], w_im[gp], cfg[c].rho, st, tans ? &tans[c] : nullptr, pp, pt);
+    int total_units = 0;
+    for (int p = 0; p < np; ++p) total_units += pp[p].n_units;
+    // claim the units with a compare-and-swap that REFUSES instead of overshooting, so the queue never holds an
+    // unwritten descriptor (the queue holds chunk x max_units_pt units: a refusal needs hand-made options)
+    unsigned base = 0;
+    {
+        unsigned cur = *(volatile unsigned*)&cc->n_units;
+        for (;;) {
+            if ((unsigned long long)cur + (unsigned)total_units > cap_units) { st |= UL_ST_UNIT_OVF; np = 0; total_units = 0; break; }
+            const unsigned prev = atomicCAS(&cc->n_units, cur, cur + (unsigned)total_units);
+            if (prev == cur) { base = cur; break; }
+            cur = prev;
         }
-        int u = base;
-        for (int p = 0; p < np; ++p) { W.patch[p].unit0 = u; u += W.patch[p].n_units; patches[(long long)i * UL_MAXP + p] = W.patch[p]; if (tans) ptans[(long long)i * UL_MAXP + p] = W.ptan[p]; }
-        n_patch[i] = np;
-        status[i] |= st;                                 // k_roots wrote the word first
-        atomicAdd(&ctr->n_limb_solves, (unsigned long long)tot_solves);
-        atomicAdd(&ctr->n_patches, (unsigned long long)np);
     }
-    np = __shfl_sync(0xffffffffu, np, 0);
-    __syncwarp();
+    unsigned u = base;
     for (int p = 0; p < np; ++p) {
-        int nu = W.patch[p].n_units, u0 = W.patch[p].unit0;
-        for (int b = lane; b < nu; b += 32) unit_desc[u0 + b] = ((unsigned)(i * UL_MAXP + p) << 11) | (unsigned)b;
+        const int nu = pp[p].n_units;
+        pp[p].unit0 = (int)u;
+        for (int b = 0; b < nu; ++b) unit_desc[u + b] = ((unsigned)(i * UL_MAXP + p) << 11) | (unsigned)b;
+        u += nu;
     }
+    n_patch[i] = np;
+    if (st) status[i] |= st;
+    atomicAdd(&ctr->n_patches, (unsigned long long)np);
 }
 
 // One warp per 32-ring work unit, one lane per ring (Sec. 3.3; App. A). Units are pulled from a device counter.
@@ -949,6 +969,7 @@ extern "C" int ulens_create(ulens_ctx** out, int cuda_device, const ulens_option
     if (e == cudaSuccess) e = cudaMalloc(&ctx->c_zr, sizeof(double) * 10 * (size_t)ctx->chunk);
     if (e == cudaSuccess) e = cudaMalloc(&ctx->c_zi, sizeof(double) * 10 * (size_t)ctx->chunk);
     if (e == cudaSuccess) e = cudaMalloc(&ctx->c_mask, sizeof(unsigned) * (size_t)ctx->chunk);
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->n_boxes, sizeof(int) * (size_t)ctx->chunk);
     if (e == cudaSuccess) e = cudaMalloc(&ctx->unit_desc, sizeof(unsigned) * ctx->cap_units);
     if (e == cudaSuccess) e = cudaMalloc(&ctx->unit_sum, sizeof(double) * ctx->cap_units);
     if (e == cudaSuccess) e = cudaMalloc(&ctx->unit_odd, sizeof(double) * ctx->cap_units);
@@ -966,6 +987,7 @@ extern "C" void ulens_destroy(ulens_ctx* ctx)
     cudaSetDevice(ctx->device);
     cudaDeviceSynchronize();
     cudaFree(ctx->c_zr); cudaFree(ctx->c_zi); cudaFree(ctx->c_mask);
+    cudaFree(ctx->boxes); cudaFree(ctx->exts); cudaFree(ctx->n_boxes);
     cudaFree(ctx->ptans); cudaFree(ctx->unit_tan); cudaFree(ctx->grad5); cudaFree(ctx->tan_dev);
     cudaFree(ctx->patches); cudaFree(ctx->n_patch); cudaFree(ctx->status_ws); cudaFree(ctx->unit_desc);
     cudaFree(ctx->unit_sum); cudaFree(ctx->unit_odd); cudaFree(ctx->cc); cudaFree(ctx->counters);
@@ -1075,11 +1097,18 @@ static int run_chunks(ulens_ctx* ctx, long long n_total, int n_pts, bool ld, con
         if (cudaMalloc(&ctx->unit_tan, sizeof(double) * NT * ctx->cap_units) != cudaSuccess) return ULENS_ENOMEM;
         ctx->unit_tan_nt = NT;
     }
-    // warps (= source points) per CTA of k_regions: the degree-10 work area is 30 KB per warp, so 4 warps per CTA
-    // would leave one CTA per SM; 2 per CTA lets three CTAs share the SM's shared memory (measured on C3)
-    const int wpc = (N == 3) ? 2 : 4;
-    const size_t smem = wpc * sizeof(RegionWork<DEG>) + (dual ? wpc * 32 * DEG * sizeof(BoxExt) : 0);
-    CK(cudaFuncSetAttribute(k_regions<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    // box lists of one chunk, sized for the widest lens multiplicity seen so far (first use only)
+    constexpr int BCAP = BoxCap<N>::value;
+    if (ctx->boxes_cap < BCAP) {
+        cudaFree(ctx->boxes); ctx->boxes = nullptr; ctx->boxes_cap = 0;
+        if (cudaMalloc(&ctx->boxes, sizeof(SubBox) * BCAP * (size_t)ctx->chunk) != cudaSuccess) return ULENS_ENOMEM;
+        ctx->boxes_cap = BCAP;
+    }
+    if (dual && ctx->exts_cap < BCAP) {
+        cudaFree(ctx->exts); ctx->exts = nullptr; ctx->exts_cap = 0;
+        if (cudaMalloc(&ctx->exts, sizeof(BoxExt) * BCAP * (size_t)ctx->chunk) != cudaSuccess) return ULENS_ENOMEM;
+        ctx->exts_cap = BCAP;
+    }
     int sm_count = 148;
     cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, ctx->device);
     for (long long base = 0; base < n_total; base += ctx->chunk) {
@@ -1091,10 +1120,21 @@ static int run_chunks(ulens_ctx* ctx, long long n_total, int n_pts, bool ld, con
                                                         nullptr, nullptr, nullptr, ctx->status_ws, ctx->c_zr, ctx->c_zi, ctx->c_mask, nullptr, nullptr, pmap, n_dev);
         }
         {
-            KTimer kt(ctx, ULENS_K_REGIONS, st);
-            k_regions<N><<<(n + wpc - 1) / wpc, 32 * wpc, smem, st>>>(n, (int)base, n_pts, ctx->cfg_dev, ctx->poly_dev, w_re, w_im, rp,
-                                                         ctx->patches, ctx->n_patch, ctx->status_ws, ctx->unit_desc,
-                                                         (unsigned)ctx->cap_units, ctx->cc, ctx->counters, ctx->c_zr, ctx->c_zi, ctx->c_mask, tans, ctx->ptans, pmap, n_dev);
+            KTimer kt(ctx, ULENS_K_LIMB, st);
+            if (dual)
+                k_limb<N, true><<<n, LimbGeom<N>::THREADS, 0, st>>>(n, (int)base, n_pts, ctx->cfg_dev, ctx->poly_dev, w_re, w_im, rp,
+                                                                    ctx->boxes, ctx->exts, ctx->n_boxes, ctx->status_ws, ctx->counters,
+                                                                    ctx->c_zr, ctx->c_zi, ctx->c_mask, pmap, n_dev);
+            else
+                k_limb<N, false><<<n, LimbGeom<N>::THREADS, 0, st>>>(n, (int)base, n_pts, ctx->cfg_dev, ctx->poly_dev, w_re, w_im, rp,
+                                                                     ctx->boxes, ctx->exts, ctx->n_boxes, ctx->status_ws, ctx->counters,
+                                                                     ctx->c_zr, ctx->c_zi, ctx->c_mask, pmap, n_dev);
+        }
+        {
+            KTimer kt(ctx, ULENS_K_SECTORS, st);
+            k_sectors<N><<<(n + 127) / 128, 128, 0, st>>>(n, (int)base, n_pts, ctx->cfg_dev, w_re, w_im, rp, ctx->boxes, ctx->exts,
+                                                           ctx->n_boxes, ctx->patches, ctx->n_patch, ctx->status_ws, ctx->unit_desc,
+                                                           (unsigned)ctx->cap_units, ctx->cc, ctx->counters, tans, ctx->ptans, pmap, n_dev);
         }
         // persistent grid: as many CTAs as are resident at once (occupancy API; 4-6 per SM by register count)
         int per_sm = 4;
@@ -1135,7 +1175,7 @@ static int run_chunks(ulens_ctx* ctx, long long n_total, int n_pts, bool ld, con
                 ctx->last_launches += 1;
             }
         }
-        ctx->last_launches += 4;
+        ctx->last_launches += 5;
         CK(cudaGetLastError());
     }
     return ULENS_OK;

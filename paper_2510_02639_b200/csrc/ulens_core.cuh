@@ -173,10 +173,10 @@ UL_HD bool polish_image(const Lens& L, double wx, double wy, double& zx, double&
 // Eq. 4: coefficients b_0..b_DEG of the lens polynomial for source position w
 // ------------------------------------------------------------------------------------------------
 
+// e_0..e_N = elementary symmetric polynomials of c_i = conj(w) - conj(a_i), f_k = sum_i eps_i e_k(c without c_i)
 template <int N>
-UL_HD void poly_coeffs(const Lens& L, const LensPoly& T, double wx, double wy, double* br, double* bi)
+UL_HD void poly_sym(const Lens& L, double wx, double wy, double* ex, double* ey, double* fx, double* fy)
 {
-    constexpr int DEG = N * N + 1;
     // c_i = conj(w) - conj(a_i)
     double cx[N], cy[N];
 #pragma unroll
@@ -186,8 +186,6 @@ UL_HD void poly_coeffs(const Lens& L, const LensPoly& T, double wx, double wy, d
 #pragma unroll
     for (int i = 0; i < N; ++i)
         if (cx[i] * cx[i] + cy[i] * cy[i] < 1e-26) cx[i] += 1e-13;
-    // elementary symmetric polynomials e_0..e_N of c, and f_k = sum_i eps_i e_k(c \ c_i)
-    double ex[N + 1], ey[N + 1], fx[N], fy[N];
     ex[0] = 1.0; ey[0] = 0.0;
 #pragma unroll
     for (int k = 1; k <= N; ++k) { ex[k] = 0.0; ey[k] = 0.0; }
@@ -196,8 +194,9 @@ UL_HD void poly_coeffs(const Lens& L, const LensPoly& T, double wx, double wy, d
 #pragma unroll
         for (int k = N; k >= 1; --k) {
             if (k <= i + 1) {
-                ex[k] += ex[k - 1] * cx[i] - ey[k - 1] * cy[i];
-                ey[k] += ex[k - 1] * cy[i] + ey[k - 1] * cx[i];
+                double tx = ex[k - 1] * cx[i] - ey[k - 1] * cy[i];
+                double ty = ex[k - 1] * cy[i] + ey[k - 1] * cx[i];
+                ex[k] += tx; ey[k] += ty;
             }
         }
     }
@@ -217,6 +216,14 @@ UL_HD void poly_coeffs(const Lens& L, const LensPoly& T, double wx, double wy, d
         fx[2] = L.eps[0] * p12x + L.eps[1] * p02x + L.eps[2] * p01x;
         fy[2] = L.eps[0] * p12y + L.eps[1] * p02y + L.eps[2] * p01y;
     }
+}
+
+template <int N>
+UL_HD void poly_coeffs(const Lens& L, const LensPoly& T, double wx, double wy, double* br, double* bi)
+{
+    constexpr int DEG = N * N + 1;
+    double ex[N + 1], ey[N + 1], fx[N], fy[N];
+    poly_sym<N>(L, wx, wy, ex, ey, fx, fy);
     // S(z) = sum_k e_k T_k(z)   (degree N^2),  R(z) = sum_k f_k T_{k+1}(z)   (degree N^2)
     // P = (z - w) S - R :  b_l = S_{l-1} - w S_l - R_l
     double sr[DEG], si[DEG];          // S_0..S_{N^2}  (DEG = N^2+1 entries)

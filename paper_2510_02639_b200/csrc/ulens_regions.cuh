@@ -1,19 +1,15 @@
-// ulens_regions.cuh -- image-region (sector) builder: Eq. 8 limb sampling -> image-limb points ->
-// polar (r, theta) boxes -> 1-D interval grouping in r and theta -> sectors with margins and a ray
-// grid sized from the local image scale.   PAPER.md Sec. 3.2; readings G2, G8 in DESIGN.md.
+// ulens_regions.cuh -- image-region (sector) builder, second half: polar (r, theta) boxes of the image-limb
+// arcs -> 1-D interval grouping in r and theta -> sectors with margins and a ray grid sized from the local
+// image scale.   PAPER.md Sec. 3.2; readings G2, G8 in DESIGN.md.
 //
-// One warp builds the sectors of one source point. The work is written as phases that take the lane
-// index explicitly, so the same code is also callable lane by lane from a host logic test:
-//   phase A (32 lanes)  each lane follows n_limb/32 consecutive limb points (warm-started EA, Eq. 7),
-//                       validates / polishes every root on Eq. 1 and keeps, per root slot, the polar
-//                       bounding box of the image-limb points it saw (a piece of an image boundary);
-//                       slots whose validity flips between consecutive limb points (image pairs created
-//                       or destroyed on a caustic) are linked so that their boxes overlap.
-//   phase B (32 lanes)  rank-sort the boxes by lower r and by lower theta.
-//   phase C (lane 0)    sweep the sorted intervals -> r-groups, theta-groups (periodic); every occupied
-//                       (r-group, theta-group) cell becomes one sector ("all combinations of radial and
-//                       angular bins ... empty sectors are discarded, periodic ones merged"), refined to the
-//                       min/max of its members plus a margin, with n_r x n_theta from the local image scale.
+// The first half (Eq. 8 limb sampling, warm-started Ehrlich-Aberth, Eq.-1 polish, one box per image arc) is
+// k_limb in ulens_limb.cuh: a CTA per source point, a group of N^2+1 lanes per limb arc, one lane per root.
+// This file holds the box helpers both halves use and the per-point sector construction (k_sectors, one
+// THREAD per source point; plain C++, so tests/host_logic.cpp runs it on the CPU):
+//   boxes -> disjoint r-groups (interval union); inside each r-group its member boxes -> periodic theta-groups;
+//   every occupied (r-group, theta-group) cell becomes one sector ("all combinations of radial and
+//   angular bins ... empty sectors are discarded, periodic ones merged"), refined to the min/max of its
+//   members plus a margin, with n_r x n_theta from the local image scale.
 #pragma once
 #include "ulens_core.cuh"
 #include "ulens_dual.cuh"
@@ -54,18 +50,8 @@ struct PatchTan {
     double tlo_dot[UL_NT_MAX], thi_dot[UL_NT_MAX];
 };
 
-template <int DEG>
-struct RegionWork {
-    BoxExt* ext;            // [32 * DEG] or nullptr (primal run)
-    PatchTan ptan[UL_MAXP];
-    SubBox box[32 * DEG];
-    double key_r[32 * DEG], key_t[32 * DEG];   // lower r / lower theta of the expanded boxes (sort keys; empty: 1e300)
-    short order_r[32 * DEG], order_t[32 * DEG];
-    int n_sorted;
-    unsigned status;
-    int n_patch;
-    Patch patch[UL_MAXP];
-};
+// boxes per source point in the k_limb -> k_sectors buffer: one per (arc, root slot) plus room for arcs that split
+template <int N> struct BoxCap { static constexpr int value = (N == 1) ? 96 : (N == 2) ? 192 : 384; };
 
 UL_HD double wrap_pi(double a)      // to (-pi, pi]
 {
@@ -133,353 +119,6 @@ UL_HDNI void local_extents(double zx, double zy, double gx, double gy, double rh
     ct = 1.0 / sqrt(ss / (M * M) + cc / (m * m));
 }
 
-// ---------------------------------------------------------------------------------------------- phase A
-template <int N>
-UL_HDN void regions_phaseA(int lane, const Lens& L, const LensPoly& T, double wcx, double wcy, double rho,
-                           const RegionParams& P, RegionWork<N * N + 1>& W, unsigned& status, int& n_solves,
-                           const double* czr, const double* czi, unsigned cmask)
-{
-    constexpr int DEG = N * N + 1;
-    const int chunk = P.n_limb / 32;
-    SubBox* B = &W.box[lane * DEG];
-    double t_cur[DEG];              // per BOX: unwrapped theta of its last point
-    double lastx[DEG], lasty[DEG];  // per BOX: its last point
-    int bmap[DEG];                  // slot -> the box that slot's current arc writes to
-    double h_ph[DEG][2], h_r[DEG][2], h_t[DEG][2];   // per BOX: its last two own points (limb angle, r, theta)
-    int h_n[DEG];
-#pragma unroll
-    for (int j = 0; j < DEG; ++j) { bmap[j] = -1; lastx[j] = lasty[j] = 0.0; h_n[j] = 0; }
-    double zr[DEG], zi[DEG], ozr[DEG], ozi[DEG], pvx[DEG], pvy[DEG];
-    double br[DEG + 1], bi[DEG + 1];
-    unsigned valid_prev = 0, faint_prev = 0;
-    BoxExt* E = W.ext ? &W.ext[lane * DEG] : nullptr;
-    if (E) for (int j = 0; j < DEG; ++j) { E[j].lo_r = 1e300; E[j].hi_r = -1.0; E[j].lo_x = E[j].lo_y = E[j].lo_ph = E[j].hi_x = E[j].hi_y = E[j].hi_ph = 0.0;
-        E[j].tlo_t = 1e300; E[j].thi_t = -1e300; E[j].tlo_x = E[j].tlo_y = E[j].tlo_ph = E[j].thi_x = E[j].thi_y = E[j].thi_ph = 0.0; }
-#pragma unroll
-    for (int j = 0; j < DEG; ++j) { B[j].r_lo = 1.0; B[j].r_hi = -1.0; B[j].t_lo = B[j].t_hi = 0.0; B[j].hr = B[j].ht = B[j].cr = B[j].ct = 1e300; t_cur[j] = 0.0; pvx[j] = pvy[j] = 0.0; }
-
-    // The lane walks its arc of the limb, phi in [phi0, phi0 + chunk dphi], with an ADAPTIVE step: the base
-    // step is dphi = 2 pi / n_limb (Eq. 8); a step is halved and retried (down to dphi / 4096) when an image
-    // moved by more than ~4 % of its distance from the origin -- where the limb passes close to a lens or to a
-    // cusp the image boundary races along a long arc within a fraction of dphi and uniform limb sampling
-    // would leave most of that arc unsampled -- and (down to dphi / 8) when the set of images
-    // changed, which localises the creation / destruction of an image pair on a caustic.
-    // light lenses (eps_a < 1e-2) whose planetary caustic -- centred on w_a = a_a - sum_{b != a} eps_b/conj(a_a - a_b),
-    // a few sqrt(eps_a) across -- the source overlaps or nearly so
-    unsigned near_light = 0;
-    if (N == 3) {
-#pragma unroll
-        for (int a = 0; a < N; ++a) {
-            if (!(L.eps[a] < 1e-2)) continue;
-            double tx = L.ax[a] - wcx, ty = L.ay[a] - wcy;
-#pragma unroll
-            for (int b = 0; b < N; ++b) {
-                if (b == a) continue;
-                double dx = L.ax[a] - L.ax[b], dy = L.ay[a] - L.ay[b];
-                double i2 = L.eps[b] / (dx * dx + dy * dy);
-                tx -= dx * i2; ty -= dy * i2;
-            }
-            const double R = 8.0 * sqrt(L.eps[a]) + 2.0 * rho;
-            if (tx * tx + ty * ty < R * R) near_light |= 1u << a;
-        }
-    }
-    const double dphi = 2.0 * UL_PI / P.n_limb;
-    const double ph0 = dphi * (lane * chunk), ph_end = dphi * (lane * chunk + chunk);
-    double ph = ph0, step = dphi;
-    bool first = true;
-    int guard = 0;
-    while (first || ph < ph_end - 1e-9 * dphi) {
-        const int s = first ? 0 : 1;
-        double st_try = step;
-        if (ph + st_try > ph_end - 1e-9 * dphi) st_try = ph_end - ph;      // land exactly on the arc's end
-        const double ph_new = first ? ph0 : ph + st_try;
-        double wx = wcx + rho * cos(ph_new), wy = wcy + rho * sin(ph_new);      // Eq. 8 (G2)
-        poly_coeffs_ni<N>(L, T, wx, wy, br, bi);
-        // limb solves only have to land in the basin of the Eq.-1 polish: relative step 1e-7.
-        // Warm start from the previous limb point (cap 24); cold restart from the Cauchy circle (cap 64) for the
-        // arc's first point or when the warm solve hits its cap. One call site each (code size).
-        int it;
-        bool cold = first;
-        // Triple lens: continuation first. A slot that held an image at the previous limb point follows it by
-        // damped Newton on Eq. 1 itself (exact, and independent of the conditioning of the degree-10 polynomial,
-        // SURVEY 7-2). Those roots are then FROZEN in the simultaneous iteration -- they still repel the others
-        // (implicit deflation, Eq. 7) -- so Ehrlich-Aberth only has to move the roots that are not images, which
-        // is where image pairs are born. Measured on C3: 11 % faster step, 30 % fewer rays (no sectors from
-        // noisy roots next to the light lenses), fewer flagged points; for degree 5 the warm-started EA is
-        // already as cheap and the plain order is 6 % faster, so N <= 2 keeps it.
-        unsigned frozen = 0;
-        double c_det[DEG], c_gx[DEG], c_gy[DEG];
-        if (!first) {
-#pragma unroll
-            for (int j = 0; j < DEG; ++j) { ozr[j] = zr[j]; ozi[j] = zi[j]; }
-        }
-        if (N == 3 && !first) {
-#pragma unroll 1
-            for (int j = 0; j < DEG; ++j) {
-                if (!(valid_prev & (1u << j))) continue;
-                double zx = pvx[j], zy = pvy[j], detJ, resid, gx, gy;
-                bool ok = polish_image_ni<N>(L, wx, wy, zx, zy, 10, 1e-9, detJ, resid, gx, gy);
-                double jx = zx - pvx[j], jy = zy - pvy[j];
-                ok = ok && (jx * jx + jy * jy <= 0.0016 * ul_max(zx * zx + zy * zy, 0.04));
-                if (ok) {
-#pragma unroll 1
-                    for (int q = 0; q < j; ++q) {          // two slots running into one image: the pair merges
-                        if (!(frozen & (1u << q))) continue;
-                        double ddx = zx - zr[q], ddy = zy - zi[q];
-                        if (ddx * ddx + ddy * ddy < 1e-10 * ul_max(1.0, zx * zx + zy * zy)) ok = false;
-                    }
-                }
-                if (ok) { zr[j] = zx; zi[j] = zy; frozen |= 1u << j; c_det[j] = detJ; c_gx[j] = gx; c_gy[j] = gy; }
-            }
-        }
-#pragma unroll 1
-        for (;;) {
-            if (cold) { ea_init_ni<DEG>(br, bi, zr, zi); frozen = 0; }
-            it = ea_iterate_ni<DEG>(br, bi, zr, zi, cold ? 64 : 24, UL_EA_LIMB_TOL2, frozen);
-            if (cold || it <= 24) break;
-            cold = true;
-        }
-        if (!first) {
-            if (cold && it <= 64) it = 1;
-            match_roots<DEG>(ozr, ozi, zr, zi, frozen);  // slot j keeps following the same root
-        }
-        ++n_solves;
-        const bool noconv = (first && it > 64) || (!first && it > 24);
-
-        unsigned valid = 0, faint = 0;
-        double px[DEG], py[DEG], hrr[DEG], htt[DEG], crr[DEG], ctt[DEG];
-#pragma unroll 1
-        for (int j = 0; j < DEG; ++j) {
-            double zx = zr[j], zy = zi[j], detJ, resid, gx, gy;
-            bool ok;
-            if (frozen & (1u << j)) {                    // continued image: already exact
-                ok = true; detJ = c_det[j]; gx = c_gx[j]; gy = c_gy[j];
-            } else {
-            // distance of the EA root to the nearest lens bounds how far the polish may move it
-            double dm2 = 1e300;
-#pragma unroll
-            for (int i = 0; i < N; ++i) { double dx = zx - L.ax[i], dy = zy - L.ay[i]; dm2 = ul_min(dm2, dx * dx + dy * dy); }
-            // (0.04: the acceptance test below allows a total move of 10 % of that distance, so a first step
-            // beyond 20 % is rejected either way -- after one iteration instead of six)
-            ok = polish_image_ni<N>(L, wx, wy, zx, zy, 6, 1e-9, detJ, resid, gx, gy, 0.04);
-            // along the limb a slot must follow ONE image continuously: a polish that carries the EA root
-            // further than 10 % of its distance to the nearest lens has jumped to some other image
-            double mv2 = (zx - zr[j]) * (zx - zr[j]) + (zy - zi[j]) * (zy - zi[j]);
-            ok = ok && (mv2 <= 0.01 * dm2);
-            }
-            // continuation: a slot that held an image at the previous limb point and lost it (EA cannot
-            // resolve the root clusters next to a light lens in double) is re-polished from that image
-            if (!ok && (valid_prev & (1u << j)) && (N < 3 || cold)) {
-                zx = pvx[j]; zy = pvy[j];
-                ok = polish_image_ni<N>(L, wx, wy, zx, zy, 10, 1e-9, detJ, resid, gx, gy);
-                double jx = zx - pvx[j], jy = zy - pvy[j];
-                ok = ok && (jx * jx + jy * jy <= 0.0016 * ul_max(zx * zx + zy * zy, 0.04));
-            }
-            // two slots on one image: the later one is not an image of its own
-            if (ok) {
-#pragma unroll
-                for (int q = 0; q < DEG; ++q) {
-                    if (q >= j || !(valid & (1u << q))) continue;
-                    double ddx = zx - px[q], ddy = zy - py[q];
-                    if (ddx * ddx + ddy * ddy < 1e-10 * ul_max(1.0, zx * zx + zy * zy)) ok = false;
-                }
-            }
-            px[j] = zx; py[j] = zy;
-            if (ok) {
-                valid |= 1u << j;
-                zr[j] = zx; zi[j] = zy;                 // polished image = better warm start
-                local_extents(zx, zy, gx, gy, rho, hrr[j], htt[j], crr[j], ctt[j]);
-                // an image of magnification 1/|det J| < 1e-7 (the one sitting on top of a light lens) is
-                // tracked but gets no sector: at most N of them, i.e. < 3e-7 of A >= 1
-                if (fabs(detJ) > 1e7) faint |= 1u << j;
-            } else { hrr[j] = htt[j] = crr[j] = ctt[j] = 1e300; }
-        }
-        if (first) {
-            // seed the arc's first point from the images of the source CENTRE (step a2, found with an
-            // unrestricted polish, duplicates removed, faint images seeded): damped Newton on Eq. 1 for this
-            // limb point from each of them. Whatever it converges to is an image of the limb point; if no
-            // slot holds it yet it takes a free one.
-#pragma unroll 1
-            for (int m = 0; m < DEG; ++m) {
-                if (!(cmask & (1u << m))) continue;
-                double zx = czr[m], zy = czi[m], detJ, resid, gx, gy;
-                if (!polish_image_ni<N>(L, wx, wy, zx, zy, 12, 1e-9, detJ, resid, gx, gy)) continue;
-                bool dup = false;
-                int free_slot = -1;
-#pragma unroll
-                for (int q = 0; q < DEG; ++q) {
-                    if (valid & (1u << q)) {
-                        double ddx = zx - px[q], ddy = zy - py[q];
-                        if (ddx * ddx + ddy * ddy < 1e-10 * ul_max(1.0, zx * zx + zy * zy)) dup = true;
-                    } else if (free_slot < 0) free_slot = q;
-                }
-                if (dup || free_slot < 0) continue;
-                const int q = free_slot;
-                valid |= 1u << q; px[q] = zx; py[q] = zy; zr[q] = zx; zi[q] = zy;
-                local_extents(zx, zy, gx, gy, rho, hrr[q], htt[q], crr[q], ctt[q]);
-                if (fabs(detJ) > 1e7) faint |= 1u << q;
-            }
-        }
-        if (N == 3) {
-            // Wrong image parity at this limb point: images next to a light lens are hidden in the root cluster
-            // EA cannot resolve (see centre_images). Seed Eq. 1 from that lens's Einstein ring; whatever converges to
-            // an image no slot holds yet takes a free slot and is tracked by continuation from here on.
-            int nv = 0;
-#pragma unroll
-            for (int j = 0; j < DEG; ++j) nv += (valid >> j) & 1u;
-            const bool bad_parity = (((nv - (N + 1)) & 1) != 0 || nv < N + 1);
-            // A missing PAIR leaves the parity right. Where the source sits on the planetary caustic of a light lens
-            // (near_light, below) the ring is therefore seeded at every limb point.
-            if (bad_parity || near_light) {
-#pragma unroll 1
-                for (int a = 0; a < N; ++a) {
-                    if (!(L.eps[a] < 1e-2)) continue;
-                    if (!bad_parity && !(near_light & (1u << a))) continue;
-                    const double re = sqrt(L.eps[a]);
-#pragma unroll 1
-                    // all 8 directions at the arc's first point and on a wrong parity; otherwise the even and the odd
-                    // four on alternate limb points (an image, once found, is tracked by continuation)
-                    const int k_step = (first || bad_parity) ? 1 : 2, k_0 = (first || bad_parity) ? 0 : (n_solves & 1);
-                    for (int k = k_0; k < 8; k += k_step) {
-                        double zx = L.ax[a] + re * UL_RING8_X(k), zy = L.ay[a] + re * UL_RING8_Y(k), detJ, resid, gx, gy;
-                        if (!polish_image_ni<N>(L, wx, wy, zx, zy, 12, 1e-9, detJ, resid, gx, gy)) continue;
-                        bool dup = false;
-                        int free_slot = -1;
-#pragma unroll 1
-                        for (int q = 0; q < DEG; ++q) {
-                            if (valid & (1u << q)) {
-                                double ddx = zx - px[q], ddy = zy - py[q];
-                                if (ddx * ddx + ddy * ddy < 1e-10 * ul_max(1.0, zx * zx + zy * zy)) dup = true;
-                            } else if (free_slot < 0) free_slot = q;
-                        }
-                        if (dup || free_slot < 0) continue;
-                        const int q = free_slot;
-                        valid |= 1u << q; px[q] = zx; py[q] = zy; zr[q] = zx; zi[q] = zy;
-                        local_extents(zx, zy, gx, gy, rho, hrr[q], htt[q], crr[q], ctt[q]);
-                        if (fabs(detJ) > 1e7) faint |= 1u << q;
-                    }
-                }
-            }
-        }
-        if (!first && ++guard < 4096) {
-            // largest image displacement over this step, relative to the image's distance from the origin
-            bool too_far = false;
-#pragma unroll
-            for (int j = 0; j < DEG; ++j) {
-                if (!(valid & valid_prev & ~faint & (1u << j))) continue;
-                double dx = px[j] - pvx[j], dy = py[j] - pvy[j];
-                double z2 = px[j] * px[j] + py[j] * py[j];
-                if (dx * dx + dy * dy > 0.0016 * ul_max(z2, 0.04)) too_far = true;
-            }
-            const bool flipped = (valid != valid_prev);
-            if ((too_far && st_try > dphi * (1.0 / 4096.0)) || (flipped && st_try > dphi * 0.126)) {
-#pragma unroll
-                for (int j = 0; j < DEG; ++j) { zr[j] = ozr[j]; zi[j] = ozi[j]; }
-                step = 0.5 * st_try;
-                continue;                                 // retry from the previous point with half the step
-            }
-        }
-        if (noconv) status |= UL_ST_EA_NOCONV;
-        // own points
-#pragma unroll 1
-        for (int j = 0; j < DEG; ++j) {
-            if (!(valid & ~faint & (1u << j))) continue;
-            // A box holds ONE arc. If this slot's image is nowhere near the last point of its box (the slot
-            // swapped identity with another root, or lost its image and found a different one), its new
-            // arc goes to an unused box of this lane if there is one.
-            int bi = bmap[j];
-            const double far2 = 0.0036 * ul_max(px[j] * px[j] + py[j] * py[j], 0.04);
-            if (bi >= 0) {
-                double dx = px[j] - lastx[bi], dy = py[j] - lasty[bi];
-                if (dx * dx + dy * dy > far2) bi = -1;
-            }
-            if (bi < 0) {
-                // an empty box no slot writes to; failing that, the box whose last point is nearest
-                double bd = 1e300; int nearest = 0;
-                for (int b = 0; b < DEG && bi < 0; ++b) {
-                    bool in_use = false;
-                    for (int q = 0; q < DEG; ++q) in_use = in_use || (q != j && bmap[q] == b);
-                    if (B[b].r_lo > B[b].r_hi) { if (!in_use) bi = b; continue; }
-                    double dx = px[j] - lastx[b], dy = py[j] - lasty[b], d = dx * dx + dy * dy;
-                    if (d < bd) { bd = d; nearest = b; }
-                }
-                if (bi < 0) bi = nearest;
-                bmap[j] = bi;
-                h_n[bi] = 0;                             // a new arc starts: forget the old arc's samples
-            }
-            box_add(B[bi], t_cur[bi], sqrt(px[j] * px[j] + py[j] * py[j]), atan2(py[j], px[j]), hrr[j], htt[j], crr[j], ctt[j], true);
-            lastx[bi] = px[j]; lasty[bi] = py[j];
-            {
-                // bulge of the boundary between samples: vertex of the parabola through the last three
-                const double rr = sqrt(px[j] * px[j] + py[j] * py[j]), tt = t_cur[bi];
-                if (h_n[bi] >= 2) {
-                    double yv;
-                    if (parabola_vertex(h_ph[bi][0], h_r[bi][0], h_ph[bi][1], h_r[bi][1], ph_new, rr, yv)) {
-                        B[bi].r_lo = ul_min(B[bi].r_lo, ul_max(yv, 0.0)); B[bi].r_hi = ul_max(B[bi].r_hi, yv);
-                    }
-                    if (parabola_vertex(h_ph[bi][0], h_t[bi][0], h_ph[bi][1], h_t[bi][1], ph_new, tt, yv)) {
-                        B[bi].t_lo = ul_min(B[bi].t_lo, yv); B[bi].t_hi = ul_max(B[bi].t_hi, yv);
-                    }
-                }
-                h_ph[bi][0] = h_ph[bi][1]; h_r[bi][0] = h_r[bi][1]; h_t[bi][0] = h_t[bi][1];
-                h_ph[bi][1] = ph_new; h_r[bi][1] = rr; h_t[bi][1] = tt;
-                if (h_n[bi] < 2) ++h_n[bi];
-            }
-            if (E) {
-                double rr = sqrt(px[j] * px[j] + py[j] * py[j]);
-                if (rr < E[bi].lo_r) { E[bi].lo_r = rr; E[bi].lo_x = px[j]; E[bi].lo_y = py[j]; E[bi].lo_ph = ph_new; }
-                if (rr > E[bi].hi_r) { E[bi].hi_r = rr; E[bi].hi_x = px[j]; E[bi].hi_y = py[j]; E[bi].hi_ph = ph_new; }
-                if (t_cur[bi] < E[bi].tlo_t) { E[bi].tlo_t = t_cur[bi]; E[bi].tlo_x = px[j]; E[bi].tlo_y = py[j]; E[bi].tlo_ph = ph_new; }
-                if (t_cur[bi] > E[bi].thi_t) { E[bi].thi_t = t_cur[bi]; E[bi].thi_x = px[j]; E[bi].thi_y = py[j]; E[bi].thi_ph = ph_new; }
-            }
-        }
-        // links: a slot that switched off (its last point) or on (its first point) between s-1 and s is one
-        // half of an image pair destroyed / created on a critical curve somewhere between the two partners'
-        // end points: each partner's box takes the other's end point, so that the pair's boxes overlap.
-        // Partner = the nearest other switching slot, if closer than 0.5 (unrelated flips are not linked).
-        if (s > 0) {
-            unsigned off = valid_prev & ~valid, on = valid & ~valid_prev;
-            unsigned grp = off | on;
-            if (grp && (grp & (grp - 1))) {             // at least two members
-                double ex[DEG], ey[DEG];
-#pragma unroll
-                for (int a = 0; a < DEG; ++a) { ex[a] = (off & (1u << a)) ? pvx[a] : px[a]; ey[a] = (off & (1u << a)) ? pvy[a] : py[a]; }
-#pragma unroll 1
-                for (int a = 0; a < DEG; ++a) {
-                    if (!(grp & ~(faint | faint_prev) & (1u << a))) continue;
-                    int nb = -1; double bd = 0.25;
-#pragma unroll 1
-                    for (int b = 0; b < DEG; ++b) {
-                        if (b == a || !(grp & ~(faint | faint_prev) & (1u << b))) continue;
-                        double dx = ex[a] - ex[b], dy = ey[a] - ey[b];
-                        double d = dx * dx + dy * dy;
-                        if (d < bd) { bd = d; nb = b; }
-                    }
-                    if (nb >= 0) {
-                        double ra = sqrt(ex[a] * ex[a] + ey[a] * ey[a]), ta = atan2(ey[a], ex[a]);
-                        double rb = sqrt(ex[nb] * ex[nb] + ey[nb] * ey[nb]), tb = atan2(ey[nb], ex[nb]);
-                        if (bmap[nb] >= 0) box_add(B[bmap[nb]], t_cur[bmap[nb]], ra, ta, 1e300, 1e300, 1e300, 1e300, false);
-                        if (bmap[a] >= 0) box_add(B[bmap[a]], t_cur[bmap[a]], rb, tb, 1e300, 1e300, 1e300, 1e300, false);
-                    }
-                }
-            }
-        }
-#pragma unroll
-        for (int j = 0; j < DEG; ++j) { pvx[j] = px[j]; pvy[j] = py[j]; }
-        valid_prev = valid; faint_prev = faint;
-        if (!first) { ph = ph_new; step = ul_min(2.0 * st_try, dphi); }
-        first = false;
-    }
-    // normalise theta intervals: t_lo in [-pi, pi)
-#pragma unroll
-    for (int j = 0; j < DEG; ++j) {
-        if (B[j].r_lo > B[j].r_hi) continue;
-        double sh = 2.0 * UL_PI * floor((B[j].t_lo + UL_PI) / (2.0 * UL_PI));
-        B[j].t_lo -= sh; B[j].t_hi -= sh;
-        if (B[j].t_hi - B[j].t_lo > 2.0 * UL_PI) B[j].t_hi = B[j].t_lo + 2.0 * UL_PI;
-    }
-}
-
 // margins applied to every box before grouping: a quarter of the local minor scale in both directions
 // plus 2 % of the box itself (boundary bulge between limb samples)
 UL_HD void box_expanded(const SubBox& b, double& rl, double& rh, double& tl, double& th)
@@ -494,39 +133,6 @@ UL_HD void box_expanded(const SubBox& b, double& rl, double& rh, double& tl, dou
     mt = ul_min(mt, 0.5);
     rl = ul_max(b.r_lo - mr, 0.0); rh = b.r_hi + mr;
     tl = b.t_lo - mt; th = b.t_hi + mt;
-}
-
-// ---------------------------------------------------------------------------------------------- phase B
-template <int DEG>
-UL_HDN void regions_phaseB_keys(int lane, RegionWork<DEG>& W)
-{
-    const int n = 32 * DEG;
-    for (int i = lane; i < n; i += 32) {
-        const SubBox& b = W.box[i];
-        double rl = 1e300, rh, tl = 1e300, th;
-        if (!(b.r_lo > b.r_hi)) box_expanded(b, rl, rh, tl, th);
-        W.key_r[i] = rl; W.key_t[i] = tl;
-    }
-}
-
-// rank sort on the cached keys (call regions_phaseB_keys first, then synchronise the warp)
-template <int DEG>
-UL_HDN void regions_phaseB(int lane, RegionWork<DEG>& W)
-{
-    const int n = 32 * DEG;
-    for (int i = lane; i < n; i += 32) {
-        const double rl = W.key_r[i], tl = W.key_t[i];
-        if (rl >= 1e300) continue;
-        int rank_r = 0, rank_t = 0;
-        for (int j = 0; j < n; ++j) {
-            const double rl2 = W.key_r[j], tl2 = W.key_t[j];
-            if (rl2 >= 1e300 || j == i) continue;
-            rank_r += (rl2 < rl) || (rl2 == rl && j < i);
-            rank_t += (tl2 < tl) || (tl2 == tl && j < i);
-        }
-        W.order_r[rank_r] = (short)i;
-        W.order_t[rank_t] = (short)i;
-    }
 }
 
 // dual variant: tangents of a sector's radial bounds from its extreme image-limb points
@@ -619,48 +225,96 @@ UL_HD void emit_patch(Patch& out, const RegionParams& P, int point, double rl, d
     out.n_units = n_units;
 }
 
+
+UL_HD void ext_reset(BoxExt& x)
+{
+    x.lo_r = 1e300; x.hi_r = -1.0; x.lo_x = x.lo_y = x.lo_ph = x.hi_x = x.hi_y = x.hi_ph = 0.0;
+    x.tlo_t = 1e300; x.thi_t = -1e300; x.tlo_x = x.tlo_y = x.tlo_ph = x.thi_x = x.thi_y = x.thi_ph = 0.0;
+}
+
+// union of intervals, order independent: insert [lo, hi] into the list of disjoint groups, merging every group it
+// touches; at the cap the interval joins the nearest group instead of opening a new one
+UL_HD bool interval_absorb(double* g_lo, double* g_hi, int& ng, double lo, double hi)
+{
+    int first = -1;                                      // the group that has absorbed [lo, hi] so far
+    for (bool changed = true; changed;) {
+        changed = false;
+        for (int g = 0; g < ng; ++g) {
+            if (g == first || lo > g_hi[g] || hi < g_lo[g]) continue;
+            if (first < 0) { first = g; g_lo[g] = ul_min(g_lo[g], lo); g_hi[g] = ul_max(g_hi[g], hi); }
+            else {
+                g_lo[first] = ul_min(g_lo[first], g_lo[g]); g_hi[first] = ul_max(g_hi[first], g_hi[g]);
+                --ng; g_lo[g] = g_lo[ng]; g_hi[g] = g_hi[ng];
+                if (first == ng) first = g;
+            }
+            lo = g_lo[first]; hi = g_hi[first];
+            changed = true;                              // the grown group may touch groups already passed
+            break;
+        }
+    }
+    return first >= 0;
+}
+UL_HD void interval_insert(double* g_lo, double* g_hi, int& ng, double lo, double hi)
+{
+    if (interval_absorb(g_lo, g_hi, ng, lo, hi)) return;
+    if (ng < UL_MAXG) { g_lo[ng] = lo; g_hi[ng] = hi; ++ng; return; }
+    // at the cap: join the nearest group, then absorb whatever the grown group touches
+    int best = 0; double bd = 1e300;
+    for (int g = 0; g < ng; ++g) { double d = lo > g_hi[g] ? lo - g_hi[g] : g_lo[g] - hi; if (d < bd) { bd = d; best = g; } }
+    lo = ul_min(g_lo[best], lo); hi = ul_max(g_hi[best], hi);
+    --ng; g_lo[best] = g_lo[ng]; g_hi[best] = g_hi[ng];
+    if (!interval_absorb(g_lo, g_hi, ng, lo, hi)) { g_lo[ng] = lo; g_hi[ng] = hi; ++ng; }
+}
+
+UL_HD void interval_sort(double* g_lo, double* g_hi, int ng)
+{
+    for (int a = 1; a < ng; ++a) {
+        double lo = g_lo[a], hi = g_hi[a]; int b = a - 1;
+        while (b >= 0 && g_lo[b] > lo) { g_lo[b + 1] = g_lo[b]; g_hi[b + 1] = g_hi[b]; --b; }
+        g_lo[b + 1] = lo; g_hi[b + 1] = hi;
+    }
+}
+
+// a gap much narrower than the groups on both sides is the neck between two arcs of one image (an image
+// pair about to merge on a critical curve): one group, so that the sector ends where the image ends
+UL_HD void interval_merge_necks(double* g_lo, double* g_hi, int& ng)
+{
+    for (int g = 0; g + 1 < ng;) {
+        double gap = g_lo[g + 1] - g_hi[g];
+        if (gap < 0.05 * ul_min(g_hi[g] - g_lo[g], g_hi[g + 1] - g_lo[g + 1])) {
+            g_hi[g] = ul_max(g_hi[g], g_hi[g + 1]);
+            for (int k = g + 1; k + 1 < ng; ++k) { g_lo[k] = g_lo[k + 1]; g_hi[k] = g_hi[k + 1]; }
+            --ng;
+        } else ++g;
+    }
+}
+
 // Returns the number of sectors (0 if no image-limb point was found).
-// The paper's "1-D binning in r and theta, all combinations, empty ones dropped" as interval sweeps:
+// The paper's "1-D binning in r and theta, all combinations, empty ones dropped" as interval unions:
 // boxes -> disjoint r-groups; inside each r-group its member boxes -> periodic theta-groups; every
 // (r-group, theta-group) is one sector with the tight bounds of its members.
 // The boxes only follow image BOUNDARIES. A circle r = const that lies in a gap between two r-groups (or
 // inside the innermost one) meets no boundary, so it is entirely inside or entirely outside the image:
 // one ray on it decides. Where it is inside (ring-like image around the origin, or a disk that contains
 // the origin) the gap is filled: the groups on both sides merge into one full-ring sector.
+//   box [nb], ext [nb] or nullptr (forward-mode run: the boxes' extreme own points); patch / ptan [UL_MAXP] out.
 template <int N>
-UL_HDN int regions_phaseC(RegionWork<N * N + 1>& W, const RegionParams& P, int point, const Lens& L, double wcx,
-                          double wcy, double rho, unsigned& status, const TangentTable* TT = nullptr)
+UL_HDN int sectors_from_boxes(const SubBox* box, const BoxExt* ext, int nb, const RegionParams& P, int point, const Lens& L,
+                              double wcx, double wcy, double rho, unsigned& status, const TangentTable* TT, Patch* patch,
+                              PatchTan* ptan)
 {
-    constexpr int DEG = N * N + 1;
-    const int n = 32 * DEG;
-    int nb = 0;
-    for (int i = 0; i < n; ++i) nb += !(W.box[i].r_lo > W.box[i].r_hi);
-    W.n_sorted = nb;
-    W.n_patch = 0;
     if (nb == 0) { status |= UL_ST_NO_IMAGE; return 0; }
 
     // ---- r groups
     double gr_lo[UL_MAXG], gr_hi[UL_MAXG];
     int ngr = 0;
-    {
-        double cur_hi = -1.0;
-        for (int q = 0; q < nb; ++q) {
-            double rl, rh, tl, th;
-            box_expanded(W.box[W.order_r[q]], rl, rh, tl, th);
-            if (ngr == 0 || (rl > cur_hi && ngr < UL_MAXG)) { gr_lo[ngr] = rl; gr_hi[ngr] = rh; cur_hi = rh; ++ngr; }
-            else { cur_hi = ul_max(cur_hi, rh); gr_hi[ngr - 1] = cur_hi; }
-        }
+    for (int i = 0; i < nb; ++i) {
+        double rl, rh, tl, th;
+        box_expanded(box[i], rl, rh, tl, th);
+        interval_insert(gr_lo, gr_hi, ngr, rl, rh);
     }
-    // a gap much narrower than the groups on both sides is the neck between two arcs of one image (an image
-    // pair about to merge on a critical curve): one group, so that the sector ends where the image ends
-    for (int g = 0; g + 1 < ngr;) {
-        double gap = gr_lo[g + 1] - gr_hi[g];
-        if (gap < 0.05 * ul_min(gr_hi[g] - gr_lo[g], gr_hi[g + 1] - gr_lo[g + 1])) {
-            gr_hi[g] = gr_hi[g + 1];
-            for (int k = g + 1; k + 1 < ngr; ++k) { gr_lo[k] = gr_lo[k + 1]; gr_hi[k] = gr_hi[k + 1]; }
-            --ngr;
-        } else ++g;
-    }
+    interval_sort(gr_lo, gr_hi, ngr);
+    interval_merge_necks(gr_lo, gr_hi, ngr);
     // ---- fill gaps whose circles are inside the image
     bool ring_group[UL_MAXG];
     {
@@ -692,86 +346,98 @@ UL_HDN int regions_phaseC(RegionWork<N * N + 1>& W, const RegionParams& P, int p
         if (ring_group[a]) {
             // filled ring / disk: one full-ring sector scanned along radial lines
             double hr = 1e300, ht = 1e300, cr = 1e300, ct = 1e300;
-            BoxExt xlo; xlo.lo_r = 1e300; xlo.hi_r = -1.0; xlo.lo_x = xlo.lo_y = xlo.lo_ph = xlo.hi_x = xlo.hi_y = xlo.hi_ph = 0.0;
-            xlo.tlo_t = 1e300; xlo.thi_t = -1e300; xlo.tlo_x = xlo.tlo_y = xlo.tlo_ph = xlo.thi_x = xlo.thi_y = xlo.thi_ph = 0.0;   // full ring: theta frozen
-            for (int i = 0; i < n; ++i) {
-                const SubBox& b = W.box[i];
-                if (b.r_lo > b.r_hi) continue;
+            BoxExt xlo; ext_reset(xlo);                  // full ring: theta frozen
+            for (int i = 0; i < nb; ++i) {
+                const SubBox& b = box[i];
                 double rl, rh, tl, th;
                 box_expanded(b, rl, rh, tl, th);
                 if (!(rl >= gr_lo[a] && rl <= gr_hi[a])) continue;
                 hr = ul_min(hr, b.hr); ht = ul_min(ht, b.ht); cr = ul_min(cr, b.cr); ct = ul_min(ct, b.ct);
-                if (W.ext) {
-                    const BoxExt& e = W.ext[i];
+                if (ext) {
+                    const BoxExt& e = ext[i];
                     if (e.lo_r < xlo.lo_r) { xlo.lo_r = e.lo_r; xlo.lo_x = e.lo_x; xlo.lo_y = e.lo_y; xlo.lo_ph = e.lo_ph; }
                     if (e.hi_r > xlo.hi_r) { xlo.hi_r = e.hi_r; xlo.hi_x = e.hi_x; xlo.hi_y = e.hi_y; xlo.hi_ph = e.hi_ph; }
                 }
             }
             if (np == UL_MAXP) { capped = true; break; }
-            if (W.ext && TT) patch_tangents<N>(L, *TT, xlo, gr_lo[a] <= 0.0, W.ptan[np]);
-            emit_patch(W.patch[np++], P, point, gr_lo[a], gr_hi[a], -UL_PI, UL_PI, hr, ht, cr, ct, true, true,
+            if (ext && TT) patch_tangents<N>(L, *TT, xlo, gr_lo[a] <= 0.0, ptan[np]);
+            emit_patch(patch[np++], P, point, gr_lo[a], gr_hi[a], -UL_PI, UL_PI, hr, ht, cr, ct, true, true,
                        gap_r_lo, gap_r_hi, 0.0, 0.0, units_left, status);
             continue;
         }
-        // ---- theta groups of this r-group's members (periodic)
+        // ---- theta groups of this r-group's members: intervals on the circle, t_lo in [-pi, pi), span <= 2 pi
         double gt_lo[UL_MAXG], gt_hi[UL_MAXG];
         int ngt = 0;
-        {
-            double cur_hi = -1e300;
-            for (int q = 0; q < nb; ++q) {
-                double rl, rh, tl, th;
-                box_expanded(W.box[W.order_t[q]], rl, rh, tl, th);
-                if (!(rl >= gr_lo[a] && rl <= gr_hi[a])) continue;
-                if (ngt == 0 || (tl > cur_hi && ngt < UL_MAXG)) { gt_lo[ngt] = tl; gt_hi[ngt] = th; cur_hi = th; ++ngt; }
-                else { cur_hi = ul_max(cur_hi, th); gt_hi[ngt - 1] = cur_hi; }
-            }
-            for (int g = 0; g + 1 < ngt;) {               // necks, as for r
-                double gap = gt_lo[g + 1] - gt_hi[g];
-                if (gap < 0.05 * ul_min(gt_hi[g] - gt_lo[g], gt_hi[g + 1] - gt_lo[g + 1])) {
-                    gt_hi[g] = gt_hi[g + 1];
-                    for (int k = g + 1; k + 1 < ngt; ++k) { gt_lo[k] = gt_lo[k + 1]; gt_hi[k] = gt_hi[k + 1]; }
-                    --ngt;
+        bool full_ring = false;
+        for (int i = 0; i < nb && !full_ring; ++i) {
+            double rl, rh, tl, th;
+            box_expanded(box[i], rl, rh, tl, th);
+            if (!(rl >= gr_lo[a] && rl <= gr_hi[a])) continue;
+            // merge with every group it touches, in whichever turn of the circle they meet
+            for (int g = 0; g < ngt;) {
+                int k = 2;
+                if (!(tl > gt_hi[g] || th < gt_lo[g])) k = 0;
+                else if (!(tl + 2.0 * UL_PI > gt_hi[g] || th + 2.0 * UL_PI < gt_lo[g])) k = 1;
+                else if (!(tl - 2.0 * UL_PI > gt_hi[g] || th - 2.0 * UL_PI < gt_lo[g])) k = -1;
+                if (k != 2) {
+                    tl = ul_min(tl + 2.0 * UL_PI * k, gt_lo[g]); th = ul_max(th + 2.0 * UL_PI * k, gt_hi[g]);
+                    gt_lo[g] = gt_lo[ngt - 1]; gt_hi[g] = gt_hi[ngt - 1]; --ngt;
+                    g = 0;                               // the grown interval may now touch earlier groups
                 } else ++g;
             }
-            // wrap: the group reaching furthest past +pi swallows the leading groups it covers
-            for (;;) {
-                if (ngt <= 1) break;
-                int im = 0;
-                for (int g = 1; g < ngt; ++g) if (gt_hi[g] > gt_hi[im]) im = g;
-                if (im == 0 || gt_hi[im] - 2.0 * UL_PI < gt_lo[0]) break;
-                gt_hi[im] = ul_max(gt_hi[im], gt_hi[0] + 2.0 * UL_PI);
-                for (int g = 1; g < ngt; ++g) { gt_lo[g - 1] = gt_lo[g]; gt_hi[g - 1] = gt_hi[g]; }
-                --ngt;
-            }
-            for (int g = 0; g < ngt; ++g) if (gt_hi[g] - gt_lo[g] >= 2.0 * UL_PI) { gt_lo[0] = -UL_PI; gt_hi[0] = UL_PI; ngt = 1; break; }
+            if (th - tl >= 2.0 * UL_PI) { full_ring = true; break; }
+            const double sh = 2.0 * UL_PI * floor((tl + UL_PI) / (2.0 * UL_PI));      // t_lo back to [-pi, pi)
+            tl -= sh; th -= sh;
+            if (ngt < UL_MAXG) { gt_lo[ngt] = tl; gt_hi[ngt] = th; ++ngt; }
+            else { full_ring = true; }                   // more arcs than groups: one ring around them all
         }
-        const bool full_ring = (ngt == 1 && gt_hi[0] - gt_lo[0] >= 2.0 * UL_PI - 1e-12);
+        if (!full_ring) {
+            interval_sort(gt_lo, gt_hi, ngt);
+            interval_merge_necks(gt_lo, gt_hi, ngt);
+            // the neck between the last and the first group, across the cut at -pi / +pi
+            if (ngt > 1) {
+                double gap = gt_lo[0] + 2.0 * UL_PI - gt_hi[ngt - 1];
+                if (gap < 0.05 * ul_min(gt_hi[0] - gt_lo[0], gt_hi[ngt - 1] - gt_lo[ngt - 1])) {
+                    gt_hi[ngt - 1] = gt_hi[0] + 2.0 * UL_PI;
+                    for (int k = 0; k + 1 < ngt; ++k) { gt_lo[k] = gt_lo[k + 1]; gt_hi[k] = gt_hi[k + 1]; }
+                    --ngt;
+                }
+            }
+            for (int g = 0; g < ngt; ++g) if (gt_hi[g] - gt_lo[g] >= 2.0 * UL_PI - 1e-12) full_ring = true;
+        }
+        if (full_ring) { gt_lo[0] = -UL_PI; gt_hi[0] = UL_PI; ngt = 1; }
         // ---- tight bounds of each theta-group's members
         double c_rl[UL_MAXG], c_rh[UL_MAXG], c_tl[UL_MAXG], c_th[UL_MAXG], c_hr[UL_MAXG], c_ht[UL_MAXG], c_cr[UL_MAXG], c_ct[UL_MAXG];
-        BoxExt c_ext[UL_MAXG];
-        for (int g = 0; g < ngt; ++g) { c_ext[g].lo_r = 1e300; c_ext[g].hi_r = -1.0; c_ext[g].lo_x = c_ext[g].lo_y = c_ext[g].lo_ph = c_ext[g].hi_x = c_ext[g].hi_y = c_ext[g].hi_ph = 0.0;
-            c_ext[g].tlo_t = 1e300; c_ext[g].thi_t = -1e300; c_ext[g].tlo_x = c_ext[g].tlo_y = c_ext[g].tlo_ph = c_ext[g].thi_x = c_ext[g].thi_y = c_ext[g].thi_ph = 0.0; }
+        BoxExt c_ext[UL_MAXG];                           // forward-mode run: the cells' extreme own points
         for (int g = 0; g < ngt; ++g) { c_rl[g] = 1e300; c_rh[g] = -1e300; c_tl[g] = 1e300; c_th[g] = -1e300; c_hr[g] = c_ht[g] = c_cr[g] = c_ct[g] = 1e300; }
-        for (int i = 0; i < n; ++i) {
-            const SubBox& b = W.box[i];
-            if (b.r_lo > b.r_hi) continue;
+        if (ext) for (int g = 0; g < ngt; ++g) ext_reset(c_ext[g]);
+        for (int i = 0; i < nb; ++i) {
+            const SubBox& b = box[i];
             double rl, rh, tl, th;
             box_expanded(b, rl, rh, tl, th);
             if (!(rl >= gr_lo[a] && rl <= gr_hi[a])) continue;
             int c = 0;
             if (full_ring) { tl = -UL_PI; th = UL_PI; }
             else {
+                // the group (and the turn of the circle) this box's lower end lies in -- or lies nearest to: a group's
+                // ends went through +- 2 pi shifts while it was merged, so a member can miss it by a rounding error
+                double bd = 1e300; int bk = 0;
                 for (int g = 0; g < ngt; ++g) {
-                    if (tl >= gt_lo[g] && tl <= gt_hi[g]) { c = g; break; }
-                    if (tl + 2.0 * UL_PI >= gt_lo[g] && tl + 2.0 * UL_PI <= gt_hi[g]) { c = g; tl += 2.0 * UL_PI; th += 2.0 * UL_PI; break; }
+#pragma unroll
+                    for (int k = -1; k <= 1; ++k) {
+                        const double t = tl + 2.0 * UL_PI * k;
+                        const double d = ul_max(ul_max(gt_lo[g] - t, t - gt_hi[g]), 0.0);
+                        if (d < bd) { bd = d; c = g; bk = k; }
+                    }
                 }
+                tl += 2.0 * UL_PI * bk; th += 2.0 * UL_PI * bk;
             }
             c_rl[c] = ul_min(c_rl[c], rl); c_rh[c] = ul_max(c_rh[c], rh);
             c_tl[c] = ul_min(c_tl[c], tl); c_th[c] = ul_max(c_th[c], th);
             c_hr[c] = ul_min(c_hr[c], b.hr); c_ht[c] = ul_min(c_ht[c], b.ht);
             c_cr[c] = ul_min(c_cr[c], b.cr); c_ct[c] = ul_min(c_ct[c], b.ct);
-            if (W.ext) {
-                const BoxExt& e = W.ext[i];
+            if (ext) {
+                const BoxExt& e = ext[i];
                 BoxExt& x = c_ext[c];
                 if (e.lo_r < x.lo_r) { x.lo_r = e.lo_r; x.lo_x = e.lo_x; x.lo_y = e.lo_y; x.lo_ph = e.lo_ph; }
                 if (e.hi_r > x.hi_r) { x.hi_r = e.hi_r; x.hi_x = e.hi_x; x.hi_y = e.hi_y; x.hi_ph = e.hi_ph; }
@@ -788,7 +454,7 @@ UL_HDN int regions_phaseC(RegionWork<N * N + 1>& W, const RegionParams& P, int p
                 int cp = (c + ngt - 1) % ngt, cn = (c + 1) % ngt;
                 gap_lo = gt_lo[c] - gt_hi[cp]; if (c == 0) gap_lo += 2.0 * UL_PI;
                 gap_hi = gt_lo[cn] - gt_hi[c]; if (c == ngt - 1) gap_hi += 2.0 * UL_PI;
-                // a group shifted by the wrap merge may sit a full turn away
+                // a group that reaches across the cut may sit a full turn away
                 gap_lo -= 2.0 * UL_PI * floor(gap_lo / (2.0 * UL_PI));
                 gap_hi -= 2.0 * UL_PI * floor(gap_hi / (2.0 * UL_PI));
             }
@@ -799,8 +465,8 @@ UL_HDN int regions_phaseC(RegionWork<N * N + 1>& W, const RegionParams& P, int p
             // with theta up to the two tips, which the sin-spaced lines (UL_PATCH_SINR) take care of. A sector
             // that closes on itself in theta has no tips at all (spectral convergence).
             const bool scan_r = full_ring || ((c_th[c] - c_tl[c]) * c_rh[c] > (c_rh[c] - c_rl[c]));
-            if (W.ext && TT) patch_tangents<N>(L, *TT, c_ext[c], false, W.ptan[np]);
-            emit_patch(W.patch[np++], P, point, c_rl[c], c_rh[c], c_tl[c], c_th[c], c_hr[c], c_ht[c], c_cr[c], c_ct[c],
+            if (ext && TT) patch_tangents<N>(L, *TT, c_ext[c], false, ptan[np]);
+            emit_patch(patch[np++], P, point, c_rl[c], c_rh[c], c_tl[c], c_th[c], c_hr[c], c_ht[c], c_cr[c], c_ct[c],
                        full_ring, scan_r, gap_r_lo, gap_r_hi, gap_lo, gap_hi, units_left, status);
         }
     }
@@ -808,18 +474,16 @@ UL_HDN int regions_phaseC(RegionWork<N * N + 1>& W, const RegionParams& P, int p
         // more sectors than the cap: one full-ring sector around everything (never drop an image)
         status |= UL_ST_PATCH_CAP;
         double rl = 1e300, rh = 0.0, hr = 1e300, ht = 1e300, cr = 1e300, ct = 1e300;
-        for (int i = 0; i < n; ++i) {
-            const SubBox& b = W.box[i];
-            if (b.r_lo > b.r_hi) continue;
+        for (int i = 0; i < nb; ++i) {
+            const SubBox& b = box[i];
             double a1, a2, a3, a4; box_expanded(b, a1, a2, a3, a4);
             rl = ul_min(rl, a1); rh = ul_max(rh, a2); hr = ul_min(hr, b.hr); ht = ul_min(ht, b.ht); cr = ul_min(cr, b.cr); ct = ul_min(ct, b.ct);
         }
         np = 0; units_left = P.max_units_pt;
-        for (int k = 0; k < UL_NT_MAX; ++k) { W.ptan[0].rlo_dot[k] = 0.0; W.ptan[0].rhi_dot[k] = 0.0; W.ptan[0].tlo_dot[k] = 0.0; W.ptan[0].thi_dot[k] = 0.0; }
-        emit_patch(W.patch[np++], P, point, rl, rh, -UL_PI, UL_PI, hr, ht, cr, ct, true, false, rl, 1e300, 0.0, 0.0,
+        if (ptan) for (int k = 0; k < UL_NT_MAX; ++k) { ptan[0].rlo_dot[k] = 0.0; ptan[0].rhi_dot[k] = 0.0; ptan[0].tlo_dot[k] = 0.0; ptan[0].thi_dot[k] = 0.0; }
+        emit_patch(patch[np++], P, point, rl, rh, -UL_PI, UL_PI, hr, ht, cr, ct, true, false, rl, 1e300, 0.0, 0.0,
                    units_left, status);
     }
-    W.n_patch = np;
     return np;
 }
 
