@@ -454,30 +454,37 @@ k_sectors(int n, int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cf
           const unsigned* __restrict__ n_dev = nullptr)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int lane = threadIdx.x & 31;
     if (n_dev) n = min(n, (int)*n_dev - pt_base);
-    if (i >= n) return;
-    const long long gp = pmap ? (long long)pmap[pt_base + i] : (long long)pt_base + i;
-    const int c = (int)(gp / n_pts_per_cfg);
-    const Lens L = cfg[c].lens;
+    const bool live = i < n;                             // (no early return: the warp claims its units together)
     constexpr int CAP = BoxCap<N>::value;
     Patch* pp = patches + (long long)i * UL_MAXP;
-    PatchTan* pt = tans ? ptans + (long long)i * UL_MAXP : nullptr;
     unsigned st = 0;
-    int np = sectors_from_boxes<N>(boxes + (size_t)i * CAP, tans ? exts + (size_t)i * CAP : nullptr, n_boxes[i], rp, i, L,
+    int np = 0, total_units = 0;
+    if (live) {
+        const long long gp = pmap ? (long long)pmap[pt_base + i] : (long long)pt_base + i;
+        const int c = (int)(gp / n_pts_per_cfg);
+        const Lens L = cfg[c].lens;
+        PatchTan* pt = tans ? ptans + (long long)i * UL_MAXP : nullptr;
+        np = sectors_from_boxes<N>(boxes + (size_t)i * CAP, tans ? exts + (size_t)i * CAP : nullptr, n_boxes[i], rp, i, L,
                                    w_re[gp], w_im[gp], cfg[c].rho, st, tans ? &tans[c] : nullptr, pp, pt);
-    int total_units = 0;
-    for (int p = 0; p < np; ++p) total_units += pp[p].n_units;
-    // claim the units with a compare-and-swap that REFUSES instead of overshooting, so the queue never holds an
-    // unwritten descriptor (the queue holds chunk x max_units_pt units: a refusal needs hand-made options)
-    unsigned base = 0;
-    {
-        unsigned cur = *(volatile unsigned*)&cc->n_units;
-        for (;;) {
-            if ((unsigned long long)cur + (unsigned)total_units > cap_units) { st |= UL_ST_UNIT_OVF; np = 0; total_units = 0; break; }
-            const unsigned prev = atomicCAS(&cc->n_units, cur, cur + (unsigned)total_units);
-            if (prev == cur) { base = cur; break; }
-            cur = prev;
-        }
+        for (int p = 0; p < np; ++p) total_units += pp[p].n_units;
+    }
+    // one atomicAdd per warp: exclusive prefix sum of the lanes' unit counts, lane 31 holds the warp's total
+    unsigned incl = (unsigned)total_units;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const unsigned t = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += t; }
+    unsigned wbase = 0;
+    if (lane == 31 && incl) wbase = atomicAdd(&cc->n_units, incl);
+    wbase = __shfl_sync(0xffffffffu, wbase, 31);
+    unsigned base = wbase + incl - (unsigned)total_units;
+    if (!live) return;
+    // The queue holds chunk x max_units_pt units, so this cannot fail with the built-in per-point cap. If it does
+    // (hand-made options), the point is refused and the part of the queue it claimed is filled with void descriptors,
+    // which k_shoot skips: the queue never holds an unwritten descriptor.
+    if ((unsigned long long)base + (unsigned)total_units > cap_units) {
+        for (unsigned u = base; u < cap_units && u < base + (unsigned)total_units; ++u) unit_desc[u] = 0xffffffffu;
+        st |= UL_ST_UNIT_OVF; np = 0; total_units = 0;
     }
     unsigned u = base;
     for (int p = 0; p < np; ++p) {
@@ -488,7 +495,7 @@ k_sectors(int n, int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cf
     }
     n_patch[i] = np;
     if (st) status[i] |= st;
-    atomicAdd(&ctr->n_patches, (unsigned long long)np);
+    if (np) atomicAdd(&ctr->n_patches, (unsigned long long)np);
 }
 
 // One warp per 32-ring work unit, one lane per ring (Sec. 3.3; App. A). Units are pulled from a device counter.
@@ -511,6 +518,7 @@ k_shoot(int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cfg, const 
         u = __shfl_sync(0xffffffffu, u, 0);
         if (u >= n_units) break;
         unsigned d = unit_desc[u];
+        if (d == 0xffffffffu) continue;                  // void descriptor (refused point, k_sectors)
         const Patch P = patches[d >> 11];
         int blk = (int)(d & 0x7ffu);
         long long gp = pmap ? (long long)pmap[pt_base + P.point] : (long long)pt_base + P.point;
@@ -627,6 +635,7 @@ k_shoot_dual(int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cfg, c
         u = __shfl_sync(0xffffffffu, u, 0);
         if (u >= n_units) break;
         unsigned d = unit_desc[u];
+        if (d == 0xffffffffu) continue;                  // void descriptor (refused point, k_sectors)
         const Patch P = patches[d >> 11];
         const PatchTan& PT = ptans[d >> 11];
         int blk = (int)(d & 0x7ffu);
