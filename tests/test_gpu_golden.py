@@ -1,0 +1,143 @@
+"""Full-size parity evidence. Needs a B200.
+
+BASELINE configs C1-C3 are run at FULL size in the launch configuration bench.py times; then
+  (a) the stored oracle sample (tests/golden/oracle_C<cfg>.npz: >= 2,048 seeded stratified points per config, half
+      near-caustic, plus the light-body stratum; written by tests/golden/make_oracle_golden.py from oracle/ alone) is
+      compared point by point: every admissible point with a clean status must be within 1e-4; flagged points are
+      reported separately;
+  (b) limb-sampling sensitivity: the same workload with another n_limb. A correct result does not depend on where the
+      limb samples fall, so every point on which the two runs differ by more than 5e-5 is wrong in at least one of
+      them: the oracle decides (in the test, capped), and a run that is off by more than 1e-4 there must carry a
+      status bit;
+  (c) a random sample of the FLAGGED points is checked against the oracle and the fraction within 1e-4 printed.
+"""
+import os
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+TOL_A = 1e-4
+HERE = os.path.dirname(os.path.abspath(__file__))
+N_FLAGGED_SAMPLE = int(os.environ.get("ULENS_FLAGGED_SAMPLE", "16"))     # per config; profiles/ holds a run with 256
+_cache = {}
+
+
+def _lenses(binding, wl):
+    f = binding.ulens_lens_binary if wl.kind == "binary" else binding.ulens_lens_triple
+    return [f(*p) for p in wl.lens_params]
+
+
+def _olenses(O, wl):
+    f = O.lens_binary if wl.kind == "binary" else O.lens_triple
+    return [f(*p) for p in wl.lens_params]
+
+
+def _full(torch, cfg, n_limb=0):
+    """A, err, status of the whole config (cached per (cfg, n_limb))."""
+    key = (cfg, n_limb)
+    if key not in _cache:
+        from paper_2510_02639_b200 import binding, inputs
+        wl = inputs.get(cfg)
+        ctx = binding.Context(0, n_limb=n_limb)
+        w_re = torch.tensor(np.ascontiguousarray(wl.w.real), device="cuda:0")
+        w_im = torch.tensor(np.ascontiguousarray(wl.w.imag), device="cuda:0")
+        A, err, st = ctx.ulens_mag(_lenses(binding, wl), wl.rho, wl.u1, w_re, w_im)
+        torch.cuda.synchronize()
+        _cache[key] = (wl, A.cpu().numpy(), err.cpu().numpy(), st.cpu().numpy().astype(np.uint32))
+        ctx.close()
+    return _cache[key]
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3])
+def test_stored_oracle_sample_full_size(torch_cuda, cfg):
+    from paper_2510_02639_b200 import inputs
+    wl, A, err, st = _full(torch_cuda, cfg)
+    g = np.load(os.path.join(HERE, "golden", "oracle_C%d.npz" % cfg))
+    ci, pi, zone = inputs.golden_sample(wl, cfg)
+    assert np.array_equal(ci, g["cfg_index"]) and np.array_equal(pi, g["point_index"])      # the same seeded sample
+    assert np.array_equal(wl.w[ci, pi].real, g["w_re"]) and np.array_equal(wl.w[ci, pi].imag, g["w_im"])
+    assert len(ci) >= 2048 and g["near_caustic"].sum() >= 1024
+    adm = g["err_est"] <= 2e-5
+    rel = np.abs(A[ci, pi] / g["A"] - 1)
+    flagged = (st[ci, pi] & 0xff) != 0
+    clean = adm & ~flagged
+    bad_clean = clean & ~(rel <= TOL_A)
+    fl = adm & flagged
+    print("C%d stored oracle sample: %d points (%d near-caustic, %d in a light-body zone), admissible %d; clean %d: median %.1e  "
+          "p99 %.1e  max %.1e, > 1e-4: %d; flagged %d of which > 1e-4: %d (max %.1e); light-body zone max %.1e"
+          % (cfg, len(ci), int(g["near_caustic"].sum()), int(zone.sum()), int(adm.sum()), int(clean.sum()),
+             np.median(rel[clean]), np.quantile(rel[clean], 0.99), rel[clean].max(), int(bad_clean.sum()), int(fl.sum()),
+             int((rel[fl] > TOL_A).sum()), rel[fl].max() if fl.any() else 0.0,
+             rel[clean & zone].max() if (clean & zone).any() else 0.0))
+    assert adm.mean() >= 0.9
+    assert not bad_clean.any(), list(zip(ci[bad_clean][:8], pi[bad_clean][:8], rel[bad_clean][:8], A[ci, pi][bad_clean][:8]))
+    # flagged points carry a value too; a few may miss the bar (that is what the flag says), not most of them
+    assert (rel[fl] > TOL_A).sum() <= max(2, 0.25 * fl.sum())
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3])
+def test_limb_sampling_sensitivity_full_size(torch_cuda, oracle, cfg):
+    torch = torch_cuda
+    wl, A1, e1, s1 = _full(torch, cfg)                    # production: n_limb = 512
+    _, A2, e2, s2 = _full(torch, cfg, n_limb=704)         # other limb sampling (22 instead of 17 points per arc)
+    diff = np.abs(A1 / A2 - 1) > 5e-5
+    f1 = (s1 & 0xff) != 0
+    f2 = (s2 & 0xff) != 0
+    idx = np.argwhere(diff)
+    n_diff = len(idx)
+    n_unflagged_both = int((diff & ~f1 & ~f2).sum())
+    # the oracle decides on the differing points (capped: high-magnification points cost minutes of CPU each)
+    rng = np.random.default_rng(7)
+    if len(idx) > 48:
+        # all points unflagged in production first, then a random fill
+        pri = idx[~f1[idx[:, 0], idx[:, 1]]]
+        rest = idx[f1[idx[:, 0], idx[:, 1]]]
+        pick = np.concatenate([pri[:48], rest[rng.permutation(len(rest))[:max(0, 48 - len(pri))]]])
+    else:
+        pick = idx
+    n_chk = n_bad1 = n_bad2 = 0
+    if len(pick):
+        ci, pi = pick[:, 0], pick[:, 1]
+        ref = oracle.mag_fs_batch(_olenses(oracle, wl), ci.astype(np.int32), wl.w[ci, pi].real, wl.w[ci, pi].imag,
+                                  wl.rho[ci], wl.u1[ci], 100, 8)
+        adm = ref["err_est"] <= 2e-5
+        r1 = np.abs(A1[ci, pi] / ref["A"] - 1)
+        r2 = np.abs(A2[ci, pi] / ref["A"] - 1)
+        n_chk = int(adm.sum())
+        # a run that is off by more than the bar on such a point must say so in its status word
+        w1 = adm & (r1 > TOL_A) & ~f1[ci, pi]
+        w2 = adm & (r2 > TOL_A) & ~f2[ci, pi]
+        n_bad1, n_bad2 = int(w1.sum()), int(w2.sum())
+        print("C%d limb-sampling sensitivity (n_limb 512 vs 704, full size %d points): %d points differ by > 5e-5 "
+              "(%d flagged in production, %d flagged in neither run); oracle-checked %d: production > 1e-4 on %d (unflagged: %d), "
+              "other sampling > 1e-4 on %d (unflagged: %d)"
+              % (cfg, A1.size, n_diff, int((diff & f1).sum()), n_unflagged_both, n_chk, int((adm & (r1 > TOL_A)).sum()),
+                 n_bad1, int((adm & (r2 > TOL_A)).sum()), n_bad2))
+        assert n_bad1 == 0, list(zip(ci[w1], pi[w1], r1[w1]))
+        assert n_bad2 == 0, list(zip(ci[w2], pi[w2], r2[w2]))
+    else:
+        print("C%d limb-sampling sensitivity: no point differs by > 5e-5 between n_limb 512 and 704 (%d points)" % (cfg, A1.size))
+    assert n_diff <= 2e-3 * A1.size
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3])
+def test_flagged_points_vs_oracle(torch_cuda, oracle, cfg):
+    wl, A, err, st = _full(torch_cuda, cfg)
+    idx = np.argwhere((st & 0xff) != 0)
+    rng = np.random.default_rng(100 + cfg)
+    pick = idx[rng.permutation(len(idx))[:N_FLAGGED_SAMPLE]]
+    ci, pi = pick[:, 0], pick[:, 1]
+    ref = oracle.mag_fs_batch(_olenses(oracle, wl), ci.astype(np.int32), wl.w[ci, pi].real, wl.w[ci, pi].imag,
+                              wl.rho[ci], wl.u1[ci], 100, 8)
+    adm = ref["err_est"] <= 2e-5
+    rel = np.abs(A[ci, pi] / ref["A"] - 1)
+    bits = {hex(b): int(((st[ci, pi] & b) != 0).sum()) for b in (0x1, 0x2, 0x4, 0x8, 0x10, 0x40, 0x80)}
+    print("C%d flagged points: %d of %d in the workload; random sample of %d (status bits %s): admissible %d, within 1e-4: %d "
+          "(%.0f %%), median %.1e, max %.1e" % (cfg, len(idx), A.size, len(pick), bits, int(adm.sum()), int((rel[adm] <= TOL_A).sum()),
+                                               100.0 * (rel[adm] <= TOL_A).mean() if adm.any() else 0.0,
+                                               np.median(rel[adm]) if adm.any() else 0.0, rel[adm].max() if adm.any() else 0.0))
+    assert np.all(np.isfinite(A[ci, pi]))
+    assert adm.sum() >= 0.5 * len(pick)
+    assert (rel[adm] <= 10 * TOL_A).mean() >= 0.9         # flagged means doubtful, not garbage
