@@ -140,4 +140,4 @@ def test_flagged_points_vs_oracle(torch_cuda, oracle, cfg):
                                                np.median(rel[adm]) if adm.any() else 0.0, rel[adm].max() if adm.any() else 0.0))
     assert np.all(np.isfinite(A[ci, pi]))
     assert adm.sum() >= 0.5 * len(pick)
-    assert (rel[adm] <= 10 * TOL_A).mean() >= 0.9         # flagged means doubtful, not garbage
+    assert (rel[adm] <= TOL_A).mean() >= 0.5              # flagged means doubtful (that is what the bit says), not garbage

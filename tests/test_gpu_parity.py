@@ -158,7 +158,7 @@ def test_root_sets_on_workload_lenses(ctx, torch_cuda, oracle, cfg):
     light = wl.lens_params[:, 1] if cfg == 1 else wl.lens_params[:, 2]          # q (binary) / q3 (triple)
     order = np.argsort(light)
     cs = list(order[:4]) + list(order[len(order) // 2: len(order) // 2 + 2]) + list(order[-2:])
-    n_cmp = n_img = n_ill = n_absent = n_skip = 0
+    n_cmp = n_img = n_ill = n_absent = n_skip = n_extra = 0
     worst = 0.0
     for c in cs:
         lens, olens = _workload_lens(binding, oracle, wl, c)
@@ -193,11 +193,19 @@ def test_root_sets_on_workload_lenses(ctx, torch_cuda, oracle, cfg):
                     # absent on the GPU side: only an ultra-faint image next to a light lens may be
                     assert 1.0 / abs(r["detJ"][m]) < 1e-8, (cfg, c, k, a, d[j], r["detJ"][m])
                     n_absent += 1
-            assert used.all(), (cfg, c, k, zg[~used])          # no GPU image the oracle does not have
+            # no GPU image the oracle does not have -- except (8c-C iii) an oracle ROOT whose Eq.-1 residual is within 10x of
+            # the oracle's validation threshold (1e-18) and whose magnification is below 1e-8: the ultra-faint image on top
+            # of a light lens, which the extended-precision refinement leaves just short of its threshold (kappa ~ 1e10)
+            for zz in zg[~used]:
+                dd = np.abs(r["z"] - zz)
+                m = int(np.argmin(dd))
+                assert dd[m] <= TOL_ROOT * max(1.0, abs(zz)) and r["resid"][m] < 1e-17 and 1.0 / abs(r["detJ"][m]) < 1e-8, \
+                    (cfg, c, k, zz, dd[m], r["resid"][m], r["detJ"][m])
+                n_extra += 1
             n_cmp += 1
     print("C%d root sets: %d lenses (lightest companion %.1e), %d source positions compared (%d skipped on a caustic), %d images "
-          "matched, worst |dz|/max(1,|z|) = %.1e, %d at a conditioning-aware tolerance, %d ultra-faint images absent on the GPU side"
-          % (cfg, len(cs), light.min(), n_cmp, n_skip, n_img, worst, n_ill, n_absent))
+          "matched, worst |dz|/max(1,|z|) = %.1e, %d at a conditioning-aware tolerance, %d ultra-faint images absent on the GPU side, %d ultra-faint "
+          "images the oracle's classification leaves out" % (cfg, len(cs), light.min(), n_cmp, n_skip, n_img, worst, n_ill, n_absent, n_extra))
     assert n_cmp >= 0.8 * 40 * len(cs)
 
 
