@@ -67,6 +67,10 @@ extern "C" {
 typedef struct ulens_ctx ulens_ctx;
 
 #define ULENS_OPT_NO_RETRY   0x1      /* ulens_options.flags: do not re-integrate doubtful points (see ULENS_ST_RETRIED) */
+#define ULENS_OPT_F32_SHOOT  0x2      /* mixed-precision ray shooting: the rays of ulens_mag / ulens_lightcurve_* WITHOUT
+                                         derivatives run on the FP32 pipe in segment-local coordinates (cancellation-free difference
+                                         form of Eq. 1); segment constants, edge events and accumulation stay FP64. Same sectors, same
+                                         rule, same 1e-4 bar; the forward-mode variant always runs in FP64 */
 
 /* Tunables; a zeroed struct (or NULL) selects the defaults in brackets. */
 typedef struct {
@@ -255,6 +259,9 @@ int  ulens_get_kernel_ms(ulens_ctx* ctx, int which, double* ms_total, int* launc
 /* FP64 FMA roofline denominator: runs a dependent-chain-free DFMA kernel on every SM for about
  * `ms` milliseconds and returns the achieved rate in DFMA/s (one DFMA = 2 flop). Synchronises. */
 int  ulens_fp64_peak(ulens_ctx* ctx, double ms, double* dfma_per_s);
+
+/* The same for the FP32 pipe (FFMA/s): denominator of the mixed-precision variant's roofline. Synchronises. */
+int  ulens_fp32_peak(ulens_ctx* ctx, double ms, double* ffma_per_s);
 
 const char* ulens_strerror(int code);
 const char* ulens_last_cuda_error(ulens_ctx* ctx);

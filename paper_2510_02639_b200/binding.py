@@ -21,11 +21,12 @@ KERNEL_NAMES = ["k_traj", "k_roots", "k_limb", "k_shoot", "k_finalize", "k_secto
 
 EXPORTS = ["ulens_create", "ulens_destroy", "ulens_lens_binary", "ulens_lens_triple", "ulens_mag", "ulens_mag_grad",
            "ulens_mag_host", "ulens_trajectory", "ulens_lightcurve_binary", "ulens_lightcurve_binary_host", "ulens_lightcurve_triple", "ulens_lightcurve_triple_host", "ulens_lightcurve_binary_ext", "ulens_lightcurve_binary_ext_host", "ulens_nll_marginal", "ulens_mag_point", "ulens_roots", "ulens_get_stats",
-           "ulens_reset_stats", "ulens_last_launch_count", "ulens_set_timing", "ulens_get_kernel_ms", "ulens_fp64_peak", "ulens_strerror",
+           "ulens_reset_stats", "ulens_last_launch_count", "ulens_set_timing", "ulens_get_kernel_ms", "ulens_fp64_peak", "ulens_fp32_peak", "ulens_strerror",
            "ulens_last_cuda_error"]
 
 
 ULENS_OPT_NO_RETRY = 0x1
+ULENS_OPT_F32_SHOOT = 0x2
 ULENS_ST_RETRIED = 0x2000
 ULENS_ST_POINT_SRC = 0x1000
 
@@ -86,6 +87,7 @@ def lib() -> C.CDLL:
         L.ulens_set_timing.argtypes = [vp, ip]
         L.ulens_get_kernel_ms.argtypes = [vp, ip, dp, C.POINTER(C.c_int)]
         L.ulens_fp64_peak.argtypes = [vp, C.c_double, dp]
+        L.ulens_fp32_peak.argtypes = [vp, C.c_double, dp]
         L.ulens_strerror.argtypes = [ip]
         L.ulens_strerror.restype = C.c_char_p
         L.ulens_last_cuda_error.argtypes = [vp]
@@ -421,6 +423,11 @@ class Context:
             _check(lib().ulens_get_kernel_ms(self._h, which, C.byref(ms), C.byref(n)), self._h)
             out[name] = (ms.value, n.value)
         return out
+
+    def ulens_fp32_peak(self, ms: float = 200.0) -> float:
+        out = C.c_double()
+        _check(lib().ulens_fp32_peak(self._h, ms, C.byref(out)), self._h)
+        return out.value
 
     def ulens_fp64_peak(self, ms: float = 200.0) -> float:
         out = C.c_double()

@@ -8,7 +8,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libulens.so")
 SOURCES = ["ulens_api.cu"]
-HEADERS = ["ulens_core.cuh", "ulens_regions.cuh", "ulens_limb.cuh", "ulens_dual.cuh", "ulens_host.hpp", os.path.join("..", "..", "include", "ulens.h")]
+HEADERS = ["ulens_core.cuh", "ulens_regions.cuh", "ulens_limb.cuh", "ulens_dual.cuh", "ulens_f32.cuh", "ulens_host.hpp", os.path.join("..", "..", "include", "ulens.h")]
 
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-shared", "-Xcompiler", "-fPIC"]

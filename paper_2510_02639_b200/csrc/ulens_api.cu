@@ -22,6 +22,7 @@
 #include "ulens_dual.cuh"
 #include "ulens_regions.cuh"
 #include "ulens_limb.cuh"
+#include "ulens_f32.cuh"
 #include "ulens_host.hpp"
 
 using namespace ulens;
@@ -556,6 +557,59 @@ k_shoot(int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cfg, const 
     if (lane == 0 && rays) atomicAdd(&ctr->n_rays, rays);
 }
 
+// k_shoot on the FP32 pipe (ulens_f32.cuh; ULENS_OPT_F32_SHOOT): same queue, same lines, same rule; rays in
+// segment-local single precision, segment constants / edge events / accumulation in FP64.
+template <int N, bool LD>
+__global__ void __launch_bounds__(128, UL_SHOOT_MINB)
+k_shoot_f32(int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cfg, const double* __restrict__ w_re,
+            const double* __restrict__ w_im, const Patch* __restrict__ patches, const unsigned* __restrict__ unit_desc,
+            double* __restrict__ unit_sum, double* __restrict__ unit_odd, unsigned* __restrict__ status,
+            ChunkCounters* cc, DevCounters* ctr, unsigned cap_units, const int* __restrict__ pmap = nullptr)
+{
+    const int lane = threadIdx.x & 31;
+    const unsigned n_units = min(cc->n_units, cap_units);
+    unsigned long long rays = 0;
+    for (;;) {
+        unsigned u = 0;
+        if (lane == 0) u = atomicAdd(&cc->next_unit, 1u);
+        u = __shfl_sync(0xffffffffu, u, 0);
+        if (u >= n_units) break;
+        unsigned d = unit_desc[u];
+        if (d == 0xffffffffu) continue;
+        const Patch P = patches[d >> 11];
+        int blk = (int)(d & 0x7ffu);
+        long long gp = pmap ? (long long)pmap[pt_base + P.point] : (long long)pt_base + P.point;
+        int c = (int)(gp / n_pts_per_cfg);
+        Lens L = cfg[c].lens;
+        double rho = cfg[c].rho, u1 = cfg[c].u1;
+        double wcx = w_re[gp], wcy = w_im[gp];
+        int line = blk * 32 + lane;
+        double U, S, f; bool edge, clipped;
+        if (P.flags & UL_PATCH_SCAN_R) {
+            double th, wt; line_node(P.flags, P.n_th, line, P.th0, P.dth, th, wt);
+            shoot_col_f32<N, LD>(L, wcx, wcy, rho * rho, th, P.r0, P.dr, P.n_r, U, S, edge);
+            f = ((1.0 - u1) * U + (LD ? (u1 / rho) * S : 0.0)) * wt;
+            clipped = edge || (!(P.flags & UL_PATCH_PERIODIC) && (line < 1 || line >= P.n_th - 1) && U > 0.0);
+        } else {
+            double r, wr; line_node(P.flags, P.n_r, line, P.r0, P.dr, r, wr);
+            bool periodic = (P.flags & UL_PATCH_PERIODIC) != 0;
+            shoot_ring_f32<N, LD>(L, wcx, wcy, rho * rho, r, P.th0, P.dth, P.n_th, periodic, U, S, edge);
+            f = r * ((1.0 - u1) * U + (LD ? (u1 / rho) * S : 0.0)) * P.dth * wr;
+            clipped = edge || ((line < 1 || line >= P.n_r - 1) && U > 0.0 && P.r0 > 0.0);
+        }
+        double tot = warp_sum(f);
+        double odd = warp_sum((lane & 1) ? f : 0.0);
+        unsigned any_clip = __ballot_sync(0xffffffffu, clipped);
+        if (lane == 0) {
+            unit_sum[u] = tot;
+            unit_odd[u] = 2.0 * odd;
+            if (any_clip) atomicOr(&status[P.point], UL_ST_CLIPPED);
+            rays += 32ull * (unsigned long long)(((P.flags & UL_PATCH_SCAN_R) ? P.n_r : P.n_th) + 4);
+        }
+    }
+    if (lane == 0 && rays) atomicAdd(&ctr->n_rays, rays);
+}
+
 // One thread per point: ordered (deterministic) sum over its sectors' units, normalisation (Eq. A5; F0 of P:99).
 __global__ void k_finalize(int n, int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cfg,
                            const Patch* __restrict__ patches, const int* __restrict__ n_patch,
@@ -922,6 +976,22 @@ __global__ void k_dfma_peak(int iters, double* out)
     if (s == 12345.678) out[0] = s;
 }
 
+// FP32 FMA peak: 8 independent chains per thread
+__global__ void k_ffma_peak(int iters, float* out)
+{
+    float a0 = threadIdx.x * 1e-9f, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6, a7 = a0 + 7;
+    const float m = 1.0000001f, b = 1e-9f;
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            a0 = fmaf(a0, m, b); a1 = fmaf(a1, m, b); a2 = fmaf(a2, m, b); a3 = fmaf(a3, m, b);
+            a4 = fmaf(a4, m, b); a5 = fmaf(a5, m, b); a6 = fmaf(a6, m, b); a7 = fmaf(a7, m, b);
+        }
+    }
+    float s = a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7;
+    if (s == 12345.678f) out[0] = s;
+}
+
 // ------------------------------------------------------------------------------------------------ C ABI
 
 extern "C" const char* ulens_strerror(int code)
@@ -1152,6 +1222,9 @@ static int run_chunks(ulens_ctx* ctx, long long n_total, int n_pts, bool ld, con
         if (dual) {
             if (ld) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_shoot_dual<N, true>, 128, 0);
             else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_shoot_dual<N, false>, 128, 0);
+        } else if (ctx->opt.flags & ULENS_OPT_F32_SHOOT) {
+            if (ld) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_shoot_f32<N, true>, 128, 0);
+            else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_shoot_f32<N, false>, 128, 0);
         } else {
             if (ld) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_shoot<N, true>, 128, 0);
             else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_shoot<N, false>, 128, 0);
@@ -1168,6 +1241,14 @@ static int run_chunks(ulens_ctx* ctx, long long n_total, int n_pts, bool ld, con
                 k_shoot_dual<N, false><<<grid, 128, 0, st>>>((int)base, n_pts, ctx->cfg_dev, tans, w_re, w_im, ctx->patches, ctx->ptans,
                                                              ctx->unit_desc, ctx->unit_sum, ctx->unit_odd, ctx->unit_tan, ctx->status_ws,
                                                              ctx->cc, ctx->counters, (unsigned)ctx->cap_units, pmap);
+            else if (ctx->opt.flags & ULENS_OPT_F32_SHOOT) {
+                if (ld)
+                    k_shoot_f32<N, true><<<grid, 128, 0, st>>>((int)base, n_pts, ctx->cfg_dev, w_re, w_im, ctx->patches, ctx->unit_desc,
+                                                               ctx->unit_sum, ctx->unit_odd, ctx->status_ws, ctx->cc, ctx->counters, (unsigned)ctx->cap_units, pmap);
+                else
+                    k_shoot_f32<N, false><<<grid, 128, 0, st>>>((int)base, n_pts, ctx->cfg_dev, w_re, w_im, ctx->patches, ctx->unit_desc,
+                                                                ctx->unit_sum, ctx->unit_odd, ctx->status_ws, ctx->cc, ctx->counters, (unsigned)ctx->cap_units, pmap);
+            }
             else if (ld)
                 k_shoot<N, true><<<grid, 128, 0, st>>>((int)base, n_pts, ctx->cfg_dev, w_re, w_im, ctx->patches, ctx->unit_desc,
                                                        ctx->unit_sum, ctx->unit_odd, ctx->status_ws, ctx->cc, ctx->counters, (unsigned)ctx->cap_units, pmap);
@@ -1830,5 +1911,35 @@ extern "C" int ulens_fp64_peak(ulens_ctx* ctx, double ms, double* dfma_per_s)
     }
     cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d);
     *dfma_per_s = best;
+    return ULENS_OK;
+}
+
+extern "C" int ulens_fp32_peak(ulens_ctx* ctx, double ms, double* ffma_per_s)
+{
+    if (!ctx || !ffma_per_s || !(ms > 0.0)) return ULENS_EINVAL;
+    CK(cudaSetDevice(ctx->device));
+    int sm_count = 148;
+    cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, ctx->device);
+    float* d = nullptr;
+    CK(cudaMalloc(&d, sizeof(float)));
+    cudaEvent_t e0, e1;
+    CK(cudaEventCreate(&e0)); CK(cudaEventCreate(&e1));
+    const int blocks = sm_count * 8, threads = 256;
+    int iters = 2000;
+    double best = 0.0;
+    float el = 0.f;
+    // calibrate then run ~ms
+    for (int pass = 0; pass < 3; ++pass) {
+        CK(cudaEventRecord(e0));
+        k_ffma_peak<<<blocks, threads>>>(iters, d);
+        CK(cudaEventRecord(e1));
+        CK(cudaEventSynchronize(e1));
+        CK(cudaEventElapsedTime(&el, e0, e1));
+        double rate = (double)blocks * threads * 64.0 * iters / (el * 1e-3);
+        if (pass > 0 && rate > best) best = rate;
+        if (pass == 0) { double scale = ms / (el > 1e-3 ? el : 1e-3); iters = (int)(iters * scale); if (iters < 100) iters = 100; if (iters > 50000000) iters = 50000000; }
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d);
+    *ffma_per_s = best;
     return ULENS_OK;
 }
