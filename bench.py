@@ -51,6 +51,12 @@ FP64_INSTR_PER_RAY_DUAL_EXTRA = 74
 FP64_INSTR_PER_LIMB_SOLVE = {1: 600, 2: 2400, 3: 8300}
 # FP64 FMA pipe of one B200: 148 SMs x 64 DFMA lanes / clk x 1.965 GHz (clocks.max.sm) -- DESIGN.md
 FP64_PEAK_DFMA = 148 * 64 * 1.965e9
+# Mixed-precision variant (k_shoot_f32): algorithmic FP32-pipe instructions per ray in the segment-local
+# difference form -- displacement (ring: series of sin x and cos x - 1, rotation of z0: 16; radial line: 3; mix 10), per lens
+# c + d, c (c + d), |.|^2, reciprocal, eps conj(d / p), accumulate: 16, F: 6, inside test + count: 2, sqrt on inside rays: 1.
+FP32_INSTR_PER_RAY = {(1, False): 34, (1, True): 35, (2, False): 50, (2, True): 51, (3, False): 66, (3, True): 67}
+# FP32 FMA pipe: 148 SMs x 128 FFMA lanes / clk x 1.965 GHz (checked in-run by ulens_fp32_peak)
+FP32_PEAK_FFMA = 148 * 128 * 1.965e9
 
 # cpu_baseline / --impl reference sample: seeded stratified points of the workload (half near-caustic);
 # the seed was fixed once so that the oracle's work on the sample is a few 1e8 lens-map evaluations.
@@ -202,6 +208,7 @@ class Env:
         self.torch, self.dist, self.binding, self.inputs, self.replicas = torch, dist, binding, inputs, replicas
         self.ctx, self.dev, self.local_rank, self.world = ctx, dev, local_rank, world
         self.flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)    # > 126 MB L2
+        self.ctx32 = None
 
     def barrier(self):
         if self.world > 1:
@@ -210,10 +217,14 @@ class Env:
 
 
 def measure_config(env: Env, cfg: int, steps: int, warmup: int, switch: bool = False, with_e2e: bool = True,
-                   with_clocks: bool = False) -> dict:
+                   with_clocks: bool = False, f32: bool = False) -> dict:
     """W warm-up steps, K timed steps (CUDA events on the launch stream, L2 flushed before each), per-kernel
     device times from the library's own event pairs, optionally the end-to-end leg; max over ranks."""
     torch, ctx, dev, binding, inputs, replicas = env.torch, env.ctx, env.dev, env.binding, env.inputs, env.replicas
+    if f32:                                                          # mixed-precision variant: its own context (option flag)
+        if env.ctx32 is None:
+            env.ctx32 = binding.Context(env.local_rank, flags=binding.ULENS_OPT_F32_SHOOT)
+        ctx = env.ctx32
     wl = inputs.get(cfg)                                             # every rank: the same seeded workload (replica)
     lenses = gpu_lenses(binding, wl)
     n = wl.n_cfg * wl.n_pts
@@ -315,13 +326,18 @@ def measure_config(env: Env, cfg: int, steps: int, warmup: int, switch: bool = F
     shoot_avg_s = shoot_ms * 1e-3 / max(shoot_n, 1)
     achieved = 2.0 * ipr * rays_per_launch / shoot_avg_s / 1e12
     peak = 2.0 * FP64_PEAK_DFMA / 1e12
-    roofline = {"bound": "alu", "kernel": "k_shoot_dual" if dual else "k_shoot", "achieved": achieved, "peak": peak,
+    if f32 and not dual:
+        # mixed-precision variant: FP32-pipe instructions per ray against the FP32 FMA pipe (128 lanes / clk / SM)
+        ipr = FP32_INSTR_PER_RAY[(n_lens, ld)]
+        achieved = 2.0 * ipr * rays_per_launch / shoot_avg_s / 1e12
+        peak = 2.0 * FP32_PEAK_FFMA / 1e12
+    roofline = {"bound": "alu", "kernel": ("k_shoot_f32" if f32 else "k_shoot") if not dual else "k_shoot_dual", "achieved": achieved, "peak": peak,
                 "variant": "k_shoot_dual (value + 5 tangents per ray)" if dual else "k_shoot",
                 "unit": "TFLOP/s", "frac": achieved / peak, "traffic": None,
                 "traffic_note": "the path is ALU-bound; DRAM bytes of one launch are in the ncu captures under profiles/",
                 "peak_source": "derived: 148 SM x 64 DFMA/clk x 1.965 GHz x 2 flop (DESIGN.md); "
                                "MEASURED_PEAKS.json has no FP64 entry",
-                "fp64_instr_per_ray": ipr, "rays_per_launch": rays_per_launch,
+                ("fp32_instr_per_ray" if (f32 and not dual) else "fp64_instr_per_ray"): ipr, "rays_per_launch": rays_per_launch,
                 "kernel_ms_avg": 1e3 * shoot_avg_s, "share_of_step": shoot_ms / ms}
     reg_ms, reg_n = kms["k_limb"]                          # the limb tracker; k_sectors (thread per point) is reported beside it
     sec_ms, _ = kms["k_sectors"]
@@ -372,6 +388,10 @@ def main_ours(args, rank, local_rank, world):
         for c in range(5):
             if c != args.config:
                 others["C%d" % c] = summary(measure_config(env, c, 2, 3, with_e2e=False))
+        for c in (1, 2, 3):
+            r32 = measure_config(env, c, 2, 3, with_e2e=False, f32=True)
+            others["C%d_f32" % c] = dict(summary(r32), api="ULENS_OPT_F32_SHOOT: rays on the FP32 pipe (SURVEY 8.f-1); roofline_frac is "
+                                         "against the FP32 FMA peak (%.1f TFLOP/s)" % (2.0 * FP32_PEAK_FFMA / 1e12))
         if args.config == 4 and not args.switch:
             rs = measure_config(env, 4, 2, 3, switch=True, with_e2e=False)
             others["C4_switch"] = dict(summary(rs), n_ext=rs["n_ext"], n_epochs_total=rs["n"],
@@ -381,6 +401,14 @@ def main_ours(args, rank, local_rank, world):
     if rank == 0:
         wl = r["wl"]
         peak_measured = ctx.ulens_fp64_peak(200.0)
+        if "C1_f32" in others:
+            line_f32 = {"workload": others["C1_f32"]["workload"], "kernel": "k_shoot_f32", "bound": "alu", "unit": "TFLOP/s",
+                        "peak": 2.0 * FP32_PEAK_FFMA / 1e12, "frac": others["C1_f32"]["roofline_frac"],
+                        "achieved": others["C1_f32"]["roofline_frac"] * 2.0 * FP32_PEAK_FFMA / 1e12,
+                        "peak_measured_ffma_microbench": 2.0 * ctx.ulens_fp32_peak(200.0) / 1e12,
+                        "value": others["C1_f32"]["value"], "value_fp64_path": others.get("C1", {}).get("value")}
+        else:
+            line_f32 = None
         for k in ("roofline", "roofline_regions"):
             r[k]["peak_measured_dfma_microbench"] = 2.0 * peak_measured / 1e12
             r[k]["frac_of_measured"] = r[k]["achieved"] / (2.0 * peak_measured / 1e12)
@@ -402,6 +430,8 @@ def main_ours(args, rank, local_rank, world):
         if dual and args.switch:
             line["config"]["switch_detail"] = {"api": "ulens_lightcurve_binary_ext", "selection": "library (sel_tol default 2e-5)",
                                                "n_ext": r["n_ext"], "n_epochs_total": r["n"]}
+        if line_f32:
+            line["roofline_f32"] = line_f32
         if others:
             line["all_configs"] = others
         if not args.no_cpu_baseline and world == 1:
@@ -413,6 +443,8 @@ def main_ours(args, rank, local_rank, world):
                                     "rays_per_s": nev / dt}
         print(json.dumps(line), flush=True)
     ctx.close()
+    if env.ctx32 is not None:
+        env.ctx32.close()
     if world > 1:
         dist.barrier()
         dist.destroy_process_group()

@@ -716,6 +716,20 @@ UL_HD void edge_event(double f0, double f1, double f2, double f3, bool want_S, d
     }
 }
 
+// The edge events of a scan line are DEFERRED: each of the 32 lines of a work unit meets the image edge at its own node,
+// so an event evaluated on the spot runs with 1-2 lanes of the warp active (round 1, ncu: 19 % of k_shoot's warp
+// instructions, 24 of 32 lanes active on average). The loop only notes the node index of a sign change (two slots: a line
+// through one image has an entry and an exit); the events are resolved after the loop, where the lanes of the warp are
+// together again, from the four window rays recomputed at the noted node. A third event on a line resolves the oldest
+// one on the spot. The recomputed window may differ from the loop's values in the last bit (another rounding path), which
+// can flip the sign of a node sitting exactly on the edge: the loop's classification (entering: node 1 outside, node 2
+// inside) is authoritative, a disagreeing node is moved onto the edge.
+UL_HD void enforce_crossing(double& w1, double& w2, bool entering)
+{
+    if (entering) { if (w1 < 0.0) w1 = 0.0; if (!(w2 < 0.0)) w2 = -1e-9 * fabs(w1) - 1e-300; }
+    else { if (!(w1 < 0.0)) w1 = -1e-9 * fabs(w2) - 1e-300; if (w2 < 0.0) w2 = 0.0; }
+}
+
 // Integrate one ring r over theta:  U = Int chi dtheta / dth,  S = Int chi sqrt(-F) dtheta / dth  (both in cells).
 // Rays at th0 + (j + 1/2) dth, j = -2 .. n_th+1 (two halo rays per side feed the cubic stencil; for a
 // periodic sector they are the wrapped rays). edge = true if one of the first / last two rays of a
@@ -724,28 +738,44 @@ template <int N, bool LD>
 UL_HD void shoot_ring(const Lens& L, double wcx, double wcy, double rho2, double r, double th0, double dth,
                       int n_th, bool periodic, double& U_out, double& S_out, bool& edge)
 {
-    double cd = cos(dth), sd = sin(dth);
+    const double cd = cos(dth), sd = sin(dth);
     double t = th0 - 1.5 * dth;
     double c = cos(t), s = sin(t);
-    double f0 = UL_BIG, f1 = UL_BIG, f2 = UL_BIG, f3;
+    double f1 = UL_BIG, f2 = UL_BIG;
     double U = 0.0, S = 0.0;
     edge = false;
     const int j_first = periodic ? 2 : 1;
-    // per ray: count it, then close the pair (j-2, j-1) = (f1, f2) once its stencil (f0..f3) is complete
+    int npend = 0, pj0 = 0, pj1 = 0;
+    unsigned pen = 0;
+    // the event noted at node pj: pair (pj-2, pj-1), window nodes pj-3 .. pj at angles th0 + (k + 1/2) dth
+    auto resolve = [&](int pj, bool entering) {
+        const double a = th0 + (pj - 2.5) * dth;
+        double wc = cos(a), ws = sin(a), w[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            w[k] = ray_F<N>(L, r * wc, r * ws, wcx, wcy, rho2);
+            const double cn = wc * cd - ws * sd; ws = ws * cd + wc * sd; wc = cn;
+        }
+        enforce_crossing(w[1], w[2], entering);
+        double u, dS; bool en;
+        edge_event(w[0], w[1], w[2], w[3], LD, 0.0, u, en, dS);
+        U += u - 0.5; S += dS;
+    };
+    // per ray: count it, then note the pair (j-2, j-1) = (f1, f2) if the sign changes between them. In a periodic
+    // sector pair (-1, 0) is pair (n_th-1, n_th) again: take it once.
     auto node = [&](int j, double f3) {
         if (j >= 0 && j < n_th && f3 < 0.0) {
             U += 1.0;
             if (LD) S += sqrt(-f3);
             if (!periodic && (j < 2 || j >= n_th - 2)) edge = true;
         }
-        // stencil complete once f0 = F_{j-3} exists (j >= 1). In a periodic sector pair (-1, 0) is pair
-        // (n_th-1, n_th) again: take it once.
         if (j >= j_first && ((f1 < 0.0) != (f2 < 0.0))) {
-            double u, dS; bool en;
-            edge_event(f0, f1, f2, f3, LD, 0.0, u, en, dS);
-            U += u - 0.5; S += dS;
+            if (npend == 2) { resolve(pj0, (pen & 1u) != 0); pj0 = pj1; pen >>= 1; npend = 1; }
+            if (npend == 0) pj0 = j; else pj1 = j;
+            if (!(f1 < 0.0)) pen |= 1u << npend;
+            ++npend;
         }
-        f0 = f1; f1 = f2; f2 = f3;
+        f1 = f2; f2 = f3;
     };
     // two rays in flight per iteration: their lens maps are independent, which doubles the FP64 pipe's
     // instruction-level parallelism (the rotation recurrence is the only loop-carried chain)
@@ -758,6 +788,8 @@ UL_HD void shoot_ring(const Lens& L, double wcx, double wcy, double rho2, double
         c = c2 * cd - s2 * sd;
         s = s2 * cd + c2 * sd;
     }
+    if (npend > 0) resolve(pj0, (pen & 1u) != 0);
+    if (npend > 1) resolve(pj1, (pen & 2u) != 0);
     U_out = U; S_out = S;
 }
 
@@ -784,32 +816,46 @@ template <int N, bool LD>
 UL_HD void shoot_col(const Lens& L, double wcx, double wcy, double rho2, double th, double r0, double dr,
                      int n_r, double& U_out, double& S_out, bool& edge)
 {
-    double c = cos(th), s = sin(th);
-    double f0 = UL_BIG, f1 = UL_BIG, f2 = UL_BIG, f3;
+    const double c = cos(th), s = sin(th);
+    double f1 = UL_BIG, f2 = UL_BIG;
     double U = 0.0, S = 0.0, U2 = 0.0;
     edge = false;
+    int npend = 0, pi0 = 0, pi1 = 0;
+    unsigned pen = 0;
+    // the event noted at node pi: pair (pi-2, pi-1), window nodes pi-3 .. pi (deferred, see shoot_ring)
+    auto resolve = [&](int pi, bool entering) {
+        double w[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const double rk = r0 + (pi - 3 + k + 0.5) * dr;
+            w[k] = ray_F<N>(L, rk * c, rk * s, wcx, wcy, rho2);
+        }
+        enforce_crossing(w[1], w[2], entering);
+        const double r1 = r0 + (pi - 1.5) * dr;          // node pi-2
+        const double rh = r1 + 0.5 * dr;                 // cell face between the pair
+        const double rin = entering ? r1 + dr : r1;      // first inside node
+        const double t2x = dr / ul_max(rin, 0.5 * dr);
+        double u, dS; bool en;
+        edge_event(w[0], w[1], w[2], w[3], LD, t2x, u, en, dS);
+        double rc = en ? (r1 + dr) - u * dr : r1 + u * dr;
+        rc = ul_max(rc, 0.0);
+        U2 += en ? 0.5 * (rh * rh - rc * rc) : 0.5 * (rc * rc - rh * rh);
+        S += dS * rc;
+    };
     auto node = [&](int i, double r, double f3) {
         if (i >= 0 && i < n_r && f3 < 0.0) {
             U += r;
             if (LD) S += r * sqrt(-f3);
             if ((i < 2 && r0 > 0.0) || i >= n_r - 2) edge = true;
         }
-        // pair (i-2, i-1) = (f1, f2)
-        if (i >= 1 && ((f1 < 0.0) != (f2 < 0.0))) {
-            double r1 = r0 + (i - 1.5) * dr;             // node i-2
-            double rh = r1 + 0.5 * dr;                   // cell face between the pair
-            if (rh > 0.0) {
-                double u, dS; bool en;
-                double rin = !(f1 < 0.0) ? r1 + dr : r1;  // first inside node
-                double t2x = dr / ul_max(rin, 0.5 * dr);
-                edge_event(f0, f1, f2, f3, LD, t2x, u, en, dS);
-                double rc = en ? (r1 + dr) - u * dr : r1 + u * dr;
-                rc = ul_max(rc, 0.0);
-                U2 += en ? 0.5 * (rh * rh - rc * rc) : 0.5 * (rc * rc - rh * rh);
-                S += dS * rc;
-            }
+        // pair (i-2, i-1) = (f1, f2); the cell face between the pair must lie at r > 0
+        if (i >= 1 && ((f1 < 0.0) != (f2 < 0.0)) && (r0 + (i - 1.0) * dr > 0.0)) {
+            if (npend == 2) { resolve(pi0, (pen & 1u) != 0); pi0 = pi1; pen >>= 1; npend = 1; }
+            if (npend == 0) pi0 = i; else pi1 = i;
+            if (!(f1 < 0.0)) pen |= 1u << npend;
+            ++npend;
         }
-        f0 = f1; f1 = f2; f2 = f3;
+        f1 = f2; f2 = f3;
     };
     for (int i = -2; i <= n_r + 1; i += 2) {               // two rays in flight (see shoot_ring)
         const double ra = r0 + (i + 0.5) * dr, rb = r0 + (i + 1.5) * dr;
@@ -818,6 +864,8 @@ UL_HD void shoot_col(const Lens& L, double wcx, double wcy, double rho2, double 
         node(i, ra, fa);
         if (i + 1 <= n_r + 1) node(i + 1, rb, fb);
     }
+    if (npend > 0) resolve(pi0, (pen & 1u) != 0);
+    if (npend > 1) resolve(pi1, (pen & 2u) != 0);
     U_out = U * dr + U2; S_out = S * dr;
 }
 

@@ -256,14 +256,7 @@ UL_HDNI void edge_event_adj(double f0, double f1, double f2, double f3, bool wan
 #define UL_DEFER_D 32
 #endif
 
-// The recomputed window may differ from the loop's values in the last bit (another rounding path), which can flip
-// the sign of a node sitting exactly on the edge: the loop's classification (entering: node 1 outside, node 2
-// inside) is authoritative, a disagreeing node is moved onto the edge.
-UL_HD void enforce_crossing(double& w1, double& w2, bool entering)
-{
-    if (entering) { if (w1 < 0.0) w1 = 0.0; if (!(w2 < 0.0)) w2 = -1e-9 * fabs(w1) - 1e-300; }
-    else { if (!(w1 < 0.0)) w1 = -1e-9 * fabs(w2) - 1e-300; if (w2 < 0.0) w2 = 0.0; }
-}
+// (enforce_crossing, ulens_core.cuh, keeps the loop's classification of the pair authoritative for the recomputed window)
 
 // ------------------------------------------------------------------------------------------------ scan lines
 

