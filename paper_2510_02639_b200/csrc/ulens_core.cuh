@@ -730,6 +730,48 @@ UL_HD void enforce_crossing(double& w1, double& w2, bool entering)
     else { if (!(w1 < 0.0)) w1 = -1e-9 * fabs(w2) - 1e-300; if (w2 < 0.0) w2 = 0.0; }
 }
 
+// the event noted at node pj of a ring: pair (pj-2, pj-1), window nodes pj-3 .. pj at angles th0 + (k + 1/2) dth
+template <int N, bool LD>
+UL_HD void ring_event(const Lens& L, double wcx, double wcy, double rho2, double r, double th0, double dth, double cd, double sd,
+                      int pj, bool entering, double& U, double& S)
+{
+    const double a = th0 + (pj - 2.5) * dth;
+    double wc = cos(a), ws = sin(a), w[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        w[k] = ray_F<N>(L, r * wc, r * ws, wcx, wcy, rho2);
+        const double cn = wc * cd - ws * sd; ws = ws * cd + wc * sd; wc = cn;
+    }
+    enforce_crossing(w[1], w[2], entering);
+    double u, dS; bool en;
+    edge_event(w[0], w[1], w[2], w[3], LD, 0.0, u, en, dS);
+    U += u - 0.5; S += dS;
+}
+
+// the event noted at node pi of a radial line (direction c, s): pair (pi-2, pi-1), window nodes pi-3 .. pi
+template <int N, bool LD>
+UL_HD void col_event(const Lens& L, double wcx, double wcy, double rho2, double c, double s, double r0, double dr,
+                     int pi, bool entering, double& U2, double& S)
+{
+    double w[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const double rk = r0 + (pi - 3 + k + 0.5) * dr;
+        w[k] = ray_F<N>(L, rk * c, rk * s, wcx, wcy, rho2);
+    }
+    enforce_crossing(w[1], w[2], entering);
+    const double r1 = r0 + (pi - 1.5) * dr;              // node pi-2
+    const double rh = r1 + 0.5 * dr;                     // cell face between the pair
+    const double rin = entering ? r1 + dr : r1;          // first inside node
+    const double t2x = dr / ul_max(rin, 0.5 * dr);
+    double u, dS; bool en;
+    edge_event(w[0], w[1], w[2], w[3], LD, t2x, u, en, dS);
+    double rc = en ? (r1 + dr) - u * dr : r1 + u * dr;
+    rc = ul_max(rc, 0.0);
+    U2 += en ? 0.5 * (rh * rh - rc * rc) : 0.5 * (rc * rc - rh * rh);
+    S += dS * rc;
+}
+
 // Integrate one ring r over theta:  U = Int chi dtheta / dth,  S = Int chi sqrt(-F) dtheta / dth  (both in cells).
 // Rays at th0 + (j + 1/2) dth, j = -2 .. n_th+1 (two halo rays per side feed the cubic stencil; for a
 // periodic sector they are the wrapped rays). edge = true if one of the first / last two rays of a
@@ -747,20 +789,7 @@ UL_HD void shoot_ring(const Lens& L, double wcx, double wcy, double rho2, double
     const int j_first = periodic ? 2 : 1;
     int npend = 0, pj0 = 0, pj1 = 0;
     unsigned pen = 0;
-    // the event noted at node pj: pair (pj-2, pj-1), window nodes pj-3 .. pj at angles th0 + (k + 1/2) dth
-    auto resolve = [&](int pj, bool entering) {
-        const double a = th0 + (pj - 2.5) * dth;
-        double wc = cos(a), ws = sin(a), w[4];
-#pragma unroll
-        for (int k = 0; k < 4; ++k) {
-            w[k] = ray_F<N>(L, r * wc, r * ws, wcx, wcy, rho2);
-            const double cn = wc * cd - ws * sd; ws = ws * cd + wc * sd; wc = cn;
-        }
-        enforce_crossing(w[1], w[2], entering);
-        double u, dS; bool en;
-        edge_event(w[0], w[1], w[2], w[3], LD, 0.0, u, en, dS);
-        U += u - 0.5; S += dS;
-    };
+    auto resolve = [&](int pj, bool entering) { ring_event<N, LD>(L, wcx, wcy, rho2, r, th0, dth, cd, sd, pj, entering, U, S); };
     // per ray: count it, then note the pair (j-2, j-1) = (f1, f2) if the sign changes between them. In a periodic
     // sector pair (-1, 0) is pair (n_th-1, n_th) again: take it once.
     auto node = [&](int j, double f3) {
@@ -822,26 +851,7 @@ UL_HD void shoot_col(const Lens& L, double wcx, double wcy, double rho2, double 
     edge = false;
     int npend = 0, pi0 = 0, pi1 = 0;
     unsigned pen = 0;
-    // the event noted at node pi: pair (pi-2, pi-1), window nodes pi-3 .. pi (deferred, see shoot_ring)
-    auto resolve = [&](int pi, bool entering) {
-        double w[4];
-#pragma unroll
-        for (int k = 0; k < 4; ++k) {
-            const double rk = r0 + (pi - 3 + k + 0.5) * dr;
-            w[k] = ray_F<N>(L, rk * c, rk * s, wcx, wcy, rho2);
-        }
-        enforce_crossing(w[1], w[2], entering);
-        const double r1 = r0 + (pi - 1.5) * dr;          // node pi-2
-        const double rh = r1 + 0.5 * dr;                 // cell face between the pair
-        const double rin = entering ? r1 + dr : r1;      // first inside node
-        const double t2x = dr / ul_max(rin, 0.5 * dr);
-        double u, dS; bool en;
-        edge_event(w[0], w[1], w[2], w[3], LD, t2x, u, en, dS);
-        double rc = en ? (r1 + dr) - u * dr : r1 + u * dr;
-        rc = ul_max(rc, 0.0);
-        U2 += en ? 0.5 * (rh * rh - rc * rc) : 0.5 * (rc * rc - rh * rh);
-        S += dS * rc;
-    };
+    auto resolve = [&](int pi, bool entering) { col_event<N, LD>(L, wcx, wcy, rho2, c, s, r0, dr, pi, entering, U2, S); };
     auto node = [&](int i, double r, double f3) {
         if (i >= 0 && i < n_r && f3 < 0.0) {
             U += r;

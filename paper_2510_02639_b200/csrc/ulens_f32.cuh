@@ -13,9 +13,10 @@
 // scale (rho^2) times |d| / rho, instead of ~1e-7 / rho. The displacement d itself is formed without cancellation: along
 // a radial line d = t (cos th, sin th); along a ring d = z0 (e^{i x} - 1) with x the angle from the reference ray and
 // sin x, cos x - 1 from their Taylor series (|x| <= 1/2 by the choice of the segment length).
-// The window of F values that locates the image edge (App. A.1) is kept in FP32; the edge event itself (cubic root,
-// Hurwitz-zeta end correction: rare) runs in FP64 on the promoted window; counts are integers, sums of sqrt(-F) are
-// FP32 within a segment and FP64 across segments.
+// The loop only needs the SIGN of F at every node (inside / outside) and sqrt(-F) on inside rays; where the sign changes
+// between two nodes it notes the node, and the edge event (cubic root, Hurwitz-zeta end correction: two per line) is
+// resolved after the loop in FP64 from four recomputed FP64 rays, by the very code the FP64 kernel uses (ring_event /
+// col_event, ulens_core.cuh). Counts are integers, sums of sqrt(-F) are FP32 within a segment and FP64 across segments.
 #pragma once
 #include "ulens_core.cuh"
 
@@ -77,10 +78,13 @@ __device__ __forceinline__ void shoot_ring_f32(const Lens& L, double wcx, double
     int half = (int)(0.5 / dth);
     half = half > 32 ? 32 : (half < 1 ? 1 : half);
     const float dthf = (float)dth;
-    float f0 = UL_F32_BIG, f1 = UL_F32_BIG, f2 = UL_F32_BIG;
+    float f1 = UL_F32_BIG, f2 = UL_F32_BIG;
     double U = 0.0, S = 0.0;
     edge = false;
     const int j_first = periodic ? 2 : 1;
+    const double cd = cos(dth), sd = sin(dth);
+    int npend = 0, pj0 = 0, pj1 = 0;
+    unsigned pen = 0;
     // reference ray of the first segment, then rotated from segment to segment in FP64
     double sn, cs, sstep, cstep;
     sincos(th0 + (-2 + half + 0.5) * dth, &sn, &cs);
@@ -104,16 +108,22 @@ __device__ __forceinline__ void shoot_ring_f32(const Lens& L, double wcx, double
                 if (!periodic && (j < 2 || j >= n_th - 2)) edge = true;
             }
             if (j >= j_first && ((f1 < 0.0f) != (f2 < 0.0f))) {
-                double u, dS; bool en;
-                edge_event((double)f0, (double)f1, (double)f2, (double)f3, LD, 0.0, u, en, dS);
-                U += u - 0.5; S += dS;
+                if (npend == 2) {
+                    ring_event<N, LD>(L, wcx, wcy, rho2, r, th0, dth, cd, sd, pj0, (pen & 1u) != 0, U, S);
+                    pj0 = pj1; pen >>= 1; npend = 1;
+                }
+                if (npend == 0) pj0 = j; else pj1 = j;
+                if (!(f1 < 0.0f)) pen |= 1u << npend;
+                ++npend;
             }
-            f0 = f1; f1 = f2; f2 = f3;
+            f1 = f2; f2 = f3;
         }
         U += (double)cnt; S += (double)ssum;
         const double cn = cs * cstep - sn * sstep;
         sn = sn * cstep + cs * sstep; cs = cn;
     }
+    if (npend > 0) ring_event<N, LD>(L, wcx, wcy, rho2, r, th0, dth, cd, sd, pj0, (pen & 1u) != 0, U, S);
+    if (npend > 1) ring_event<N, LD>(L, wcx, wcy, rho2, r, th0, dth, cd, sd, pj1, (pen & 2u) != 0, U, S);
     U_out = U; S_out = S;
 }
 
@@ -126,9 +136,11 @@ __device__ __forceinline__ void shoot_col_f32(const Lens& L, double wcx, double 
     sincos(th, &sn, &cs);
     const float cf = (float)cs, sf = (float)sn, drf = (float)dr;
     constexpr int half = 32;
-    float f0 = UL_F32_BIG, f1 = UL_F32_BIG, f2 = UL_F32_BIG;
+    float f1 = UL_F32_BIG, f2 = UL_F32_BIG;
     double U = 0.0, S = 0.0, U2 = 0.0;
     edge = false;
+    int npend = 0, pi0 = 0, pi1 = 0;
+    unsigned pen = 0;
     for (int i0 = -2; i0 <= n_r + 1; i0 += 2 * half) {
         const double rc = r0 + (i0 + half + 0.5) * dr;     // reference node i0 + half
         SegRef<N> R;
@@ -144,27 +156,24 @@ __device__ __forceinline__ void shoot_col_f32(const Lens& L, double wcx, double 
                 if (LD) { const float sq = sqrt_approx(-f3); ssum += sq; tssum += t * sq; }
                 if ((i < 2 && r0 > 0.0) || i >= n_r - 2) edge = true;
             }
-            // pair (i-2, i-1) = (f1, f2)
-            if (i >= 1 && ((f1 < 0.0f) != (f2 < 0.0f))) {
-                const double r1 = r0 + (i - 1.5) * dr;       // node i-2
-                const double rh = r1 + 0.5 * dr;             // cell face between the pair
-                if (rh > 0.0) {
-                    double u, dS; bool en;
-                    const double rin = !(f1 < 0.0f) ? r1 + dr : r1;
-                    const double t2x = dr / ul_max(rin, 0.5 * dr);
-                    edge_event((double)f0, (double)f1, (double)f2, (double)f3, LD, t2x, u, en, dS);
-                    double rcr = en ? (r1 + dr) - u * dr : r1 + u * dr;
-                    rcr = ul_max(rcr, 0.0);
-                    U2 += en ? 0.5 * (rh * rh - rcr * rcr) : 0.5 * (rcr * rcr - rh * rh);
-                    S += dS * rcr;
+            // pair (i-2, i-1) = (f1, f2); the cell face between the pair must lie at r > 0
+            if (i >= 1 && ((f1 < 0.0f) != (f2 < 0.0f)) && (r0 + (i - 1.0) * dr > 0.0)) {
+                if (npend == 2) {
+                    col_event<N, LD>(L, wcx, wcy, rho2, cs, sn, r0, dr, pi0, (pen & 1u) != 0, U2, S);
+                    pi0 = pi1; pen >>= 1; npend = 1;
                 }
+                if (npend == 0) pi0 = i; else pi1 = i;
+                if (!(f1 < 0.0f)) pen |= 1u << npend;
+                ++npend;
             }
-            f0 = f1; f1 = f2; f2 = f3;
+            f1 = f2; f2 = f3;
         }
         // sum over the inside nodes of r = rc + t, and of r sqrt(-F)
         U += (double)cnt * rc + (double)tsum;
         S += rc * (double)ssum + (double)tssum;
     }
+    if (npend > 0) col_event<N, LD>(L, wcx, wcy, rho2, cs, sn, r0, dr, pi0, (pen & 1u) != 0, U2, S);
+    if (npend > 1) col_event<N, LD>(L, wcx, wcy, rho2, cs, sn, r0, dr, pi1, (pen & 2u) != 0, U2, S);
     U_out = U * dr + U2; S_out = S * dr;
 }
 
