@@ -15,14 +15,6 @@
 #include <math.h>
 #include <stdint.h>
 
-// warp vote used by the dual scan-line loops to batch their (rare, expensive) edge events across the 32 lines
-// of a work unit; in a host build every "warp" is one line
-#if defined(__CUDA_ARCH__)
-#define UL_WARP_ANY(p) (__any_sync(0xffffffffu, (p)) != 0)
-#else
-#define UL_WARP_ANY(p) (p)
-#endif
-
 #if defined(__CUDACC__)
 #define UL_HD __host__ __device__ __forceinline__
 #define UL_HDN __host__ __device__

@@ -248,14 +248,9 @@ UL_HDNI void edge_event_adj(double f0, double f1, double f2, double f3, bool wan
     }
 }
 
-// Edge events in the tangent loops are DEFERRED and BATCHED: each of the 32 lines of a work unit meets the image
-// edge at its own node; evaluated on the spot, 1-2 lanes would be active in the event code. A lane that sees a
-// sign change remembers the node index, and the warp evaluates all pending events together -- at the latest
-// UL_DEFER_D nodes later, or when one of the lanes meets its next crossing -- recomputing the four window rays.
-#ifndef UL_DEFER_D
-#define UL_DEFER_D 32
-#endif
-
+// Edge events in the tangent loops are DEFERRED as in the primal loops (ulens_core.cuh shoot_ring): the loop notes the node
+// of a sign change (two slots), the events are resolved in two extra passes after the rays, where the lanes of the warp
+// are together again, from the four window rays recomputed at the noted node.
 // (enforce_crossing, ulens_core.cuh, keeps the loop's classification of the pair authoritative for the recomputed window)
 
 // ------------------------------------------------------------------------------------------------ scan lines
@@ -274,9 +269,10 @@ UL_HD void shoot_ring_t(const Lens& L, double wcx, double wcy, double rho2, doub
     stat_zero(SU); stat_zero(SS);
     edge = false;
     const int j_first = periodic ? 2 : 1;
-    bool pend = false, pen = false; int pj = 0;
-    auto flush = [&]() {
-        if (pend) {
+    int npend = 0, pj0 = 0, pj1 = 0;
+    unsigned penb = 0;
+    auto flush = [&](int pj, bool pen) {
+        {
             // window nodes pj-3 .. pj at angles th0 + (k + 1/2) dth
             const double a = th0 + (pj - 2.5) * dth;
             double wc = cos(a), ws = sin(a);
@@ -302,11 +298,10 @@ UL_HD void shoot_ring_t(const Lens& L, double wcx, double wcy, double rho2, doub
                 if (LD) stat_add(SS, aS[k], B);
                 const double cn = wc * cd - ws * sd; ws = ws * cd + wc * sd; wc = cn;
             }
-            pend = false;
         }
     };
-    // (one more pass than there are rays: the last one only flushes what is still pending -- one flush site)
-    for (int j = -2; j <= n_th + 2; ++j) {
+    // (the loop runs up to two passes beyond the rays: they resolve the noted events -- one flush site in the code)
+    for (int j = -2; j <= n_th + 3; ++j) {
         const bool last = j > n_th + 1;
         RayCore<N> R;
         ray_core<N>(L, r * c, r * s, wcx, wcy, rho2, R);
@@ -323,9 +318,16 @@ UL_HD void shoot_ring_t(const Lens& L, double wcx, double wcy, double rho2, doub
             if (!periodic && (j < 2 || j >= n_th - 2)) edge = true;
         }
         const bool ev = !last && j >= j_first && ((f1 < 0.0) != (f2 < 0.0));
-        // flush for the whole warp when a pending event is old enough or its lane meets its next crossing
-        if (UL_WARP_ANY(pend && (ev || last || j - pj >= UL_DEFER_D))) flush();
-        if (ev) { pj = j; pend = true; pen = !(f1 < 0.0); }
+        // a noted event is resolved after the rays (the two extra passes), or on the spot when a third one arrives
+        if (npend > 0 && (last || (ev && npend == 2))) {
+            flush(pj0, (penb & 1u) != 0);
+            pj0 = pj1; penb >>= 1; --npend;
+        }
+        if (ev) {
+            if (npend == 0) pj0 = j; else pj1 = j;
+            if (!(f1 < 0.0)) penb |= 1u << npend;
+            ++npend;
+        }
         f1 = f2; f2 = f3;
         const double cn = c * cd - s * sd;
         s = s * cd + c * sd;
@@ -345,9 +347,10 @@ UL_HD void shoot_col_t(const Lens& L, double wcx, double wcy, double rho2, doubl
     double U = 0.0, S = 0.0, U2 = 0.0;
     stat_zero(SU); stat_zero(SS);
     edge = false;
-    bool pend = false, pen = false; int pi = 0;
-    auto flush = [&]() {
-        if (pend) {
+    int npend = 0, pi0 = 0, pi1 = 0;
+    unsigned penb = 0;
+    auto flush = [&](int pi, bool pen) {
+        {
             double w[4];
             RayCore<N> R;
 #pragma unroll
@@ -379,10 +382,9 @@ UL_HD void shoot_col_t(const Lens& L, double wcx, double wcy, double rho2, doubl
                 stat_add(SU, rc_free ? rc * dr * au[k] : 0.0, B);
                 if (LD) stat_add(SS, rc * aS[k] + dS * drc * au[k], B);          // (the caller scales the S set by dr)
             }
-            pend = false;
         }
     };
-    for (int i = -2; i <= n_r + 2; ++i) {                 // (last pass: flush only)
+    for (int i = -2; i <= n_r + 3; ++i) {                 // (last two passes: resolve the noted events)
         const bool last = i > n_r + 1;
         const double r = r0 + dr * (i + 0.5);
         RayCore<N> R;
@@ -401,8 +403,15 @@ UL_HD void shoot_col_t(const Lens& L, double wcx, double wcy, double rho2, doubl
         }
         // pair (i-2, i-1) = (f1, f2); the cell face between the pair must lie at r > 0
         const bool ev = !last && i >= 1 && ((f1 < 0.0) != (f2 < 0.0)) && (r0 + dr * (i - 1.0) > 0.0);
-        if (UL_WARP_ANY(pend && (ev || last || i - pi >= UL_DEFER_D))) flush();
-        if (ev) { pi = i; pend = true; pen = !(f1 < 0.0); }
+        if (npend > 0 && (last || (ev && npend == 2))) {
+            flush(pi0, (penb & 1u) != 0);
+            pi0 = pi1; penb >>= 1; --npend;
+        }
+        if (ev) {
+            if (npend == 0) pi0 = i; else pi1 = i;
+            if (!(f1 < 0.0)) penb |= 1u << npend;
+            ++npend;
+        }
         f1 = f2; f2 = f3;
     }
     U_out = U * dr + U2; S_out = S * dr;
