@@ -407,41 +407,40 @@ __global__ void k_ext_scatter(int n, const unsigned char* __restrict__ flag, con
     if (f) map[blk[blockIdx.x] + wsum[w] + __popc(b & ((1u << l) - 1u))] = i;
 }
 
-// Image-region builder, first half (ulens_limb.cuh): one CTA per source point, a group of N^2+1 lanes per limb arc,
-// one lane per root. Writes the point's box list.
-// CTAs per SM asked of the compiler: 3 x 160 threads for the binary lens (measured: 87 -> 75 ms on C1 against 2; 4 is no
-// better), 2 x 320 for the triple lens
+// Image-region builder, first half (ulens_limb.cuh): a group of N^2+1 lanes per limb arc, one lane per root; a warp holds
+// GPW arcs, and the WARPS warps that share a source point are independent work items (4 per CTA, any mix of points).
+// Appends to the point's box list (n_boxes zeroed before the launch).
 #ifndef UL_LIMB_MINB
-#define UL_LIMB_MINB(N) ((N) == 3 ? 2 : 3)
+#define UL_LIMB_MINB(N) ((N) == 3 ? 4 : 4)
 #endif
 template <int N, bool DUAL>
-__global__ void __launch_bounds__(LimbGeom<N>::THREADS, UL_LIMB_MINB(N))
+__global__ void __launch_bounds__(128, UL_LIMB_MINB(N))
 k_limb(int n, int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cfg, const LensPoly* __restrict__ poly,
        const double* __restrict__ w_re, const double* __restrict__ w_im, RegionParams rp,
        SubBox* __restrict__ boxes, BoxExt* __restrict__ exts, int* __restrict__ n_boxes, unsigned* __restrict__ status,
        DevCounters* ctr, const double* __restrict__ c_zr, const double* __restrict__ c_zi,
        const unsigned* __restrict__ c_mask, const int* __restrict__ pmap = nullptr, const unsigned* __restrict__ n_dev = nullptr)
 {
-    __shared__ LimbShared<N> sh;
-    __shared__ LensPoly sT;
-    const int i = blockIdx.x;
+    typedef LimbGeom<N> G;
+    __shared__ LimbShared<N> sh[4];
+    const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (n_dev) n = min(n, (int)*n_dev - pt_base);
-    if (i >= n) return;                                  // whole CTA leaves together
+    const long long item = (long long)blockIdx.x * 4 + wib;          // (point, warp of the point)
+    const int i = (int)(item / G::WARPS), w = (int)(item % G::WARPS);
+    if (i >= n) return;                                  // whole warp leaves together
     const long long gp = pmap ? (long long)pmap[pt_base + i] : (long long)pt_base + i;
     const int c = (int)(gp / n_pts_per_cfg);
-    if (threadIdx.x == 0) { sh.n_box = 0; sh.status = 0; sh.n_solves = 0; }
-    for (int k = threadIdx.x; k < (int)(sizeof(LensPoly) / sizeof(double)); k += blockDim.x)
-        reinterpret_cast<double*>(&sT)[k] = reinterpret_cast<const double*>(&poly[c])[k];
-    __syncthreads();
     const Lens L = cfg[c].lens;
     constexpr int CAP = BoxCap<N>::value;
-    limb_track<N, DUAL>(sh, L, sT, w_re[gp], w_im[gp], cfg[c].rho, rp, c_zr + (long long)i * 10, c_zi + (long long)i * 10,
-                        c_mask[i], boxes + (size_t)i * CAP, DUAL ? exts + (size_t)i * CAP : nullptr, CAP);
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        n_boxes[i] = min(sh.n_box, CAP);
-        if (sh.status) status[i] |= sh.status;           // k_roots wrote the word first
-        atomicAdd(&ctr->n_limb_solves, (unsigned long long)sh.n_solves);
+    int n_solves = 0;
+    unsigned st = limb_track<N, DUAL>(sh[wib], w, L, poly[c], w_re[gp], w_im[gp], cfg[c].rho, rp, c_zr + (long long)i * 10,
+                                      c_zi + (long long)i * 10, c_mask[i], boxes + (size_t)i * CAP,
+                                      DUAL ? exts + (size_t)i * CAP : nullptr, n_boxes + i, CAP, n_solves);
+    st = __reduce_or_sync(0xffffffffu, st);
+    n_solves = __reduce_add_sync(0xffffffffu, n_solves);
+    if (lane == 0) {
+        if (st) atomicOr(&status[i], st);                // k_roots wrote the word first
+        atomicAdd(&ctr->n_limb_solves, (unsigned long long)n_solves);
     }
 }
 
@@ -469,7 +468,7 @@ k_sectors(int n, int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cf
         const int c = (int)(gp / n_pts_per_cfg);
         const Lens L = cfg[c].lens;
         PatchTan* pt = tans ? ptans + (long long)i * UL_MAXP : nullptr;
-        np = sectors_from_boxes<N>(boxes + (size_t)i * CAP, tans ? exts + (size_t)i * CAP : nullptr, n_boxes[i], rp, i, L,
+        np = sectors_from_boxes<N>(boxes + (size_t)i * CAP, tans ? exts + (size_t)i * CAP : nullptr, min(n_boxes[i], CAP), rp, i, L,
                                    w_re[gp], w_im[gp], cfg[c].rho, st, tans ? &tans[c] : nullptr, pp, pt);
         for (int p = 0; p < np; ++p) total_units += pp[p].n_units;
     }
@@ -1202,12 +1201,14 @@ static int run_chunks(ulens_ctx* ctx, long long n_total, int n_pts, bool ld, con
         }
         {
             KTimer kt(ctx, ULENS_K_LIMB, st);
+            CK(cudaMemsetAsync(ctx->n_boxes, 0, sizeof(int) * (size_t)n, st));
+            const unsigned limb_grid = (unsigned)(((long long)n * LimbGeom<N>::WARPS + 3) / 4);
             if (dual)
-                k_limb<N, true><<<n, LimbGeom<N>::THREADS, 0, st>>>(n, (int)base, n_pts, ctx->cfg_dev, ctx->poly_dev, w_re, w_im, rp,
+                k_limb<N, true><<<limb_grid, 128, 0, st>>>(n, (int)base, n_pts, ctx->cfg_dev, ctx->poly_dev, w_re, w_im, rp,
                                                                     ctx->boxes, ctx->exts, ctx->n_boxes, ctx->status_ws, ctx->counters,
                                                                     ctx->c_zr, ctx->c_zi, ctx->c_mask, pmap, n_dev);
             else
-                k_limb<N, false><<<n, LimbGeom<N>::THREADS, 0, st>>>(n, (int)base, n_pts, ctx->cfg_dev, ctx->poly_dev, w_re, w_im, rp,
+                k_limb<N, false><<<limb_grid, 128, 0, st>>>(n, (int)base, n_pts, ctx->cfg_dev, ctx->poly_dev, w_re, w_im, rp,
                                                                      ctx->boxes, ctx->exts, ctx->n_boxes, ctx->status_ws, ctx->counters,
                                                                      ctx->c_zr, ctx->c_zi, ctx->c_mask, pmap, n_dev);
         }

@@ -4,8 +4,10 @@
 //
 // Parallel layout (round 2; round 1 ran one LANE per limb arc with ~1.5 KB of per-lane state in local memory:
 // 250 registers, 8 warps per SM, 6 % of the FP64 pipe):
-//   one CTA per source point; the limb is cut into NARC arcs of consecutive limb points; an arc is followed by a
-//   GROUP of DEG = N^2+1 lanes, ONE LANE PER ROOT of the lens polynomial. Everything indexed by root slot in the
+//   the limb of a source point is cut into NARC arcs of consecutive limb points; an arc is followed by a GROUP of
+//   DEG = N^2+1 lanes, ONE LANE PER ROOT of the lens polynomial; a warp holds GPW groups, and the WARPS = NARC / GPW warps
+//   of a point run independently of each other (no barrier: a first version with one CTA per point spent a quarter
+//   of its stall samples waiting at the CTA's final barrier for its slowest warp). Everything indexed by root slot in the
 //   paper's algorithm is then a per-lane scalar in registers: the root, the image it polishes to, the previous
 //   image (warm start / continuation), the box of the arc this slot is drawing. What couples the roots goes
 //   through the group: the polynomial coefficients (lane l computes b_l; shared memory), the Aberth repulsion sum
@@ -35,13 +37,11 @@ struct LimbGeom {
     static constexpr int THREADS = 32 * WARPS;
 };
 
+// shared memory of ONE WARP (its GPW arcs); the warps of a CTA are independent of each other
 template <int N>
 struct LimbShared {
-    double2 coef[LimbGeom<N>::NARC][N * N + 2];          // b_0 .. b_DEG of the arc's current limb point
-    double2 z[LimbGeom<N>::NARC][N * N + 1];             // the roots during the simultaneous iteration
-    int n_box;
-    unsigned status;
-    int n_solves;
+    double2 coef[LimbGeom<N>::GPW][N * N + 2];           // b_0 .. b_DEG of the arc's current limb point
+    double2 z[LimbGeom<N>::GPW][N * N + 1];              // the roots during the simultaneous iteration
 };
 
 #define UL_FULL 0xffffffffu
@@ -91,7 +91,7 @@ __device__ __forceinline__ int ea_coop(bool run, bool frozen, const double2* coe
 {
     bool done = !run || frozen;
     bool bad = false;
-    double prev = 1e300;
+    double prev_s2 = 1e300, prev_den = 1.0;             // the previous step as (|step|^2, |z|^2): rel = s2 / den without dividing
     int its = 0;
     if (run) zs[j] = make_double2(zr, zi);
     __syncwarp();
@@ -126,10 +126,11 @@ __device__ __forceinline__ int ea_coop(bool run, bool frozen, const double2* coe
                 if (a2 > 1e-300) { const double ia = 1.0 / a2; stx = (nx * ax + ny * ay) * ia; sty = (ny * ax - nx * ay) * ia; }
                 else { stx = nx; sty = ny; }
                 nzr = zr - stx; nzi = zi - sty;
-                const double rel = (stx * stx + sty * sty) / (nzr * nzr + nzi * nzi + 1e-12);
-                if (!(rel == rel)) bad = true;
-                if (rel < tol2 || (rel < 1e-6 && rel > 0.5 * prev)) done = true;
-                prev = rel;
+                const double s2 = stx * stx + sty * sty, den = nzr * nzr + nzi * nzi + 1e-12;
+                if (!(s2 == s2) || !(den == den)) bad = true;
+                // rel < tol2  ||  (rel < 1e-6 && rel > 0.5 prev),  rel = s2 / den
+                if (s2 < tol2 * den || (s2 < 1e-6 * den && s2 * prev_den > 0.5 * prev_s2 * den)) done = true;
+                prev_s2 = s2; prev_den = den;
             }
         }
         __syncwarp();                                    // everyone has read the old positions
@@ -203,23 +204,25 @@ __device__ __forceinline__ void adopt_candidates(bool run, int j, int gbase, uns
     (void)DEG;
 }
 
-// The limb tracker of one source point. All threads of the CTA call it.
+// The limb tracker of one warp of one source point (warp = 0 .. WARPS-1: which arcs). All 32 lanes call it.
+// n_box: the point's box counter (global memory, zeroed before the launch); returns this lane's status bits and
+// adds the warp's limb solves to n_solves_out.
 template <int N, bool DUAL>
-__device__ void limb_track(LimbShared<N>& sh, const Lens& L, const LensPoly& T, double wcx, double wcy, double rho,
-                           const RegionParams& P, const double* __restrict__ czr, const double* __restrict__ czi,
-                           unsigned cmask, SubBox* boxes, BoxExt* exts, int box_cap)
+__device__ unsigned limb_track(LimbShared<N>& sh, int warp, const Lens& L, const LensPoly& T, double wcx, double wcy, double rho,
+                               const RegionParams& P, const double* __restrict__ czr, const double* __restrict__ czi,
+                               unsigned cmask, SubBox* boxes, BoxExt* exts, int* n_box, int box_cap, int& n_solves_out)
 {
     typedef LimbGeom<N> G;
     constexpr int DEG = G::DEG;
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int lane = threadIdx.x & 31;
     const int gw = lane / DEG;
     const bool active = gw < G::GPW;
     const int gbase = active ? gw * DEG : 0;
     const int j = active ? lane - gbase : 0;
     const int arc = active ? warp * G::GPW + gw : 0;
     const unsigned gmask = active ? (((1u << DEG) - 1u) << gbase) : 0u;
-    double2* coef = sh.coef[arc];
-    double2* zs = sh.z[arc];
+    double2* coef = sh.coef[active ? gw : 0];
+    double2* zs = sh.z[active ? gw : 0];
 
     // light lenses (eps_a < 1e-2) whose planetary caustic -- centred on w_a = a_a - sum_{b != a} eps_b/conj(a_a - a_b),
     // a few sqrt(eps_a) across -- the source overlaps or nearly so (triple lens: images hidden in a root cluster)
@@ -319,16 +322,20 @@ __device__ void limb_track(LimbShared<N>& sh, const Lens& L, const LensPoly& T, 
         // ---- Eq. 7. Warm start from the previous limb point (cap 24); cold from the Cauchy circle (cap 64) for the
         // arc's first point or when the warm solve hits its cap.
         // (`first` is the same for every running group of the warp: all arcs take their first point in the same pass)
+        // One call site for both passes (code size: the kernel is instruction-fetch bound): pass 0 is the warm solve
+        // (cold at an arc's first point), pass 1 the cold restart of the groups whose warm solve failed.
         bool cold = first;
-        if (run && cold) ea_init_sh<DEG>(coef, j, zr, zi);
-        int it = ea_coop<DEG>(run, frozen, coef, zs, j, gmask, zr, zi, __any_sync(UL_FULL, run && first) ? 64 : 24, UL_EA_LIMB_TOL2);
-        {
-            const bool need_cold = run && !cold && it > 24;
-            if (__any_sync(UL_FULL, need_cold)) {
-                if (need_cold) { frozen = false; ea_init_sh<DEG>(coef, j, zr, zi); }
-                const int it2 = ea_coop<DEG>(need_cold, false, coef, zs, j, gmask, zr, zi, 64, UL_EA_LIMB_TOL2);
-                if (need_cold) { it = it2; cold = true; }
-            }
+        int it = 0;
+        bool go = run;
+#pragma unroll 1
+        for (int pass = 0; pass < 2; ++pass) {
+            if (go && cold) { frozen = false; ea_init_sh<DEG>(coef, j, zr, zi); }
+            const int cap = __any_sync(UL_FULL, go && cold) ? 64 : 24;
+            const int itp = ea_coop<DEG>(go, frozen, coef, zs, j, gmask, zr, zi, cap, UL_EA_LIMB_TOL2);
+            if (go) it = itp;
+            go = run && !cold && it > 24;                // warm solve hit its cap: restart this group from the Cauchy circle
+            if (!__any_sync(UL_FULL, go)) break;
+            if (go) cold = true;
         }
         const bool noconv = run && it > (cold ? 64 : 24);
         if (run && j == 0) ++n_solves;
@@ -368,7 +375,7 @@ __device__ void limb_track(LimbShared<N>& sh, const Lens& L, const LensPoly& T, 
                 for (int i = 0; i < N; ++i) { double dx = zr - L.ax[i], dy = zi - L.ay[i]; dm2 = ul_min(dm2, dx * dx + dy * dy); }
                 // (0.04: the acceptance test below allows a total move of 10 % of that distance, so a first step
                 // beyond 20 % is rejected either way -- after one iteration instead of six)
-                ok = polish_image<N>(L, wx, wy, px, py, 6, 1e-9, detJ, resid, gx, gy, 0.04, false);
+                ok = polish_image<N>(L, wx, wy, px, py, 6, 1e-9, detJ, resid, gx, gy, 0.04, false);   // (inlined: measured 12 % faster on C4 than the out-of-line copy)
                 // along the limb a slot must follow ONE image continuously: a polish that carries the EA root
                 // further than 10 % of its distance to the nearest lens has jumped to some other image
                 const double mv2 = (px - zr) * (px - zr) + (py - zi) * (py - zi);
@@ -478,7 +485,7 @@ __device__ void limb_track(LimbShared<N>& sh, const Lens& L, const LensPoly& T, 
                 // finished and a new one starts.
                 if (ab.open) {
                     const double dx = px - ab.lastx, dy = py - ab.lasty;
-                    if (dx * dx + dy * dy > 0.0036 * ul_max(rr * rr, 0.04)) arcbox_flush<DUAL>(ab, E, &sh.n_box, box_cap, boxes, exts, status);
+                    if (dx * dx + dy * dy > 0.0036 * ul_max(rr * rr, 0.04)) arcbox_flush<DUAL>(ab, E, n_box, box_cap, boxes, exts, status);
                 }
                 if (!ab.open) { arcbox_start(ab); if (DUAL) ext_reset(E); }
                 box_add(ab.B, ab.t_cur, rr, atan2(py, px), hr, ht, cr, ct, true);
@@ -541,9 +548,9 @@ __device__ void limb_track(LimbShared<N>& sh, const Lens& L, const LensPoly& T, 
             if (!(ph < ph_end - 1e-9 * dphi)) arc_done = true;
         }
     }
-    arcbox_flush<DUAL>(ab, E, &sh.n_box, box_cap, boxes, exts, status);
-    if (status) atomicOr(&sh.status, status);
-    if (n_solves) atomicAdd(&sh.n_solves, n_solves);
+    arcbox_flush<DUAL>(ab, E, n_box, box_cap, boxes, exts, status);
+    n_solves_out = n_solves;
+    return status;
 }
 
 }  // namespace ulens

@@ -98,25 +98,29 @@ UL_HDNI bool parabola_vertex(double x0, double y0, double x1, double y1, double 
 // radius rho is an ellipse with semi-axes rho/(1+|g|) (along arg(g)/2) and rho/|1-|g|| (perpendicular);
 // hr, ht = its half-extents (projections) along the radial / azimuthal direction at z; cr, ct = its
 // half-chords through the centre along those directions.
+// (single precision: the extents only size the ray grid and the box margins)
 UL_HDNI void local_extents(double zx, double zy, double gx, double gy, double rho, double& hr, double& ht,
                          double& cr, double& ct)
 {
-    double ga = sqrt(gx * gx + gy * gy);
-    double m = rho / (1.0 + ga);
-    double den = fabs(1.0 - ga);
-    double M = den > 1e-6 ? rho / den : rho * 1e6;
-    double z2 = zx * zx + zy * zy;
-    double c2 = 0.0;                                    // cos(2 phi), phi = angle(major axis) - angle(radial)
-    if (ga > 1e-300 && z2 > 1e-300) {
+    const float fgx = (float)gx, fgy = (float)gy, fzx = (float)zx, fzy = (float)zy, frho = (float)rho;
+    const float ga = sqrtf(fgx * fgx + fgy * fgy);
+    const float m = frho / (1.0f + ga);
+    const float den = fabsf((float)(1.0 - sqrt(gx * gx + gy * gy)));     // 1 - |g| in double: |g| -> 1 on a critical curve
+    const float M = den > 1e-6f ? frho / den : frho * 1e6f;
+    const float z2 = fzx * fzx + fzy * fzy;
+    float c2 = 0.0f;                                     // cos(2 phi), phi = angle(major axis) - angle(radial)
+    if (ga > 1e-30f && z2 > 1e-30f) {
         // Re(g conj(z)^2) / (|g||z|^2) = cos(arg g - 2 theta);  major axis at arg(g)/2 + pi/2
-        double re = gx * (zx * zx - zy * zy) + gy * (2.0 * zx * zy);
+        const float re = fgx * (fzx * fzx - fzy * fzy) + fgy * (2.0f * fzx * fzy);
         c2 = -re / (ga * z2);
+        c2 = c2 > 1.0f ? 1.0f : (c2 < -1.0f ? -1.0f : c2);
     }
-    double cc = 0.5 * (1.0 + c2), ss = 0.5 * (1.0 - c2);
-    hr = sqrt(M * M * cc + m * m * ss);
-    ht = sqrt(M * M * ss + m * m * cc);
-    cr = 1.0 / sqrt(cc / (M * M) + ss / (m * m));
-    ct = 1.0 / sqrt(ss / (M * M) + cc / (m * m));
+    const float cc = 0.5f * (1.0f + c2), ss = 0.5f * (1.0f - c2);
+    const float M2 = M * M, m2 = m * m;
+    hr = (double)sqrtf(M2 * cc + m2 * ss);
+    ht = (double)sqrtf(M2 * ss + m2 * cc);
+    cr = (double)(1.0f / sqrtf(cc / M2 + ss / m2));
+    ct = (double)(1.0f / sqrtf(ss / M2 + cc / m2));
 }
 
 // margins applied to every box before grouping: a quarter of the local minor scale in both directions
