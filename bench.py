@@ -381,7 +381,7 @@ def main_ours(args, rank, local_rank, world):
     ctx = binding.Context(local_rank)
     env = Env(torch, dist, binding, inputs, replicas, ctx, dev, local_rank, world)
 
-    r = measure_config(env, args.config, args.steps, args.warmup, switch=args.switch, with_e2e=True, with_clocks=True)
+    r = measure_config(env, args.config, args.steps, args.warmup, switch=args.switch, with_e2e=True, with_clocks=True, f32=args.f32)
     others = {}
     if args.all_configs and world == 1:
         # the other BASELINE configs through the same code path, short runs (W = 3 warm-up, 2 timed steps)
@@ -419,7 +419,7 @@ def main_ours(args, rank, local_rank, world):
                 "config": {"workload": workload_name(wl), "rho": [float(wl.rho.min()), float(wl.rho.max())],
                            "u1": [float(wl.u1.min()), float(wl.u1.max())],
                            "outputs": "A and dA/d(t0,u0,tE,s,q,rho,alpha) per epoch (forward-mode variant, step a8)" if dual else "A per point",
-                           "switch": bool(args.switch),
+                           "switch": bool(args.switch), "f32_shoot": bool(args.f32),
                            "l2": "flushed between timed steps (256 MiB fill)",
                            "parallelism": "replicas" if world > 1 else "1 GPU"},
                 "rays_per_s": r["rays_per_s"], "rays_per_point": r["rays_per_point"],
@@ -499,10 +499,15 @@ def main():
     ap.add_argument("--switch", action="store_true",
                     help="config 4 only: ulens_lightcurve_binary_ext (point-source value for the far epochs, P:153; "
                          "library selection at the default tolerance) instead of the finite-source path on every epoch")
+    ap.add_argument("--f32", action="store_true",
+                    help="configs 0-3 only: the mixed-precision variant (ULENS_OPT_F32_SHOOT, SURVEY 8.f-1) as the measured path; "
+                         "roofline is then k_shoot_f32 against the FP32 FMA peak")
     ap.add_argument("--stub", action="store_true", help=argparse.SUPPRESS)
     args = ap.parse_args()
     if args.switch and args.config != 4:
         ap.error("--switch needs --config 4")
+    if args.f32 and args.config == 4:
+        ap.error("--f32: the forward-mode variant (config 4) always runs in FP64")
     if args.gpus < 1:
         ap.error("--gpus must be >= 1")
     if "WORLD_SIZE" not in os.environ and args.gpus > 1 and args.impl != "reference":

@@ -574,17 +574,17 @@ UL_HDN unsigned centre_images(const Lens& L, const LensPoly& T, double wx, doubl
 // ------------------------------------------------------------------------------------------------
 
 // zeta(-1/2, u) and zeta(-3/2, u) for u in (0, 1]: Hurwitz zeta = u^(-s) + zeta(s, 1+u); the smooth part
-// zeta(s, 1+u) is a degree-9 least-squares fit on Chebyshev nodes of [0,1] (max error 7e-10 / 2e-10). The ONE copy
+// zeta(s, 1+u) is a degree-9 least-squares fit at 64 Chebyshev nodes of [0,1] (max error 6e-10 / 2e-10). The ONE copy
 // of the tables; paper_2510_02639_b200/csrc/fit_zeta_tables.py regenerates them (mpmath) and tests/test_host_logic.py
-// checks them against mpmath.zeta to 1e-9.
-#define UL_ZETA_M12_COEFFS {-0.207886224314425946, -0.730177387536053191, -0.326542433690562406, \
-                            0.0837832566266219698, -0.0435998186937335486, 0.0271396135617846347, \
-                            -0.0165300041688832568, 0.00823252937110980637, -0.00274063185833692022, \
-                            0.000434876090612478912}
-#define UL_ZETA_M32_COEFFS {-0.0254852020522020475, -0.311829304876540199, -0.547634035662697937, \
-                            -0.163258961591498412, 0.0313415948971861593, -0.0127998326381573904, \
-                            0.00616325441161647825, -0.00268571587959467142, 0.000828839924548779593, \
-                            -0.0001258385180165005}
+// checks them against mpmath.zeta to 1e-9 and against the script's output.
+#define UL_ZETA_M12_COEFFS {-0.207886224399935288, -0.730177374187579331, -0.326542779711049336, \
+                            0.0837867303083785903, -0.0436173603868350857, 0.0271895277281179355, \
+                            -0.0166136306767131411, 0.00831433648693249115, -0.00278385068661135939, \
+                            0.0004444009766404081}
+#define UL_ZETA_M32_COEFFS {-0.0254852020332272215, -0.311829307850673643, -0.547633958335979165, \
+                            -0.163259739667364207, 0.0313455313556175105, -0.0128110506256419159, \
+                            0.00618207285304185443, -0.0027041446390176113, 0.000838584837043554769, \
+                            -0.000127987893602585462}
 // value and derivative of the degree-9 polynomial c[0] + c[1] u + ...
 UL_HD void zeta_poly(const double (&c)[10], double u, double& p, double& dp)
 {

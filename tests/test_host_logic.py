@@ -131,3 +131,34 @@ def test_resolution_knobs_converge(exe):
     assert coarse_limb["n_patch"] == base["n_patch"]
     assert abs(coarse_limb["A"] / base["A"] - 1) < 3e-5
     assert fine["rays"] > 4 * base["rays"]
+
+
+def _zeta_tables():
+    import re
+    src = open(os.path.join(HERE, "..", "paper_2510_02639_b200", "csrc", "ulens_core.cuh")).read()
+    out = {}
+    for name in ("UL_ZETA_M12_COEFFS", "UL_ZETA_M32_COEFFS"):
+        body = re.search(r"#define %s \{([^}]*)\}" % name, src, re.S).group(1).replace("\\", " ")
+        out[name] = np.array([float(x) for x in body.split(",")])
+    return out
+
+
+def test_hurwitz_zeta_tables_against_mpmath():
+    """The one copy of the end-correction tables (ulens_core.cuh): zeta(s, u) = u^(-s) + poly(u) against mpmath.zeta for
+    s = -1/2, -3/2 on (0, 1] to 1e-9, and identical to what the committed fit script produces."""
+    import mpmath as mp
+    import subprocess
+    import sys
+    tabs = _zeta_tables()
+    for name, s in (("UL_ZETA_M12_COEFFS", -0.5), ("UL_ZETA_M32_COEFFS", -1.5)):
+        c = tabs[name]
+        assert len(c) == 10
+        for u in np.linspace(1e-6, 1.0, 257):
+            mine = u ** (-s) + np.polynomial.polynomial.polyval(u, c)
+            assert abs(mine - float(mp.zeta(s, mp.mpf(float(u))))) < 1e-9, (name, u)
+    out = subprocess.run([sys.executable, os.path.join(HERE, "..", "paper_2510_02639_b200", "csrc", "fit_zeta_tables.py")],
+                         capture_output=True, text=True, check=True).stdout
+    for name in tabs:
+        line = [ln for ln in out.splitlines() if name in ln][0]
+        vals = np.array([float(x) for x in line[line.index("{") + 1: line.index("}")].split(",")])
+        assert np.array_equal(vals, tabs[name])
