@@ -28,6 +28,7 @@ struct SubBox {
 #endif
 #define UL_MAXP 12          // sector cap per point ("capped based on the maximum expected number of images")
 #define UL_MAXG 16          // groups per axis
+#define UL_MAXG_TMP 64      // ... while the boxes are still arriving: disjoint groups form first and are bridged later
 
 struct RegionParams {
     int n_limb;             // multiple of 32
@@ -236,8 +237,10 @@ UL_HD void ext_reset(BoxExt& x)
     x.tlo_t = 1e300; x.thi_t = -1e300; x.tlo_x = x.tlo_y = x.tlo_ph = x.thi_x = x.thi_y = x.thi_ph = 0.0;
 }
 
-// union of intervals, order independent: insert [lo, hi] into the list of disjoint groups, merging every group it
-// touches; at the cap the interval joins the nearest group instead of opening a new one
+// union of intervals, order independent: insert [lo, hi] into the list of disjoint groups (room for UL_MAXG_TMP), merging
+// every group it touches; at that cap the interval joins the nearest group instead of opening a new one (the only
+// order-dependent step: 64 disjoint groups at once have not been seen). interval_reduce brings the final, sorted list
+// down to UL_MAXG by closing the narrowest gaps.
 UL_HD bool interval_absorb(double* g_lo, double* g_hi, int& ng, double lo, double hi)
 {
     int first = -1;                                      // the group that has absorbed [lo, hi] so far
@@ -261,7 +264,7 @@ UL_HD bool interval_absorb(double* g_lo, double* g_hi, int& ng, double lo, doubl
 UL_HD void interval_insert(double* g_lo, double* g_hi, int& ng, double lo, double hi)
 {
     if (interval_absorb(g_lo, g_hi, ng, lo, hi)) return;
-    if (ng < UL_MAXG) { g_lo[ng] = lo; g_hi[ng] = hi; ++ng; return; }
+    if (ng < UL_MAXG_TMP) { g_lo[ng] = lo; g_hi[ng] = hi; ++ng; return; }
     // at the cap: join the nearest group, then absorb whatever the grown group touches
     int best = 0; double bd = 1e300;
     for (int g = 0; g < ng; ++g) { double d = lo > g_hi[g] ? lo - g_hi[g] : g_lo[g] - hi; if (d < bd) { bd = d; best = g; } }
@@ -276,6 +279,17 @@ UL_HD void interval_sort(double* g_lo, double* g_hi, int ng)
         double lo = g_lo[a], hi = g_hi[a]; int b = a - 1;
         while (b >= 0 && g_lo[b] > lo) { g_lo[b + 1] = g_lo[b]; g_hi[b + 1] = g_hi[b]; --b; }
         g_lo[b + 1] = lo; g_hi[b + 1] = hi;
+    }
+}
+
+UL_HD void interval_reduce(double* g_lo, double* g_hi, int& ng, int cap)
+{
+    while (ng > cap) {                                   // (sorted list) close the narrowest gap
+        int best = 0; double bd = 1e300;
+        for (int g = 0; g + 1 < ng; ++g) { const double d = g_lo[g + 1] - g_hi[g]; if (d < bd) { bd = d; best = g; } }
+        g_hi[best] = ul_max(g_hi[best], g_hi[best + 1]);
+        for (int k = best + 1; k + 1 < ng; ++k) { g_lo[k] = g_lo[k + 1]; g_hi[k] = g_hi[k + 1]; }
+        --ng;
     }
 }
 
@@ -310,7 +324,7 @@ UL_HDN int sectors_from_boxes(const SubBox* box, const BoxExt* ext, int nb, cons
     if (nb == 0) { status |= UL_ST_NO_IMAGE; return 0; }
 
     // ---- r groups
-    double gr_lo[UL_MAXG], gr_hi[UL_MAXG];
+    double gr_lo[UL_MAXG_TMP], gr_hi[UL_MAXG_TMP];
     int ngr = 0;
     for (int i = 0; i < nb; ++i) {
         double rl, rh, tl, th;
@@ -319,6 +333,7 @@ UL_HDN int sectors_from_boxes(const SubBox* box, const BoxExt* ext, int nb, cons
     }
     interval_sort(gr_lo, gr_hi, ngr);
     interval_merge_necks(gr_lo, gr_hi, ngr);
+    interval_reduce(gr_lo, gr_hi, ngr, UL_MAXG);
     // ---- fill gaps whose circles are inside the image
     bool ring_group[UL_MAXG];
     {
@@ -370,7 +385,7 @@ UL_HDN int sectors_from_boxes(const SubBox* box, const BoxExt* ext, int nb, cons
             continue;
         }
         // ---- theta groups of this r-group's members: intervals on the circle, t_lo in [-pi, pi), span <= 2 pi
-        double gt_lo[UL_MAXG], gt_hi[UL_MAXG];
+        double gt_lo[UL_MAXG_TMP], gt_hi[UL_MAXG_TMP];
         int ngt = 0;
         bool full_ring = false;
         for (int i = 0; i < nb && !full_ring; ++i) {
@@ -392,8 +407,8 @@ UL_HDN int sectors_from_boxes(const SubBox* box, const BoxExt* ext, int nb, cons
             if (th - tl >= 2.0 * UL_PI) { full_ring = true; break; }
             const double sh = 2.0 * UL_PI * floor((tl + UL_PI) / (2.0 * UL_PI));      // t_lo back to [-pi, pi)
             tl -= sh; th -= sh;
-            if (ngt < UL_MAXG) { gt_lo[ngt] = tl; gt_hi[ngt] = th; ++ngt; }
-            else { full_ring = true; }                   // more arcs than groups: one ring around them all
+            if (ngt < UL_MAXG_TMP) { gt_lo[ngt] = tl; gt_hi[ngt] = th; ++ngt; }
+            else { full_ring = true; }                   // more disjoint arcs at once than there is room for: one ring
         }
         if (!full_ring) {
             interval_sort(gt_lo, gt_hi, ngt);
@@ -408,6 +423,7 @@ UL_HDN int sectors_from_boxes(const SubBox* box, const BoxExt* ext, int nb, cons
                 }
             }
             for (int g = 0; g < ngt; ++g) if (gt_hi[g] - gt_lo[g] >= 2.0 * UL_PI - 1e-12) full_ring = true;
+            if (ngt > UL_MAXG) full_ring = true;         // more arcs than sectors: one ring around them all
         }
         if (full_ring) { gt_lo[0] = -UL_PI; gt_hi[0] = UL_PI; ngt = 1; }
         // ---- tight bounds of each theta-group's members
@@ -452,15 +468,21 @@ UL_HDN int sectors_from_boxes(const SubBox* box, const BoxExt* ext, int nb, cons
         }
         for (int c = 0; c < ngt; ++c) {
             if (c_rl[c] > c_rh[c]) continue;
+            // free space to the neighbouring cells, from the cells' TIGHT bounds (minima / maxima of member values: the same
+            // whatever order the boxes arrived in; the group bounds gt_* went through +- 2 pi shifts while they were merged
+            // and carry order-dependent rounding in their last bits)
             double gap_lo, gap_hi;
-            if (ngt == 1) { gap_lo = gap_hi = 2.0 * UL_PI - (gt_hi[0] - gt_lo[0]); }
+            if (ngt == 1) { gap_lo = gap_hi = 2.0 * UL_PI - (c_th[0] - c_tl[0]); }
             else {
                 int cp = (c + ngt - 1) % ngt, cn = (c + 1) % ngt;
-                gap_lo = gt_lo[c] - gt_hi[cp]; if (c == 0) gap_lo += 2.0 * UL_PI;
-                gap_hi = gt_lo[cn] - gt_hi[c]; if (c == ngt - 1) gap_hi += 2.0 * UL_PI;
-                // a group that reaches across the cut may sit a full turn away
+                while (c_rl[cp] > c_rh[cp] && cp != c) cp = (cp + ngt - 1) % ngt;          // (skip cells without members)
+                while (c_rl[cn] > c_rh[cn] && cn != c) cn = (cn + 1) % ngt;
+                gap_lo = c_tl[c] - c_th[cp];
+                gap_hi = c_tl[cn] - c_th[c];
+                // neighbouring cells live in their own turns of the circle
                 gap_lo -= 2.0 * UL_PI * floor(gap_lo / (2.0 * UL_PI));
                 gap_hi -= 2.0 * UL_PI * floor(gap_hi / (2.0 * UL_PI));
+                if (cp == c) gap_lo = gap_hi = 2.0 * UL_PI - (c_th[c] - c_tl[c]);
             }
             if (np == UL_MAXP) { capped = true; break; }
             // Scan lines run ACROSS the long axis of the sector. Images near the Einstein ring are arcs that
