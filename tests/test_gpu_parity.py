@@ -145,6 +145,25 @@ def test_root_sets_match_oracle(ctx, torch_cuda, oracle, kind):
     assert n_cmp > 0.9 * n
 
 
+def _newton_eq1_mp(olens, w, z0, digits=50):
+    """Newton on Eq. 1 itself (w = z - sum eps_i / conj(z - a_i)) in multi-precision arithmetic from z0:
+    dz = (b - g conj(b)) / (1 - |g|^2), b = w - w(z), g = sum eps_i / conj(z - a_i)^2. Returns (z, |residual|)."""
+    import mpmath as mp
+    with mp.workdps(digits):
+        eps = [mp.mpf(float(e)) for e in olens.masses()]
+        a = [mp.mpc(complex(x)) for x in olens.positions()]
+        z, wq = mp.mpc(z0), mp.mpc(w)
+        for _ in range(60):
+            f = z - sum(e / mp.conj(z - ai) for e, ai in zip(eps, a)) - wq
+            if abs(f) < mp.mpf(10) ** (-(digits - 5)):
+                break
+            g = sum(e / mp.conj(z - ai) ** 2 for e, ai in zip(eps, a))
+            b = -f
+            z = z + (b - g * mp.conj(b)) / (1 - abs(g) ** 2)
+        f = z - sum(e / mp.conj(z - ai) for e, ai in zip(eps, a)) - wq
+        return complex(z), float(abs(f))
+
+
 @pytest.mark.parametrize("cfg", [1, 3])
 def test_root_sets_on_workload_lenses(ctx, torch_cuda, oracle, cfg):
     """Root-set parity on the lens draws of BASELINE C1 / C3 themselves, including the lightest companions (C1: q down to
@@ -193,16 +212,17 @@ def test_root_sets_on_workload_lenses(ctx, torch_cuda, oracle, cfg):
                     # absent on the GPU side: only an ultra-faint image next to a light lens may be
                     assert 1.0 / abs(r["detJ"][m]) < 1e-8, (cfg, c, k, a, d[j], r["detJ"][m])
                     n_absent += 1
-            # no GPU image the oracle does not have -- except (8c-C iii) an oracle ROOT that misses the oracle's validation
-            # threshold (1e-18) narrowly: Eq.-1 residual < 1e-14, six orders below the smallest residual of a spurious root
-            # (> 1e-8, test_oracle_pins). These are faint images next to a light lens (kappa 1e5 ... 1e10), which the
-            # extended-precision refinement of the POLYNOMIAL root leaves at a residual of a few 1e-17 on Eq. 1; the GPU side
-            # polishes on Eq. 1 itself. Counted and printed.
+            # no GPU image the oracle does not have -- except images the oracle's classification leaves out: next to a light
+            # lens (kappa 1e5 ... 1e10) the extended-precision refinement of the POLYNOMIAL root can stall short of the
+            # oracle's validation threshold on Eq. 1 (8c-C iii). Such a GPU image must (a) coincide with an oracle root and
+            # (b) be an image by the definition itself: Newton on Eq. 1 in 50-digit arithmetic, started from it, converges
+            # (residual < 1e-40) without leaving its 1e-10 neighbourhood. Counted and printed.
             for zz in zg[~used]:
                 dd = np.abs(r["z"] - zz)
                 m = int(np.argmin(dd))
-                assert dd[m] <= TOL_ROOT * max(1.0, abs(zz)) and r["resid"][m] < 1e-14, \
-                    (cfg, c, k, zz, dd[m], r["resid"][m], r["detJ"][m])
+                z50, res50 = _newton_eq1_mp(olens, complex(w[k]), complex(zz))
+                assert dd[m] <= TOL_ROOT * max(1.0, abs(zz)) and res50 < 1e-40 and abs(z50 - zz) <= TOL_ROOT * max(1.0, abs(zz)), \
+                    (cfg, c, k, zz, dd[m], r["resid"][m], res50, abs(z50 - zz))
                 n_extra += 1
             n_cmp += 1
     print("C%d root sets: %d lenses (lightest companion %.1e), %d source positions compared (%d skipped on a caustic), %d images "
