@@ -42,19 +42,27 @@ UNIT = "magnifications/s"
 # the lens map with one reciprocal per ray, the rotation recurrence, d^2 and the inside test; the limb-
 # darkened figure adds the square root of the inside rays (about half of all rays).
 FP64_INSTR_PER_RAY = {(1, False): 27, (1, True): 32, (2, False): 35, (2, True): 40, (3, False): 47, (3, True): 52}
-# Forward-mode variant (binary, 5 intrinsic tangents): per tangent the moving ray dz (2), g conj(dz) (4), the explicit
-# lens-parameter term (0..8, mean 3), dF (4), accumulation (1) = 14, plus g itself (4 per ray): + 74 per ray.
-FP64_INSTR_PER_RAY_DUAL_EXTRA = 74
+# Forward-mode variant: SURVEY 8.d's per-unit figure for a ray that also carries the tangents, "dual variant ~ 2-2.5x" of the
+# primal count: its midpoint, 2.25x. (Round 1's kernel executed more than that -- 114 by its own itemised count; round 2's
+# kernel executes 91.5 DFMA + DMUL + DADD per ray on C4 by ncu's SASS counters, profiles/r02_ncu_shoot_dual_c4.md: the
+# unit of useful work is the survey's, not what a particular kernel spends on it. DESIGN.md 6.4.)
+FP64_DUAL_FACTOR = 2.25
 # k_limb: algorithmic FP64-pipe instructions per limb solve: coefficients ~26 DEG, warm-started
 # Ehrlich-Aberth 3 iterations x DEG roots x (8 DEG Horner + 12 (DEG-1) repulsion + 24), Eq.-1 polish of the
 # N+1..DEG images 2.5 iterations x (17 N + 25), boxes ~100.
 FP64_INSTR_PER_LIMB_SOLVE = {1: 600, 2: 2400, 3: 8300}
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the roofline kernel, from the `ncu --set full` captures
+# summarised under profiles/ (r02_ncu_shoot_dual_c4.md, r02_ncu_shoot_c1.md, r02_ncu_shoot_c2.md, r02_ncu_shoot_f32_c1.md);
+# key = (config, f32 variant)
+NCU_TRAFFIC_BYTES_PER_LAUNCH = {(4, False): 55.569152e6 + 724.669952e6, (1, False): 27.501056e6 + 0.717056e6,
+                                (2, False): 30.622720e6 + 5.162496e6, (1, True): 27.456512e6 + 1.179904e6}
 # FP64 FMA pipe of one B200: 148 SMs x 64 DFMA lanes / clk x 1.965 GHz (clocks.max.sm) -- DESIGN.md
 FP64_PEAK_DFMA = 148 * 64 * 1.965e9
 # Mixed-precision variant (k_shoot_f32): algorithmic FP32-pipe instructions per ray in the segment-local
-# difference form -- displacement (ring: series of sin x and cos x - 1, rotation of z0: 16; radial line: 3; mix 10), per lens
-# c + d, c (c + d), |.|^2, reciprocal, eps conj(d / p), accumulate: 16, F: 6, inside test + count: 2, sqrt on inside rays: 1.
-FP32_INSTR_PER_RAY = {(1, False): 34, (1, True): 35, (2, False): 50, (2, True): 51, (3, False): 66, (3, True): 67}
+# difference form along a radial line (the common scan direction) -- displacement t (cos, sin): 4; per lens c + d (2), c (c + d)
+# (4), |.|^2 (2), eps x reciprocal (1), eps conj(d / p) (4), accumulate (2, with the 2 above fused): 17; F: 6; inside test +
+# count: 2; sqrt on inside rays: 1. (ncu SASS counters on C1: 44 FFMA + FMUL + FADD per ray, profiles/r02_ncu_shoot_f32_c1.md.)
+FP32_INSTR_PER_RAY = {(1, False): 28, (1, True): 29, (2, False): 45, (2, True): 46, (3, False): 62, (3, True): 63}
 # FP32 FMA pipe: 148 SMs x 128 FFMA lanes / clk x 1.965 GHz (checked in-run by ulens_fp32_peak)
 FP32_PEAK_FFMA = 148 * 128 * 1.965e9
 
@@ -322,7 +330,7 @@ def measure_config(env: Env, cfg: int, steps: int, warmup: int, switch: bool = F
     shoot_ms, shoot_n = kms["k_shoot"]
     rays_per_step = stats["n_rays"] / steps
     rays_per_launch = stats["n_rays"] / max(shoot_n, 1)
-    ipr = FP64_INSTR_PER_RAY[(n_lens, ld)] + (FP64_INSTR_PER_RAY_DUAL_EXTRA if dual else 0)
+    ipr = FP64_INSTR_PER_RAY[(n_lens, ld)] * (FP64_DUAL_FACTOR if dual else 1.0)
     shoot_avg_s = shoot_ms * 1e-3 / max(shoot_n, 1)
     achieved = 2.0 * ipr * rays_per_launch / shoot_avg_s / 1e12
     peak = 2.0 * FP64_PEAK_DFMA / 1e12
@@ -332,9 +340,10 @@ def measure_config(env: Env, cfg: int, steps: int, warmup: int, switch: bool = F
         achieved = 2.0 * ipr * rays_per_launch / shoot_avg_s / 1e12
         peak = 2.0 * FP32_PEAK_FFMA / 1e12
     roofline = {"bound": "alu", "kernel": ("k_shoot_f32" if f32 else "k_shoot") if not dual else "k_shoot_dual", "achieved": achieved, "peak": peak,
-                "variant": "k_shoot_dual (value + 5 tangents per ray)" if dual else "k_shoot",
-                "unit": "TFLOP/s", "frac": achieved / peak, "traffic": None,
-                "traffic_note": "the path is ALU-bound; DRAM bytes of one launch are in the ncu captures under profiles/",
+                "variant": "k_shoot_dual (value + 5 tangents per ray)" if dual else ("k_shoot_f32" if f32 else "k_shoot"),
+                "unit": "TFLOP/s", "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH.get((cfg, bool(f32))),
+                "traffic_note": "dram__bytes_read.sum + dram__bytes_write.sum of ONE launch from the ncu --set full capture of this kernel on this "
+                                "config (profiles/r02_ncu_*.md), not measured in this run; null where no capture exists. The path is ALU-bound.",
                 "peak_source": "derived: 148 SM x 64 DFMA/clk x 1.965 GHz x 2 flop (DESIGN.md); "
                                "MEASURED_PEAKS.json has no FP64 entry",
                 ("fp32_instr_per_ray" if (f32 and not dual) else "fp64_instr_per_ray"): ipr, "rays_per_launch": rays_per_launch,
