@@ -609,13 +609,15 @@ UL_HD double zeta_m32(double u)
     return u * sqrt(u) + p;
 }
 // the same with d/du (forward-mode variant). d sqrt(u)/du is singular at u = 0 (a node exactly on the edge: the
-// rule is not differentiable there): that term is dropped below u = 1e-8
-UL_HD void zeta_m12_du(double u, double& z, double& dz)
+// rule is not differentiable there). That term is the counterpart of the first inside node's own weight
+// -1/(2 sqrt(-F)): the two cancel to leading order, so they are kept or dropped TOGETHER. keep_sing = the scan loop
+// kept the node's weight (-F above UL_DUAL_SING_FLOOR rho^2, ulens_dual.cuh).
+UL_HD void zeta_m12_du(double u, bool keep_sing, double& z, double& dz)
 {
     const double c[10] = UL_ZETA_M12_COEFFS;
     double p, dp; zeta_poly(c, u, p, dp);
     const double su = sqrt(u);
-    z = su + p; dz = (u > 1e-8 ? 0.5 / su : 0.0) + dp;
+    z = su + p; dz = ((keep_sing && u > 1e-14) ? 0.5 / su : 0.0) + dp;
 }
 UL_HD void zeta_m32_du(double u, double& z, double& dz)
 {

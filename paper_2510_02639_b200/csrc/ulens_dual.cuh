@@ -179,7 +179,7 @@ UL_HD void stat_contract(const Lens& L, const TangentTable& T, double rho, const
 // for the discrete rule);  d p'(x) = sum_k l_k'(x) df_k + p''(x) dx,  d p''(x) = sum_k l_k''(x) df_k + p'''(x) dx;
 // u, sigma, tau and the Hurwitz-zeta end correction are smooth functions of (x, p', p'').
 // (out of line: an event is rare next to the rays, and inlined at the flush site it costs the scan loops ~60 registers)
-UL_HDNI void edge_event_adj(double f0, double f1, double f2, double f3, bool want_S, double t2_extra,
+UL_HDNI void edge_event_adj(double f0, double f1, double f2, double f3, bool want_S, bool keep_sing, double t2_extra,
                             double& u, bool& entering, double& dS, double* au, double* aS)
 {
     // rows: coefficient of x^0..x^3; columns: f0..f3
@@ -232,7 +232,7 @@ UL_HDNI void edge_event_adj(double f0, double f1, double f2, double f3, bool wan
         if (sigma > 0.0) {
             const double ss = sqrt(sigma);
             double z12, dz12, z32, dz32;
-            zeta_m12_du(u, z12, dz12);
+            zeta_m12_du(u, keep_sing, z12, dz12);
             zeta_m32_du(u, z32, dz32);
             const double t2 = tau / (2.0 * sigma) + (entering ? t2_extra : -t2_extra);
             const bool use32 = fabs(t2) < 0.5;
@@ -247,6 +247,10 @@ UL_HDNI void edge_event_adj(double f0, double f1, double f2, double f3, bool wan
         }
     }
 }
+
+// A node whose -F is below this fraction of rho^2 sits on the edge to rounding (the sector grids are anchored at limb
+// points, i.e. at exact edge points, so this happens ~1e-5 per source point, not ~1e-10): d sqrt(-F) does not exist there.
+#define UL_DUAL_SING_FLOOR 1e-10
 
 // Edge events in the tangent loops are DEFERRED as in the primal loops (ulens_core.cuh shoot_ring): the loop notes the node
 // of a sign change (two slots), the events are resolved in two extra passes after the rays, where the lanes of the warp
@@ -284,9 +288,10 @@ UL_HD void shoot_ring_t(const Lens& L, double wcx, double wcy, double rho2, doub
                 w[k] = R.F;
                 const double cn = wc * cd - ws * sd; ws = ws * cd + wc * sd; wc = cn;
             }
+            const bool keep = -w[pen ? 2 : 1] > UL_DUAL_SING_FLOOR * rho2;     // the loop's rule for the first inside node
             enforce_crossing(w[1], w[2], pen);
             double u, dS, au[4], aS[4]; bool en;
-            edge_event_adj(w[0], w[1], w[2], w[3], LD, 0.0, u, en, dS, au, aS);
+            edge_event_adj(w[0], w[1], w[2], w[3], LD, keep, 0.0, u, en, dS, au, aS);
             U += u - 0.5; S += dS;
             wc = cos(a); ws = sin(a);
 #pragma unroll 1
@@ -311,9 +316,13 @@ UL_HD void shoot_ring_t(const Lens& L, double wcx, double wcy, double rho2, doub
             if (LD) {
                 const double sq = sqrt(-f3);
                 S += sq;
-                RayBasis<N> B;
-                ray_basis<N, false>(L, R, r, c, s, B);
-                stat_add(SS, -0.5 / sq, B);              // d sqrt(-F) = -dF / (2 sqrt(-F))
+                // d sqrt(-F) = -dF / (2 sqrt(-F)); a node (numerically) ON the edge has no such derivative: its weight
+                // and its counterpart in the end correction (zeta_m12_du) are dropped together
+                if (-f3 > UL_DUAL_SING_FLOOR * rho2) {
+                    RayBasis<N> B;
+                    ray_basis<N, false>(L, R, r, c, s, B);
+                    stat_add(SS, -0.5 / sq, B);
+                }
             }
             if (!periodic && (j < 2 || j >= n_th - 2)) edge = true;
         }
@@ -359,13 +368,14 @@ UL_HD void shoot_col_t(const Lens& L, double wcx, double wcy, double rho2, doubl
                 ray_core<N>(L, rk * c, rk * s, wcx, wcy, rho2, R);
                 w[k] = R.F;
             }
+            const bool keep = -w[pen ? 2 : 1] > UL_DUAL_SING_FLOOR * rho2;
             enforce_crossing(w[1], w[2], pen);
             const double r1 = r0 + dr * (pi - 1.5);       // node pi - 2
             const double rh = r1 + 0.5 * dr;              // cell face between the pair
             const double rin = pen ? r1 + dr : r1;        // first inside node
             const double t2x = dr / ul_max(rin, 0.5 * dr);
             double u, dS, au[4], aS[4]; bool en;
-            edge_event_adj(w[0], w[1], w[2], w[3], LD, t2x, u, en, dS, au, aS);
+            edge_event_adj(w[0], w[1], w[2], w[3], LD, keep, t2x, u, en, dS, au, aS);
             double rc = en ? (r1 + dr) - u * dr : r1 + u * dr;
             const bool rc_free = rc > 0.0;
             rc = ul_max(rc, 0.0);
@@ -395,9 +405,11 @@ UL_HD void shoot_col_t(const Lens& L, double wcx, double wcy, double rho2, doubl
             if (LD) {
                 const double sq = sqrt(-f3);
                 S += r * sq;
-                RayBasis<N> B;
-                ray_basis<N, true>(L, R, r, c, s, B);
-                stat_add(SS, -0.5 * r / sq, B);
+                if (-f3 > UL_DUAL_SING_FLOOR * rho2) {
+                    RayBasis<N> B;
+                    ray_basis<N, true>(L, R, r, c, s, B);
+                    stat_add(SS, -0.5 * r / sq, B);
+                }
             }
             if ((i < 2 && r0 > 0.0) || i >= n_r - 2) edge = true;
         }
