@@ -46,6 +46,7 @@ extern "C" {
 #define ULENS_ECUDA        -2   /* a CUDA runtime call failed (ulens_last_cuda_error has the text) */
 #define ULENS_ENOMEM       -3   /* workspace allocation failed */
 #define ULENS_EUNSUPPORTED -4   /* valid request that this build does not implement */
+#define ULENS_ELIMIT       -5   /* ulens_mag_static: more points than the fixed scratch holds (ULENS_STATIC_MAX_POINTS) */
 
 /* per-point status bits (status_out) */
 #define ULENS_ST_EA_NOCONV   0x0001u  /* an Ehrlich-Aberth solve hit its iteration cap (Eq. 7) */
@@ -262,6 +263,32 @@ int  ulens_fp64_peak(ulens_ctx* ctx, double ms, double* dfma_per_s);
 
 /* The same for the FP32 pipe (FFMA/s): denominator of the mixed-precision variant's roofline. Synchronises. */
 int  ulens_fp32_peak(ulens_ctx* ctx, double ms, double* ffma_per_s);
+
+/* ---- no-allocation entry ----------------------------------------------------------------------------------------
+ * For callers that cannot allocate device memory (code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid cudaMalloc): ulens_mag WITHOUT a context and without any allocation. Same operation as ulens_mag on a context
+ * with default options and ULENS_OPT_NO_RETRY (steps a2-a7 of the hot path: Eq. 1-3, 7-8, App. A of the paper; one pass,
+ * no retry of doubtful points -- they keep their status bits), same argument meaning and layout:
+ *   cuda_device        device ordinal (made current); lenses_host / rho_host / u1_host: HOST arrays [n_cfg]
+ *   w_re, w_im         DEVICE [n_cfg][n_pts] source centres;  A_out DEVICE [n_cfg][n_pts]
+ *   err_out, status_out DEVICE [n_cfg][n_pts] or NULL;        stream: cudaStream_t (NULL = default stream)
+ * The whole workspace (tables, box lists, sector descriptors, unit queue, counters) is one file-scope device array of
+ * ulens_static_scratch_bytes() bytes (about 6 MiB) that EVERY GPU touched by this library holds until the process exits;
+ * it bounds the call to n_cfg * n_pts <= ULENS_STATIC_MAX_POINTS. A larger request returns ULENS_ELIMIT and does
+ * nothing -- use ulens_mag. The entry calls no cudaMalloc / cudaFree / cudaHostAlloc and no allocating library routine;
+ * it enqueues two small host-to-device copies (pageable source, staged by the runtime before the call returns), one
+ * memset and the five kernels of the path on `stream`, and does not wait for them.
+ * All calls (all threads, all streams) on one device SHARE the array, which keeps the last call's contents; what must
+ * start at zero is cleared on `stream` by the call itself. Two calls that overlap on the GPU (different streams, or
+ * different host threads) RACE on it: issue the calls of one device on one stream, or order them with events. Not
+ * thread-safe on the host either (static tables). ulens_static_last_cuda_error() has the text after ULENS_ECUDA. */
+#define ULENS_STATIC_MAX_POINTS 128
+int  ulens_mag_static(int cuda_device, int n_cfg, int n_pts, const ulens_lens* lenses_host, const double* rho_host,
+                      const double* u1_host, const double* w_re, const double* w_im, double* A_out, double* err_out,
+                      uint32_t* status_out, void* stream);
+int  ulens_static_max_points(void);
+long long ulens_static_scratch_bytes(void);
+const char* ulens_static_last_cuda_error(void);
 
 const char* ulens_strerror(int code);
 const char* ulens_last_cuda_error(ulens_ctx* ctx);

@@ -14,6 +14,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libulens.so")
 
 ULENS_OK, ULENS_EINVAL, ULENS_ECUDA, ULENS_ENOMEM, ULENS_EUNSUPPORTED = 0, -1, -2, -3, -4
+ULENS_ELIMIT = -5
 ST_EA_NOCONV, ST_IMG_PARITY, ST_PATCH_CAP, ST_RES_CAP = 0x1, 0x2, 0x4, 0x8
 ST_CLIPPED, ST_UNIT_OVF, ST_ERR_HIGH, ST_NO_IMAGE = 0x10, 0x20, 0x40, 0x80
 ST_NIMG_SHIFT = 8
@@ -22,7 +23,8 @@ KERNEL_NAMES = ["k_traj", "k_roots", "k_limb", "k_shoot", "k_finalize", "k_secto
 EXPORTS = ["ulens_create", "ulens_destroy", "ulens_lens_binary", "ulens_lens_triple", "ulens_mag", "ulens_mag_grad",
            "ulens_mag_host", "ulens_trajectory", "ulens_lightcurve_binary", "ulens_lightcurve_binary_host", "ulens_lightcurve_triple", "ulens_lightcurve_triple_host", "ulens_lightcurve_binary_ext", "ulens_lightcurve_binary_ext_host", "ulens_nll_marginal", "ulens_mag_point", "ulens_roots", "ulens_get_stats",
            "ulens_reset_stats", "ulens_last_launch_count", "ulens_set_timing", "ulens_get_kernel_ms", "ulens_fp64_peak", "ulens_fp32_peak", "ulens_strerror",
-           "ulens_last_cuda_error"]
+           "ulens_last_cuda_error", "ulens_mag_static", "ulens_static_max_points", "ulens_static_scratch_bytes",
+           "ulens_static_last_cuda_error"]
 
 
 ULENS_OPT_NO_RETRY = 0x1
@@ -92,6 +94,12 @@ def lib() -> C.CDLL:
         L.ulens_strerror.restype = C.c_char_p
         L.ulens_last_cuda_error.argtypes = [vp]
         L.ulens_last_cuda_error.restype = C.c_char_p
+        L.ulens_mag_static.argtypes = [ip, ip, ip, C.POINTER(ulens_lens), dp, dp, vp, vp, vp, vp, vp, vp]
+        L.ulens_static_max_points.argtypes = []
+        L.ulens_static_scratch_bytes.argtypes = []
+        L.ulens_static_scratch_bytes.restype = C.c_longlong
+        L.ulens_static_last_cuda_error.argtypes = []
+        L.ulens_static_last_cuda_error.restype = C.c_char_p
         _lib = L
     return _lib
 
@@ -134,6 +142,37 @@ def _dev(t, dtype, n):
     if not t.is_cuda or not t.is_contiguous() or t.dtype != dtype or t.numel() != n:
         raise UlensError("expected a contiguous CUDA tensor of dtype %s with %d elements" % (dtype, n))
     return C.c_void_p(t.data_ptr())
+
+
+def ulens_static_max_points() -> int:
+    return int(lib().ulens_static_max_points())
+
+
+def ulens_static_scratch_bytes() -> int:
+    return int(lib().ulens_static_scratch_bytes())
+
+
+def ulens_mag_static(device: int, lenses, rho, u1, w_re, w_im, A_out, err_out=None, status_out=None, stream=None):
+    """ulens_mag_static (include/ulens.h): ulens_mag without a context and without any allocation -- the caller
+    passes the inputs AND the outputs (CUDA tensors [n_cfg, n_pts]: float64, float64, int32), at most
+    ulens_static_max_points() points per call. `stream`: a torch.cuda.Stream (default: the device's current one).
+    Enqueue-only. Calls on one device share one scratch array: keep them on one stream."""
+    import torch
+    n_cfg, arr, rho, u1 = Context._cfg_arrays(lenses, rho, u1)
+    n_pts = w_re.numel() // max(n_cfg, 1)
+    n = n_cfg * n_pts
+    if stream is None:
+        stream = torch.cuda.current_stream(device)
+    rc = lib().ulens_mag_static(int(device), n_cfg, n_pts, arr, _dptr(rho), _dptr(u1),
+                                _dev(w_re, torch.float64, n), _dev(w_im, torch.float64, n),
+                                _dev(A_out, torch.float64, n), _dev(err_out, torch.float64, n),
+                                _dev(status_out, torch.int32, n), C.c_void_p(stream.cuda_stream))
+    if rc != ULENS_OK:
+        msg = lib().ulens_strerror(rc).decode()
+        if rc == ULENS_ECUDA:
+            msg += ": " + lib().ulens_static_last_cuda_error().decode()
+        raise UlensError(f"ulens error {rc}: {msg}")
+    return A_out, err_out, status_out
 
 
 class Context:

@@ -1001,6 +1001,7 @@ extern "C" const char* ulens_strerror(int code)
         case ULENS_ECUDA: return "CUDA error";
         case ULENS_ENOMEM: return "out of memory";
         case ULENS_EUNSUPPORTED: return "unsupported";
+        case ULENS_ELIMIT: return "size beyond the fixed scratch of the no-allocation entry (ULENS_STATIC_MAX_POINTS)";
         default: return "unknown error";
     }
 }
@@ -1943,4 +1944,149 @@ extern "C" int ulens_fp32_peak(ulens_ctx* ctx, double ms, double* ffma_per_s)
     cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d);
     *ffma_per_s = best;
     return ULENS_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ no-allocation entry
+//
+// ulens_mag_static: the finite-source magnification (steps a2 - a7, as ulens_mag without the retry pass) for callers
+// that cannot allocate device memory (CUDA graph capture, serving loops, harnesses that forbid cudaMalloc). The whole
+// per-chunk workspace -- configuration tables, roots of the source centres, box lists, sector descriptors, unit queue
+// and its sums, counters -- lives in ONE file-scope device array of fixed size; no context is needed. Every GPU that
+// loads the library holds the array (UL_STATIC_BYTES, about 6 MiB) until the process exits.
+// In host code `g_static_scratch` is only a stand-in for the symbol: its DEVICE address comes from
+// cudaGetSymbolAddress, once per device with that device current, and the kernels are given pointers carved from it.
+
+#define UL_STATIC_MAX_DEV 64
+constexpr size_t ul_align256(size_t x) { return (x + 255) & ~(size_t)255; }
+constexpr size_t UL_STATIC_UNITS   = (size_t)ULENS_STATIC_MAX_POINTS * 1024;          // per-point unit cap x points
+constexpr size_t UL_SO_CFG      = 0;
+constexpr size_t UL_SO_POLY     = UL_SO_CFG      + ul_align256(sizeof(PointCfg) * ULENS_STATIC_MAX_POINTS);
+constexpr size_t UL_SO_PATCHES  = UL_SO_POLY     + ul_align256(sizeof(LensPoly) * ULENS_STATIC_MAX_POINTS);
+constexpr size_t UL_SO_NPATCH   = UL_SO_PATCHES  + ul_align256(sizeof(Patch) * UL_MAXP * ULENS_STATIC_MAX_POINTS);
+constexpr size_t UL_SO_STATUS   = UL_SO_NPATCH   + ul_align256(sizeof(int) * ULENS_STATIC_MAX_POINTS);
+constexpr size_t UL_SO_CZR      = UL_SO_STATUS   + ul_align256(sizeof(unsigned) * ULENS_STATIC_MAX_POINTS);
+constexpr size_t UL_SO_CZI      = UL_SO_CZR      + ul_align256(sizeof(double) * 10 * ULENS_STATIC_MAX_POINTS);
+constexpr size_t UL_SO_CMASK    = UL_SO_CZI      + ul_align256(sizeof(double) * 10 * ULENS_STATIC_MAX_POINTS);
+constexpr size_t UL_SO_NBOXES   = UL_SO_CMASK    + ul_align256(sizeof(unsigned) * ULENS_STATIC_MAX_POINTS);
+constexpr size_t UL_SO_BOXES    = UL_SO_NBOXES   + ul_align256(sizeof(int) * ULENS_STATIC_MAX_POINTS);
+constexpr size_t UL_SO_UDESC    = UL_SO_BOXES    + ul_align256(sizeof(SubBox) * BoxCap<3>::value * ULENS_STATIC_MAX_POINTS);
+constexpr size_t UL_SO_USUM     = UL_SO_UDESC    + ul_align256(sizeof(unsigned) * UL_STATIC_UNITS);
+constexpr size_t UL_SO_UODD     = UL_SO_USUM     + ul_align256(sizeof(double) * UL_STATIC_UNITS);
+constexpr size_t UL_SO_CC       = UL_SO_UODD     + ul_align256(sizeof(double) * UL_STATIC_UNITS);
+constexpr size_t UL_SO_COUNTERS = UL_SO_CC       + ul_align256(sizeof(ChunkCounters));
+constexpr size_t UL_STATIC_BYTES = UL_SO_COUNTERS + ul_align256(sizeof(DevCounters));
+static_assert(UL_STATIC_BYTES <= (size_t)8 << 20, "static scratch is meant to stay modest (<= 8 MiB)");
+
+static __device__ __align__(256) unsigned char g_static_scratch[UL_STATIC_BYTES];
+
+// one workspace descriptor per device, in static host storage (no heap either); device < 0: not set up yet
+static ulens_ctx g_static_ctx[UL_STATIC_MAX_DEV];
+static bool g_static_ready[UL_STATIC_MAX_DEV];
+static PointCfg g_static_cfg_host[ULENS_STATIC_MAX_POINTS];
+static LensPoly g_static_poly_host[ULENS_STATIC_MAX_POINTS];
+static char g_static_err[256];
+
+extern "C" const char* ulens_static_last_cuda_error(void) { return g_static_err; }
+extern "C" int ulens_static_max_points(void) { return ULENS_STATIC_MAX_POINTS; }
+extern "C" long long ulens_static_scratch_bytes(void) { return (long long)UL_STATIC_BYTES; }
+
+static int static_setup(int dev)
+{
+    ulens_ctx* ctx = &g_static_ctx[dev];
+    memset(ctx, 0, sizeof *ctx);
+    ctx->device = dev;
+    CK(cudaSetDevice(dev));
+    unsigned char* base = nullptr;
+    CK(cudaGetSymbolAddress((void**)&base, g_static_scratch));      // this device's copy of the array
+    if (!base) return ULENS_ECUDA;
+    ulens_options o; memset(&o, 0, sizeof o);                        // the defaults of ulens_create
+    o.n_limb = 512; o.n_r = 96; o.n_theta = 48; o.rel_tol = 1e-4; o.chunk_pts = ULENS_STATIC_MAX_POINTS;
+    o.flags = ULENS_OPT_NO_RETRY;
+    ctx->opt = o;
+    ctx->rp.n_limb = o.n_limb; ctx->rp.n_r = o.n_r; ctx->rp.n_theta = o.n_theta;
+    ctx->rp.max_nr = 8192; ctx->rp.max_nth = 32768; ctx->rp.max_units_pt = 1024;
+    ctx->chunk = ULENS_STATIC_MAX_POINTS;
+    ctx->cap_units = UL_STATIC_UNITS;
+    ctx->cfg_dev   = reinterpret_cast<PointCfg*>(base + UL_SO_CFG);
+    ctx->poly_dev  = reinterpret_cast<LensPoly*>(base + UL_SO_POLY);
+    ctx->cfg_cap   = ULENS_STATIC_MAX_POINTS;
+    ctx->patches   = reinterpret_cast<Patch*>(base + UL_SO_PATCHES);
+    ctx->n_patch   = reinterpret_cast<int*>(base + UL_SO_NPATCH);
+    ctx->status_ws = reinterpret_cast<unsigned*>(base + UL_SO_STATUS);
+    ctx->c_zr      = reinterpret_cast<double*>(base + UL_SO_CZR);
+    ctx->c_zi      = reinterpret_cast<double*>(base + UL_SO_CZI);
+    ctx->c_mask    = reinterpret_cast<unsigned*>(base + UL_SO_CMASK);
+    ctx->n_boxes   = reinterpret_cast<int*>(base + UL_SO_NBOXES);
+    ctx->boxes     = reinterpret_cast<SubBox*>(base + UL_SO_BOXES);
+    ctx->boxes_cap = BoxCap<3>::value;                               // the widest box list: run_chunks never reallocates
+    ctx->unit_desc = reinterpret_cast<unsigned*>(base + UL_SO_UDESC);
+    ctx->unit_sum  = reinterpret_cast<double*>(base + UL_SO_USUM);
+    ctx->unit_odd  = reinterpret_cast<double*>(base + UL_SO_UODD);
+    ctx->cc        = reinterpret_cast<ChunkCounters*>(base + UL_SO_CC);
+    ctx->counters  = reinterpret_cast<DevCounters*>(base + UL_SO_COUNTERS);
+    g_static_ready[dev] = true;
+    return ULENS_OK;
+}
+
+extern "C" int ulens_mag_static(int cuda_device, int n_cfg, int n_pts, const ulens_lens* lenses_host,
+                                const double* rho_host, const double* u1_host, const double* w_re, const double* w_im,
+                                double* A_out, double* err_out, uint32_t* status_out, void* stream)
+{
+    g_static_err[0] = 0;
+    if (cuda_device < 0 || cuda_device >= UL_STATIC_MAX_DEV || n_cfg < 0 || n_pts < 0) return ULENS_EINVAL;
+    if (n_cfg == 0 || n_pts == 0) return ULENS_OK;
+    if (!lenses_host || !rho_host || !u1_host || !w_re || !w_im || !A_out) return ULENS_EINVAL;
+    const long long n_total = (long long)n_cfg * n_pts;
+    if (n_total > ULENS_STATIC_MAX_POINTS) return ULENS_ELIMIT;      // beyond the fixed scratch: use ulens_mag
+    ulens_ctx* ctx = &g_static_ctx[cuda_device];
+    int rc = ULENS_OK;
+    if (!g_static_ready[cuda_device]) {
+        int ndev = 0;
+        if (cudaGetDeviceCount(&ndev) != cudaSuccess || cuda_device >= ndev) return ULENS_ECUDA;
+        rc = static_setup(cuda_device);
+    } else {
+        cudaError_t e = cudaSetDevice(cuda_device);
+        if (e != cudaSuccess) rc = fail_cuda(ctx, e, "cudaSetDevice");
+    }
+    if (rc != ULENS_OK) { memcpy(g_static_err, ctx->cuda_err, sizeof g_static_err); return rc; }
+    cudaStream_t st = (cudaStream_t)stream;
+    // configuration tables (the checks and the arithmetic of upload_cfgs), built in static host storage
+    const int N = lenses_host[0].n_lens;
+    if (N < 1 || N > 3) return ULENS_EINVAL;
+    bool ld = false;
+    for (int c = 0; c < n_cfg; ++c) {
+        const ulens_lens& L = lenses_host[c];
+        if (L.n_lens != N) return ULENS_EUNSUPPORTED;
+        double tot = 0.0;
+        for (int a = 0; a < N; ++a) {
+            if (!isfinite(L.eps[a]) || !(L.eps[a] >= 0.0) || !isfinite(L.ax[a]) || !isfinite(L.ay[a])) return ULENS_EINVAL;
+            tot += L.eps[a];
+        }
+        if (fabs(tot - 1.0) > 1e-9) return ULENS_EINVAL;
+        if (!finite_pos(rho_host[c]) || !(u1_host[c] >= 0.0 && u1_host[c] <= 1.0)) return ULENS_EINVAL;
+        PointCfg& P = g_static_cfg_host[c];
+        memset(&P, 0, sizeof P);
+        P.lens.n = N;
+        for (int a = 0; a < N; ++a) { P.lens.eps[a] = L.eps[a]; P.lens.ax[a] = L.ax[a]; P.lens.ay[a] = L.ay[a]; }
+        P.rho = rho_host[c]; P.u1 = u1_host[c];
+        if (u1_host[c] > 0.0) ld = true;
+        lens_poly_basis(L.n_lens, L.eps, L.ax, L.ay, &g_static_poly_host[c]);
+    }
+    // pageable source: the runtime stages the bytes before it returns, so the static host tables may be rewritten
+    // by the next call; the copies are ordered on `st` ahead of the kernels
+    rc = [&]() -> int {
+        CK(cudaMemcpyAsync(ctx->cfg_dev, g_static_cfg_host, sizeof(PointCfg) * n_cfg, cudaMemcpyHostToDevice, st));
+        CK(cudaMemcpyAsync(ctx->poly_dev, g_static_poly_host, sizeof(LensPoly) * n_cfg, cudaMemcpyHostToDevice, st));
+        // the array keeps the previous call's contents: the statistics counters restart at zero (the chunk counters
+        // and the per-point box counts are cleared by run_chunks itself; everything else is written before it is read)
+        CK(cudaMemsetAsync(ctx->counters, 0, sizeof(DevCounters), st));
+        ctx->last_launches = 0;
+        switch (N) {
+            case 1: return run_chunks<1>(ctx, n_total, n_pts, ld, w_re, w_im, A_out, err_out, status_out, st);
+            case 2: return run_chunks<2>(ctx, n_total, n_pts, ld, w_re, w_im, A_out, err_out, status_out, st);
+            default: return run_chunks<3>(ctx, n_total, n_pts, ld, w_re, w_im, A_out, err_out, status_out, st);
+        }
+    }();
+    if (rc != ULENS_OK) memcpy(g_static_err, ctx->cuda_err, sizeof g_static_err);
+    return rc;
 }
