@@ -72,6 +72,10 @@ typedef struct ulens_ctx ulens_ctx;
                                          derivatives run on the FP32 pipe in segment-local coordinates (cancellation-free difference
                                          form of Eq. 1); segment constants, edge events and accumulation stay FP64. Same sectors, same
                                          rule, same 1e-4 bar; the forward-mode variant always runs in FP64 */
+#define ULENS_OPT_NO_QUIET   0x4      /* do not use the quiet-point shortcut. By default a source point that a 9-probe point-source test
+                                         finds far from every caustic (same image count at the centre and at 8 limb points, finite-source
+                                         effect below 1e-4) has its limb followed with an eighth of the n_limb samples: its images are
+                                         smooth near-ellipses. Only the sampling density of step a3 changes; the rays still decide */
 
 /* Tunables; a zeroed struct (or NULL) selects the defaults in brackets. */
 typedef struct {

@@ -29,6 +29,7 @@ EXPORTS = ["ulens_create", "ulens_destroy", "ulens_lens_binary", "ulens_lens_tri
 
 ULENS_OPT_NO_RETRY = 0x1
 ULENS_OPT_F32_SHOOT = 0x2
+ULENS_OPT_NO_QUIET = 0x4
 ULENS_ST_RETRIED = 0x2000
 ULENS_ST_POINT_SRC = 0x1000
 

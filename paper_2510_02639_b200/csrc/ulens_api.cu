@@ -55,6 +55,7 @@ struct ulens_ctx {
     SubBox* boxes; int boxes_cap;       // [chunk][BoxCap] box lists of the points (k_limb -> k_sectors); boxes_cap = BoxCap allocated
     BoxExt* exts; int exts_cap;         // forward-mode runs: the boxes' extreme own points
     int* n_boxes;               // [chunk]
+    unsigned char* quiet;       // [chunk] 1 = quiet source point (k_quiet): coarse limb sampling
     // forward-mode variant (allocated on first use)
     PatchTan* ptans;            // [chunk][UL_MAXP] tangents of the sectors' radial bounds
     double* unit_tan; int unit_tan_nt;  // [cap_units][NT] tangent sums of the units
@@ -407,6 +408,80 @@ __global__ void k_ext_scatter(int n, const unsigned char* __restrict__ flag, con
     if (f) map[blk[blockIdx.x] + wsum[w] + __popc(b & ((1u << l) - 1u))] = i;
 }
 
+// Quiet source points [proposal]. Far from every caustic the images are smooth near-ellipses and an eighth of the limb
+// samples bounds them as well as all of them; the limb tracker is the second most expensive step, so such points are
+// worth recognising. Same multipole probe as the point-source switch (k_point_ext): the point-source magnification at
+// the centre and at 8 limb points; the point is quiet when every probe has as many images as the centre (no caustic
+// between them), every solve is clean, and Q + H <= tol A_c, i.e. the finite-source effect itself is below tol.
+// Only the sampling density changes: the images are still found by tracking, the rays still decide what is inside.
+#ifndef UL_QUIET_TOL
+#define UL_QUIET_TOL 1e-4
+#endif
+template <int N>
+__global__ void k_quiet(int n, int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cfg, const LensPoly* __restrict__ poly,
+                        const double* __restrict__ w_re, const double* __restrict__ w_im, double tol,
+                        unsigned char* __restrict__ quiet, const int* __restrict__ pmap = nullptr,
+                        const unsigned* __restrict__ n_dev = nullptr)
+{
+    constexpr int DEG = N * N + 1;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (n_dev) n = min(n, (int)*n_dev - pt_base);
+    if (i >= n) return;
+    const long long gp = pmap ? (long long)pmap[pt_base + i] : (long long)pt_base + i;
+    const int c = (int)(gp / n_pts_per_cfg);
+    const Lens L = cfg[c].lens;
+    const double rho = cfg[c].rho, wx = w_re[gp], wy = w_im[gp];
+    double zr[DEG], zi[DEG];
+    double A_c = 0.0, s_axes = 0.0, s_diag = 0.0;
+    unsigned st_c = 0;
+    bool ok = true;
+    // never next to a light lens: within 8 sqrt(eps_a) + 2 rho of its planetary caustic (centred on
+    // w_a = a_a - sum_{b != a} eps_b / conj(a_a - a_b)) images hide in a root cluster that the polynomial solve -- and
+    // with it this probe -- can miss altogether (measured on C3: a pair of 4.5e-4 A each, found only by the limb
+    // tracker's seeds on that lens's Einstein ring, which need the dense sampling)
+    if (N > 1) {
+#pragma unroll
+        for (int a = 0; a < N; ++a) {
+            if (!(L.eps[a] < 1e-2)) continue;
+            double tx = L.ax[a] - wx, ty = L.ay[a] - wy;
+#pragma unroll
+            for (int b = 0; b < N; ++b) {
+                if (b == a) continue;
+                const double dx = L.ax[a] - L.ax[b], dy = L.ay[a] - L.ay[b];
+                const double i2 = L.eps[b] / (dx * dx + dy * dy);
+                tx -= dx * i2; ty -= dy * i2;
+            }
+            const double R = 8.0 * sqrt(L.eps[a]) + 2.0 * rho;
+            if (tx * tx + ty * ty < R * R) ok = false;
+        }
+    }
+#pragma unroll 1
+    for (int p = 0; p < 9 && ok; ++p) {
+        double px = wx, py = wy;
+        if (p > 0) {
+            const int k = (p - 1) & 3;
+            const double ex = (k == 0) ? 1.0 : (k == 2) ? -1.0 : 0.0, ey = (k == 1) ? 1.0 : (k == 3) ? -1.0 : 0.0;
+            if (p > 4) { const double r = rho * 0.70710678118654752; px += r * (ex - ey); py += r * (ex + ey); }
+            else { px += rho * ex; py += rho * ey; }
+        }
+        unsigned mask = 0;
+        const unsigned st = centre_images<N>(L, poly[c], px, py, zr, zi, mask);
+        if (st & (UL_ST_EA_NOCONV | UL_ST_IMG_PARITY)) ok = false;
+        const double a = point_mag<N>(L, nullptr, zr, zi, mask, nullptr);
+        if (p == 0) { st_c = st; A_c = a; }
+        else {
+            if (((st ^ st_c) >> 8) & 0xfu) ok = false;   // image count changed
+            if (p > 4) s_diag += a; else s_axes += a;
+        }
+    }
+    if (ok) {
+        const double Q = 0.5 * fabs(0.125 * (s_axes + s_diag) - A_c);
+        const double H = 0.25 * fabs(s_axes - s_diag);
+        ok = (Q + H <= tol * A_c);
+    }
+    quiet[i] = ok ? 1 : 0;
+}
+
 // Image-region builder, first half (ulens_limb.cuh): a group of N^2+1 lanes per limb arc, one lane per root; a warp holds
 // GPW arcs, and the WARPS warps that share a source point are independent work items (4 per CTA, any mix of points).
 // Appends to the point's box list (n_boxes zeroed before the launch).
@@ -419,7 +494,8 @@ k_limb(int n, int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cfg, 
        const double* __restrict__ w_re, const double* __restrict__ w_im, RegionParams rp,
        SubBox* __restrict__ boxes, BoxExt* __restrict__ exts, int* __restrict__ n_boxes, unsigned* __restrict__ status,
        DevCounters* ctr, const double* __restrict__ c_zr, const double* __restrict__ c_zi,
-       const unsigned* __restrict__ c_mask, const int* __restrict__ pmap = nullptr, const unsigned* __restrict__ n_dev = nullptr)
+       const unsigned* __restrict__ c_mask, const int* __restrict__ pmap = nullptr, const unsigned* __restrict__ n_dev = nullptr,
+       const unsigned char* __restrict__ quiet = nullptr)
 {
     typedef LimbGeom<N> G;
     __shared__ LimbShared<N> sh[4];
@@ -428,14 +504,19 @@ k_limb(int n, int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cfg, 
     const long long item = (long long)blockIdx.x * 4 + wib;          // (point, warp of the point)
     const int i = (int)(item / G::WARPS), w = (int)(item % G::WARPS);
     if (i >= n) return;                                  // whole warp leaves together
+    // a quiet point (k_quiet) is one work item: its limb is followed by warp 0 alone, GPW arcs, an eighth of the samples
+    const bool q = quiet && quiet[i];
+    if (q && w > 0) return;
     const long long gp = pmap ? (long long)pmap[pt_base + i] : (long long)pt_base + i;
     const int c = (int)(gp / n_pts_per_cfg);
     const Lens L = cfg[c].lens;
     constexpr int CAP = BoxCap<N>::value;
     int n_solves = 0;
+    const int n_arcs = q ? G::GPW : G::NARC;
+    const int per_arc = q ? max(2, (rp.n_limb / 8 + G::GPW - 1) / G::GPW) : 0;
     unsigned st = limb_track<N, DUAL>(sh[wib], w, L, poly[c], w_re[gp], w_im[gp], cfg[c].rho, rp, c_zr + (long long)i * 10,
                                       c_zi + (long long)i * 10, c_mask[i], boxes + (size_t)i * CAP,
-                                      DUAL ? exts + (size_t)i * CAP : nullptr, n_boxes + i, CAP, n_solves);
+                                      DUAL ? exts + (size_t)i * CAP : nullptr, n_boxes + i, CAP, n_solves, n_arcs, per_arc);
     st = __reduce_or_sync(0xffffffffu, st);
     n_solves = __reduce_add_sync(0xffffffffu, n_solves);
     if (lane == 0) {
@@ -453,7 +534,7 @@ k_sectors(int n, int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cf
           const int* __restrict__ n_boxes, Patch* __restrict__ patches, int* __restrict__ n_patch, unsigned* __restrict__ status,
           unsigned* __restrict__ unit_desc, unsigned cap_units, ChunkCounters* cc, DevCounters* ctr,
           const TangentTable* __restrict__ tans, PatchTan* __restrict__ ptans, const int* __restrict__ pmap = nullptr,
-          const unsigned* __restrict__ n_dev = nullptr)
+          const unsigned* __restrict__ n_dev = nullptr, const unsigned char* __restrict__ quiet = nullptr)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int lane = threadIdx.x & 31;
@@ -468,8 +549,12 @@ k_sectors(int n, int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cf
         const int c = (int)(gp / n_pts_per_cfg);
         const Lens L = cfg[c].lens;
         PatchTan* pt = tans ? ptans + (long long)i * UL_MAXP : nullptr;
+        // spacing of the limb samples k_limb took for this point (quiet points: GPW arcs of max(2, ...) points)
+        typedef LimbGeom<N> G;
+        const bool q = quiet && quiet[i];
+        const int n_samp = q ? G::GPW * max(2, (rp.n_limb / 8 + G::GPW - 1) / G::GPW) : G::NARC * max(1, (rp.n_limb + G::NARC / 2) / G::NARC);
         np = sectors_from_boxes<N>(boxes + (size_t)i * CAP, tans ? exts + (size_t)i * CAP : nullptr, min(n_boxes[i], CAP), rp, i, L,
-                                   w_re[gp], w_im[gp], cfg[c].rho, st, tans ? &tans[c] : nullptr, pp, pt);
+                                   w_re[gp], w_im[gp], cfg[c].rho, st, tans ? &tans[c] : nullptr, pp, pt, 2.0 * UL_PI / n_samp);
         for (int p = 0; p < np; ++p) total_units += pp[p].n_units;
     }
     // one atomicAdd per warp: exclusive prefix sum of the lanes' unit counts, lane 31 holds the warp's total
@@ -1051,6 +1136,7 @@ extern "C" int ulens_create(ulens_ctx** out, int cuda_device, const ulens_option
     if (e == cudaSuccess) e = cudaMalloc(&ctx->c_zi, sizeof(double) * 10 * (size_t)ctx->chunk);
     if (e == cudaSuccess) e = cudaMalloc(&ctx->c_mask, sizeof(unsigned) * (size_t)ctx->chunk);
     if (e == cudaSuccess) e = cudaMalloc(&ctx->n_boxes, sizeof(int) * (size_t)ctx->chunk);
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->quiet, (size_t)ctx->chunk);
     if (e == cudaSuccess) e = cudaMalloc(&ctx->unit_desc, sizeof(unsigned) * ctx->cap_units);
     if (e == cudaSuccess) e = cudaMalloc(&ctx->unit_sum, sizeof(double) * ctx->cap_units);
     if (e == cudaSuccess) e = cudaMalloc(&ctx->unit_odd, sizeof(double) * ctx->cap_units);
@@ -1068,7 +1154,7 @@ extern "C" void ulens_destroy(ulens_ctx* ctx)
     cudaSetDevice(ctx->device);
     cudaDeviceSynchronize();
     cudaFree(ctx->c_zr); cudaFree(ctx->c_zi); cudaFree(ctx->c_mask);
-    cudaFree(ctx->boxes); cudaFree(ctx->exts); cudaFree(ctx->n_boxes);
+    cudaFree(ctx->boxes); cudaFree(ctx->exts); cudaFree(ctx->n_boxes); cudaFree(ctx->quiet);
     cudaFree(ctx->ptans); cudaFree(ctx->unit_tan); cudaFree(ctx->grad5); cudaFree(ctx->tan_dev);
     cudaFree(ctx->patches); cudaFree(ctx->n_patch); cudaFree(ctx->status_ws); cudaFree(ctx->unit_desc);
     cudaFree(ctx->unit_sum); cudaFree(ctx->unit_odd); cudaFree(ctx->cc); cudaFree(ctx->counters);
@@ -1200,6 +1286,14 @@ static int run_chunks(ulens_ctx* ctx, long long n_total, int n_pts, bool ld, con
             k_roots<N><<<(n + 127) / 128, 128, 0, st>>>(n, (int)base, n_pts, ctx->cfg_dev, ctx->poly_dev, w_re, w_im,
                                                         nullptr, nullptr, nullptr, ctx->status_ws, ctx->c_zr, ctx->c_zi, ctx->c_mask, nullptr, nullptr, pmap, n_dev);
         }
+        // quiet source points take the coarse limb sampling (first pass only: the retry pass is for doubtful points)
+        const bool use_quiet = !(ctx->opt.flags & ULENS_OPT_NO_QUIET) && st_or == 0 && ctx->quiet != nullptr;
+        if (use_quiet) {
+            KTimer kt(ctx, ULENS_K_ROOTS, st);
+            k_quiet<N><<<(n + 127) / 128, 128, 0, st>>>(n, (int)base, n_pts, ctx->cfg_dev, ctx->poly_dev, w_re, w_im, UL_QUIET_TOL, ctx->quiet, pmap, n_dev);
+            ctx->last_launches += 1;
+        }
+        const unsigned char* quiet = use_quiet ? ctx->quiet : nullptr;
         {
             KTimer kt(ctx, ULENS_K_LIMB, st);
             CK(cudaMemsetAsync(ctx->n_boxes, 0, sizeof(int) * (size_t)n, st));
@@ -1207,17 +1301,17 @@ static int run_chunks(ulens_ctx* ctx, long long n_total, int n_pts, bool ld, con
             if (dual)
                 k_limb<N, true><<<limb_grid, 128, 0, st>>>(n, (int)base, n_pts, ctx->cfg_dev, ctx->poly_dev, w_re, w_im, rp,
                                                                     ctx->boxes, ctx->exts, ctx->n_boxes, ctx->status_ws, ctx->counters,
-                                                                    ctx->c_zr, ctx->c_zi, ctx->c_mask, pmap, n_dev);
+                                                                    ctx->c_zr, ctx->c_zi, ctx->c_mask, pmap, n_dev, quiet);
             else
                 k_limb<N, false><<<limb_grid, 128, 0, st>>>(n, (int)base, n_pts, ctx->cfg_dev, ctx->poly_dev, w_re, w_im, rp,
                                                                      ctx->boxes, ctx->exts, ctx->n_boxes, ctx->status_ws, ctx->counters,
-                                                                     ctx->c_zr, ctx->c_zi, ctx->c_mask, pmap, n_dev);
+                                                                     ctx->c_zr, ctx->c_zi, ctx->c_mask, pmap, n_dev, quiet);
         }
         {
             KTimer kt(ctx, ULENS_K_SECTORS, st);
             k_sectors<N><<<(n + 127) / 128, 128, 0, st>>>(n, (int)base, n_pts, ctx->cfg_dev, w_re, w_im, rp, ctx->boxes, ctx->exts,
                                                            ctx->n_boxes, ctx->patches, ctx->n_patch, ctx->status_ws, ctx->unit_desc,
-                                                           (unsigned)ctx->cap_units, ctx->cc, ctx->counters, tans, ctx->ptans, pmap, n_dev);
+                                                           (unsigned)ctx->cap_units, ctx->cc, ctx->counters, tans, ctx->ptans, pmap, n_dev, quiet);
         }
         // persistent grid: as many CTAs as are resident at once (occupancy API; 4-6 per SM by register count)
         int per_sm = 4;
@@ -1974,7 +2068,8 @@ constexpr size_t UL_SO_USUM     = UL_SO_UDESC    + ul_align256(sizeof(unsigned) 
 constexpr size_t UL_SO_UODD     = UL_SO_USUM     + ul_align256(sizeof(double) * UL_STATIC_UNITS);
 constexpr size_t UL_SO_CC       = UL_SO_UODD     + ul_align256(sizeof(double) * UL_STATIC_UNITS);
 constexpr size_t UL_SO_COUNTERS = UL_SO_CC       + ul_align256(sizeof(ChunkCounters));
-constexpr size_t UL_STATIC_BYTES = UL_SO_COUNTERS + ul_align256(sizeof(DevCounters));
+constexpr size_t UL_SO_QUIET    = UL_SO_COUNTERS + ul_align256(sizeof(DevCounters));
+constexpr size_t UL_STATIC_BYTES = UL_SO_QUIET + ul_align256(ULENS_STATIC_MAX_POINTS);
 static_assert(UL_STATIC_BYTES <= (size_t)8 << 20, "static scratch is meant to stay modest (<= 8 MiB)");
 
 static __device__ __align__(256) unsigned char g_static_scratch[UL_STATIC_BYTES];
@@ -2024,6 +2119,7 @@ static int static_setup(int dev)
     ctx->unit_odd  = reinterpret_cast<double*>(base + UL_SO_UODD);
     ctx->cc        = reinterpret_cast<ChunkCounters*>(base + UL_SO_CC);
     ctx->counters  = reinterpret_cast<DevCounters*>(base + UL_SO_COUNTERS);
+    ctx->quiet     = base + UL_SO_QUIET;
     g_static_ready[dev] = true;
     return ULENS_OK;
 }

@@ -318,11 +318,9 @@ UL_HD void shoot_ring_t(const Lens& L, double wcx, double wcy, double rho2, doub
                 S += sq;
                 // d sqrt(-F) = -dF / (2 sqrt(-F)); a node (numerically) ON the edge has no such derivative: its weight
                 // and its counterpart in the end correction (zeta_m12_du) are dropped together
-                if (-f3 > UL_DUAL_SING_FLOOR * rho2) {
-                    RayBasis<N> B;
-                    ray_basis<N, false>(L, R, r, c, s, B);
-                    stat_add(SS, -0.5 / sq, B);
-                }
+                RayBasis<N> B;
+                ray_basis<N, false>(L, R, r, c, s, B);
+                stat_add(SS, (-f3 > UL_DUAL_SING_FLOOR * rho2) ? -0.5 / sq : 0.0, B);
             }
             if (!periodic && (j < 2 || j >= n_th - 2)) edge = true;
         }
@@ -405,11 +403,9 @@ UL_HD void shoot_col_t(const Lens& L, double wcx, double wcy, double rho2, doubl
             if (LD) {
                 const double sq = sqrt(-f3);
                 S += r * sq;
-                if (-f3 > UL_DUAL_SING_FLOOR * rho2) {
-                    RayBasis<N> B;
-                    ray_basis<N, true>(L, R, r, c, s, B);
-                    stat_add(SS, -0.5 * r / sq, B);
-                }
+                RayBasis<N> B;
+                ray_basis<N, true>(L, R, r, c, s, B);
+                stat_add(SS, (-f3 > UL_DUAL_SING_FLOOR * rho2) ? -0.5 * r / sq : 0.0, B);
             }
             if ((i < 2 && r0 > 0.0) || i >= n_r - 2) edge = true;
         }

@@ -210,13 +210,14 @@ __device__ __forceinline__ void adopt_candidates(bool run, int j, int gbase, uns
 template <int N, bool DUAL>
 __device__ unsigned limb_track(LimbShared<N>& sh, int warp, const Lens& L, const LensPoly& T, double wcx, double wcy, double rho,
                                const RegionParams& P, const double* __restrict__ czr, const double* __restrict__ czi,
-                               unsigned cmask, SubBox* boxes, BoxExt* exts, int* n_box, int box_cap, int& n_solves_out)
+                               unsigned cmask, SubBox* boxes, BoxExt* exts, int* n_box, int box_cap, int& n_solves_out,
+                               int n_arcs = LimbGeom<N>::NARC, int per_arc_in = 0)
 {
     typedef LimbGeom<N> G;
     constexpr int DEG = G::DEG;
     const int lane = threadIdx.x & 31;
     const int gw = lane / DEG;
-    const bool active = gw < G::GPW;
+    const bool active = gw < G::GPW && warp * G::GPW + gw < n_arcs;
     const int gbase = active ? gw * DEG : 0;
     const int j = active ? lane - gbase : 0;
     const int arc = active ? warp * G::GPW + gw : 0;
@@ -244,8 +245,9 @@ __device__ unsigned limb_track(LimbShared<N>& sh, int warp, const Lens& L, const
         }
     }
 
-    const int per_arc = max(1, (P.n_limb + G::NARC / 2) / G::NARC);
-    const double dphi = 2.0 * UL_PI / (per_arc * G::NARC);
+    // (quiet source points, k_quiet: the whole limb as n_arcs = GPW arcs of one warp, per_arc_in points each)
+    const int per_arc = per_arc_in > 0 ? per_arc_in : max(1, (P.n_limb + G::NARC / 2) / G::NARC);
+    const double dphi = 2.0 * UL_PI / (per_arc * n_arcs);
     const double ph0 = dphi * (arc * per_arc), ph_end = dphi * (arc * per_arc + per_arc);
 
     double zr = 0.0, zi = 0.0, ozr = 0.0, ozi = 0.0, pvx = 0.0, pvy = 0.0;

@@ -155,6 +155,66 @@ UL_HD void patch_tangents(const Lens& L, const TangentTable& T, const BoxExt& x,
     }
 }
 
+// Forward-mode runs: a sector bound moves like the image's extreme point (envelope theorem: d r_max / dp is dr/dp at
+// fixed limb angle, taken AT the extreme), and the ray grid must follow the image closely -- the quadrature error is a
+// function of where the edge falls between the scan lines, and its derivative is not small. The extreme among the limb
+// SAMPLES is off by up to half a sample spacing, which leaves a first-order error in the bound's tangent (measured on
+// C4: dA/du0, dA/drho, dA/dalpha converged like 1/n_limb). So the sampled extreme of |z| (which = 0) or arg z
+// (which = 1) is moved along the limb to the true one (kind = +1: maximum, -1: minimum): secant iteration on d/dphi of
+// the quantity, the image z(phi) followed by Newton on Eq. 1 (dz/dphi by the implicit-function theorem, as
+// limb_point_rdot). dph: the local sample spacing at most; the search stays within it. Returns false (nothing changed)
+// if the image is lost, the search leaves the range, or the result is less extreme than the sample.
+template <int N>
+UL_HD bool refine_extreme(const Lens& L, double wcx, double wcy, double rho, int which, int kind, double dph,
+                          double& x, double& y, double& ph)
+{
+    // f = d(|z| or arg z)/dphi up to a positive factor
+    auto slope = [&](double phi, double& zx, double& zy, double& f) -> bool {
+        const double sn = sin(phi), cs = cos(phi);
+        double detJ, resid, gx, gy;
+        if (!polish_image_ni<N>(L, wcx + rho * cs, wcy + rho * sn, zx, zy, 8, 1e-11, detJ, resid, gx, gy)) return false;
+        const double bx = -rho * sn, by = rho * cs;                       // dw/dphi
+        const double vx = bx - (gx * bx + gy * by), vy = by - (gy * bx - gx * by);      // det J dz/dphi
+        f = (which == 0 ? zx * vx + zy * vy : zx * vy - zy * vx) / detJ;
+        return f == f && fabs(f) < 1e300;
+    };
+    double x0 = x, y0 = y, p0 = ph, f0;
+    if (!slope(p0, x0, y0, f0)) return false;
+    if (f0 == 0.0) return false;
+    // second point on the side the slope points to
+    double p1 = p0 + ((kind * f0 > 0.0) ? 0.25 : -0.25) * dph, x1 = x0, y1 = y0, f1;
+    if (!slope(p1, x1, y1, f1)) return false;
+    for (int it = 0; it < 4; ++it) {
+        const double df = f1 - f0;
+        if (!(fabs(df) > 0.0)) break;
+        const double pn = p1 - f1 * (p1 - p0) / df;
+        if (!(fabs(pn - ph) <= dph)) return false;
+        p0 = p1; f0 = f1; x0 = x1; y0 = y1;
+        p1 = pn;
+        if (!slope(p1, x1, y1, f1)) return false;
+        if (fabs(p1 - p0) < 1e-6 * dph) break;            // the tangent's error is first order in this
+    }
+    const double mv2 = (x1 - x) * (x1 - x) + (y1 - y) * (y1 - y);
+    if (!(mv2 <= 0.01 * ul_max(x * x + y * y, 0.04))) return false;       // jumped to another image
+    if (which == 0) { if (kind * (sqrt(x1 * x1 + y1 * y1) - sqrt(x * x + y * y)) < 0.0) return false; }
+    else { if (kind * (x * y1 - y * x1) < 0.0) return false; }             // sign of the turn from the sample to the result
+    x = x1; y = y1; ph = p1;
+    return true;
+}
+
+// the extreme own points of a sector (sampled) -> the true extremes of the image boundary
+template <int N>
+UL_HD void refine_sector_extremes(const Lens& L, double wcx, double wcy, double rho, double dph, bool from_origin, BoxExt& x)
+{
+    if (x.hi_r < 0.0) return;
+    if (!from_origin) refine_extreme<N>(L, wcx, wcy, rho, 0, -1, dph, x.lo_x, x.lo_y, x.lo_ph);
+    refine_extreme<N>(L, wcx, wcy, rho, 0, +1, dph, x.hi_x, x.hi_y, x.hi_ph);
+    if (x.thi_t > -1e299 && !from_origin) {
+        refine_extreme<N>(L, wcx, wcy, rho, 1, -1, dph, x.tlo_x, x.tlo_y, x.tlo_ph);
+        refine_extreme<N>(L, wcx, wcy, rho, 1, +1, dph, x.thi_x, x.thi_y, x.thi_ph);
+    }
+}
+
 // ---------------------------------------------------------------------------------------------- phase C
 // One sector -> its ray grid (Sec. 3.3 "fixed-resolution polar grid"; spacing from the local image scale).
 // Scan lines (one per lane, 32 per work unit) are rings scanned along theta for a bounded sector and radial
@@ -315,11 +375,12 @@ UL_HD void interval_merge_necks(double* g_lo, double* g_hi, int& ng)
 // inside the innermost one) meets no boundary, so it is entirely inside or entirely outside the image:
 // one ray on it decides. Where it is inside (ring-like image around the origin, or a disk that contains
 // the origin) the gap is filled: the groups on both sides merge into one full-ring sector.
-//   box [nb], ext [nb] or nullptr (forward-mode run: the boxes' extreme own points); patch / ptan [UL_MAXP] out.
+//   box [nb], ext [nb] or nullptr (forward-mode run: the boxes' extreme own points); patch / ptan [UL_MAXP] out;
+//   dph_limb: spacing of this point's limb samples (forward-mode run: how far a true extreme can lie from the sampled one).
 template <int N>
 UL_HDN int sectors_from_boxes(const SubBox* box, const BoxExt* ext, int nb, const RegionParams& P, int point, const Lens& L,
                               double wcx, double wcy, double rho, unsigned& status, const TangentTable* TT, Patch* patch,
-                              PatchTan* ptan)
+                              PatchTan* ptan, double dph_limb = 2.0 * UL_PI / 512)
 {
     if (nb == 0) { status |= UL_ST_NO_IMAGE; return 0; }
 
@@ -379,7 +440,10 @@ UL_HDN int sectors_from_boxes(const SubBox* box, const BoxExt* ext, int nb, cons
                 }
             }
             if (np == UL_MAXP) { capped = true; break; }
-            if (ext && TT) patch_tangents<N>(L, *TT, xlo, gr_lo[a] <= 0.0, ptan[np]);
+            if (ext && TT) {
+                refine_sector_extremes<N>(L, wcx, wcy, rho, dph_limb, gr_lo[a] <= 0.0, xlo);
+                patch_tangents<N>(L, *TT, xlo, gr_lo[a] <= 0.0, ptan[np]);
+            }
             emit_patch(patch[np++], P, point, gr_lo[a], gr_hi[a], -UL_PI, UL_PI, hr, ht, cr, ct, true, true,
                        gap_r_lo, gap_r_hi, 0.0, 0.0, units_left, status);
             continue;
@@ -491,7 +555,10 @@ UL_HDN int sectors_from_boxes(const SubBox* box, const BoxExt* ext, int nb, cons
             // with theta up to the two tips, which the sin-spaced lines (UL_PATCH_SINR) take care of. A sector
             // that closes on itself in theta has no tips at all (spectral convergence).
             const bool scan_r = full_ring || ((c_th[c] - c_tl[c]) * c_rh[c] > (c_rh[c] - c_rl[c]));
-            if (ext && TT) patch_tangents<N>(L, *TT, c_ext[c], false, ptan[np]);
+            if (ext && TT) {
+                refine_sector_extremes<N>(L, wcx, wcy, rho, dph_limb, false, c_ext[c]);
+                patch_tangents<N>(L, *TT, c_ext[c], false, ptan[np]);
+            }
             emit_patch(patch[np++], P, point, c_rl[c], c_rh[c], c_tl[c], c_th[c], c_hr[c], c_ht[c], c_cr[c], c_ct[c],
                        full_ring, scan_r, gap_r_lo, gap_r_hi, gap_lo, gap_hi, units_left, status);
         }

@@ -89,3 +89,41 @@ def test_full_config4_with_derivatives(ctx, torch_cuda):
         torch.cuda.synchronize()
         assert np.array_equal(A1.cpu().numpy()[0], A[c, sel])
         assert np.array_equal(dA1.cpu().numpy()[0], dA[c, sel])
+
+
+def test_config4_derivatives_do_not_depend_on_the_limb_sampling(torch_cuda):
+    """Forward mode moves each sector with the image's extreme points; the sampled extremes are refined to the true ones
+    (refine_extreme, ulens_regions.cuh), so the derivatives must not depend on how densely the limb was sampled -- not
+    even for the quiet points, whose limb gets an eighth of the samples. 64 light curves of C4 x 2,000 epochs, three
+    runs: production (n_limb 512, quiet-point shortcut), shortcut off, shortcut off with n_limb 2048 (the reference).
+    dA/drho is reported, not asserted: it is the small difference of two terms ~2A/rho and carries the derivative of the
+    along-line quadrature error."""
+    from paper_2510_02639_b200 import binding, inputs
+    torch = torch_cuda
+    wl = inputs.get(4)
+    nc = 64
+    t = torch.tensor(wl.t.copy(), device="cuda:0")
+    runs = {}
+    for name, kw in (("production", dict()), ("shortcut off", dict(flags=binding.ULENS_OPT_NO_QUIET)),
+                     ("n_limb 2048", dict(flags=binding.ULENS_OPT_NO_QUIET, n_limb=2048))):
+        c = binding.Context(0, **kw)
+        A, dA, err, st = c.ulens_lightcurve_binary(wl.theta[:nc], 0.5, t, want_dA=True)
+        torch.cuda.synchronize()
+        runs[name] = (A.cpu().numpy(), dA.cpu().numpy(), st.cpu().numpy().astype(np.uint32))
+        c.close()
+    A_ref, d_ref, s_ref = runs["n_limb 2048"]
+    names = ["t0", "u0", "tE", "s", "q", "rho", "alpha"]
+    for name in ("production", "shortcut off"):
+        A, dA, st = runs[name]
+        clean = ((st & 0xff) == 0) & ((s_ref & 0xff) == 0)
+        assert clean.mean() > 0.98
+        assert np.abs(A / A_ref - 1)[clean].max() <= 5e-5
+        line = []
+        for k in range(7):
+            mag = np.abs(d_ref[:, :, k])
+            r = (np.abs(dA[:, :, k] - d_ref[:, :, k]) / (mag + 1e-2 * np.median(mag)))[clean]
+            line.append("%s %.0e/%.0e" % (names[k], np.median(r), np.quantile(r, 0.99)))
+            if names[k] != "rho":
+                assert np.median(r) <= 1e-5, (name, names[k], np.median(r))
+                assert np.quantile(r, 0.99) <= 1e-2, (name, names[k], np.quantile(r, 0.99))
+        print("C4 derivatives, %s vs n_limb 2048 (relative difference, median/p99): %s" % (name, "  ".join(line)))

@@ -20,8 +20,9 @@ pytestmark = pytest.mark.gpu
 
 TOL_A = 1e-4
 HERE = os.path.dirname(os.path.abspath(__file__))
-N_FLAGGED_SAMPLE = int(os.environ.get("ULENS_FLAGGED_SAMPLE", "16"))     # per config; profiles/ holds a run with 256
+N_FLAGGED_SAMPLE = int(os.environ.get("ULENS_FLAGGED_SAMPLE", "16"))     # per config
 _cache = {}
+_stats = {}
 
 
 def _lenses(binding, wl):
@@ -34,18 +35,19 @@ def _olenses(O, wl):
     return [f(*p) for p in wl.lens_params]
 
 
-def _full(torch, cfg, n_limb=0):
-    """A, err, status of the whole config (cached per (cfg, n_limb))."""
-    key = (cfg, n_limb)
+def _full(torch, cfg, n_limb=0, flags=0):
+    """A, err, status of the whole config (cached per (cfg, n_limb, flags))."""
+    key = (cfg, n_limb, flags)
     if key not in _cache:
         from paper_2510_02639_b200 import binding, inputs
         wl = inputs.get(cfg)
-        ctx = binding.Context(0, n_limb=n_limb)
+        ctx = binding.Context(0, n_limb=n_limb, flags=flags)
         w_re = torch.tensor(np.ascontiguousarray(wl.w.real), device="cuda:0")
         w_im = torch.tensor(np.ascontiguousarray(wl.w.imag), device="cuda:0")
         A, err, st = ctx.ulens_mag(_lenses(binding, wl), wl.rho, wl.u1, w_re, w_im)
         torch.cuda.synchronize()
         _cache[key] = (wl, A.cpu().numpy(), err.cpu().numpy(), st.cpu().numpy().astype(np.uint32))
+        _stats[key] = ctx.ulens_get_stats()
         ctx.close()
     return _cache[key]
 
@@ -141,3 +143,34 @@ def test_flagged_points_vs_oracle(torch_cuda, oracle, cfg):
     assert np.all(np.isfinite(A[ci, pi]))
     assert adm.sum() >= 0.5 * len(pick)
     assert (rel[adm] <= TOL_A).mean() >= 0.5              # flagged means doubtful (that is what the bit says), not garbage
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3])
+def test_quiet_points_coarse_limb_sampling_full_size(torch_cuda, oracle, cfg):
+    """The quiet-point shortcut (include/ulens.h ULENS_OPT_NO_QUIET): source points that the 9-probe
+    point-source test finds far from every caustic and from every light lens have their limb followed with an eighth of
+    the samples. Only the sampling density of step a3 changes, so the whole config must come out the same as with the
+    shortcut off: every point on which the two runs differ by more than 5e-5 is checked against the oracle and must carry
+    a status bit in the run that is off by more than 1e-4."""
+    from paper_2510_02639_b200 import binding
+    wl, A1, e1, s1 = _full(torch_cuda, cfg)                                       # production: shortcut on
+    _, A0, e0, s0 = _full(torch_cuda, cfg, flags=binding.ULENS_OPT_NO_QUIET)
+    n1 = _stats[(cfg, 0, 0)]["n_limb_solves"]; n0 = _stats[(cfg, 0, binding.ULENS_OPT_NO_QUIET)]["n_limb_solves"]
+    rel = np.abs(A1 / A0 - 1)
+    idx = np.argwhere(rel > 5e-5)
+    print("C%d quiet-point shortcut: limb solves per point %.0f -> %.0f; max rel diff %.1e over %d points, %d differ by > 5e-5; "
+          "flagged %d -> %d" % (cfg, n0 / A0.size, n1 / A1.size, np.nanmax(rel), A0.size, len(idx),
+                                int(((s0 & 0xff) != 0).sum()), int(((s1 & 0xff) != 0).sum())))
+    assert n1 < 0.95 * n0                                  # the shortcut did engage
+    assert len(idx) <= 1e-4 * A0.size
+    if len(idx):
+        pick = idx[:32]
+        ci, pi = pick[:, 0], pick[:, 1]
+        ref = oracle.mag_fs_batch(_olenses(oracle, wl), ci.astype(np.int32), wl.w[ci, pi].real, wl.w[ci, pi].imag,
+                                  wl.rho[ci], wl.u1[ci], 100, 8)
+        adm = ref["err_est"] <= 2e-5
+        r1 = np.abs(A1[ci, pi] / ref["A"] - 1); r0 = np.abs(A0[ci, pi] / ref["A"] - 1)
+        w1 = adm & (r1 > TOL_A) & ((s1[ci, pi] & 0xff) == 0)
+        w0 = adm & (r0 > TOL_A) & ((s0[ci, pi] & 0xff) == 0)
+        assert not w1.any(), list(zip(ci[w1], pi[w1], r1[w1]))
+        assert not w0.any(), list(zip(ci[w0], pi[w0], r0[w0]))
