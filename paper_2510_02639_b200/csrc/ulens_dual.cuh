@@ -314,13 +314,14 @@ UL_HD void shoot_ring_t(const Lens& L, double wcx, double wcy, double rho2, doub
         if (j >= 0 && j < n_th && f3 < 0.0) {
             U += 1.0;
             if (LD) {
-                const double sq = sqrt(-f3);
-                S += sq;
-                // d sqrt(-F) = -dF / (2 sqrt(-F)); a node (numerically) ON the edge has no such derivative: its weight
-                // and its counterpart in the end correction (zeta_m12_du) are dropped together
+                // sqrt(-F) and its derivative -dF / (2 sqrt(-F)) from one reciprocal square root (no division). A node
+                // (numerically) ON the edge has no such derivative: its weight and its counterpart in the end correction
+                // (zeta_m12_du) are dropped together
+                const double rs = ul_rsqrt(-f3);
+                S += -f3 * rs;
                 RayBasis<N> B;
                 ray_basis<N, false>(L, R, r, c, s, B);
-                stat_add(SS, (-f3 > UL_DUAL_SING_FLOOR * rho2) ? -0.5 / sq : 0.0, B);
+                stat_add(SS, (-f3 > UL_DUAL_SING_FLOOR * rho2) ? -0.5 * rs : 0.0, B);
             }
             if (!periodic && (j < 2 || j >= n_th - 2)) edge = true;
         }
@@ -401,11 +402,11 @@ UL_HD void shoot_col_t(const Lens& L, double wcx, double wcy, double rho2, doubl
         if (i >= 0 && i < n_r && f3 < 0.0) {
             U += r;
             if (LD) {
-                const double sq = sqrt(-f3);
-                S += r * sq;
+                const double rs = ul_rsqrt(-f3);
+                S += r * (-f3 * rs);
                 RayBasis<N> B;
                 ray_basis<N, true>(L, R, r, c, s, B);
-                stat_add(SS, (-f3 > UL_DUAL_SING_FLOOR * rho2) ? -0.5 * r / sq : 0.0, B);
+                stat_add(SS, (-f3 > UL_DUAL_SING_FLOOR * rho2) ? -0.5 * r * rs : 0.0, B);
             }
             if ((i < 2 && r0 > 0.0) || i >= n_r - 2) edge = true;
         }
