@@ -52,10 +52,11 @@ FP64_DUAL_FACTOR = 2.25
 # N+1..DEG images 2.5 iterations x (17 N + 25), boxes ~100.
 FP64_INSTR_PER_LIMB_SOLVE = {1: 600, 2: 2400, 3: 8300}
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the roofline kernel, from the `ncu --set full` captures
-# summarised under profiles/ (r02_ncu_shoot_dual_c4.md, r02_ncu_shoot_c1.md, r02_ncu_shoot_c2.md, r02_ncu_shoot_f32_c1.md);
+# summarised under profiles/ (r02_ncu_shoot_dual_c4.md, r02_ncu_shoot_c1.md, r02_ncu_shoot_c2.md, r02_ncu_shoot_c3.md, r02_ncu_shoot_f32_c1.md);
 # key = (config, f32 variant)
-NCU_TRAFFIC_BYTES_PER_LAUNCH = {(4, False): 55.569152e6 + 724.669952e6, (1, False): 27.501056e6 + 0.717056e6,
-                                (2, False): 30.622720e6 + 5.162496e6, (1, True): 27.456512e6 + 1.179904e6}
+NCU_TRAFFIC_BYTES_PER_LAUNCH = {(4, False): 54.152704e6 + 660.615424e6, (1, False): 27.450880e6 + 0.672000e6,
+                                (2, False): 30.332672e6 + 4.473856e6, (3, False): 33.317888e6 + 2.782464e6,
+                                (1, True): 27.550464e6 + 0.452864e6}
 # FP64 FMA pipe of one B200: 148 SMs x 64 DFMA lanes / clk x 1.965 GHz (clocks.max.sm) -- DESIGN.md
 FP64_PEAK_DFMA = 148 * 64 * 1.965e9
 # Mixed-precision variant (k_shoot_f32): algorithmic FP32-pipe instructions per ray in the segment-local

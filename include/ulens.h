@@ -75,7 +75,9 @@ typedef struct ulens_ctx ulens_ctx;
 #define ULENS_OPT_NO_QUIET   0x4      /* do not use the quiet-point shortcut. By default a source point that a 9-probe point-source test
                                          finds far from every caustic (same image count at the centre and at 8 limb points, finite-source
                                          effect below 1e-4) has its limb followed with an eighth of the n_limb samples: its images are
-                                         smooth near-ellipses. Only the sampling density of step a3 changes; the rays still decide */
+                                         smooth near-ellipses. Only the sampling density of step a3 changes; the rays still decide.
+                                         Never next to a light lens (within 8 sqrt(eps) + 2 rho of its planetary caustic) and never in
+                                         the retry pass; a point's result does not depend on what it is batched with */
 
 /* Tunables; a zeroed struct (or NULL) selects the defaults in brackets. */
 typedef struct {

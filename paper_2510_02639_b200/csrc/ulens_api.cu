@@ -1287,6 +1287,7 @@ static int run_chunks(ulens_ctx* ctx, long long n_total, int n_pts, bool ld, con
                                                         nullptr, nullptr, nullptr, ctx->status_ws, ctx->c_zr, ctx->c_zi, ctx->c_mask, nullptr, nullptr, pmap, n_dev);
         }
         // quiet source points take the coarse limb sampling (first pass only: the retry pass is for doubtful points)
+        // (whatever the size of the call or the chunk: a point's result must not depend on what it is batched with)
         const bool use_quiet = !(ctx->opt.flags & ULENS_OPT_NO_QUIET) && st_or == 0 && ctx->quiet != nullptr;
         if (use_quiet) {
             KTimer kt(ctx, ULENS_K_ROOTS, st);
