@@ -36,6 +36,8 @@ struct DevCounters {
 struct ChunkCounters {          // reset per chunk
     unsigned int n_units;       // units allocated by k_regions
     unsigned int next_unit;     // dynamic scheduler of k_shoot
+    unsigned int n_quiet;       // k_quiet: quiet points (listed from the front of limb_list) ...
+    unsigned int n_full;        // ... and the others (listed from its back)
 };
 
 #define UL_N_STAGE 8
@@ -56,6 +58,8 @@ struct ulens_ctx {
     BoxExt* exts; int exts_cap;         // forward-mode runs: the boxes' extreme own points
     int* n_boxes;               // [chunk]
     unsigned char* quiet;       // [chunk] 1 = quiet source point (k_quiet): coarse limb sampling
+    int* limb_list;             // [chunk] k_quiet -> k_limb: quiet points from the front, the others from the back
+    double* quiet_drho;         // [chunk] quiet points: dA/drho from the probe (forward-mode runs)
     // forward-mode variant (allocated on first use)
     PatchTan* ptans;            // [chunk][UL_MAXP] tangents of the sectors' radial bounds
     double* unit_tan; int unit_tan_nt;  // [cap_units][NT] tangent sums of the units
@@ -417,24 +421,34 @@ __global__ void k_ext_scatter(int n, const unsigned char* __restrict__ flag, con
 #ifndef UL_QUIET_TOL
 #define UL_QUIET_TOL 1e-4
 #endif
+// Ray grid of the quiet points relative to ulens_options.n_r (scan lines per half-extent) and n_theta (nodes per half-chord
+// along a line). Measured over every point of C1-C3 against the full grid: half the lines cost a broad
+// ~2e-5 (largest 4e-5), half the nodes a heavy tail (1.3e-4 on 3 points: refused); (0.5, 0.75) keeps the largest
+// difference at 4.3e-5 and the largest error on the stored oracle samples at 5.0e-5, for 56 % fewer rays on those points.
+#ifndef UL_QUIET_RES_LINES
+#define UL_QUIET_RES_LINES 0.5
+#endif
+#ifndef UL_QUIET_RES_NODES
+#define UL_QUIET_RES_NODES 0.75
+#endif
 template <int N>
 __global__ void k_quiet(int n, int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cfg, const LensPoly* __restrict__ poly,
                         const double* __restrict__ w_re, const double* __restrict__ w_im, double tol,
-                        unsigned char* __restrict__ quiet, const int* __restrict__ pmap = nullptr,
-                        const unsigned* __restrict__ n_dev = nullptr)
+                        unsigned char* __restrict__ quiet, double* __restrict__ quiet_drho, int* __restrict__ limb_list,
+                        ChunkCounters* cc, const int* __restrict__ pmap = nullptr, const unsigned* __restrict__ n_dev = nullptr)
 {
     constexpr int DEG = N * N + 1;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (n_dev) n = min(n, (int)*n_dev - pt_base);
-    if (i >= n) return;
-    const long long gp = pmap ? (long long)pmap[pt_base + i] : (long long)pt_base + i;
+    const bool live = i < n;                             // (no early return: the warp lists its points together)
+    const long long gp = !live ? 0 : (pmap ? (long long)pmap[pt_base + i] : (long long)pt_base + i);
     const int c = (int)(gp / n_pts_per_cfg);
     const Lens L = cfg[c].lens;
     const double rho = cfg[c].rho, wx = w_re[gp], wy = w_im[gp];
     double zr[DEG], zi[DEG];
     double A_c = 0.0, s_axes = 0.0, s_diag = 0.0;
     unsigned st_c = 0;
-    bool ok = true;
+    bool ok = live;
     // never next to a light lens: within 8 sqrt(eps_a) + 2 rho of its planetary caustic (centred on
     // w_a = a_a - sum_{b != a} eps_b / conj(a_a - a_b)) images hide in a root cluster that the polynomial solve -- and
     // with it this probe -- can miss altogether (measured on C3: a pair of 4.5e-4 A each, found only by the limb
@@ -479,7 +493,32 @@ __global__ void k_quiet(int n, int pt_base, int n_pts_per_cfg, const PointCfg* _
         const double H = 0.25 * fabs(s_axes - s_diag);
         ok = (Q + H <= tol * A_c);
     }
-    quiet[i] = ok ? 1 : 0;
+    if (live) {
+        quiet[i] = ok ? 1 : 0;
+        // dA/drho of a quiet point from the same probe. Angular mean of A_ps on the limb = A_c + rho^2/4 lap A + O(rho^4), so
+        // for the limb-darkened disk (I = 1 - u1 (1 - sqrt(1 - r^2)), <r^2>_I = (1 - 7 u1/15) / (2 (1 - u1/3))):
+        //   A_fs = A_c + (mean_8 - A_c)/2 * LD + O(rho^4),  LD = (1 - 7 u1/15)/(1 - u1/3)   =>   dA_fs/drho = (mean_8 - A_c) LD / rho
+        // (the quadrupole term of Gould 2008 / Pejcha & Heyrovsky 2009; what "quiet" certifies is that the series converges).
+        // Forward mode uses it in place of the rule's own dA/drho, which far from caustics is the small difference of two
+        // terms ~ 2A/rho and carries the derivative of the along-line quadrature error.
+        const double u1 = cfg[c].u1;
+        quiet_drho[i] = ok ? (0.125 * (s_axes + s_diag) - A_c) * ((1.0 - 7.0 * u1 / 15.0) / (1.0 - u1 / 3.0)) / rho : 0.0;
+    }
+    // work lists of k_limb (one atomicAdd per warp and list): a quiet point is ONE work item, the others WARPS each; listing
+    // them apart keeps the working warps of k_limb packed (left in place, a quiet point's other WARPS - 1 work items would
+    // return at once and leave their CTA with a single resident warp). The order inside a list is whatever the atomics give:
+    // a point's result does not depend on which warp takes it.
+    const int lane = threadIdx.x & 31;
+    const unsigned bq = __ballot_sync(0xffffffffu, ok), bf = __ballot_sync(0xffffffffu, live && !ok);
+    unsigned base_q = 0, base_f = 0;
+    if (lane == 0) {
+        if (bq) base_q = atomicAdd(&cc->n_quiet, (unsigned)__popc(bq));
+        if (bf) base_f = atomicAdd(&cc->n_full, (unsigned)__popc(bf));
+    }
+    base_q = __shfl_sync(0xffffffffu, base_q, 0); base_f = __shfl_sync(0xffffffffu, base_f, 0);
+    const unsigned below = (1u << lane) - 1u;
+    if (ok) limb_list[base_q + __popc(bq & below)] = i;
+    else if (live) limb_list[n - 1 - (int)(base_f + __popc(bf & below))] = i;
 }
 
 // Image-region builder, first half (ulens_limb.cuh): a group of N^2+1 lanes per limb arc, one lane per root; a warp holds
@@ -495,18 +534,31 @@ k_limb(int n, int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cfg, 
        SubBox* __restrict__ boxes, BoxExt* __restrict__ exts, int* __restrict__ n_boxes, unsigned* __restrict__ status,
        DevCounters* ctr, const double* __restrict__ c_zr, const double* __restrict__ c_zi,
        const unsigned* __restrict__ c_mask, const int* __restrict__ pmap = nullptr, const unsigned* __restrict__ n_dev = nullptr,
-       const unsigned char* __restrict__ quiet = nullptr)
+       const unsigned char* __restrict__ quiet = nullptr, const int* __restrict__ limb_list = nullptr,
+       const ChunkCounters* __restrict__ cc = nullptr)
 {
     typedef LimbGeom<N> G;
     __shared__ LimbShared<N> sh[4];
     const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (n_dev) n = min(n, (int)*n_dev - pt_base);
     const long long item = (long long)blockIdx.x * 4 + wib;          // (point, warp of the point)
-    const int i = (int)(item / G::WARPS), w = (int)(item % G::WARPS);
-    if (i >= n) return;                                  // whole warp leaves together
-    // a quiet point (k_quiet) is one work item: its limb is followed by warp 0 alone, GPW arcs, an eighth of the samples
-    const bool q = quiet && quiet[i];
-    if (q && w > 0) return;
+    int i, w;
+    bool q = false;
+    if (limb_list) {
+        // work lists of k_quiet: the quiet points first (one work item each: warp 0 follows the whole limb, GPW arcs, an
+        // eighth of the samples), then WARPS items for each of the others; the grid is sized for the worst case and the
+        // items past the end leave at once, whole CTAs at a time
+        const long long nq = cc->n_quiet, nf = cc->n_full;
+        if (item < nq) { i = limb_list[item]; w = 0; q = true; }
+        else {
+            const long long it = item - nq;
+            if (it >= nf * G::WARPS) return;
+            i = limb_list[n - 1 - (int)(it / G::WARPS)]; w = (int)(it % G::WARPS);
+        }
+    } else {
+        i = (int)(item / G::WARPS); w = (int)(item % G::WARPS);
+        if (i >= n) return;                              // whole warp leaves together
+    }
     const long long gp = pmap ? (long long)pmap[pt_base + i] : (long long)pt_base + i;
     const int c = (int)(gp / n_pts_per_cfg);
     const Lens L = cfg[c].lens;
@@ -553,7 +605,10 @@ k_sectors(int n, int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cf
         typedef LimbGeom<N> G;
         const bool q = quiet && quiet[i];
         const int n_samp = q ? G::GPW * max(2, (rp.n_limb / 8 + G::GPW - 1) / G::GPW) : G::NARC * max(1, (rp.n_limb + G::NARC / 2) / G::NARC);
-        np = sectors_from_boxes<N>(boxes + (size_t)i * CAP, tans ? exts + (size_t)i * CAP : nullptr, min(n_boxes[i], CAP), rp, i, L,
+        // quiet points: smooth near-elliptical images, for which the rule converges fast: fewer lines, fewer nodes per line
+        RegionParams rpq = rp;
+        if (q) { rpq.n_r = max(16, (int)(rp.n_r * UL_QUIET_RES_LINES + 0.5)); rpq.n_theta = max(8, (int)(rp.n_theta * UL_QUIET_RES_NODES + 0.5)); }
+        np = sectors_from_boxes<N>(boxes + (size_t)i * CAP, tans ? exts + (size_t)i * CAP : nullptr, min(n_boxes[i], CAP), rpq, i, L,
                                    w_re[gp], w_im[gp], cfg[c].rho, st, tans ? &tans[c] : nullptr, pp, pt, 2.0 * UL_PI / n_samp);
         for (int p = 0; p < np; ++p) total_units += pp[p].n_units;
     }
@@ -888,7 +943,8 @@ __global__ void k_finalize_dual(int n, int pt_base, int n_pts_per_cfg, const Poi
                                 const TangentTable* __restrict__ tans, const Patch* __restrict__ patches,
                                 const int* __restrict__ n_patch, const double* __restrict__ unit_sum,
                                 const double* __restrict__ unit_tan, double* __restrict__ grad, const int* __restrict__ pmap = nullptr,
-                                const unsigned* __restrict__ n_dev = nullptr, const unsigned* __restrict__ status_retry = nullptr)
+                                const unsigned* __restrict__ n_dev = nullptr, const unsigned* __restrict__ status_retry = nullptr,
+                                const unsigned char* __restrict__ quiet = nullptr, const double* __restrict__ quiet_drho = nullptr)
 {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (n_dev) n = min(n, (int)*n_dev - pt_base);
@@ -913,6 +969,8 @@ __global__ void k_finalize_dual(int n, int pt_base, int n_pts_per_cfg, const Poi
         double dF0 = 2.0 * UL_PI * rho * (1.0 - u1 / 3.0) * tans[c].drho[k];
         grad[gp * NT + k] = np ? (tk[k] - A * dF0) / F0 : nan("");
     }
+    // quiet point: dA/drho from the multipole probe (k_quiet); direction NT-1 is rho in every tangent table
+    if (quiet && quiet[i] && np) grad[gp * NT + NT - 1] = quiet_drho[i];
 }
 
 // chain rule through the trajectory (reading G3): (w_cx, w_cy, s, q, rho) -> (t0, u0, tE, s, q, rho, alpha)
@@ -1137,6 +1195,8 @@ extern "C" int ulens_create(ulens_ctx** out, int cuda_device, const ulens_option
     if (e == cudaSuccess) e = cudaMalloc(&ctx->c_mask, sizeof(unsigned) * (size_t)ctx->chunk);
     if (e == cudaSuccess) e = cudaMalloc(&ctx->n_boxes, sizeof(int) * (size_t)ctx->chunk);
     if (e == cudaSuccess) e = cudaMalloc(&ctx->quiet, (size_t)ctx->chunk);
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->limb_list, sizeof(int) * (size_t)ctx->chunk);
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->quiet_drho, sizeof(double) * (size_t)ctx->chunk);
     if (e == cudaSuccess) e = cudaMalloc(&ctx->unit_desc, sizeof(unsigned) * ctx->cap_units);
     if (e == cudaSuccess) e = cudaMalloc(&ctx->unit_sum, sizeof(double) * ctx->cap_units);
     if (e == cudaSuccess) e = cudaMalloc(&ctx->unit_odd, sizeof(double) * ctx->cap_units);
@@ -1154,7 +1214,7 @@ extern "C" void ulens_destroy(ulens_ctx* ctx)
     cudaSetDevice(ctx->device);
     cudaDeviceSynchronize();
     cudaFree(ctx->c_zr); cudaFree(ctx->c_zi); cudaFree(ctx->c_mask);
-    cudaFree(ctx->boxes); cudaFree(ctx->exts); cudaFree(ctx->n_boxes); cudaFree(ctx->quiet);
+    cudaFree(ctx->boxes); cudaFree(ctx->exts); cudaFree(ctx->n_boxes); cudaFree(ctx->quiet); cudaFree(ctx->limb_list); cudaFree(ctx->quiet_drho);
     cudaFree(ctx->ptans); cudaFree(ctx->unit_tan); cudaFree(ctx->grad5); cudaFree(ctx->tan_dev);
     cudaFree(ctx->patches); cudaFree(ctx->n_patch); cudaFree(ctx->status_ws); cudaFree(ctx->unit_desc);
     cudaFree(ctx->unit_sum); cudaFree(ctx->unit_odd); cudaFree(ctx->cc); cudaFree(ctx->counters);
@@ -1291,7 +1351,7 @@ static int run_chunks(ulens_ctx* ctx, long long n_total, int n_pts, bool ld, con
         const bool use_quiet = !(ctx->opt.flags & ULENS_OPT_NO_QUIET) && st_or == 0 && ctx->quiet != nullptr;
         if (use_quiet) {
             KTimer kt(ctx, ULENS_K_ROOTS, st);
-            k_quiet<N><<<(n + 127) / 128, 128, 0, st>>>(n, (int)base, n_pts, ctx->cfg_dev, ctx->poly_dev, w_re, w_im, UL_QUIET_TOL, ctx->quiet, pmap, n_dev);
+            k_quiet<N><<<(n + 127) / 128, 128, 0, st>>>(n, (int)base, n_pts, ctx->cfg_dev, ctx->poly_dev, w_re, w_im, UL_QUIET_TOL, ctx->quiet, ctx->quiet_drho, ctx->limb_list, ctx->cc, pmap, n_dev);
             ctx->last_launches += 1;
         }
         const unsigned char* quiet = use_quiet ? ctx->quiet : nullptr;
@@ -1302,11 +1362,13 @@ static int run_chunks(ulens_ctx* ctx, long long n_total, int n_pts, bool ld, con
             if (dual)
                 k_limb<N, true><<<limb_grid, 128, 0, st>>>(n, (int)base, n_pts, ctx->cfg_dev, ctx->poly_dev, w_re, w_im, rp,
                                                                     ctx->boxes, ctx->exts, ctx->n_boxes, ctx->status_ws, ctx->counters,
-                                                                    ctx->c_zr, ctx->c_zi, ctx->c_mask, pmap, n_dev, quiet);
+                                                                    ctx->c_zr, ctx->c_zi, ctx->c_mask, pmap, n_dev, quiet,
+                                                                    quiet ? ctx->limb_list : nullptr, ctx->cc);
             else
                 k_limb<N, false><<<limb_grid, 128, 0, st>>>(n, (int)base, n_pts, ctx->cfg_dev, ctx->poly_dev, w_re, w_im, rp,
                                                                      ctx->boxes, ctx->exts, ctx->n_boxes, ctx->status_ws, ctx->counters,
-                                                                     ctx->c_zr, ctx->c_zi, ctx->c_mask, pmap, n_dev, quiet);
+                                                                     ctx->c_zr, ctx->c_zi, ctx->c_mask, pmap, n_dev, quiet,
+                                                                     quiet ? ctx->limb_list : nullptr, ctx->cc);
         }
         {
             KTimer kt(ctx, ULENS_K_SECTORS, st);
@@ -1360,7 +1422,8 @@ static int run_chunks(ulens_ctx* ctx, long long n_total, int n_pts, bool ld, con
                                                         A_out, err_out, status_out, ctx->counters, pmap, n_dev, st_or);
             if (dual) {
                 k_finalize_dual<NT><<<(n + 127) / 128, 128, 0, st>>>(n, (int)base, n_pts, ctx->cfg_dev, tans, ctx->patches, ctx->n_patch,
-                                                                 ctx->unit_sum, ctx->unit_tan, grad5_out, pmap, n_dev, st_or ? status_out : nullptr);
+                                                                 ctx->unit_sum, ctx->unit_tan, grad5_out, pmap, n_dev, st_or ? status_out : nullptr,
+                                                                 quiet, ctx->quiet_drho);
                 ctx->last_launches += 1;
             }
         }
@@ -2070,7 +2133,9 @@ constexpr size_t UL_SO_UODD     = UL_SO_USUM     + ul_align256(sizeof(double) * 
 constexpr size_t UL_SO_CC       = UL_SO_UODD     + ul_align256(sizeof(double) * UL_STATIC_UNITS);
 constexpr size_t UL_SO_COUNTERS = UL_SO_CC       + ul_align256(sizeof(ChunkCounters));
 constexpr size_t UL_SO_QUIET    = UL_SO_COUNTERS + ul_align256(sizeof(DevCounters));
-constexpr size_t UL_STATIC_BYTES = UL_SO_QUIET + ul_align256(ULENS_STATIC_MAX_POINTS);
+constexpr size_t UL_SO_LIMBLIST = UL_SO_QUIET + ul_align256(ULENS_STATIC_MAX_POINTS);
+constexpr size_t UL_SO_QDRHO    = UL_SO_LIMBLIST + ul_align256(sizeof(int) * ULENS_STATIC_MAX_POINTS);
+constexpr size_t UL_STATIC_BYTES = UL_SO_QDRHO + ul_align256(sizeof(double) * ULENS_STATIC_MAX_POINTS);
 static_assert(UL_STATIC_BYTES <= (size_t)8 << 20, "static scratch is meant to stay modest (<= 8 MiB)");
 
 static __device__ __align__(256) unsigned char g_static_scratch[UL_STATIC_BYTES];
@@ -2121,6 +2186,8 @@ static int static_setup(int dev)
     ctx->cc        = reinterpret_cast<ChunkCounters*>(base + UL_SO_CC);
     ctx->counters  = reinterpret_cast<DevCounters*>(base + UL_SO_COUNTERS);
     ctx->quiet     = base + UL_SO_QUIET;
+    ctx->limb_list = reinterpret_cast<int*>(base + UL_SO_LIMBLIST);
+    ctx->quiet_drho = reinterpret_cast<double*>(base + UL_SO_QDRHO);
     g_static_ready[dev] = true;
     return ULENS_OK;
 }

@@ -93,11 +93,13 @@ def test_full_config4_with_derivatives(ctx, torch_cuda):
 
 def test_config4_derivatives_do_not_depend_on_the_limb_sampling(torch_cuda):
     """Forward mode moves each sector with the image's extreme points; the sampled extremes are refined to the true ones
-    (refine_extreme, ulens_regions.cuh), so the derivatives must not depend on how densely the limb was sampled -- not
-    even for the quiet points, whose limb gets an eighth of the samples. 64 light curves of C4 x 2,000 epochs, three
-    runs: production (n_limb 512, quiet-point shortcut), shortcut off, shortcut off with n_limb 2048 (the reference).
-    dA/drho is reported, not asserted: it is the small difference of two terms ~2A/rho and carries the derivative of the
-    along-line quadrature error."""
+    (refine_extreme, ulens_regions.cuh), so the derivatives must not depend on how densely the limb was sampled. 64 light
+    curves of C4 x 2,000 epochs, three runs: shortcut off at n_limb 512 against shortcut off at n_limb 2048 (the
+    reference) -- median relative difference <= 1e-5 (measured 1e-10; 1e-3 before the refinement) -- and production
+    (quiet points: an eighth of the limb samples AND the coarser ray grid) against the same reference: <= 2e-4, a tenth of
+    the derivative bar. dA/drho is reported, not asserted: the rule's own dA/drho is the small difference of two terms
+    ~2A/rho and carries the derivative of the along-line quadrature error, and production replaces it by
+    the quadrupole term on the quiet points (tested against finite differences in test_gpu_dual.py)."""
     from paper_2510_02639_b200 import binding, inputs
     torch = torch_cuda
     wl = inputs.get(4)
@@ -113,7 +115,7 @@ def test_config4_derivatives_do_not_depend_on_the_limb_sampling(torch_cuda):
         c.close()
     A_ref, d_ref, s_ref = runs["n_limb 2048"]
     names = ["t0", "u0", "tE", "s", "q", "rho", "alpha"]
-    for name in ("production", "shortcut off"):
+    for name, med_tol in (("production", 2e-4), ("shortcut off", 1e-5)):
         A, dA, st = runs[name]
         clean = ((st & 0xff) == 0) & ((s_ref & 0xff) == 0)
         assert clean.mean() > 0.98
@@ -124,6 +126,6 @@ def test_config4_derivatives_do_not_depend_on_the_limb_sampling(torch_cuda):
             r = (np.abs(dA[:, :, k] - d_ref[:, :, k]) / (mag + 1e-2 * np.median(mag)))[clean]
             line.append("%s %.0e/%.0e" % (names[k], np.median(r), np.quantile(r, 0.99)))
             if names[k] != "rho":
-                assert np.median(r) <= 1e-5, (name, names[k], np.median(r))
+                assert np.median(r) <= med_tol, (name, names[k], np.median(r))
                 assert np.quantile(r, 0.99) <= 1e-2, (name, names[k], np.quantile(r, 0.99))
         print("C4 derivatives, %s vs n_limb 2048 (relative difference, median/p99): %s" % (name, "  ".join(line)))
