@@ -138,7 +138,11 @@ int  ulens_mag(ulens_ctx* ctx, int n_cfg, int n_pts,
  *   n_lens = 1, 2: dA5_out device [n_cfg*n_pts][5] = dA/d(w_cx, w_cy, s, q, rho)   (s, q columns zero for n_lens = 1)
  *   n_lens = 3   : dA5_out device [n_cfg*n_pts][8] = dA/d(w_cx, w_cy, s, q, q3, r3, psi, rho)
  * The lens-parameter columns are defined in the geometry of ulens_lens_binary / ulens_lens_triple (the parameters are
- * recovered from the lens; any other geometry is EUNSUPPORTED). */
+ * recovered from the lens; any other geometry is EUNSUPPORTED).
+ * The derivatives are those of the quadrature rule on a ray grid that moves with the image, with one
+ * exception: on a quiet source point (see ULENS_OPT_NO_QUIET) the rho column is the quadrupole term of the finite-source
+ * expansion, (<A_ps>_limb - A_ps(w_c)) (1 - 7 u1/15)/(1 - u1/3) / rho. Far from caustics dA/drho is the small difference of two
+ * terms ~2A/rho and the rule's own value there is cancellation noise of size ~1e-4 A/rho (also with ULENS_OPT_NO_QUIET). */
 int  ulens_mag_grad(ulens_ctx* ctx, int n_cfg, int n_pts,
                const ulens_lens* lenses_host, const double* rho_host, const double* u1_host,
                const double* w_re, const double* w_im,
