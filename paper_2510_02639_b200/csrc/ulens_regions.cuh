@@ -202,6 +202,13 @@ UL_HD bool refine_extreme(const Lens& L, double wcx, double wcy, double rho, int
     return true;
 }
 
+// "more extreme" with a total order: boxes arrive in any order, and two boxes that share a limb point (the end of one arc is the
+// start of the next) can hold the same extreme value to the last bit with coordinates that differ in theirs
+UL_HD bool ext_before(double v, double ph, double x, double v0, double ph0, double x0)
+{
+    return v < v0 || (v == v0 && (ph < ph0 || (ph == ph0 && x < x0)));
+}
+
 // the extreme own points of a sector (sampled) -> the true extremes of the image boundary
 template <int N>
 UL_HD void refine_sector_extremes(const Lens& L, double wcx, double wcy, double rho, double dph, bool from_origin, BoxExt& x)
@@ -435,8 +442,8 @@ UL_HDN int sectors_from_boxes(const SubBox* box, const BoxExt* ext, int nb, cons
                 hr = ul_min(hr, b.hr); ht = ul_min(ht, b.ht); cr = ul_min(cr, b.cr); ct = ul_min(ct, b.ct);
                 if (ext) {
                     const BoxExt& e = ext[i];
-                    if (e.lo_r < xlo.lo_r) { xlo.lo_r = e.lo_r; xlo.lo_x = e.lo_x; xlo.lo_y = e.lo_y; xlo.lo_ph = e.lo_ph; }
-                    if (e.hi_r > xlo.hi_r) { xlo.hi_r = e.hi_r; xlo.hi_x = e.hi_x; xlo.hi_y = e.hi_y; xlo.hi_ph = e.hi_ph; }
+                    if (ext_before(e.lo_r, e.lo_ph, e.lo_x, xlo.lo_r, xlo.lo_ph, xlo.lo_x)) { xlo.lo_r = e.lo_r; xlo.lo_x = e.lo_x; xlo.lo_y = e.lo_y; xlo.lo_ph = e.lo_ph; }
+                    if (ext_before(-e.hi_r, e.hi_ph, e.hi_x, -xlo.hi_r, xlo.hi_ph, xlo.hi_x)) { xlo.hi_r = e.hi_r; xlo.hi_x = e.hi_x; xlo.hi_y = e.hi_y; xlo.hi_ph = e.hi_ph; }
                 }
             }
             if (np == UL_MAXP) { capped = true; break; }
@@ -523,11 +530,11 @@ UL_HDN int sectors_from_boxes(const SubBox* box, const BoxExt* ext, int nb, cons
             if (ext) {
                 const BoxExt& e = ext[i];
                 BoxExt& x = c_ext[c];
-                if (e.lo_r < x.lo_r) { x.lo_r = e.lo_r; x.lo_x = e.lo_x; x.lo_y = e.lo_y; x.lo_ph = e.lo_ph; }
-                if (e.hi_r > x.hi_r) { x.hi_r = e.hi_r; x.hi_x = e.hi_x; x.hi_y = e.hi_y; x.hi_ph = e.hi_ph; }
+                if (ext_before(e.lo_r, e.lo_ph, e.lo_x, x.lo_r, x.lo_ph, x.lo_x)) { x.lo_r = e.lo_r; x.lo_x = e.lo_x; x.lo_y = e.lo_y; x.lo_ph = e.lo_ph; }
+                if (ext_before(-e.hi_r, e.hi_ph, e.hi_x, -x.hi_r, x.hi_ph, x.hi_x)) { x.hi_r = e.hi_r; x.hi_x = e.hi_x; x.hi_y = e.hi_y; x.hi_ph = e.hi_ph; }
                 // theta ends in the cell's own unwrapping: this box's interval is [tl, th] after the shifts above
-                if (tl < x.tlo_t) { x.tlo_t = tl; x.tlo_x = e.tlo_x; x.tlo_y = e.tlo_y; x.tlo_ph = e.tlo_ph; }
-                if (th > x.thi_t) { x.thi_t = th; x.thi_x = e.thi_x; x.thi_y = e.thi_y; x.thi_ph = e.thi_ph; }
+                if (ext_before(tl, e.tlo_ph, e.tlo_x, x.tlo_t, x.tlo_ph, x.tlo_x)) { x.tlo_t = tl; x.tlo_x = e.tlo_x; x.tlo_y = e.tlo_y; x.tlo_ph = e.tlo_ph; }
+                if (ext_before(-th, e.thi_ph, e.thi_x, -x.thi_t, x.thi_ph, x.thi_x)) { x.thi_t = th; x.thi_x = e.thi_x; x.thi_y = e.thi_y; x.thi_ph = e.thi_ph; }
             }
         }
         for (int c = 0; c < ngt; ++c) {
