@@ -425,8 +425,13 @@ __global__ void k_ext_scatter(int n, const unsigned char* __restrict__ flag, con
 // along a line). Measured over every point of C1-C3 against the full grid: half the lines cost a broad
 // ~2e-5 (largest 4e-5), half the nodes a heavy tail (1.3e-4 on 3 points: refused); (0.5, 0.75) keeps the largest
 // difference at 4.3e-5 and the largest error on the stored oracle samples at 5.0e-5, for 56 % fewer rays on those points.
+// Ray grid of a quiet point's sectors that end at the true extremes of their image (ulens_regions.cuh quiet_image_extremes),
+// relative to ulens_options.n_r (scan lines per half-extent) and n_theta (nodes per half-chord along a line). Measured over
+// every point of C1-C3 and 1.4 M random-lens points against the full treatment, and on the stored oracle samples
+// (DESIGN.md 5.3): with exact ends (3/8, 3/4) stays within 3.3e-5 of the full grid; 5/8 of the nodes puts single points at
+// 6.7e-5 (refused); a quarter of the lines costs a broad 2e-5 ... 5e-5 (refused).
 #ifndef UL_QUIET_RES_LINES
-#define UL_QUIET_RES_LINES 0.5
+#define UL_QUIET_RES_LINES 0.375
 #endif
 #ifndef UL_QUIET_RES_NODES
 #define UL_QUIET_RES_NODES 0.75
@@ -586,7 +591,9 @@ k_sectors(int n, int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cf
           const int* __restrict__ n_boxes, Patch* __restrict__ patches, int* __restrict__ n_patch, unsigned* __restrict__ status,
           unsigned* __restrict__ unit_desc, unsigned cap_units, ChunkCounters* cc, DevCounters* ctr,
           const TangentTable* __restrict__ tans, PatchTan* __restrict__ ptans, const int* __restrict__ pmap = nullptr,
-          const unsigned* __restrict__ n_dev = nullptr, const unsigned char* __restrict__ quiet = nullptr)
+          const unsigned* __restrict__ n_dev = nullptr, const unsigned char* __restrict__ quiet = nullptr,
+          const double* __restrict__ c_zr = nullptr, const double* __restrict__ c_zi = nullptr,
+          const unsigned* __restrict__ c_mask = nullptr)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int lane = threadIdx.x & 31;
@@ -605,11 +612,13 @@ k_sectors(int n, int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cf
         typedef LimbGeom<N> G;
         const bool q = quiet && quiet[i];
         const int n_samp = q ? G::GPW * max(2, (rp.n_limb / 8 + G::GPW - 1) / G::GPW) : G::NARC * max(1, (rp.n_limb + G::NARC / 2) / G::NARC);
-        // quiet points: smooth near-elliptical images, for which the rule converges fast: fewer lines, fewer nodes per line
+        // quiet points: a sector that ends at the true extremes of a smooth near-elliptical image (quiet_image_extremes) is
+        // shot with fewer lines and fewer nodes per line: with exact ends the sin-spaced rule across the lines is all but exact
         RegionParams rpq = rp;
-        if (q) { rpq.n_r = max(16, (int)(rp.n_r * UL_QUIET_RES_LINES + 0.5)); rpq.n_theta = max(8, (int)(rp.n_theta * UL_QUIET_RES_NODES + 0.5)); }
-        np = sectors_from_boxes<N>(boxes + (size_t)i * CAP, tans ? exts + (size_t)i * CAP : nullptr, min(n_boxes[i], CAP), rpq, i, L,
-                                   w_re[gp], w_im[gp], cfg[c].rho, st, tans ? &tans[c] : nullptr, pp, pt, 2.0 * UL_PI / n_samp);
+        rpq.n_r = max(16, (int)(rp.n_r * UL_QUIET_RES_LINES + 0.5)); rpq.n_theta = max(8, (int)(rp.n_theta * UL_QUIET_RES_NODES + 0.5));
+        np = sectors_from_boxes<N>(boxes + (size_t)i * CAP, tans ? exts + (size_t)i * CAP : nullptr, min(n_boxes[i], CAP), rp, i, L,
+                                   w_re[gp], w_im[gp], cfg[c].rho, st, tans ? &tans[c] : nullptr, pp, pt, 2.0 * UL_PI / n_samp,
+                                   q ? &rpq : nullptr, c_zr + (long long)i * 10, c_zi + (long long)i * 10, c_mask[i]);
         for (int p = 0; p < np; ++p) total_units += pp[p].n_units;
     }
     // one atomicAdd per warp: exclusive prefix sum of the lanes' unit counts, lane 31 holds the warp's total
@@ -1374,7 +1383,8 @@ static int run_chunks(ulens_ctx* ctx, long long n_total, int n_pts, bool ld, con
             KTimer kt(ctx, ULENS_K_SECTORS, st);
             k_sectors<N><<<(n + 127) / 128, 128, 0, st>>>(n, (int)base, n_pts, ctx->cfg_dev, w_re, w_im, rp, ctx->boxes, ctx->exts,
                                                            ctx->n_boxes, ctx->patches, ctx->n_patch, ctx->status_ws, ctx->unit_desc,
-                                                           (unsigned)ctx->cap_units, ctx->cc, ctx->counters, tans, ctx->ptans, pmap, n_dev, quiet);
+                                                           (unsigned)ctx->cap_units, ctx->cc, ctx->counters, tans, ctx->ptans, pmap, n_dev, quiet,
+                                                           ctx->c_zr, ctx->c_zi, ctx->c_mask);
         }
         // persistent grid: as many CTAs as are resident at once (occupancy API; 4-6 per SM by register count)
         int per_sm = 4;

@@ -166,7 +166,7 @@ UL_HD void patch_tangents(const Lens& L, const TangentTable& T, const BoxExt& x,
 // if the image is lost, the search leaves the range, or the result is less extreme than the sample.
 template <int N>
 UL_HD bool refine_extreme(const Lens& L, double wcx, double wcy, double rho, int which, int kind, double dph,
-                          double& x, double& y, double& ph)
+                          double& x, double& y, double& ph, bool from_sample = true)
 {
     // f = d(|z| or arg z)/dphi up to a positive factor
     auto slope = [&](double phi, double& zx, double& zy, double& f) -> bool {
@@ -196,8 +196,10 @@ UL_HD bool refine_extreme(const Lens& L, double wcx, double wcy, double rho, int
     }
     const double mv2 = (x1 - x) * (x1 - x) + (y1 - y) * (y1 - y);
     if (!(mv2 <= 0.01 * ul_max(x * x + y * y, 0.04))) return false;       // jumped to another image
-    if (which == 0) { if (kind * (sqrt(x1 * x1 + y1 * y1) - sqrt(x * x + y * y)) < 0.0) return false; }
-    else { if (kind * (x * y1 - y * x1) < 0.0) return false; }             // sign of the turn from the sample to the result
+    if (from_sample) {                                   // (a start that is only a prediction may lie beyond the true extreme)
+        if (which == 0) { if (kind * (sqrt(x1 * x1 + y1 * y1) - sqrt(x * x + y * y)) < 0.0) return false; }
+        else { if (kind * (x * y1 - y * x1) < 0.0) return false; }         // sign of the turn from the sample to the result
+    }
     x = x1; y = y1; ph = p1;
     return true;
 }
@@ -207,6 +209,46 @@ UL_HD bool refine_extreme(const Lens& L, double wcx, double wcy, double rho, int
 UL_HD bool ext_before(double v, double ph, double x, double v0, double ph0, double x0)
 {
     return v < v0 || (v == v0 && (ph < ph0 || (ph == ph0 && x < x0)));
+}
+
+// Quiet points: the image around a centre image z_c is close to the Jacobian ellipse z_c + rho (e^{i phi} - g e^{-i phi}) / D,
+// D = 1 - |g|^2, whose extremes along the radial direction n = z_c/|z_c| and across it are known in closed form:
+//   Re(conj(n) dz) D / rho = Re((conj(n) - n conj(g)) e^{i phi}),   Im(conj(n) dz) D / rho = Im((conj(n) + n conj(g)) e^{i phi}).
+// From those limb angles the four TRUE extremes of the image are found by refine_extreme (Newton on Eq. 1 along the limb).
+// With them a sector ends exactly where its image ends, which is what the sin-spaced lines across it want: the bounds from
+// the limb samples are good to ~1e-3 of the image and carry a safety margin of 0.5 %, and that offset -- not the number of
+// lines -- is what limits the rule on a smooth image. Returns false (nothing usable) if any of the four is not found.
+template <int N>
+UL_HD bool quiet_image_extremes(const Lens& L, double wcx, double wcy, double rho, double zcx, double zcy, BoxExt& x)
+{
+    double fx, fy, gx, gy, dm2;
+    lens_resid<N>(L, zcx, zcy, wcx, wcy, fx, fy, gx, gy, dm2);
+    const double D = 1.0 - (gx * gx + gy * gy);
+    const double rc = sqrt(zcx * zcx + zcy * zcy);
+    if (!(fabs(D) > 1e-3) || !(rc > 0.0)) return false;
+    const double nx = zcx / rc, ny = zcy / rc;
+    // n conj(g)
+    const double ngx = nx * gx + ny * gy, ngy = ny * gx - nx * gy;
+    // radial: q_r = conj(n) - n conj(g);  azimuthal: q_t = conj(n) + n conj(g)
+    const double qrx = nx - ngx, qry = -ny - ngy, qtx = nx + ngx, qty = -ny + ngy;
+    const double sgn = D > 0.0 ? 1.0 : -1.0;
+    const double ph_r = -atan2(qry, qrx), ph_t = 0.5 * UL_PI - atan2(qty, qtx);
+    bool ok = true;
+    for (int e = 0; e < 4 && ok; ++e) {
+        const int which = e >> 1, kind = (e & 1) ? -1 : +1;                 // r max, r min, theta max, theta min
+        double ph = (which == 0 ? ph_r : ph_t) + ((kind * sgn > 0.0) ? 0.0 : UL_PI);
+        const double c = cos(ph), sn = sin(ph);
+        // dz = rho (e^{i phi} - g e^{-i phi}) / D
+        double px = zcx + rho * (c - (gx * c + gy * sn)) / D, py = zcy + rho * (sn - (gy * c - gx * sn)) / D;
+        ok = refine_extreme<N>(L, wcx, wcy, rho, which, kind, 0.6, px, py, ph, false);
+        if (!ok) break;
+        const double r = sqrt(px * px + py * py);
+        if (e == 0) { x.hi_r = r; x.hi_x = px; x.hi_y = py; x.hi_ph = ph; }
+        else if (e == 1) { x.lo_r = r; x.lo_x = px; x.lo_y = py; x.lo_ph = ph; }
+        else if (e == 2) { x.thi_t = atan2(py, px); x.thi_x = px; x.thi_y = py; x.thi_ph = ph; }
+        else { x.tlo_t = atan2(py, px); x.tlo_x = px; x.tlo_y = py; x.tlo_ph = ph; }
+    }
+    return ok;
 }
 
 // the extreme own points of a sector (sampled) -> the true extremes of the image boundary
@@ -383,11 +425,15 @@ UL_HD void interval_merge_necks(double* g_lo, double* g_hi, int& ng)
 // one ray on it decides. Where it is inside (ring-like image around the origin, or a disk that contains
 // the origin) the gap is filled: the groups on both sides merge into one full-ring sector.
 //   box [nb], ext [nb] or nullptr (forward-mode run: the boxes' extreme own points); patch / ptan [UL_MAXP] out;
-//   dph_limb: spacing of this point's limb samples (forward-mode run: how far a true extreme can lie from the sampled one).
+//   dph_limb: spacing of this point's limb samples (forward-mode run: how far a true extreme can lie from the sampled one);
+//   Pquiet, czr / czi / cmask: a quiet point (k_quiet) and the images of its centre: a sector that holds exactly one of them ends
+//   at the true extremes of that image (quiet_image_extremes) and takes the coarser ray grid *Pquiet; any other sector of the
+//   point keeps its bounds from the limb samples and the full grid P.
 template <int N>
 UL_HDN int sectors_from_boxes(const SubBox* box, const BoxExt* ext, int nb, const RegionParams& P, int point, const Lens& L,
                               double wcx, double wcy, double rho, unsigned& status, const TangentTable* TT, Patch* patch,
-                              PatchTan* ptan, double dph_limb = 2.0 * UL_PI / 512)
+                              PatchTan* ptan, double dph_limb = 2.0 * UL_PI / 512, const RegionParams* Pquiet = nullptr,
+                              const double* czr = nullptr, const double* czi = nullptr, unsigned cmask = 0)
 {
     if (nb == 0) { status |= UL_ST_NO_IMAGE; return 0; }
 
@@ -537,6 +583,39 @@ UL_HDN int sectors_from_boxes(const SubBox* box, const BoxExt* ext, int nb, cons
                 if (ext_before(-th, e.thi_ph, e.thi_x, -x.thi_t, x.thi_ph, x.thi_x)) { x.thi_t = th; x.thi_x = e.thi_x; x.thi_y = e.thi_y; x.thi_ph = e.thi_ph; }
             }
         }
+        // ---- quiet point: a cell that holds exactly one image of the centre ends at that image's true extremes
+        bool c_exact[UL_MAXG];
+        for (int c = 0; c < ngt; ++c) c_exact[c] = false;
+        if (Pquiet && czr && !full_ring) {
+            constexpr int DEG = N * N + 1;
+            for (int c = 0; c < ngt; ++c) {
+                if (c_rl[c] > c_rh[c] || !(c_rl[c] > 0.0)) continue;
+                int cnt = 0, kk = -1;
+                for (int k = 0; k < DEG; ++k) {
+                    if (!((cmask >> k) & 1u)) continue;
+                    const double r = sqrt(czr[k] * czr[k] + czi[k] * czi[k]);
+                    if (!(r >= c_rl[c] && r <= c_rh[c])) continue;
+                    double t = atan2(czi[k], czr[k]);
+                    t += 2.0 * UL_PI * floor((0.5 * (c_tl[c] + c_th[c]) - t) / (2.0 * UL_PI) + 0.5);     // the turn nearest to the cell
+                    if (t >= c_tl[c] && t <= c_th[c]) { ++cnt; kk = k; }
+                }
+                if (cnt != 1) continue;
+                BoxExt x; ext_reset(x);
+                if (!quiet_image_extremes<N>(L, wcx, wcy, rho, czr[kk], czi[kk], x)) continue;
+                const double mid = 0.5 * (c_tl[c] + c_th[c]);
+                x.tlo_t += 2.0 * UL_PI * floor((mid - x.tlo_t) / (2.0 * UL_PI) + 0.5);
+                x.thi_t += 2.0 * UL_PI * floor((mid - x.thi_t) / (2.0 * UL_PI) + 0.5);
+                // the true extremes must agree with what the limb samples bounded (else: not the image this cell holds)
+                const double er = 0.1 * (c_rh[c] - c_rl[c]), et = 0.1 * (c_th[c] - c_tl[c]);
+                if (!(x.lo_r < x.hi_r && x.tlo_t < x.thi_t && x.lo_r >= c_rl[c] - er && x.lo_r <= c_rl[c] + er &&
+                      x.hi_r >= c_rh[c] - er && x.hi_r <= c_rh[c] + er && x.tlo_t >= c_tl[c] - et && x.tlo_t <= c_tl[c] + et &&
+                      x.thi_t >= c_th[c] - et && x.thi_t <= c_th[c] + et)) continue;
+                const double mr = 2e-4 * (x.hi_r - x.lo_r), mt = 2e-4 * (x.thi_t - x.tlo_t);
+                c_rl[c] = ul_max(x.lo_r - mr, 0.0); c_rh[c] = x.hi_r + mr; c_tl[c] = x.tlo_t - mt; c_th[c] = x.thi_t + mt;
+                c_exact[c] = true;
+                if (ext) c_ext[c] = x;
+            }
+        }
         for (int c = 0; c < ngt; ++c) {
             if (c_rl[c] > c_rh[c]) continue;
             // free space to the neighbouring cells, from the cells' TIGHT bounds (minima / maxima of member values: the same
@@ -563,10 +642,10 @@ UL_HDN int sectors_from_boxes(const SubBox* box, const BoxExt* ext, int nb, cons
             // that closes on itself in theta has no tips at all (spectral convergence).
             const bool scan_r = full_ring || ((c_th[c] - c_tl[c]) * c_rh[c] > (c_rh[c] - c_rl[c]));
             if (ext && TT) {
-                refine_sector_extremes<N>(L, wcx, wcy, rho, dph_limb, false, c_ext[c]);
+                if (!c_exact[c]) refine_sector_extremes<N>(L, wcx, wcy, rho, dph_limb, false, c_ext[c]);
                 patch_tangents<N>(L, *TT, c_ext[c], false, ptan[np]);
             }
-            emit_patch(patch[np++], P, point, c_rl[c], c_rh[c], c_tl[c], c_th[c], c_hr[c], c_ht[c], c_cr[c], c_ct[c],
+            emit_patch(patch[np++], c_exact[c] ? *Pquiet : P, point, c_rl[c], c_rh[c], c_tl[c], c_th[c], c_hr[c], c_ht[c], c_cr[c], c_ct[c],
                        full_ring, scan_r, gap_r_lo, gap_r_hi, gap_lo, gap_hi, units_left, status);
         }
     }

@@ -5,7 +5,8 @@ Seeded random families -- binaries with s in [0.32, 3.2] and q in [1e-5, 1], pla
 [-2, 2]^2, half of them drawn towards the lens -- are run with the shortcut (production) and with ULENS_OPT_NO_QUIET.
 The shortcut only changes how densely quiet points are sampled and shot, so the two runs must agree: no point that is
 clean in both may differ by more than 1e-4, and the flagged sets must (nearly) coincide. The worst clean points are then
-sent to the oracle. Measured: largest difference 6.6e-5 over 1.6 M points; the worst points are within 6.3e-5 of the oracle.
+sent to the oracle. Measured (1.4 M points): largest difference 3.3e-5; the worst points are within 3.4e-5 of the oracle
+(before the quiet points' sectors ended at the true extremes of their images: 6.3e-5 and 6.1e-5).
 """
 import numpy as np
 import pytest
@@ -61,7 +62,7 @@ def test_quiet_shortcut_on_random_lenses(torch_cuda, oracle, name, seed, n_cfg):
     rel[f0 | f1 | np.isnan(rel)] = 0.0
     assert n1 < 0.8 * n0                                   # the shortcut did engage
     assert abs(int(f0.sum()) - int(f1.sum())) <= 0.01 * max(int(f0.sum()), 100)
-    assert rel.max() <= 1e-4, np.argwhere(rel > 1e-4)[:8]
+    assert rel.max() <= 6e-5, np.argwhere(rel > 6e-5)[:8]
     # the worst clean points against the oracle (magnification < 30 keeps the oracle affordable)
     cand = np.where(A0 < 30, rel, 0.0)
     order = np.argsort(cand.ravel())[::-1][:12]
@@ -73,4 +74,4 @@ def test_quiet_shortcut_on_random_lenses(torch_cuda, oracle, name, seed, n_cfg):
     print("%s: %d points, limb solves per point %.0f -> %.0f, flagged %d -> %d; largest difference between the runs %.1e (%d above 5e-5); "
           "the 12 worst points against the oracle: max %.1e" % (name, A0.size, n0, n1, int(f0.sum()), int(f1.sum()), rel.max(),
                                                                  int((rel > 5e-5).sum()), r1.max() if len(r1) else 0.0))
-    assert adm.sum() >= 8 and r1.max() <= 1e-4
+    assert adm.sum() >= 8 and r1.max() <= 6e-5
