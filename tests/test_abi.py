@@ -71,3 +71,27 @@ def test_product_does_not_import_oracle():
             if f.endswith((".py", ".cu", ".cuh", ".hpp", ".h")):
                 txt = open(os.path.join(dirpath, f)).read()
                 assert "import oracle" not in txt and "from oracle" not in txt and "ulens_oracle" not in txt, f
+
+
+def test_static_entry_argument_checks_need_no_gpu(built_lib):
+    """ulens_mag_static (the no-allocation entry) checks its sizes before it touches CUDA: a request beyond the fixed scratch is
+    refused with ULENS_ELIMIT, bad arguments with ULENS_EINVAL, an empty request succeeds -- with or without a device."""
+    from paper_2510_02639_b200 import binding
+    lib = binding.lib()
+    cap = binding.ulens_static_max_points()
+    assert cap == 128 and 0 < binding.ulens_static_scratch_bytes() <= 8 << 20
+    L = (binding.ulens_lens * 3)(*[binding.ulens_lens_binary(1.0, 0.1)] * 3)
+    rho = (C.c_double * 3)(0.01, 0.01, 0.01)
+    u1 = (C.c_double * 3)(0.3, 0.3, 0.3)
+    fake = C.c_void_p(0x1000)                               # never dereferenced: every call below returns before any work
+    dp = C.POINTER(C.c_double)
+    call = lambda dev, n_cfg, n_pts, w=fake, out=fake: lib.ulens_mag_static(dev, n_cfg, n_pts, L, C.cast(rho, dp), C.cast(u1, dp),
+                                                                          w, w, out, None, None, None)
+    assert call(0, 1, cap + 1) == binding.ULENS_ELIMIT
+    assert call(0, 3, 43) == binding.ULENS_ELIMIT           # n_cfg x n_pts counts
+    assert b"ULENS_STATIC_MAX_POINTS" in lib.ulens_strerror(binding.ULENS_ELIMIT)
+    assert call(-1, 1, 4) == binding.ULENS_EINVAL
+    assert call(0, -1, 4) == binding.ULENS_EINVAL
+    assert call(0, 1, 4, w=None) == binding.ULENS_EINVAL
+    assert call(0, 1, 4, out=None) == binding.ULENS_EINVAL
+    assert call(0, 0, 4) == binding.ULENS_OK and call(0, 1, 0) == binding.ULENS_OK
