@@ -484,7 +484,8 @@ __global__ void k_quiet(int n, int pt_base, int n_pts_per_cfg, const PointCfg* _
             else { px += rho * ex; py += rho * ey; }
         }
         unsigned mask = 0;
-        const unsigned st = centre_images<N>(L, poly[c], px, py, zr, zi, mask);
+        // (the limb probes start the simultaneous iteration from the previous probe's roots, one source radius away)
+        const unsigned st = centre_images<N>(L, poly[c], px, py, zr, zi, mask, p > 0);
         if (st & (UL_ST_EA_NOCONV | UL_ST_IMG_PARITY)) ok = false;
         const double a = point_mag<N>(L, nullptr, zr, zi, mask, nullptr);
         if (p == 0) { st_c = st; A_c = a; }

@@ -457,12 +457,13 @@ UL_HDNI void poly_coeffs_ni(const Lens& L, const LensPoly& T, double wx, double 
 // (UL_ST_EA_NOCONV, UL_ST_IMG_PARITY, image count << 8).
 // ------------------------------------------------------------------------------------------------
 template <int N>
-UL_HDN unsigned centre_images(const Lens& L, const LensPoly& T, double wx, double wy, double* zr, double* zi, unsigned& mask)
+UL_HDN unsigned centre_images(const Lens& L, const LensPoly& T, double wx, double wy, double* zr, double* zi, unsigned& mask,
+                              bool warm = false)
 {
     constexpr int DEG = N * N + 1;
     double br[DEG + 1], bi[DEG + 1];
     poly_coeffs<N>(L, T, wx, wy, br, bi);
-    ea_init<DEG>(br, bi, zr, zi);
+    if (!warm) ea_init<DEG>(br, bi, zr, zi);            // warm: zr, zi hold the roots of a nearby source position
     int it = ea_iterate<DEG>(br, bi, zr, zi, 100);
     unsigned st = (it > 100) ? UL_ST_EA_NOCONV : 0u;
     // validate + polish (G7): damped Newton on Eq. 1 from every root; accept converged, un-moved, distinct ones
