@@ -430,6 +430,9 @@ __global__ void k_ext_scatter(int n, const unsigned char* __restrict__ flag, con
 // every point of C1-C3 and 1.4 M random-lens points against the full treatment, and on the stored oracle samples
 // (DESIGN.md 5.3): with exact ends (3/8, 3/4) stays within 3.3e-5 of the full grid; 5/8 of the nodes puts single points at
 // 6.7e-5 (refused); a quarter of the lines costs a broad 2e-5 ... 5e-5 (refused).
+#ifndef UL_QUIET_LIMB_DIV
+#define UL_QUIET_LIMB_DIV 8       // quiet points: n_limb / this many limb samples (16: 2 points each of C1 and C3 wrong by 1e-2 ... 3.5e-2: refused)
+#endif
 #ifndef UL_QUIET_RES_LINES
 #define UL_QUIET_RES_LINES 0.375
 #endif
@@ -571,7 +574,7 @@ k_limb(int n, int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cfg, 
     constexpr int CAP = BoxCap<N>::value;
     int n_solves = 0;
     const int n_arcs = q ? G::GPW : G::NARC;
-    const int per_arc = q ? max(2, (rp.n_limb / 8 + G::GPW - 1) / G::GPW) : 0;
+    const int per_arc = q ? max(2, (rp.n_limb / UL_QUIET_LIMB_DIV + G::GPW - 1) / G::GPW) : 0;
     unsigned st = limb_track<N, DUAL>(sh[wib], w, L, poly[c], w_re[gp], w_im[gp], cfg[c].rho, rp, c_zr + (long long)i * 10,
                                       c_zi + (long long)i * 10, c_mask[i], boxes + (size_t)i * CAP,
                                       DUAL ? exts + (size_t)i * CAP : nullptr, n_boxes + i, CAP, n_solves, n_arcs, per_arc);
@@ -612,7 +615,7 @@ k_sectors(int n, int pt_base, int n_pts_per_cfg, const PointCfg* __restrict__ cf
         // spacing of the limb samples k_limb took for this point (quiet points: GPW arcs of max(2, ...) points)
         typedef LimbGeom<N> G;
         const bool q = quiet && quiet[i];
-        const int n_samp = q ? G::GPW * max(2, (rp.n_limb / 8 + G::GPW - 1) / G::GPW) : G::NARC * max(1, (rp.n_limb + G::NARC / 2) / G::NARC);
+        const int n_samp = q ? G::GPW * max(2, (rp.n_limb / UL_QUIET_LIMB_DIV + G::GPW - 1) / G::GPW) : G::NARC * max(1, (rp.n_limb + G::NARC / 2) / G::NARC);
         // quiet points: a sector that ends at the true extremes of a smooth near-elliptical image (quiet_image_extremes) is
         // shot with fewer lines and fewer nodes per line: with exact ends the sin-spaced rule across the lines is all but exact
         RegionParams rpq = rp;
