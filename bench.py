@@ -54,9 +54,9 @@ FP64_INSTR_PER_LIMB_SOLVE = {1: 600, 2: 2400, 3: 8300}
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the roofline kernel, from the `ncu --set full` captures
 # summarised under profiles/ (r02_ncu_shoot_dual_c4.md, r02_ncu_shoot_c1.md, r02_ncu_shoot_c2.md, r02_ncu_shoot_c3.md, r02_ncu_shoot_f32_c1.md);
 # key = (config, f32 variant)
-NCU_TRAFFIC_BYTES_PER_LAUNCH = {(4, False): 50.790400e6 + 295.828224e6, (1, False): 26.636544e6 + 0.340992e6,
-                                (2, False): 29.690368e6 + 3.653888e6, (3, False): 31.650048e6 + 1.225984e6,
-                                (1, True): 26.133504e6 + 0.177664e6}
+NCU_TRAFFIC_BYTES_PER_LAUNCH = {(4, False): 50.039808e6 + 300.790784e6, (1, False): 26.111488e6 + 0.337408e6,
+                                (2, False): 29.666304e6 + 3.572480e6, (3, False): 31.663360e6 + 1.320960e6,
+                                (1, True): 26.103296e6 + 0.195840e6}
 # FP64 FMA pipe of one B200: 148 SMs x 64 DFMA lanes / clk x 1.965 GHz (clocks.max.sm) -- DESIGN.md
 FP64_PEAK_DFMA = 148 * 64 * 1.965e9
 # Mixed-precision variant (k_shoot_f32): algorithmic FP32-pipe instructions per ray in the segment-local
