@@ -325,7 +325,8 @@ __global__ void k_point_ext(int n, int n_pts_per_cfg, const PointCfg* __restrict
             else { px += r * ex; py += r * ey; }
         }
         unsigned mask = 0;
-        unsigned st = centre_images<N>(L, poly[c], px, py, zr, zi, mask);
+        // (the limb probes start the simultaneous iteration from the previous probe's roots, as in k_quiet)
+        unsigned st = centre_images<N>(L, poly[c], px, py, zr, zi, mask, p > 0);
         if (p == 0) {
             st_c = st;
             A_c = point_mag<N>(L, grad5 ? &tans[c] : nullptr, zr, zi, mask, grad5 ? g5 : nullptr);
